@@ -1,0 +1,161 @@
+/* sps.h -- C ABI of the B200-native SPS photometry / HMC library (libsps_b200.so).
+ *
+ * The library computes, on one NVIDIA B200 (sm_100a), the data-parallel hot path of
+ * arXiv:2506.19919 ("Bayesian posteriors with stellar population synthesis on GPUs"): the batched
+ * galaxy-photometry log-likelihood and its gradient inside every HMC / NUTS leapfrog step.
+ * Citations are PAPER.md:<line> of the reference text; R# are the readings listed in DESIGN.md.
+ *
+ * Conventions (all entry points):
+ *   - `*_dev` / "device" pointers are raw CUDA device pointers owned by the CALLER (e.g. torch
+ *     data_ptr()); "host" pointers are ordinary host memory.  The library never frees caller memory.
+ *   - Arrays are row-major, float32 unless stated.  n rows of D = 13 parameters in the order
+ *       logM, tau, alpha, beta, F_burst, logT_peak, logT_max, logZ, sigma_logZ, A_V, delta, F_floor, z
+ *     (z per BASELINE.json).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and
+ *     return without synchronising unless stated.
+ *   - Every call returns an sps_status; no exception crosses the ABI; sps_last_error() gives a
+ *     thread-local message for the last non-OK status.
+ *   - There is NO CPU fallback: without a compute-capability-10.x device every compute call returns
+ *     SPS_EUNSUPPORTED.
+ */
+#ifndef SPS_H_
+#define SPS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPS_NDIM 13
+
+typedef enum {
+  SPS_OK = 0,
+  SPS_EINVAL = 1,        /* null pointer, bad enum, non-monotonic grid ...            */
+  SPS_ESHAPE = 2,        /* a size is out of the supported range                      */
+  SPS_ECUDA = 3,         /* a CUDA runtime call failed (message has the CUDA string)  */
+  SPS_ENOMEM = 4,
+  SPS_EUNSUPPORTED = 5   /* no sm_100 device                                          */
+} sps_status;
+
+enum { SPS_PATH_EXACT = 0, SPS_PATH_APPROX = 1 };
+enum { SPS_SAMPLER_HMC = 0, SPS_SAMPLER_NUTS = 1 };
+
+typedef struct sps_table sps_table;      /* opaque; owns device memory */
+
+/* Everything that is fixed before the analysis.  HOST pointers; copied. */
+typedef struct {
+  int32_t n_age, n_Z, n_wave, n_band, n_z;   /* n_age<=128, n_Z<=16, n_band<=16, n_z>=2           */
+  const double* log10_age_yr;  /* [n_age]  increasing                                              */
+  const double* log10_Z;       /* [n_Z]    increasing, log10(Z/Zsun)                               */
+  const double* wave_A;        /* [n_wave] strictly increasing rest-frame wavelength, Angstrom     */
+  const float*  ssp;           /* [n_age*n_Z][n_wave] L_SSP(lambda|age_i,Z_j), row = i*n_Z + j     */
+  const double* filt_mu_A;     /* [n_band] Gaussian filter centre, observed frame   */
+  const double* filt_sigma_A;  /* [n_band] Gaussian sigma; support truncated at 5 sigma (R4)       */
+  double z_min, z_max;         /* uniform redshift grid of the c_SSP lookup table    */
+  double H0, Om;               /* flat LCDM for t_obs(z) (R11)                       */
+  double log10_mass_unit;      /* M_star is expressed in 10^this Msun so that fluxes are O(1)      */
+} sps_table_desc;
+
+/* Per-parameter hyper-parameters, HOST arrays of SPS_NDIM doubles each.
+ * Bounding sigmoid Eq. (C1): theta = y_lo + (y_hi-y_lo)/(1+exp(-k(theta~-x0))).
+ * Skew-normal prior on theta~ Eq. (C2): (2/omega) N(u) Phi(s u), u=(theta~-xi)/omega. */
+typedef struct {
+  const double *y_lo, *y_hi, *k, *x0, *xi, *omega, *skew;
+} sps_prior;
+
+/* sps_create_table: upload the grids, precompute quadrature weights (R4), per-wavelength dust
+ * constants (Eq. A8, R10), lambda_eff (Eq. 5) and the c_SSP[n_z][n_age][n_Z][n_band] lookup table
+ * (Eq. 7) ON THE GPU, and build the tensor-core operand layouts of the SSP table.
+ * Synchronises.  On success *out owns all device memory until sps_destroy_table. */
+sps_status sps_create_table(const sps_table_desc* desc, sps_table** out);
+sps_status sps_destroy_table(sps_table* t);
+
+/* Copy the c_SSP table to a HOST buffer of n_z*n_age*n_Z*n_band floats (diagnostic; synchronises). */
+sps_status sps_table_cssp(const sps_table* t, float* cssp_host);
+
+/* sps_weights (diagnostic observable for the 1e-5 weights tolerance): Eq. (A3)-(A7), (2).
+ * theta_dev [n,13]; unbounded != 0 means theta_dev holds theta~ and needs `prior` for Eq. (C1)
+ * (prior may be NULL when unbounded == 0).  Outputs (device): w_age [n,n_age] = P_SFH (Eq. A6),
+ * w_met [n,n_Z] = P_met, mstar [n] = M_star / mass_unit (Eq. A3). */
+sps_status sps_weights(const sps_table* t, const sps_prior* prior, const float* theta_dev, int64_t n,
+                       int unbounded, float* w_age_dev, float* w_met_dev, float* mstar_dev, void* stream);
+
+/* sps_photometry: band fluxes by the exact path (Eq. 4: tensor-core contraction
+ * against the SSP table, dust and redshifted filters in the epilogue) or the approximate path
+ * (Eq. 6: F_att(lambda_eff) times P_SSP-weighted sums of the z-interpolated c_SSP).
+ * flux_dev [n,n_band] out.  If flux_bar_dev [n,n_band] and theta_bar_dev [n,13] are both non-NULL the
+ * vector-Jacobian product theta_bar = flux_bar^T dflux/dtheta is also written (w.r.t. theta~ when
+ * unbounded != 0, else w.r.t. theta) (R20). */
+sps_status sps_photometry(const sps_table* t, const sps_prior* prior, int path, const float* theta_dev,
+                          int64_t n, int unbounded, float* flux_dev, const float* flux_bar_dev,
+                          float* theta_bar_dev, void* stream);
+
+/* sps_loglike_grad: logP(theta~) = -1/2 sum_b((flux_b-d_b)/sigma_b)^2 + sum_p log SN(theta~_p)
+ * (R12) and its gradient w.r.t. theta~ (fused reverse mode).
+ * theta_unb_dev [n,13]; gal_of_row_dev [n] int32 row -> galaxy index (NULL: row r uses galaxy r);
+ * obs_flux_dev, obs_sigma_dev [n_gal,n_band]; outputs logp_dev [n], grad_dev [n,13]. */
+sps_status sps_loglike_grad(const sps_table* t, const sps_prior* prior, int path,
+                            const float* theta_unb_dev, int64_t n, const int32_t* gal_of_row_dev,
+                            const float* obs_flux_dev, const float* obs_sigma_dev, float* logp_dev,
+                            float* grad_dev, void* stream);
+
+/* sps_leapfrog (diagnostic for the trajectory tolerance): n_steps leapfrog steps
+ * p += eps/2 grad; theta~ += eps invM*p; p += eps/2 grad from (theta0, p0); per-row eps
+ * [n] and diagonal inverse mass [n,13].  traj_dev [n_steps,n,2,13] receives (theta~, p) after each
+ * step; logp_traj_dev [n_steps,n] the log-posterior. */
+sps_status sps_leapfrog(const sps_table* t, const sps_prior* prior, int path, const float* theta0_dev,
+                        const float* p0_dev, const float* eps_dev, const float* inv_mass_dev, int64_t n,
+                        const int32_t* gal_of_row_dev, const float* obs_flux_dev,
+                        const float* obs_sigma_dev, int32_t n_steps, float* traj_dev,
+                        float* logp_traj_dev, void* stream);
+
+typedef struct {
+  int32_t sampler;        /* SPS_SAMPLER_HMC | SPS_SAMPLER_NUTS          */
+  int32_t path;           /* default path; overridden per galaxy by path_of_gal_dev when non-NULL     */
+  int32_t n_chain;        /* chains per galaxy                                                        */
+  int32_t n_warmup;       /* adaptation transitions (R14: windowed dual averaging + diagonal mass)    */
+  int32_t n_sample;       /* kept transitions                                                         */
+  int32_t n_leapfrog;     /* HMC trajectory length                                                    */
+  int32_t max_depth;      /* NUTS maximum tree depth (<= 10)                                          */
+  float   eps0;           /* initial step size                                                        */
+  float   target_accept;  /* dual-averaging target (0.8)                                              */
+  uint64_t seed;          /* Philox4x32-10 key (R16)                                                  */
+} sps_hmc_config;
+
+/* Per-chain summaries, DEVICE pointers, any may be NULL.  Chain index c = gal*n_chain + chain. */
+typedef struct {
+  float* mean;          /* [n_gal*n_chain,13] posterior mean of theta~ over kept samples              */
+  float* sd;            /* [n_gal*n_chain,13] posterior standard deviation (n-1)                      */
+  float* accept;        /* [n_gal*n_chain]    mean accept statistic over the sampling phase           */
+  float* eps;           /* [n_gal*n_chain]    adapted step size                                       */
+  float* inv_mass;      /* [n_gal*n_chain,13] adapted diagonal inverse mass                           */
+  int32_t* n_leapfrog;  /* [n_gal*n_chain]    total leapfrog steps taken                              */
+  int32_t* divergences; /* [n_gal*n_chain]    divergent transitions in the sampling phase             */
+  float* rhat;          /* [n_gal,13]         Gelman-Rubin statistic over the galaxy's chains */
+} sps_hmc_summary;
+
+/* sps_hmc_run: n_gal galaxies x n_chain chains of (n_warmup + n_sample) transitions.
+ * obs_flux_dev/obs_sigma_dev [n_gal,n_band]; path_of_gal_dev [n_gal] int32 or NULL;
+ * theta0_unb_dev [n_gal*n_chain,13] or NULL (R17: xi + 0.1 omega N(0,1));
+ * samples_dev [n_gal*n_chain, n_sample, 13] or NULL.  Synchronises before returning. */
+sps_status sps_hmc_run(const sps_table* t, const sps_prior* prior, const sps_hmc_config* cfg,
+                       const float* obs_flux_dev, const float* obs_sigma_dev, int64_t n_gal,
+                       const int32_t* path_of_gal_dev, const float* theta0_unb_dev, float* samples_dev,
+                       const sps_hmc_summary* summary, void* stream);
+
+/* Raw Philox4x32-10 words for the bit-exact RNG parity test (R16): out_dev [n,4] uint32 for counters
+ * (chain = first_chain + i, transition, purpose, index), key from seed. */
+sps_status sps_philox_words(uint64_t seed, uint32_t first_chain, uint32_t transition, uint32_t purpose,
+                            uint32_t index, int64_t n, uint32_t* out_dev, void* stream);
+
+/* Number of kernels this library launched since load (for bench.py's gpu_launches). */
+int64_t sps_launch_count(void);
+
+const char* sps_last_error(void);
+const char* sps_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPS_H_ */

@@ -1,0 +1,212 @@
+"""Thin ctypes binding of libsps_b200.so (include/sps.h).  Argument marshalling only: every step of
+the hot path runs in the CUDA kernels behind the C ABI.  torch is used for device memory and streams.
+
+There is no CPU fallback: if the shared library is missing or cannot be loaded, every call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsps_b200.so")
+NDIM = 13
+PATH_EXACT, PATH_APPROX = 0, 1
+SAMPLER_HMC, SAMPLER_NUTS = 0, 1
+
+EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
+           "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_launch_count",
+           "sps_last_error", "sps_version")
+
+
+class SpsError(RuntimeError):
+    pass
+
+
+class _TableDesc(C.Structure):
+    _fields_ = [("n_age", C.c_int32), ("n_Z", C.c_int32), ("n_wave", C.c_int32), ("n_band", C.c_int32), ("n_z", C.c_int32),
+                ("log10_age_yr", C.POINTER(C.c_double)), ("log10_Z", C.POINTER(C.c_double)), ("wave_A", C.POINTER(C.c_double)),
+                ("ssp", C.POINTER(C.c_float)), ("filt_mu_A", C.POINTER(C.c_double)), ("filt_sigma_A", C.POINTER(C.c_double)),
+                ("z_min", C.c_double), ("z_max", C.c_double), ("H0", C.c_double), ("Om", C.c_double),
+                ("log10_mass_unit", C.c_double)]
+
+
+class _Prior(C.Structure):
+    _fields_ = [(n, C.POINTER(C.c_double)) for n in ("y_lo", "y_hi", "k", "x0", "xi", "omega", "skew")]
+
+
+class _HmcConfig(C.Structure):
+    _fields_ = [("sampler", C.c_int32), ("path", C.c_int32), ("n_chain", C.c_int32), ("n_warmup", C.c_int32),
+                ("n_sample", C.c_int32), ("n_leapfrog", C.c_int32), ("max_depth", C.c_int32), ("eps0", C.c_float),
+                ("target_accept", C.c_float), ("seed", C.c_uint64)]
+
+
+class _HmcSummary(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat")]
+
+
+_lib = None
+
+
+def lib():
+    """Load the shared library (once).  Raises loudly when it is missing: no fallback exists."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise SpsError(f"{LIB_PATH} is missing: build it with `python -m paper_2506_19919_b200.build` "
+                           "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.sps_last_error.restype = C.c_char_p
+        L.sps_version.restype = C.c_char_p
+        L.sps_launch_count.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _check(status: int, what: str):
+    if status != 0:
+        raise SpsError(f"{what} failed with status {status}: {lib().sps_last_error().decode()}")
+
+
+def _dptr(t):
+    if t is None:
+        return C.c_void_p(0)
+    import torch
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous(), "need a contiguous CUDA tensor"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+class PriorHandle:
+    """Holds the host arrays of an sps_prior alive."""
+
+    def __init__(self, prior_array):
+        a = _f64(prior_array)
+        assert a.shape == (7, NDIM)
+        self._rows = [np.ascontiguousarray(a[i]) for i in range(7)]
+        self.c = _Prior(*[r.ctypes.data_as(C.POINTER(C.c_double)) for r in self._rows])
+
+    def ref(self):
+        return C.byref(self.c)
+
+
+class Table:
+    """Owner of an sps_table handle."""
+
+    def __init__(self, grid):
+        self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z = grid.n_age, grid.n_Z, grid.n_wave, grid.n_band, grid.n_z
+        keep = [_f64(grid.log10_age_yr), _f64(grid.log10_Z), _f64(grid.wave_A),
+                np.ascontiguousarray(grid.ssp, dtype=np.float32), _f64(grid.filt_mu_A), _f64(grid.filt_sigma_A)]
+        assert keep[3].shape == (self.n_age * self.n_Z, self.n_wave)
+        dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        d = _TableDesc(self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z, dp(keep[0]), dp(keep[1]), dp(keep[2]),
+                       keep[3].ctypes.data_as(C.POINTER(C.c_float)), dp(keep[4]), dp(keep[5]),
+                       float(grid.z_min), float(grid.z_max), float(grid.H0), float(grid.Om), float(grid.log10_mass_unit))
+        h = C.c_void_p()
+        _check(lib().sps_create_table(C.byref(d), C.byref(h)), "sps_create_table")
+        self.handle = h
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().sps_destroy_table(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def sps_create_table(grid) -> Table:
+    return Table(grid)
+
+
+def sps_table_cssp(table: Table) -> np.ndarray:
+    out = np.empty((table.n_z, table.n_age * table.n_Z, table.n_band), np.float32)
+    _check(lib().sps_table_cssp(table.handle, out.ctypes.data_as(C.POINTER(C.c_float))), "sps_table_cssp")
+    return out
+
+
+def _new(shape, dtype=None, like=None):
+    import torch
+    return torch.empty(shape, dtype=dtype or torch.float32, device=like.device if like is not None else "cuda")
+
+
+def sps_weights(table, prior, theta, unbounded=True):
+    n = theta.shape[0]
+    w_age, w_met, mstar = _new((n, table.n_age), like=theta), _new((n, table.n_Z), like=theta), _new((n,), like=theta)
+    _check(lib().sps_weights(table.handle, prior.ref() if prior else None, _dptr(theta), C.c_int64(n), int(unbounded),
+                             _dptr(w_age), _dptr(w_met), _dptr(mstar), _stream()), "sps_weights")
+    return w_age, w_met, mstar
+
+
+def sps_photometry(table, prior, path, theta, unbounded=True, flux_bar=None):
+    n = theta.shape[0]
+    flux = _new((n, table.n_band), like=theta)
+    theta_bar = _new((n, NDIM), like=theta) if flux_bar is not None else None
+    _check(lib().sps_photometry(table.handle, prior.ref() if prior else None, int(path), _dptr(theta), C.c_int64(n),
+                                int(unbounded), _dptr(flux), _dptr(flux_bar), _dptr(theta_bar), _stream()), "sps_photometry")
+    return (flux, theta_bar) if flux_bar is not None else flux
+
+
+def sps_loglike_grad(table, prior, path, theta_unb, obs_flux, obs_sigma, gal_of_row=None, want_grad=True, out=None):
+    n = theta_unb.shape[0]
+    logp, grad = out if out is not None else (_new((n,), like=theta_unb), _new((n, NDIM), like=theta_unb) if want_grad else None)
+    _check(lib().sps_loglike_grad(table.handle, prior.ref(), int(path), _dptr(theta_unb), C.c_int64(n), _dptr(gal_of_row),
+                                  _dptr(obs_flux), _dptr(obs_sigma), _dptr(logp), _dptr(grad), _stream()), "sps_loglike_grad")
+    return logp, grad
+
+
+def sps_leapfrog(table, prior, path, theta0, p0, eps, inv_mass, obs_flux, obs_sigma, n_steps, gal_of_row=None):
+    n = theta0.shape[0]
+    traj = _new((n_steps, n, 2, NDIM), like=theta0)
+    logp = _new((n_steps, n), like=theta0)
+    _check(lib().sps_leapfrog(table.handle, prior.ref(), int(path), _dptr(theta0), _dptr(p0), _dptr(eps), _dptr(inv_mass),
+                              C.c_int64(n), _dptr(gal_of_row), _dptr(obs_flux), _dptr(obs_sigma), C.c_int32(n_steps),
+                              _dptr(traj), _dptr(logp), _stream()), "sps_leapfrog")
+    return traj, logp
+
+
+def sps_hmc_run(table, prior, obs_flux, obs_sigma, *, sampler=SAMPLER_HMC, path=PATH_APPROX, n_chain=4, n_warmup=500,
+                n_sample=500, n_leapfrog=16, max_depth=8, eps0=0.05, target_accept=0.8, seed=1, path_of_gal=None,
+                theta0=None, keep_samples=False):
+    import torch
+    n_gal = obs_flux.shape[0]
+    nc = n_gal * n_chain
+    dev = obs_flux.device
+    f32 = lambda *s: torch.zeros(s, dtype=torch.float32, device=dev)
+    i32 = lambda *s: torch.zeros(s, dtype=torch.int32, device=dev)
+    out = dict(mean=f32(nc, NDIM), sd=f32(nc, NDIM), accept=f32(nc), eps=f32(nc), inv_mass=f32(nc, NDIM),
+               n_leapfrog=i32(nc), divergences=i32(nc), rhat=f32(n_gal, NDIM))
+    samples = f32(nc, n_sample, NDIM) if keep_samples else None
+    cfg = _HmcConfig(int(sampler), int(path), int(n_chain), int(n_warmup), int(n_sample), int(n_leapfrog), int(max_depth),
+                     float(eps0), float(target_accept), int(seed))
+    summ = _HmcSummary(*[out[k].data_ptr() for k in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat")])
+    _check(lib().sps_hmc_run(table.handle, prior.ref(), C.byref(cfg), _dptr(obs_flux), _dptr(obs_sigma), C.c_int64(n_gal),
+                             _dptr(path_of_gal), _dptr(theta0), _dptr(samples), C.byref(summ), _stream()), "sps_hmc_run")
+    if keep_samples:
+        out["samples"] = samples
+    return out
+
+
+def sps_philox_words(seed, first_chain, transition, purpose, index, n):
+    import torch
+    out = torch.empty((n, 4), dtype=torch.int32, device="cuda")
+    _check(lib().sps_philox_words(C.c_uint64(seed), C.c_uint32(first_chain), C.c_uint32(transition), C.c_uint32(purpose),
+                                  C.c_uint32(index), C.c_int64(n), _dptr(out), _stream()), "sps_philox_words")
+    return out
+
+
+def sps_launch_count() -> int:
+    return int(lib().sps_launch_count())

@@ -1,0 +1,82 @@
+// sps_common.cuh -- shared declarations of the CUDA path (sm_100a only).
+// No code is shared with oracle/ ; formulas are restated from PAPER.md (line numbers cited) and
+// the DESIGN.md readings R#.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sps.h"
+
+#define SPS_MAX_AGE 128
+#define SPS_MAX_Z 16
+#define SPS_MAX_BAND 16
+#define SPS_AGE_PER_LANE 4          // ceil(SPS_MAX_AGE / 32)
+#define FULL_MASK 0xffffffffu
+
+// ---------------------------------------------------------------------------------------------
+// device-side view of a table (passed to kernels by value; arrays live in device memory)
+// ---------------------------------------------------------------------------------------------
+struct TableDev {
+  int n_age, n_Z, n_wave, n_band, n_z, K;     // K = n_age * n_Z
+  int n_wave_pad;                              // n_wave rounded up for the tensor-core tiles
+  int cs_stride;                               // floats between consecutive ages in a c_SSP slice (n_Z*n_band padded)
+  // age grid (R5): A[i] lower age edge of bin i in Gyr (A[0] = 0, A[n_age] = +huge)
+  const float* A_edge;      // [n_age+1]
+  const float* A_mid;       // [n_age]   (A[i]+A[i+1])/2   (last: unused)
+  const float* A_half;      // [n_age]   (A[i+1]-A[i])/2   (last: +huge)
+  const float* e_edge;      // [n_age+1] log10(age/yr) of the edges (-huge, ..., +huge)
+  const float* g_mid;       // [n_Z-1]   log10 Z bin edges (midpoints)
+  // wavelength grid and per-wavelength constants (exact path)
+  const float* wave;        // [n_wave_pad] Angstrom (padding: copies of the last value)
+  const float* dlam;        // [n_wave_pad] trapezoid weights (R4), 0 in the padding
+  const float* k0;          // [n_wave_pad] Calzetti k0(lambda) (R10)
+  const float* drude;       // [n_wave_pad] Drude profile (R10)
+  const float* l2r;         // [n_wave_pad] log2(lambda / 5500 A)
+  const float* ssp;         // [K][n_wave_pad] fp32
+  // filters
+  float filt_mu[SPS_MAX_BAND], filt_sigma[SPS_MAX_BAND], lam_eff[SPS_MAX_BAND];
+  // c_SSP lookup table (Eq. 7): [n_z][n_age][cs_stride], entry (j*n_band + b) inside a row
+  const float* cssp;
+  float z_min, dz, inv_dz;
+  // cosmology (R11): t = t_pref * asinh(t_arg * (1+z)^-1.5)  [Gyr];  H0 in 1/Gyr
+  float t_pref, t_arg, H0_gyr, Om, OL;
+  float log10_mass_unit;
+};
+
+struct PriorDev {
+  float y_lo[SPS_NDIM], y_hi[SPS_NDIM], k[SPS_NDIM], x0[SPS_NDIM];
+  float xi[SPS_NDIM], omega[SPS_NDIM], skew[SPS_NDIM];
+};
+
+// Per-row intermediate record exchanged between the prologue, contraction and epilogue kernels.
+// All sizes padded so rows are 16-byte aligned.
+#define ROW_A_STRIDE 128      // a_i / a_bar_i
+#define ROW_M_STRIDE 16       // m_j / m_bar_j
+struct RowScalars {           // 16 floats
+  float Mn;                   // M_star / mass_unit
+  float z;                    // bounded redshift
+  float zfrac;                // position inside the z cell [0,1)
+  int   zbin;                 // lower z-grid index
+  float AV, delta, Ffloor;    // bounded dust parameters
+  float logp_like;            // filled by the contraction: -1/2 chi^2
+  float Mn_bar;               // d logL / d Mn
+  float z_bar;                // direct d logL / d z (table interpolation + dust at lambda_eff/(1+z) or filter shift)
+  float AV_bar, delta_bar, Ffloor_bar;
+  float pad0, pad1, pad2;
+};
+
+// ---------------------------------------------------------------------------------------------
+// small device helpers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL_MASK, v, o);
+  return v;
+}
+
+__device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+
+// launch counter (host side)
+extern "C" int64_t sps_launch_count(void);
+void sps_count_launch(int n = 1);
+void sps_set_error(const char* fmt, ...);
+sps_status sps_check_cuda(cudaError_t e, const char* what);

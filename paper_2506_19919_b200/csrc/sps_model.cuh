@@ -1,0 +1,274 @@
+// sps_model.cuh -- warp-level device functions of the SPS model: one warp owns one parameter row.
+// Steps a0-a5 of the hot path (C1 unbounding, t_obs(z), smooth/burst age weights, MDF weights) and
+// their reverse mode.  Lane l owns age bins l, l+32, l+64, l+96 and metallicity bin l.
+#pragma once
+#include "sps_common.cuh"
+
+#define LN2F 0.69314718055994531f
+#define LOG2EF 1.4426950408889634f
+#define LN10F 2.3025850929940457f
+
+// ---- a0: Eq. (C1) PAPER.md:429 -----------------------------------------------------------------
+// Every lane returns all 13 bounded parameters (th) and d theta / d theta~ (dth).
+__device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PriorDev& pr,
+                                            float th[SPS_NDIM], float dth[SPS_NDIM]) {
+  const int l = lane_id();
+  float v = 0.f, d = 1.f;
+  if (l < SPS_NDIM) {
+    v = row[l];
+    if (unbounded) {
+      float s = 1.f / (1.f + expf(-pr.k[l] * (v - pr.x0[l])));
+      float w = pr.y_hi[l] - pr.y_lo[l];
+      v = pr.y_lo[l] + w * s;
+      d = w * pr.k[l] * s * (1.f - s);
+    }
+  }
+#pragma unroll
+  for (int p = 0; p < SPS_NDIM; ++p) {
+    th[p] = __shfl_sync(FULL_MASK, v, p);
+    dth[p] = __shfl_sync(FULL_MASK, d, p);
+  }
+}
+
+// ---- a1: age of the universe (R11), Gyr, and dt/dz ------------------------------------------------
+__device__ __forceinline__ void cosmic_time(const TableDev& T, float z, float& t, float& dt_dz) {
+  float zp = 1.f + z, zp3 = zp * zp * zp;
+  t = T.t_pref * asinhf(T.t_arg * rsqrtf(zp3));
+  dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp3 + T.OL));
+}
+
+// ---- a2: double power law, Eq. (A4) PAPER.md:346 ---------------------------------------------------
+// f = 1/(x^alpha + x^-beta) at x = 2^lx2, plus q = f^2 (alpha x^alpha - beta x^-beta)  (df/dtau = q/tau,
+// df/dt = -q/t), fa = df/dalpha, fb = df/dbeta.
+__device__ __forceinline__ void sfr_node(float lx2, float alpha, float beta, float& f, float& q, float& fa, float& fb) {
+  float xa = exp2f(fminf(alpha * lx2, 60.f));
+  float xb = exp2f(fminf(-beta * lx2, 60.f));
+  f = __frcp_rn(xa + xb);
+  float f2 = f * f, lx = lx2 * LN2F;
+  q = f2 * (alpha * xa - beta * xb);
+  fa = -f2 * xa * lx;
+  fb = f2 * xb * lx;
+}
+__device__ __forceinline__ float sfr_value(float t, float tau, float alpha, float beta) {
+  if (!(t > 0.f)) return 0.f;
+  float lx2 = log2f(t / tau);
+  return __frcp_rn(exp2f(fminf(alpha * lx2, 60.f)) + exp2f(fminf(-beta * lx2, 60.f)));
+}
+
+struct AgeQuad {                       // per lane: its (up to) 4 bins, for M_formed = 1
+  float dM[SPS_AGE_PER_LANE];          // int_bin f dt            (Eq. A5 numerator)
+  float g_tau[SPS_AGE_PER_LANE], g_al[SPS_AGE_PER_LANE], g_be[SPS_AGE_PER_LANE], g_t[SPS_AGE_PER_LANE];
+};
+
+// Gauss-Legendre nodes/weights on [-1,1]
+__device__ __constant__ float GL2_X[2] = {-0.5773502691896257f, 0.5773502691896257f};
+__device__ __constant__ float GL4_X[4] = {-0.8611363115940526f, -0.3399810435848563f, 0.3399810435848563f, 0.8611363115940526f};
+__device__ __constant__ float GL4_W[4] = {0.3478548451374538f, 0.6521451548625461f, 0.6521451548625461f, 0.3478548451374538f};
+__device__ __constant__ float GL8_X[8] = {-0.9602898564975363f, -0.7966664774136267f, -0.5255324099163290f, -0.1834346424956498f,
+                                          0.1834346424956498f, 0.5255324099163290f, 0.7966664774136267f, 0.9602898564975363f};
+__device__ __constant__ float GL8_W[8] = {0.1012285362903763f, 0.2223810344533745f, 0.3137066458778873f, 0.3626837833783620f,
+                                          0.3626837833783620f, 0.3137066458778873f, 0.2223810344533745f, 0.1012285362903763f};
+
+// Mass formed per age bin (Eq. A5; R5, R6 restated for fp32):
+//  * bins whose span in ln t is small against the width 1/(alpha+beta) of the SFR turnover are
+//    integrated by 2- or 4-point Gauss-Legendre in linear t with the tabulated bin width (no
+//    t_obs - age cancellation in the width);
+//  * the few old bins near age ~ t_obs (and the one that reaches t = 0) are integrated by the whole
+//    warp: 8-point Gauss-Legendre panels in v = ln t, cut at ln t_hi - 16/(beta+1).
+template <bool WANT_GRAD>
+__device__ __forceinline__ void smooth_bins(const TableDev& T, float t_obs, float tau, float alpha, float beta, AgeQuad& Q) {
+  const int l = lane_id();
+  const float l2tau = log2f(tau);
+  const float ab = alpha + beta;
+  unsigned problem_mask[SPS_AGE_PER_LANE];
+  float t_lo_q[SPS_AGE_PER_LANE], t_hi_q[SPS_AGE_PER_LANE];
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    const int i = l + 32 * q;
+    Q.dM[q] = Q.g_tau[q] = Q.g_al[q] = Q.g_be[q] = Q.g_t[q] = 0.f;
+    float t_hi = 0.f, t_lo = 0.f, half = 0.f, t_mid = 1.f;
+    int kind = 0;                       // 0 empty, 1 GL2, 2 GL4, 3 warp-cooperative
+    if (i < T.n_age) {
+      t_hi = t_obs - T.A_edge[i];
+      t_lo = fmaxf(t_obs - T.A_edge[i + 1], 0.f);
+      half = T.A_half[i];
+      t_mid = t_obs - T.A_mid[i];
+      if (t_hi > 0.f) {
+        float s = (t_lo > 0.f) ? (half / t_mid) * ab * 0.3183098861837907f : 1e9f;   // half-width / pole distance
+        kind = (s < 0.06f) ? 1 : (s < 0.36f ? 2 : 3);
+      } else t_hi = 0.f;
+    }
+    t_lo_q[q] = t_lo; t_hi_q[q] = t_hi;
+    problem_mask[q] = __ballot_sync(FULL_MASK, kind == 3);
+    const bool any4 = __any_sync(FULL_MASK, kind == 2);
+    if (kind == 1 || kind == 2) {
+      float s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+      if (!any4) {
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          float t = t_mid + half * GL2_X[k], f, qq, fa, fb;
+          sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
+          s0 += f;
+          if (WANT_GRAD) { s1 += qq; s2 += fa; s3 += fb; s4 -= qq / t; }
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          float t = t_mid + half * GL4_X[k], f, qq, fa, fb, w = GL4_W[k];
+          sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
+          s0 += w * f;
+          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; s4 -= w * qq / t; }
+        }
+      }
+      Q.dM[q] = half * s0;
+      if (WANT_GRAD) { Q.g_tau[q] = half * s1 / tau; Q.g_al[q] = half * s2; Q.g_be[q] = half * s3; Q.g_t[q] = half * s4; }
+    }
+  }
+  // warp-cooperative bins
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    unsigned m = problem_mask[q];
+    while (m) {
+      const int src = __ffs(m) - 1;
+      m &= m - 1;
+      const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], src);
+      const float t_lo = __shfl_sync(FULL_MASK, t_lo_q[q], src);
+      const float v_hi = logf(t_hi);
+      float v_lo = v_hi - 16.f / (beta + 1.f);
+      if (t_lo > 0.f) v_lo = fmaxf(v_lo, logf(t_lo));
+      const float dv = v_hi - v_lo;
+      const float w_target = fminf(fmaxf(6.5f / ab, 0.5f), 2.0f);
+      const int n_pan = max(1, (int)ceilf(dv / w_target));
+      const float wp = dv / (float)n_pan;
+      const float ln_tau = l2tau * LN2F;
+      float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+      for (int n = l; n < n_pan * 8; n += 32) {
+        const int pan = n >> 3, k = n & 7;
+        const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
+        const float w = 0.5f * wp * GL8_W[k] * expf(v);        // dt = t dv
+        float f, qq, fa, fb;
+        sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
+        s0 += w * f;
+        if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; }
+      }
+      s0 = warp_sum(s0);
+      if (WANT_GRAD) { s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3); }
+      if (l == src) {
+        Q.dM[q] = s0;
+        if (WANT_GRAD) {
+          Q.g_tau[q] = s1 / tau; Q.g_al[q] = s2; Q.g_be[q] = s3;
+          Q.g_t[q] = sfr_value(t_hi, tau, alpha, beta) - sfr_value(t_lo, tau, alpha, beta);   // Leibniz
+        }
+      }
+    }
+  }
+}
+
+// ---- a3: triweight burst, Eq. (A6)-(A7) PAPER.md:358-372 (R7: CDF differences over the age-bin edges) ----
+// P_i = int_{y_lo}^{y_hi} (35/32)(1-y^2)^3 dy with y = clip((e - logT_peak)/(logT_max - logT_peak), -1, 1);
+// the integrand is a degree-6 polynomial, so 4-point Gauss-Legendre is exact and free of cancellation.
+__device__ __forceinline__ float tri_pdf_y(float y) { float u = 1.f - y * y; return (35.f / 32.f) * u * u * u; }
+
+struct BurstQuad { float P[SPS_AGE_PER_LANE], d_ltp[SPS_AGE_PER_LANE], d_ltm[SPS_AGE_PER_LANE]; };
+
+__device__ __forceinline__ void burst_bins(const TableDev& T, float ltp, float ltm, BurstQuad& B) {
+  const int l = lane_id();
+  const float inv_s3 = 1.f / (ltm - ltp);
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    const int i = l + 32 * q;
+    B.P[q] = B.d_ltp[q] = B.d_ltm[q] = 0.f;
+    if (i < T.n_age) {
+      float ya = fminf(fmaxf((T.e_edge[i] - ltp) * inv_s3, -1.f), 1.f);
+      float yb = fminf(fmaxf((T.e_edge[i + 1] - ltp) * inv_s3, -1.f), 1.f);
+      float half = 0.5f * (yb - ya), mid = 0.5f * (yb + ya), s = 0.f;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) s += GL4_W[k] * tri_pdf_y(mid + half * GL4_X[k]);
+      B.P[q] = half * s;
+      float pa = tri_pdf_y(ya), pb = tri_pdf_y(yb);           // zero at the clips
+      // dy/dlogT_peak = (y-1)/s3, dy/dlogT_max = -y/s3
+      B.d_ltp[q] = (pb * (yb - 1.f) - pa * (ya - 1.f)) * inv_s3;
+      B.d_ltm[q] = (-pb * yb + pa * ya) * inv_s3;
+    }
+  }
+}
+
+// ---- a4: lognormal MDF PAPER.md:378 (R9).  Lane j < n_Z owns metallicity bin j. -------------------
+__device__ __forceinline__ void met_bin(const TableDev& T, float lz, float s, float& m, float& d_lz, float& d_s) {
+  const int j = lane_id();
+  m = d_lz = d_s = 0.f;
+  if (j < T.n_Z) {
+    const float inv_s = 1.f / s;
+    const bool has_lo = j > 0, has_hi = j < T.n_Z - 1;
+    float ua = has_lo ? (T.g_mid[j - 1] - lz) * inv_s : -1e30f;
+    float ub = has_hi ? (T.g_mid[j] - lz) * inv_s : 1e30f;
+    const float r2 = 0.7071067811865476f;
+    // normal-CDF difference through the tail that keeps relative accuracy
+    if (ua > 0.f) m = 0.5f * (erfcf(ua * r2) - (has_hi ? erfcf(ub * r2) : 0.f));
+    else if (ub < 0.f) m = 0.5f * (erfcf(-ub * r2) - (has_lo ? erfcf(-ua * r2) : 0.f));
+    else m = 1.f - 0.5f * ((has_hi ? erfcf(ub * r2) : 0.f) + (has_lo ? erfcf(-ua * r2) : 0.f));
+    const float c = 0.3989422804014327f;
+    float pa = has_lo ? c * expf(-0.5f * ua * ua) : 0.f;
+    float pb = has_hi ? c * expf(-0.5f * ub * ub) : 0.f;
+    d_lz = -(pb - pa) * inv_s;
+    d_s = -(pb * (has_hi ? ub : 0.f) - pa * (has_lo ? ua : 0.f)) * inv_s;
+  }
+}
+
+// ---- a8: dust, Eq. (A8)-(A9) PAPER.md:386-392 (R10) at an arbitrary rest wavelength (approximate path) ----
+#define CALZ_SWITCH_INV_UM 1.2809053864877329f
+__device__ __forceinline__ void dust_at(float lam, float AV, float delta, float Ffl,
+                                        float& F, float& F_av, float& F_del, float& F_fl, float& F_lam) {
+  const float u = 1.0e4f / lam;
+  float k0, dk_du;
+  if (u > CALZ_SWITCH_INV_UM) {
+    k0 = 2.659f * (-2.156f + u * (1.509f + u * (-0.198f + u * 0.011f))) + 4.05f;
+    dk_du = 2.659f * (1.509f + u * (-0.396f + u * 0.033f));
+  } else {
+    k0 = 2.659f * (-1.857f + 1.040f * u) + 4.05f;
+    dk_du = 2.659f * 1.040f;
+  }
+  float dk0 = dk_du * (-u / lam);
+  if (!(k0 > 0.f)) { k0 = 0.f; dk0 = 0.f; }
+  const float l0 = 2175.f, w = 350.f;
+  const float n = (lam * w) * (lam * w);
+  const float dl = lam * lam - l0 * l0;
+  const float den = dl * dl + n;
+  const float dn = 2.f * lam * w * w;
+  const float dd = 4.f * lam * dl + dn;
+  const float dr = n / den, ddr = (dn * den - n * dd) / (den * den);
+  const float l2r = log2f(lam * (1.f / 5500.f));
+  const float pw = exp2f(delta * l2r);
+  const float Eb = 0.85f - 1.9f * delta;
+  const float br = k0 * pw + Eb * dr;
+  float A = AV * (1.f / 4.05f) * br;
+  float A_av = br * (1.f / 4.05f);
+  float A_del = AV * (1.f / 4.05f) * (k0 * pw * l2r * LN2F - 1.9f * dr);
+  float A_lam = AV * (1.f / 4.05f) * (dk0 * pw + k0 * delta * pw / lam + Eb * ddr);
+  if (!(A > 0.f)) { A = 0.f; A_av = A_del = A_lam = 0.f; }
+  const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+  const float dF_dA = -(1.f - Ffl) * 0.4f * LN10F * Tt;
+  F = Ffl + (1.f - Ffl) * Tt;
+  F_av = dF_dA * A_av; F_del = dF_dA * A_del; F_fl = 1.f - Tt; F_lam = dF_dA * A_lam;
+}
+
+// ---- a9 (prior part): log skew-normal, Eq. (C2), and d/dtheta~ ---------------------------
+__device__ __forceinline__ void log_skew_normal(float x, float xi, float om, float s, float& lp, float& dlp) {
+  const float u = (x - xi) / om;
+  const float a = s * u;
+  // log Phi(a) through erfc (scaled form for the far lower tail)
+  const float r2 = 0.7071067811865476f;
+  float logPhi, ratio;   // ratio = phi(a)/Phi(a)
+  const float Phi = 0.5f * erfcf(-a * r2);
+  if (a > -5.f) {
+    logPhi = logf(Phi);
+    ratio = 0.3989422804014327f * expf(-0.5f * a * a) / Phi;
+  } else {               // asymptotic: Phi(a) ~ phi(a)/(-a) (1 - 1/a^2 + 3/a^4)
+    const float ia2 = 1.f / (a * a);
+    const float corr = 1.f - ia2 + 3.f * ia2 * ia2;
+    logPhi = -0.5f * a * a - 0.9189385332046727f - logf(-a) + logf(corr);
+    ratio = -a / corr;
+  }
+  lp = 0.6931471805599453f - logf(om) - 0.9189385332046727f - 0.5f * u * u + logPhi;
+  dlp = (-u + s * ratio) / om;
+}

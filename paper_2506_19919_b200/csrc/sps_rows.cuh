@@ -1,0 +1,27 @@
+// sps_rows.cuh -- buffers exchanged between the per-row prologue / epilogue kernels (one warp per
+// parameter row; shared by the exact and the approximate photometry paths) and the contraction kernels.
+#pragma once
+#include "sps_model.cuh"
+
+// Work buffers for n rows (device memory owned by the library, grown on demand).
+struct RowBuffers {
+  float* a;        // [n][ROW_A_STRIDE]  P_SFH (Eq. A6)
+  float* m;        // [n][ROW_M_STRIDE]  P_met
+  float* a_bar;    // [n][ROW_A_STRIDE]  d logL / d a_i
+  float* m_bar;    // [n][ROW_M_STRIDE]  d logL / d m_j
+  RowScalars* sc;  // [n]
+  float* flux;     // [n][SPS_MAX_BAND]  model band fluxes
+  int64_t capacity;
+};
+
+// kernels (sps_kernels.cu)
+void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
+                     const int* rows, RowBuffers B, cudaStream_t s);
+void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
+                            const float* obs_flux, const float* obs_sigma, const float* flux_bar,
+                            bool want_grad, RowBuffers B, cudaStream_t s);
+void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
+                     bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s);
+void launch_copy_weights(const TableDev& T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar,
+                         cudaStream_t s);
+void launch_copy_flux(const TableDev& T, int64_t n, RowBuffers B, float* flux, cudaStream_t s);

@@ -1,0 +1,170 @@
+// sps_table.cu -- sps_create_table / sps_destroy_table: device-resident grids, per-wavelength
+// constants and the c_SSP lookup table (Eq. 7), which is built on the GPU.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include "sps_internal.h"
+
+// T_b(lambda_obs): Gaussian transmission truncated at 5 sigma (R4)
+__device__ __forceinline__ float filter_T(float lam_obs, float mu, float sigma) {
+  const float x = (lam_obs - mu) / sigma;
+  return (fabsf(x) <= 5.f) ? expf(-0.5f * x * x) : 0.f;
+}
+
+// c_SSP[t][i][j*n_band+b] = sum_k L_ij(lam_k) T_b(lam_k (1+z_t)) dlam_k.  One warp per (t, ij).
+__global__ void __launch_bounds__(256) cssp_build_kernel(TableDev T, float* __restrict__ cssp) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w >= (int64_t)T.n_z * T.K) return;
+  const int t = (int)(w / T.K), ij = (int)(w % T.K);
+  const int i = ij / T.n_Z, j = ij % T.n_Z;
+  const int l = threadIdx.x & 31;
+  const float zp = 1.f + T.z_min + T.dz * (float)t;
+  const float* L = T.ssp + (int64_t)ij * T.n_wave_pad;
+  for (int b = 0; b < T.n_band; ++b) {
+    const float mu = T.filt_mu[b], sg = T.filt_sigma[b];
+    const float lo = (mu - 5.f * sg) / zp, hi = (mu + 5.f * sg) / zp;
+    // first k with wave[k] >= lo (binary search; a slightly wide window is harmless: T = 0 outside)
+    int a = 0, c = T.n_wave;
+    while (a < c) { int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
+    int k0 = max(a - 1, 0);
+    a = k0; c = T.n_wave;
+    while (a < c) { int mid = (a + c) >> 1; if (T.wave[mid] <= hi) a = mid + 1; else c = mid; }
+    const int k1 = min(a + 1, T.n_wave);
+    float acc = 0.f, comp = 0.f;                   // Kahan: up to ~1500 terms
+    for (int k = k0 + l; k < k1; k += 32) {
+      const float term = L[k] * filter_T(T.wave[k] * zp, mu, sg) * T.dlam[k];
+      const float y = term - comp, s = acc + y;
+      comp = (s - acc) - y; acc = s;
+    }
+    acc = warp_sum(acc);
+    if (l == 0) cssp[((int64_t)t * T.n_age + i) * T.cs_stride + j * T.n_band + b] = acc;
+  }
+}
+
+template <class T>
+static T* upload(const std::vector<T>& v, sps_status& st) {
+  T* d = nullptr;
+  if (st != SPS_OK) return nullptr;
+  if (cudaMalloc(&d, v.size() * sizeof(T)) != cudaSuccess) { st = SPS_ENOMEM; sps_set_error("cudaMalloc of %zu bytes failed", v.size() * sizeof(T)); return nullptr; }
+  if (cudaMemcpy(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) { st = SPS_ECUDA; sps_set_error("cudaMemcpy H2D failed"); }
+  return d;
+}
+
+static double calz_k0(double lam_A) {
+  const double u = 1.0e4 / lam_A;
+  double k = (u > 1.2809053864877329) ? 2.659 * (-2.156 + 1.509 * u - 0.198 * u * u + 0.011 * u * u * u) + 4.05
+                                       : 2.659 * (-1.857 + 1.040 * u) + 4.05;
+  return k > 0 ? k : 0.0;
+}
+static double drude_profile(double lam) {
+  const double l0 = 2175.0, w = 350.0, n = (lam * w) * (lam * w), d = (lam * lam - l0 * l0);
+  return n / (d * d + n);
+}
+
+extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out) {
+  if (!d || !out) { sps_set_error("sps_create_table: null argument"); return SPS_EINVAL; }
+  *out = nullptr;
+  if (!d->log10_age_yr || !d->log10_Z || !d->wave_A || !d->ssp || !d->filt_mu_A || !d->filt_sigma_A) {
+    sps_set_error("sps_create_table: null array in descriptor"); return SPS_EINVAL; }
+  if (d->n_age < 2 || d->n_age > SPS_MAX_AGE || d->n_Z < 2 || d->n_Z > SPS_MAX_Z || d->n_band < 1 ||
+      d->n_band > SPS_MAX_BAND || d->n_wave < 8 || d->n_z < 2 || d->n_Z * d->n_band > 128) {
+    sps_set_error("sps_create_table: size out of range (n_age<=128, n_Z<=16, n_band<=16, n_Z*n_band<=128, n_wave>=8, n_z>=2)");
+    return SPS_ESHAPE; }
+  for (int i = 1; i < d->n_age; ++i) if (!(d->log10_age_yr[i] > d->log10_age_yr[i - 1])) { sps_set_error("age grid not increasing"); return SPS_EINVAL; }
+  for (int i = 1; i < d->n_Z; ++i) if (!(d->log10_Z[i] > d->log10_Z[i - 1])) { sps_set_error("Z grid not increasing"); return SPS_EINVAL; }
+  for (int i = 1; i < d->n_wave; ++i) if (!(d->wave_A[i] > d->wave_A[i - 1])) { sps_set_error("wavelength grid not increasing"); return SPS_EINVAL; }
+  if (!(d->z_max > d->z_min) || !(d->H0 > 0) || !(d->Om > 0 && d->Om < 1)) { sps_set_error("bad z grid or cosmology"); return SPS_EINVAL; }
+  sps_status st = sps_require_device();
+  if (st != SPS_OK) return st;
+
+  sps_table* t = new sps_table();
+  TableDev& T = t->dev;
+  memset(&T, 0, sizeof(T));
+  T.n_age = d->n_age; T.n_Z = d->n_Z; T.n_wave = d->n_wave; T.n_band = d->n_band; T.n_z = d->n_z;
+  T.K = d->n_age * d->n_Z;
+  T.n_wave_pad = (d->n_wave + 255) / 256 * 256;
+  int E4 = (d->n_Z * d->n_band + 3) / 4;
+  if ((E4 & 1) == 0) E4 += 1;                       // odd number of float4 per age row: conflict-free smem tiles
+  T.cs_stride = 4 * E4;
+  const int na = d->n_age;
+  std::vector<float> A_edge(na + 1), A_mid(na), A_half(na), e_edge(na + 1), g_mid(d->n_Z - 1 > 0 ? d->n_Z - 1 : 1);
+  std::vector<double> Ae(na + 1);
+  Ae[0] = 0.0; e_edge[0] = -1e30f;
+  for (int i = 1; i < na; ++i) { const double mid = 0.5 * (d->log10_age_yr[i] + d->log10_age_yr[i - 1]); Ae[i] = pow(10.0, mid - 9.0); e_edge[i] = (float)mid; }
+  Ae[na] = 1e30; e_edge[na] = 1e30f;
+  for (int i = 0; i <= na; ++i) A_edge[i] = (float)Ae[i];
+  for (int i = 0; i < na; ++i) { A_mid[i] = (float)(0.5 * (Ae[i] + Ae[i + 1])); A_half[i] = (float)(0.5 * (Ae[i + 1] - Ae[i])); }
+  for (int j = 0; j + 1 < d->n_Z; ++j) g_mid[j] = (float)(0.5 * (d->log10_Z[j] + d->log10_Z[j + 1]));
+  const int nw = d->n_wave, nwp = T.n_wave_pad;
+  std::vector<float> wave(nwp), dlam(nwp, 0.f), k0(nwp), dr(nwp), l2r(nwp);
+  for (int k = 0; k < nwp; ++k) {
+    const double lam = d->wave_A[k < nw ? k : nw - 1];
+    wave[k] = (float)lam; k0[k] = (float)calz_k0(lam); dr[k] = (float)drude_profile(lam); l2r[k] = (float)log2(lam / 5500.0);
+  }
+  for (int k = 0; k < nw; ++k) {                     // R4: trapezoid weights
+    const double lo = d->wave_A[k > 0 ? k - 1 : 0], hi = d->wave_A[k < nw - 1 ? k + 1 : nw - 1];
+    dlam[k] = (float)(0.5 * (hi - lo));
+  }
+  std::vector<float> ssp((size_t)T.K * nwp, 0.f);
+  for (int r = 0; r < T.K; ++r) memcpy(&ssp[(size_t)r * nwp], d->ssp + (size_t)r * nw, sizeof(float) * nw);
+  for (int b = 0; b < d->n_band; ++b) {
+    const double mu = d->filt_mu_A[b], sg = d->filt_sigma_A[b];
+    if (!(sg > 0) || !(mu - 5 * sg > 0)) { sps_set_error("filter %d: need sigma > 0 and mu - 5 sigma > 0", b); delete t; return SPS_EINVAL; }
+    T.filt_mu[b] = (float)mu; T.filt_sigma[b] = (float)sg;
+    // Eq. (5) PAPER.md:73 at z = 0 on the filter's own grid
+    const int nq = 4001; double num = 0, den = 0;
+    for (int q = 0; q < nq; ++q) {
+      const double lam = mu - 5 * sg + 10 * sg * q / (nq - 1), x = (lam - mu) / sg, w = (q == 0 || q == nq - 1) ? 0.5 : 1.0;
+      const double Tq = exp(-0.5 * x * x); num += w * lam * Tq; den += w * Tq;
+    }
+    T.lam_eff[b] = (float)(num / den);
+  }
+  T.z_min = (float)d->z_min; T.dz = (float)((d->z_max - d->z_min) / (d->n_z - 1)); T.inv_dz = (float)((d->n_z - 1) / (d->z_max - d->z_min));
+  const double OL = 1.0 - d->Om, inv_H0 = 977.7922216807891 / d->H0;
+  T.t_pref = (float)(2.0 * inv_H0 / (3.0 * sqrt(OL))); T.t_arg = (float)sqrt(OL / d->Om);
+  T.H0_gyr = (float)(1.0 / inv_H0); T.Om = (float)d->Om; T.OL = (float)OL;
+  T.log10_mass_unit = (float)d->log10_mass_unit;
+
+  T.A_edge = upload(A_edge, st); T.A_mid = upload(A_mid, st); T.A_half = upload(A_half, st); T.e_edge = upload(e_edge, st);
+  T.g_mid = upload(g_mid, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
+  T.drude = upload(dr, st); T.l2r = upload(l2r, st); T.ssp = upload(ssp, st);
+  float* cssp = nullptr;
+  const size_t cs_n = (size_t)T.n_z * T.n_age * T.cs_stride;
+  if (st == SPS_OK && cudaMalloc(&cssp, cs_n * sizeof(float)) != cudaSuccess) { st = SPS_ENOMEM; sps_set_error("cudaMalloc c_SSP failed"); }
+  if (st == SPS_OK) {
+    cudaMemset(cssp, 0, cs_n * sizeof(float));
+    T.cssp = cssp;
+    const int64_t warps = (int64_t)T.n_z * T.K;
+    cssp_build_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256>>>(T, cssp);
+    sps_count_launch();
+    st = sps_check_cuda(cudaDeviceSynchronize(), "c_SSP build");
+  }
+  if (st == SPS_OK) st = sps_exact_setup(t);
+  if (st != SPS_OK) { sps_destroy_table(t); return st; }
+  *out = t;
+  return SPS_OK;
+}
+
+extern "C" sps_status sps_destroy_table(sps_table* t) {
+  if (!t) return SPS_OK;
+  TableDev& T = t->dev;
+  const void* ptrs[] = {T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
+  for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
+  sps_exact_teardown(t);
+  sps_free_row_buffers(t);
+  delete t;
+  return SPS_OK;
+}
+
+extern "C" sps_status sps_table_cssp(const sps_table* t, float* host) {
+  if (!t || !host) { sps_set_error("sps_table_cssp: null argument"); return SPS_EINVAL; }
+  const TableDev& T = t->dev;
+  const int E = T.n_Z * T.n_band;
+  std::vector<float> tmp((size_t)T.n_z * T.n_age * T.cs_stride);
+  sps_status st = sps_check_cuda(cudaMemcpy(tmp.data(), T.cssp, tmp.size() * sizeof(float), cudaMemcpyDeviceToHost), "c_SSP D2H");
+  if (st != SPS_OK) return st;
+  for (int64_t r = 0; r < (int64_t)T.n_z * T.n_age; ++r) memcpy(host + r * E, &tmp[r * T.cs_stride], sizeof(float) * E);
+  return SPS_OK;
+}
