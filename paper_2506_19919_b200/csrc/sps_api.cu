@@ -94,10 +94,10 @@ sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* thet
 
 extern "C" sps_status sps_weights(const sps_table* tc, const sps_prior* prior, const float* theta, int64_t n, int unbounded,
                                   float* w_age, float* w_met, float* mstar, void* stream) {
-  REQUIRE(tc && theta, "null table or theta");
   REQUIRE(n >= 0, "negative n");
-  REQUIRE(!unbounded || prior, "unbounded parameters need a prior (bounds)");
   if (n == 0) return SPS_OK;
+  REQUIRE(tc && theta, "null table or theta");
+  REQUIRE(!unbounded || prior, "unbounded parameters need a prior (bounds)");
   sps_table* t = const_cast<sps_table*>(tc);
   PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
   st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
@@ -109,8 +109,9 @@ extern "C" sps_status sps_weights(const sps_table* tc, const sps_prior* prior, c
 
 extern "C" sps_status sps_photometry(const sps_table* tc, const sps_prior* prior, int path, const float* theta, int64_t n,
                                      int unbounded, float* flux, const float* flux_bar, float* theta_bar, void* stream) {
-  REQUIRE(tc && theta && flux, "null table, theta or flux");
   REQUIRE(n >= 0, "negative n");
+  if (n == 0) return SPS_OK;
+  REQUIRE(tc && theta && flux, "null table, theta or flux");
   REQUIRE(path == SPS_PATH_EXACT || path == SPS_PATH_APPROX, "bad path");
   REQUIRE(!unbounded || prior, "unbounded parameters need a prior (bounds)");
   REQUIRE((flux_bar == nullptr) == (theta_bar == nullptr), "flux_bar and theta_bar must be given together");
@@ -131,9 +132,10 @@ extern "C" sps_status sps_photometry(const sps_table* tc, const sps_prior* prior
 extern "C" sps_status sps_loglike_grad(const sps_table* tc, const sps_prior* prior, int path, const float* theta_unb, int64_t n,
                                        const int32_t* gal_of_row, const float* obs_flux, const float* obs_sigma, float* logp,
                                        float* grad, void* stream) {
+  REQUIRE(n >= 0, "negative n");
+  if (n == 0) return SPS_OK;
   REQUIRE(tc && prior && theta_unb && obs_flux && obs_sigma, "null argument");
   REQUIRE(logp || grad, "nothing to compute");
-  REQUIRE(n >= 0, "negative n");
   REQUIRE(path == SPS_PATH_EXACT || path == SPS_PATH_APPROX, "bad path");
   if (n == 0) return SPS_OK;
   sps_table* t = const_cast<sps_table*>(tc);

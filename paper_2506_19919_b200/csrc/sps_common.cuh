@@ -20,6 +20,8 @@ struct TableDev {
   int n_wave_pad;                              // n_wave rounded up for the tensor-core tiles
   int cs_stride;                               // floats between consecutive ages in a c_SSP slice (n_Z*n_band padded)
   // age grid (R5): A[i] lower age edge of bin i in Gyr (A[0] = 0, A[n_age] = +huge)
+  const double* A_edge_d;   // [n_age+1] the same in double: t_obs - A is formed in double (old bins cancel)
+  const double* A_mid_d;    // [n_age]
   const float* A_edge;      // [n_age+1]
   const float* A_mid;       // [n_age]   (A[i]+A[i+1])/2   (last: unused)
   const float* A_half;      // [n_age]   (A[i+1]-A[i])/2   (last: +huge)
@@ -34,11 +36,13 @@ struct TableDev {
   const float* ssp;         // [K][n_wave_pad] fp32
   // filters
   float filt_mu[SPS_MAX_BAND], filt_sigma[SPS_MAX_BAND], lam_eff[SPS_MAX_BAND];
-  // c_SSP lookup table (Eq. 7): [n_z][n_age][cs_stride], entry (j*n_band + b) inside a row
+  // c_SSP lookup table (Eq. 7): [n_z][2][n_age][cs_stride]: per z slice the values c_t and the increments
+  // c_{t+1} - c_t; entry (j*n_band + b) inside a row
   const float* cssp;
   float z_min, dz, inv_dz;
   // cosmology (R11): t = t_pref * asinh(t_arg * (1+z)^-1.5)  [Gyr];  H0 in 1/Gyr
   float t_pref, t_arg, H0_gyr, Om, OL;
+  double t_pref_d, t_arg_d;
   float log10_mass_unit;
 };
 

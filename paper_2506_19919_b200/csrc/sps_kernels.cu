@@ -9,7 +9,8 @@
 // ---------------------------------------------------------------------------------------------
 struct RowFwd {
   float th[SPS_NDIM], dth[SPS_NDIM];
-  float t_obs, dt_dz, Msum, Mf;
+  double t_obs_d, z_d;
+  float dt_dz, Msum, Mf;
   AgeQuad Q;
   BurstQuad Bq;
   float m, dm_lz, dm_s;
@@ -18,9 +19,9 @@ struct RowFwd {
 template <bool WANT_GRAD>
 __device__ __forceinline__ void row_forward(const TableDev& T, const PriorDev& P, const float* __restrict__ row,
                                             bool unbounded, RowFwd& R) {
-  load_params(row, unbounded, P, R.th, R.dth);
-  cosmic_time(T, R.th[12], R.t_obs, R.dt_dz);
-  smooth_bins<WANT_GRAD>(T, R.t_obs, R.th[1], R.th[2], R.th[3], R.Q);
+  load_params(row, unbounded, P, R.th, R.dth, R.z_d);
+  cosmic_time(T, R.z_d, R.t_obs_d, R.dt_dz);
+  smooth_bins<WANT_GRAD>(T, R.t_obs_d, R.th[1], R.th[2], R.th[3], R.Q);
   float s = 0.f;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) s += R.Q.dM[q];
@@ -64,10 +65,10 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 // a7 + a9 + a10: approximate photometry (Eq. 6) fused with the Gaussian likelihood
 // and the reverse pass over the c_SSP table.  v0: one warp per row, the two z-slices are read from
 // L2; lane l owns the entries e = 4l..4l+3 of a slice row (e = j*n_band + b).
-//   pass 1:  Q^(s)_e = sum_i a_i c^(s)[i][e]            (s = lower/upper z slice)
-//   S^(s)_b = sum_j m_j Q^(s)_{jb};  flux_b = F_att,b Mn [(1-f) S^(0)_b + f S^(1)_b]
+//   pass 1:  Q^(s)_e = sum_i a_i c^(s)[i][e]            (s = 0: c_t, s = 1: D_t = c_{t+1} - c_t)
+//   S^(s)_b = sum_j m_j Q^(s)_{jb};  flux_b = F_att,b Mn [S^(0)_b + f S^(1)_b]
 //   g_b = d logL / d flux_b = -(flux_b - d_b)/sigma_b^2   (or the caller's flux_bar)
-//   pass 2:  a_bar_i = sum_e [v^(0)_e c^(0)[i][e] + v^(1)_e c^(1)[i][e]],  v^(s)_e = g_b F_b Mn {1-f, f} m_j
+//   pass 2:  a_bar_i = sum_e [v^(0)_e c^(0)[i][e] + v^(1)_e c^(1)[i][e]],  v^(s)_e = g_b F_b Mn {1, f} m_j
 // ---------------------------------------------------------------------------------------------
 struct ApproxSmem {
   float a[ROW_A_STRIDE];
@@ -91,7 +92,7 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, cons
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) S.a[l + 32 * q] = B.a[row * ROW_A_STRIDE + l + 32 * q];
   if (l < ROW_M_STRIDE) S.m[l] = B.m[row * ROW_M_STRIDE + l];
   __syncwarp();
-  const float* c0p = T.cssp + ((int64_t)sc.zbin * T.n_age) * T.cs_stride + 4 * l;
+  const float* c0p = T.cssp + ((int64_t)sc.zbin * 2 * T.n_age) * T.cs_stride + 4 * l;     // c_t, then D_t
   const float* c1p = c0p + (int64_t)T.n_age * T.cs_stride;
   const bool act = 4 * l < T.cs_stride;
   float4 q0 = make_float4(0, 0, 0, 0), q1 = make_float4(0, 0, 0, 0);
@@ -117,7 +118,7 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, cons
     for (int j = 0; j < T.n_Z; ++j) { S0 += S.m[j] * S.Q0[j * T.n_band + l]; S1 += S.m[j] * S.Q1[j * T.n_band + l]; }
     lam_r = T.lam_eff[l] / (1.f + sc.z);
     dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
-    const float Sint = (1.f - f) * S0 + f * S1;
+    const float Sint = S0 + f * S1;
     flux = F * sc.Mn * Sint;
     B.flux[row * SPS_MAX_BAND + l] = flux;
     if (flux_bar) g = flux_bar[row * T.n_band + l];
@@ -135,9 +136,9 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, cons
     return;
   }
   {
-    const float Sint = (1.f - f) * S0 + f * S1;
+    const float Sint = S0 + f * S1;
     float Mn_bar = warp_sum(isb ? g * F * Sint : 0.f);
-    float z_bar = warp_sum(isb ? g * (F * sc.Mn * (S1 - S0) * T.inv_dz + sc.Mn * Sint * F_lam * (-lam_r / (1.f + sc.z))) : 0.f);
+    float z_bar = warp_sum(isb ? g * (F * sc.Mn * S1 * T.inv_dz + sc.Mn * Sint * F_lam * (-lam_r / (1.f + sc.z))) : 0.f);
     float av_bar = warp_sum(isb ? g * sc.Mn * Sint * F_av : 0.f);
     float del_bar = warp_sum(isb ? g * sc.Mn * Sint * F_del : 0.f);
     float fl_bar = warp_sum(isb ? g * sc.Mn * Sint * F_fl : 0.f);
@@ -153,7 +154,7 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, cons
   if (l < ROW_M_STRIDE) {
     float mb = 0.f;
     if (l < T.n_Z)
-      for (int b = 0; b < T.n_band; ++b) mb += S.sbar[b] * ((1.f - f) * S.Q0[l * T.n_band + b] + f * S.Q1[l * T.n_band + b]);
+      for (int b = 0; b < T.n_band; ++b) mb += S.sbar[b] * (S.Q0[l * T.n_band + b] + f * S.Q1[l * T.n_band + b]);
     B.m_bar[row * ROW_M_STRIDE + l] = mb;
   }
   // v quads
@@ -163,7 +164,7 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, cons
     const int e = 4 * l + k;
     float v = 0.f;
     if (e < E) { const int j = e / T.n_band, b = e - j * T.n_band; v = S.sbar[b] * S.m[j]; }
-    v0[k] = (1.f - f) * v; v1[k] = f * v;
+    v0[k] = v; v1[k] = f * v;
   }
   // pass 2
   float abar[SPS_AGE_PER_LANE] = {0.f, 0.f, 0.f, 0.f};

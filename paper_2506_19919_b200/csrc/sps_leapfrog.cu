@@ -1,0 +1,101 @@
+// sps_leapfrog.cu -- sps_leapfrog (trajectory diagnostic) and the per-run problem
+// description shared by the samplers.
+#include <vector>
+#include "sps_sampler.cuh"
+
+__global__ void gal_of_chain_kernel(int* out, int64_t n, int n_chain) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = (int)(i / n_chain);
+}
+
+sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
+                             const float* obs_flux, const float* obs_sigma) {
+  memset(&Q, 0, sizeof(Q));
+  Q.n = n_gal * cfg->n_chain; Q.obs_flux = obs_flux; Q.obs_sigma = obs_sigma;
+  sps_status st = sps_check_cuda(cudaMalloc(&Q.gal_of_chain, Q.n * sizeof(int)), "gal_of_chain allocation");
+  if (st != SPS_OK) return st;
+  gal_of_chain_kernel<<<(unsigned)((Q.n + 255) / 256), 256>>>(Q.gal_of_chain, Q.n, cfg->n_chain); sps_count_launch();
+  if (!path_of_gal_dev) {
+    if (cfg->path != SPS_PATH_EXACT && cfg->path != SPS_PATH_APPROX) { sps_set_error("bad path"); return SPS_EINVAL; }
+    Q.n_rows_path[cfg->path] = Q.n;
+    return SPS_OK;
+  }
+  std::vector<int32_t> pg(n_gal);
+  st = sps_check_cuda(cudaMemcpy(pg.data(), path_of_gal_dev, n_gal * sizeof(int32_t), cudaMemcpyDeviceToHost), "path_of_gal D2H");
+  if (st != SPS_OK) return st;
+  std::vector<int> rows[2];
+  for (int64_t g = 0; g < n_gal; ++g) {
+    if (pg[g] != 0 && pg[g] != 1) { sps_set_error("path_of_gal[%lld] = %d is not 0/1", (long long)g, pg[g]); return SPS_EINVAL; }
+    for (int k = 0; k < cfg->n_chain; ++k) rows[pg[g]].push_back((int)(g * cfg->n_chain + k));
+  }
+  for (int p = 0; p < 2; ++p) {
+    Q.n_rows_path[p] = (int64_t)rows[p].size();
+    if (rows[p].empty()) continue;
+    st = sps_check_cuda(cudaMalloc(&Q.rows_path[p], rows[p].size() * sizeof(int)), "row list allocation");
+    if (st != SPS_OK) return st;
+    cudaMemcpy(Q.rows_path[p], rows[p].data(), rows[p].size() * sizeof(int), cudaMemcpyHostToDevice);
+  }
+  return SPS_OK;
+}
+
+void hmc_problem_free(HmcProblem& Q) {
+  if (Q.gal_of_chain) cudaFree(Q.gal_of_chain);
+  for (int p = 0; p < 2; ++p) if (Q.rows_path[p]) cudaFree(Q.rows_path[p]);
+  memset(&Q, 0, sizeof(Q));
+}
+
+// first half kick + drift from (theta0, p0) with the gradient at theta0
+__global__ void lf_first_kernel(int64_t n, const float* __restrict__ theta0, const float* __restrict__ p0, const float* __restrict__ grad0,
+                                const float* __restrict__ eps, const float* __restrict__ inv_mass, float* theta_w, float* p_w) {
+  const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= n * SPS_NDIM) return;
+  const float e = eps[o / SPS_NDIM];
+  const float p = p0[o] + 0.5f * e * grad0[o];
+  p_w[o] = p;
+  theta_w[o] = theta0[o] + e * inv_mass[o] * p;
+}
+// finish step k (half kick), record, and start step k+1 (half kick + drift)
+__global__ void lf_record_kernel(int64_t n, int step, const float* __restrict__ grad_w, const float* __restrict__ logp_w,
+                                 const float* __restrict__ eps, const float* __restrict__ inv_mass, float* theta_w, float* p_w,
+                                 float* __restrict__ traj, float* __restrict__ logp_traj) {
+  const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= n * SPS_NDIM) return;
+  const int64_t r = o / SPS_NDIM; const int d = (int)(o % SPS_NDIM);
+  const float e = eps[r];
+  float p = p_w[o] + 0.5f * e * grad_w[o];
+  const float th = theta_w[o];
+  traj[(((int64_t)step * n + r) * 2 + 0) * SPS_NDIM + d] = th;
+  traj[(((int64_t)step * n + r) * 2 + 1) * SPS_NDIM + d] = p;
+  if (d == 0) logp_traj[(int64_t)step * n + r] = logp_w[r];
+  p += 0.5f * e * grad_w[o];
+  p_w[o] = p;
+  theta_w[o] = th + e * inv_mass[o] * p;
+}
+
+extern "C" sps_status sps_leapfrog(const sps_table* tc, const sps_prior* prior, int path, const float* theta0, const float* p0,
+                                   const float* eps, const float* inv_mass, int64_t n, const int32_t* gal_of_row,
+                                   const float* obs_flux, const float* obs_sigma, int32_t n_steps, float* traj, float* logp_traj,
+                                   void* stream) {
+  if (!tc || !prior || !theta0 || !p0 || !eps || !inv_mass || !obs_flux || !obs_sigma || !traj || !logp_traj) {
+    sps_set_error("sps_leapfrog: null argument"); return SPS_EINVAL; }
+  if (n < 0 || n_steps < 0 || (path != SPS_PATH_EXACT && path != SPS_PATH_APPROX)) { sps_set_error("sps_leapfrog: bad argument"); return SPS_EINVAL; }
+  if (n == 0 || n_steps == 0) return SPS_OK;
+  sps_table* t = const_cast<sps_table*>(tc);
+  cudaStream_t s = (cudaStream_t)stream;
+  PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
+  st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
+  float* w = nullptr;
+  const size_t nv = (size_t)n * SPS_NDIM;
+  st = sps_check_cuda(cudaMalloc(&w, (3 * nv + n) * sizeof(float)), "sps_leapfrog scratch"); if (st != SPS_OK) return st;
+  float *theta_w = w, *p_w = w + nv, *grad_w = w + 2 * nv, *logp_w = w + 3 * nv;
+  const unsigned eb = (unsigned)((nv + 255) / 256);
+  st = sps_eval(t, P, path, theta0, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
+  if (st == SPS_OK) { lf_first_kernel<<<eb, 256, 0, s>>>(n, theta0, p0, grad_w, eps, inv_mass, theta_w, p_w); sps_count_launch(); }
+  for (int k = 0; k < n_steps && st == SPS_OK; ++k) {
+    st = sps_eval(t, P, path, theta_w, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
+    if (st == SPS_OK) { lf_record_kernel<<<eb, 256, 0, s>>>(n, k, grad_w, logp_w, eps, inv_mass, theta_w, p_w, traj, logp_traj); sps_count_launch(); }
+  }
+  cudaStreamSynchronize(s);
+  cudaFree(w);
+  return st == SPS_OK ? sps_check_cuda(cudaGetLastError(), "sps_leapfrog") : st;
+}

@@ -10,19 +10,27 @@
 
 // ---- a0: Eq. (C1) PAPER.md:429 -----------------------------------------------------------------
 // Every lane returns all 13 bounded parameters (th) and d theta / d theta~ (dth).
+// The redshift (lane 12) is also returned in double: t_obs(z) - age cancels for the oldest bins.
 __device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PriorDev& pr,
-                                            float th[SPS_NDIM], float dth[SPS_NDIM]) {
+                                            float th[SPS_NDIM], float dth[SPS_NDIM], double& z_d) {
   const int l = lane_id();
   float v = 0.f, d = 1.f;
+  double vd = 0.0;
   if (l < SPS_NDIM) {
     v = row[l];
+    vd = (double)v;
     if (unbounded) {
       float s = 1.f / (1.f + expf(-pr.k[l] * (v - pr.x0[l])));
       float w = pr.y_hi[l] - pr.y_lo[l];
+      if (l == SPS_NDIM - 1) {
+        const double sd = 1.0 / (1.0 + exp(-(double)pr.k[l] * ((double)v - (double)pr.x0[l])));
+        vd = (double)pr.y_lo[l] + ((double)pr.y_hi[l] - (double)pr.y_lo[l]) * sd;
+      }
       v = pr.y_lo[l] + w * s;
       d = w * pr.k[l] * s * (1.f - s);
     }
   }
+  z_d = __shfl_sync(FULL_MASK, vd, SPS_NDIM - 1);
 #pragma unroll
   for (int p = 0; p < SPS_NDIM; ++p) {
     th[p] = __shfl_sync(FULL_MASK, v, p);
@@ -31,9 +39,10 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
 }
 
 // ---- a1: age of the universe (R11), Gyr, and dt/dz ------------------------------------------------
-__device__ __forceinline__ void cosmic_time(const TableDev& T, float z, float& t, float& dt_dz) {
-  float zp = 1.f + z, zp3 = zp * zp * zp;
-  t = T.t_pref * asinhf(T.t_arg * rsqrtf(zp3));
+__device__ __forceinline__ void cosmic_time(const TableDev& T, double z_d, double& t_d, float& dt_dz) {
+  const double zpd = 1.0 + z_d;
+  t_d = T.t_pref_d * asinh(T.t_arg_d * rsqrt(zpd * zpd * zpd));
+  const float zp = (float)zpd, zp3 = zp * zp * zp;
   dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp3 + T.OL));
 }
 
@@ -76,7 +85,7 @@ __device__ __constant__ float GL8_W[8] = {0.1012285362903763f, 0.222381034453374
 //  * the few old bins near age ~ t_obs (and the one that reaches t = 0) are integrated by the whole
 //    warp: 8-point Gauss-Legendre panels in v = ln t, cut at ln t_hi - 16/(beta+1).
 template <bool WANT_GRAD>
-__device__ __forceinline__ void smooth_bins(const TableDev& T, float t_obs, float tau, float alpha, float beta, AgeQuad& Q) {
+__device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, float tau, float alpha, float beta, AgeQuad& Q) {
   const int l = lane_id();
   const float l2tau = log2f(tau);
   const float ab = alpha + beta;
@@ -89,12 +98,14 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, float t_obs, floa
     float t_hi = 0.f, t_lo = 0.f, half = 0.f, t_mid = 1.f;
     int kind = 0;                       // 0 empty, 1 GL2, 2 GL4, 3 warp-cooperative
     if (i < T.n_age) {
-      t_hi = t_obs - T.A_edge[i];
-      t_lo = fmaxf(t_obs - T.A_edge[i + 1], 0.f);
+      t_hi = (float)(t_obs_d - T.A_edge_d[i]);
+      t_lo = fmaxf((float)(t_obs_d - T.A_edge_d[i + 1]), 0.f);
       half = T.A_half[i];
-      t_mid = t_obs - T.A_mid[i];
+      t_mid = (float)(t_obs_d - T.A_mid_d[i]);
       if (t_hi > 0.f) {
-        float s = (t_lo > 0.f) ? (half / t_mid) * ab * 0.3183098861837907f : 1e9f;   // half-width / pole distance
+        // half-width over the distance to the nearest singularity: the turnover poles at Im ln t = pi/(alpha+beta)
+        // and the branch point of t^beta at t = 0
+        float s = (t_lo > 0.f) ? (half / t_mid) * fmaxf(ab * 0.3183098861837907f, 1.f) : 1e9f;
         kind = (s < 0.06f) ? 1 : (s < 0.36f ? 2 : 3);
       } else t_hi = 0.f;
     }

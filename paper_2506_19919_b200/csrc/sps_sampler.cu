@@ -1,13 +1,16 @@
-// sps_sampler.cu -- counter-based RNG, leapfrog, HMC / NUTS engine.  [RNG only for now]
-#include "sps_internal.h"
-#include "sps_philox.cuh"
+// sps_sampler.cu -- counter-based RNG, leapfrog, fixed-length HMC with windowed warmup (a11, a12).
+// One warp owns one chain (lane p < 13 owns parameter p); the model evaluation between the
+// sampler kernels is the batch-wide prologue / contraction / epilogue pipeline (sps_eval).
+// NUTS lives in sps_nuts.cu and reuses the state and helpers declared in sps_sampler.cuh.
+#include <vector>
+#include "sps_sampler.cuh"
 
+// ---------------------------------------------------------------------------------------------
 __global__ void philox_words_kernel(uint32_t k0, uint32_t k1, uint32_t first_chain, uint32_t transition, uint32_t purpose,
                                     uint32_t index, int64_t n, uint32_t* out) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  uint4 w = philox4x32_10(make_uint4(first_chain + (uint32_t)i, transition, purpose, index), make_uint2(k0, k1));
-  reinterpret_cast<uint4*>(out)[i] = w;
+  reinterpret_cast<uint4*>(out)[i] = philox4x32_10(make_uint4(first_chain + (uint32_t)i, transition, purpose, index), make_uint2(k0, k1));
 }
 
 extern "C" sps_status sps_philox_words(uint64_t seed, uint32_t first_chain, uint32_t transition, uint32_t purpose,
@@ -19,4 +22,238 @@ extern "C" sps_status sps_philox_words(uint64_t seed, uint32_t first_chain, uint
                                                                                  transition, purpose, index, n, out);
   sps_count_launch();
   return sps_check_cuda(cudaGetLastError(), "philox launch");
+}
+
+// ---------------------------------------------------------------------------------------------
+// chain initialisation (R17): theta~_0 = xi + 0.1 omega N(0,1) from (chain, transition 0, purpose 5)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) chain_init_kernel(ChainState C, PriorDev P, const float* __restrict__ theta0, float eps0, uint2 key) {
+  CHAIN_WARP_PROLOGUE(C.n);
+  if (l < SPS_NDIM) {
+    float v;
+    if (theta0) v = theta0[c * SPS_NDIM + l];
+    else v = P.xi[l] + 0.1f * P.omega[l] * chain_normal(key, (uint32_t)c, 0u, RNG_INIT, l);
+    C.theta[c * SPS_NDIM + l] = v;
+    C.inv_mass[c * SPS_NDIM + l] = 1.f;
+    C.w_mean[c * SPS_NDIM + l] = 0.f; C.w_m2[c * SPS_NDIM + l] = 0.f;
+    C.s_mean[c * SPS_NDIM + l] = 0.f; C.s_m2[c * SPS_NDIM + l] = 0.f;
+  }
+  if (l == 0) {
+    C.eps[c] = eps0; C.da_mu[c] = logf(10.f * eps0); C.da_hbar[c] = 0.f; C.da_logepsbar[c] = 0.f; C.da_m[c] = 0;
+    C.acc_sum[c] = 0.f; C.n_leapfrog[c] = 0; C.n_div[c] = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// HMC transition (R-step 13).  Draw order: 13 normals (purpose 0), one uniform (purpose 1).
+// begin: p = N / sqrt(invM); H0 = -logP + 1/2 sum invM p^2; first half kick and drift.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, uint32_t transition, uint2 key) {
+  CHAIN_WARP_PROLOGUE(C.n);
+  float kin = 0.f;
+  if (l < SPS_NDIM) {
+    const int64_t o = c * SPS_NDIM + l;
+    const float v = C.inv_mass[o], eps = C.eps[c];
+    float p = chain_normal(key, (uint32_t)c, transition, RNG_MOMENTUM, l) * rsqrtf(v);
+    kin = 0.5f * v * p * p;
+    p += 0.5f * eps * C.grad[o];
+    C.p_w[o] = p;
+    C.theta_w[o] = C.theta[o] + eps * v * p;
+  }
+  kin = warp_sum(kin);
+  if (l == 0) C.H0[c] = -C.logp[c] + kin;
+}
+
+// between two gradient evaluations: p += eps * grad ; theta += eps * invM * p   (two half kicks merged)
+__global__ void __launch_bounds__(256) leapfrog_mid_kernel(ChainState C) {
+  const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= C.n * SPS_NDIM) return;
+  const int64_t c = o / SPS_NDIM;
+  const float eps = C.eps[c];
+  const float p = C.p_w[o] + eps * C.grad_w[o];
+  C.p_w[o] = p;
+  C.theta_w[o] += eps * C.inv_mass[o] * p;
+}
+
+// end: last half kick, Metropolis test, warmup adaptation (R14), running summaries.
+__global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, uint32_t transition, uint2 key, int n_leapfrog, AdaptFlags A,
+                                                      float* __restrict__ samples, int sample_index, int n_sample) {
+  CHAIN_WARP_PROLOGUE(C.n);
+  const int64_t o = c * SPS_NDIM + (l < SPS_NDIM ? l : 0);
+  const bool act = l < SPS_NDIM;
+  const float v = C.inv_mass[o], eps = C.eps[c];
+  const float gw = C.grad_w[o], thw = C.theta_w[o];
+  const float p = C.p_w[o] + 0.5f * eps * gw;
+  const float kin = warp_sum(act ? 0.5f * v * p * p : 0.f);
+  const float lpw = C.logp_w[c];
+  const float dH = (-lpw + kin) - C.H0[c];
+  const bool fin = __all_sync(FULL_MASK, !act || (isfinite(gw) && isfinite(thw))) && isfinite(dH);
+  const float acc_prob = fin ? fminf(1.f, expf(fminf(0.f, -dH))) : 0.f;
+  const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, transition, RNG_ACCEPT, 0u), key).x);
+  const bool accept = fin && (u < acc_prob);
+  float th = C.theta[o];
+  if (accept) {
+    th = thw;
+    if (act) { C.theta[o] = thw; C.grad[o] = gw; }
+    if (l == 0) C.logp[c] = lpw;
+  }
+  chain_adapt_and_record(C, c, l, act, o, th, acc_prob, n_leapfrog, 0, A, samples, sample_index, n_sample);
+}
+
+// ---------------------------------------------------------------------------------------------
+// finalisation: mean / sd per chain, Gelman-Rubin R-hat per galaxy
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain, int n_sample, sps_hmc_summary S) {
+  const int64_t gidx = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int l = threadIdx.x & 31;
+  const int64_t n_gal = C.n / n_chain;
+  if (gidx >= n_gal || l >= SPS_NDIM) return;
+  float mean_of_means = 0.f, W = 0.f;
+  for (int k = 0; k < n_chain; ++k) {
+    const int64_t c = gidx * n_chain + k, o = c * SPS_NDIM + l;
+    const float mu = C.s_mean[o], var = n_sample > 1 ? C.s_m2[o] / (float)(n_sample - 1) : 0.f;
+    if (S.mean) S.mean[o] = mu;
+    if (S.sd) S.sd[o] = sqrtf(var);
+    if (S.inv_mass) S.inv_mass[o] = C.inv_mass[o];
+    if (l == 0) {
+      if (S.accept) S.accept[c] = C.acc_sum[c] / (float)max(n_sample, 1);
+      if (S.eps) S.eps[c] = C.eps[c];
+      if (S.n_leapfrog) S.n_leapfrog[c] = C.n_leapfrog[c];
+      if (S.divergences) S.divergences[c] = C.n_div[c];
+    }
+    mean_of_means += mu; W += var;
+  }
+  mean_of_means /= n_chain; W /= n_chain;
+  float Bn = 0.f;                                   // B/n: variance of the chain means
+  for (int k = 0; k < n_chain; ++k) { const float d = C.s_mean[(gidx * n_chain + k) * SPS_NDIM + l] - mean_of_means; Bn += d * d; }
+  Bn = n_chain > 1 ? Bn / (float)(n_chain - 1) : 0.f;
+  if (S.rhat) {
+    const float ns = (float)n_sample;
+    S.rhat[gidx * SPS_NDIM + l] = (W > 0.f && n_chain > 1) ? sqrtf(((ns - 1.f) / ns * W + Bn) / W) : 1.f;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+sps_status chain_state_alloc(ChainState& C, int64_t n, int ckpt_vectors) {
+  memset(&C, 0, sizeof(C));
+  C.n = n;
+  const size_t nv = 11 + (size_t)ckpt_vectors;      // vectors of 13 floats per chain
+  const size_t ns = 16;                             // scalars per chain
+  const size_t bytes = n * (nv * SPS_NDIM + ns) * sizeof(float);
+  float* base = nullptr;
+  sps_status st = sps_check_cuda(cudaMalloc(&base, bytes), "chain state allocation");
+  if (st != SPS_OK) return st;
+  cudaMemset(base, 0, bytes);
+  C.base = base;
+  float* p = base;
+  auto vec = [&]() { float* r = p; p += n * SPS_NDIM; return r; };
+  auto sca = [&]() { float* r = p; p += n; return r; };
+  C.theta = vec(); C.grad = vec(); C.theta_w = vec(); C.p_w = vec(); C.grad_w = vec(); C.inv_mass = vec();
+  C.w_mean = vec(); C.w_m2 = vec(); C.s_mean = vec(); C.s_m2 = vec(); C.extra = vec();
+  C.nuts = p; p += n * (size_t)ckpt_vectors * SPS_NDIM;
+  C.logp = sca(); C.logp_w = sca(); C.H0 = sca(); C.eps = sca(); C.da_mu = sca(); C.da_hbar = sca(); C.da_logepsbar = sca();
+  C.acc_sum = sca();
+  C.da_m = (int*)sca(); C.n_leapfrog = (int*)sca(); C.n_div = (int*)sca();
+  C.nuts_sc = sca();   // 5 scalars left for NUTS
+  return SPS_OK;
+}
+void chain_state_free(ChainState& C) { if (C.base) cudaFree(C.base); C.base = nullptr; }
+
+// R14 windows (restated): <20 warmup steps: step size only.  >=150: 75 | 25,50,100,... | 50; else 15% | one window | 10%.
+void warmup_schedule(int W, std::vector<int>& ends, int& slow_lo, int& slow_hi) {
+  ends.clear();
+  if (W < 20) { slow_lo = slow_hi = W; return; }
+  int init, term, base;
+  if (W >= 150) { init = 75; term = 50; base = 25; }
+  else { init = (int)(0.15 * W); term = (int)(0.1 * W); base = W - init - term; }
+  int start = init, size = base; const int stop = W - term;
+  while (start < stop) {
+    int end = start + size;
+    if (end + 2 * size > stop) end = stop;
+    ends.push_back(end);
+    start = end; size *= 2;
+  }
+  slow_lo = init; slow_hi = stop;
+}
+
+AdaptFlags adapt_flags_for(int it, int n_warmup, const std::vector<int>& ends, int slow_lo, int slow_hi, float target) {
+  AdaptFlags A; A.warmup = it < n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == n_warmup); A.welford_n = 0;
+  A.target = target;
+  if (A.warmup && it >= slow_lo && it < slow_hi) {
+    A.in_window = 1;
+    int start = slow_lo;
+    for (int e : ends) { if (it < e) { A.welford_n = it - start + 1; A.window_end = (it + 1 == e); break; } start = e; }
+  }
+  return A;
+}
+
+static inline unsigned chain_blocks(int64_t n) { return (unsigned)((n * 32 + 255) / 256); }
+
+static sps_status eval_working(sps_table* t, const PriorDev& P, const HmcProblem& Q, ChainState& C, cudaStream_t s) {
+  // groups of rows per path: path_rows[0] exact, [1] approx (index lists) or all rows on one path
+  sps_status st = SPS_OK;
+  for (int path = 0; path < 2 && st == SPS_OK; ++path) {
+    if (Q.n_rows_path[path] == 0) continue;
+    st = sps_eval(t, P, path, C.theta_w, Q.n_rows_path[path], true, true, Q.rows_path[path], Q.gal_of_chain, Q.obs_flux,
+                  Q.obs_sigma, nullptr, true, C.logp_w, C.grad_w, s);
+  }
+  return st;
+}
+
+sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
+                             const float* obs_flux, const float* obs_sigma);
+void hmc_problem_free(HmcProblem& Q);
+sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples, cudaStream_t s);
+
+extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, const sps_hmc_config* cfg, const float* obs_flux,
+                                  const float* obs_sigma, int64_t n_gal, const int32_t* path_of_gal, const float* theta0,
+                                  float* samples, const sps_hmc_summary* summary, void* stream) {
+  if (!tc || !prior || !cfg || !obs_flux || !obs_sigma) { sps_set_error("sps_hmc_run: null argument"); return SPS_EINVAL; }
+  if (n_gal < 0 || cfg->n_chain < 1 || cfg->n_warmup < 0 || cfg->n_sample < 0 || !(cfg->eps0 > 0)) { sps_set_error("sps_hmc_run: bad config"); return SPS_EINVAL; }
+  if (cfg->sampler == SPS_SAMPLER_HMC && cfg->n_leapfrog < 1) { sps_set_error("sps_hmc_run: n_leapfrog < 1"); return SPS_EINVAL; }
+  if (cfg->sampler == SPS_SAMPLER_NUTS && (cfg->max_depth < 1 || cfg->max_depth > 10)) { sps_set_error("sps_hmc_run: max_depth must be 1..10"); return SPS_EINVAL; }
+  if (cfg->sampler != SPS_SAMPLER_HMC && cfg->sampler != SPS_SAMPLER_NUTS) { sps_set_error("sps_hmc_run: bad sampler"); return SPS_EINVAL; }
+  if (n_gal == 0) return SPS_OK;
+  sps_table* t = const_cast<sps_table*>(tc);
+  cudaStream_t s = (cudaStream_t)stream;
+  PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
+  const int64_t n = n_gal * cfg->n_chain;
+  st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
+  HmcProblem Q; ChainState C;
+  st = hmc_problem_setup(Q, cfg, n_gal, path_of_gal, obs_flux, obs_sigma); if (st != SPS_OK) return st;
+  st = chain_state_alloc(C, n, cfg->sampler == SPS_SAMPLER_NUTS ? NUTS_VECTORS : 0);
+  if (st != SPS_OK) { hmc_problem_free(Q); return st; }
+  const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
+  chain_init_kernel<<<chain_blocks(n), 256, 0, s>>>(C, P, theta0, cfg->eps0, key); sps_count_launch();
+  // logp / grad at the start: evaluate through the working buffers
+  cudaMemcpyAsync(C.theta_w, C.theta, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
+  st = eval_working(t, P, Q, C, s);
+  cudaMemcpyAsync(C.grad, C.grad_w, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
+  cudaMemcpyAsync(C.logp, C.logp_w, n * sizeof(float), cudaMemcpyDeviceToDevice, s);
+  if (st == SPS_OK && cfg->sampler == SPS_SAMPLER_HMC) {
+    std::vector<int> ends; int slow_lo, slow_hi;
+    warmup_schedule(cfg->n_warmup, ends, slow_lo, slow_hi);
+    const unsigned eb = (unsigned)((n * SPS_NDIM + 255) / 256);
+    for (int it = 0; it < cfg->n_warmup + cfg->n_sample && st == SPS_OK; ++it) {
+      hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it, key); sps_count_launch();
+      for (int k = 0; k < cfg->n_leapfrog && st == SPS_OK; ++k) {
+        st = eval_working(t, P, Q, C, s);
+        if (k + 1 < cfg->n_leapfrog) { leapfrog_mid_kernel<<<eb, 256, 0, s>>>(C); sps_count_launch(); }
+      }
+      const AdaptFlags A = adapt_flags_for(it, cfg->n_warmup, ends, slow_lo, slow_hi, cfg->target_accept);
+      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it, key, cfg->n_leapfrog, A, samples, it - cfg->n_warmup, cfg->n_sample);
+      sps_count_launch();
+    }
+  } else if (st == SPS_OK) {
+    st = nuts_run(t, P, cfg, Q, C, samples, s);
+  }
+  if (st == SPS_OK && summary) {
+    finalize_kernel<<<chain_blocks(n_gal), 256, 0, s>>>(C, cfg->n_chain, cfg->n_sample, *summary); sps_count_launch();
+  }
+  if (st == SPS_OK) st = sps_check_cuda(cudaStreamSynchronize(s), "sps_hmc_run");
+  else cudaStreamSynchronize(s);
+  chain_state_free(C); hmc_problem_free(Q);
+  return st;
 }

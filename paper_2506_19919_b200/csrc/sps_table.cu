@@ -13,33 +13,46 @@ __device__ __forceinline__ float filter_T(float lam_obs, float mu, float sigma) 
   return (fabsf(x) <= 5.f) ? expf(-0.5f * x * x) : 0.f;
 }
 
-// c_SSP[t][i][j*n_band+b] = sum_k L_ij(lam_k) T_b(lam_k (1+z_t)) dlam_k.  One warp per (t, ij).
-__global__ void __launch_bounds__(256) cssp_build_kernel(TableDev T, float* __restrict__ cssp) {
+// c_SSP[t][i][j*n_band+b] = sum_k L_ij(lam_k) T_b(lam_k (1+z_t)) dlam_k  (Eq. 7).  One warp per (t, ij).
+// Slice t of the device table holds TWO arrays: c_t and the increment D_t = c_{t+1} - c_t (zero for the
+// last slice), so that the linear interpolation c_t + f D_t and its z-derivative D_t / dz
+// carry no fp32 cancellation.  Both are accumulated in double and rounded once.
+__device__ __forceinline__ double filter_T_d(double lam_obs, double mu, double sigma) {
+  const double x = (lam_obs - mu) / sigma;
+  return (fabs(x) <= 5.0) ? exp(-0.5 * x * x) : 0.0;
+}
+__global__ void __launch_bounds__(256) cssp_build_kernel(TableDev T, const double* __restrict__ wave_d, const double* __restrict__ dlam_d,
+                                                          double z_min_d, double dz_d, float* __restrict__ cssp) {
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (w >= (int64_t)T.n_z * T.K) return;
   const int t = (int)(w / T.K), ij = (int)(w % T.K);
   const int i = ij / T.n_Z, j = ij % T.n_Z;
   const int l = threadIdx.x & 31;
-  const float zp = 1.f + T.z_min + T.dz * (float)t;
   const float* L = T.ssp + (int64_t)ij * T.n_wave_pad;
+  const bool last = (t == T.n_z - 1);
+  const double zp0 = 1.0 + z_min_d + dz_d * (double)t, zp1 = last ? zp0 : 1.0 + z_min_d + dz_d * (double)(t + 1);
   for (int b = 0; b < T.n_band; ++b) {
-    const float mu = T.filt_mu[b], sg = T.filt_sigma[b];
-    const float lo = (mu - 5.f * sg) / zp, hi = (mu + 5.f * sg) / zp;
-    // first k with wave[k] >= lo (binary search; a slightly wide window is harmless: T = 0 outside)
+    const double mu = (double)T.filt_mu[b], sg = (double)T.filt_sigma[b];
+    const double lo = (mu - 5.0 * sg) / zp1, hi = (mu + 5.0 * sg) / zp0;      // union of the two supports
     int a = 0, c = T.n_wave;
-    while (a < c) { int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
-    int k0 = max(a - 1, 0);
+    while (a < c) { int mid = (a + c) >> 1; if (wave_d[mid] < lo) a = mid + 1; else c = mid; }
+    const int k0 = max(a - 1, 0);
     a = k0; c = T.n_wave;
-    while (a < c) { int mid = (a + c) >> 1; if (T.wave[mid] <= hi) a = mid + 1; else c = mid; }
+    while (a < c) { int mid = (a + c) >> 1; if (wave_d[mid] <= hi) a = mid + 1; else c = mid; }
     const int k1 = min(a + 1, T.n_wave);
-    float acc = 0.f, comp = 0.f;                   // Kahan: up to ~1500 terms
+    double acc0 = 0.0, acc1 = 0.0;
     for (int k = k0 + l; k < k1; k += 32) {
-      const float term = L[k] * filter_T(T.wave[k] * zp, mu, sg) * T.dlam[k];
-      const float y = term - comp, s = acc + y;
-      comp = (s - acc) - y; acc = s;
+      const double Lk = (double)L[k] * dlam_d[k];
+      acc0 += Lk * filter_T_d(wave_d[k] * zp0, mu, sg);
+      acc1 += Lk * filter_T_d(wave_d[k] * zp1, mu, sg);
     }
-    acc = warp_sum(acc);
-    if (l == 0) cssp[((int64_t)t * T.n_age + i) * T.cs_stride + j * T.n_band + b] = acc;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { acc0 += __shfl_xor_sync(FULL_MASK, acc0, o); acc1 += __shfl_xor_sync(FULL_MASK, acc1, o); }
+    if (l == 0) {
+      float* row = cssp + (((int64_t)t * 2) * T.n_age + i) * T.cs_stride + j * T.n_band + b;
+      row[0] = (float)acc0;
+      row[(int64_t)T.n_age * T.cs_stride] = (float)(acc1 - acc0);
+    }
   }
 }
 
@@ -123,24 +136,36 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   }
   T.z_min = (float)d->z_min; T.dz = (float)((d->z_max - d->z_min) / (d->n_z - 1)); T.inv_dz = (float)((d->n_z - 1) / (d->z_max - d->z_min));
   const double OL = 1.0 - d->Om, inv_H0 = 977.7922216807891 / d->H0;
-  T.t_pref = (float)(2.0 * inv_H0 / (3.0 * sqrt(OL))); T.t_arg = (float)sqrt(OL / d->Om);
+  T.t_pref_d = 2.0 * inv_H0 / (3.0 * sqrt(OL)); T.t_arg_d = sqrt(OL / d->Om);
+  T.t_pref = (float)T.t_pref_d; T.t_arg = (float)T.t_arg_d;
   T.H0_gyr = (float)(1.0 / inv_H0); T.Om = (float)d->Om; T.OL = (float)OL;
   T.log10_mass_unit = (float)d->log10_mass_unit;
 
+  std::vector<double> Amid_d(na);
+  for (int i = 0; i < na; ++i) Amid_d[i] = 0.5 * (Ae[i] + Ae[i + 1]);
+  T.A_edge_d = upload(Ae, st); T.A_mid_d = upload(Amid_d, st);
   T.A_edge = upload(A_edge, st); T.A_mid = upload(A_mid, st); T.A_half = upload(A_half, st); T.e_edge = upload(e_edge, st);
   T.g_mid = upload(g_mid, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
   T.drude = upload(dr, st); T.l2r = upload(l2r, st); T.ssp = upload(ssp, st);
   float* cssp = nullptr;
-  const size_t cs_n = (size_t)T.n_z * T.n_age * T.cs_stride;
+  const size_t cs_n = (size_t)T.n_z * 2 * T.n_age * T.cs_stride;
+  std::vector<double> wave_h(d->wave_A, d->wave_A + nw), dlam_h(nw);
+  for (int k = 0; k < nw; ++k) {
+    const double lo = d->wave_A[k > 0 ? k - 1 : 0], hi = d->wave_A[k < nw - 1 ? k + 1 : nw - 1];
+    dlam_h[k] = 0.5 * (hi - lo);
+  }
+  double* wave_dd = upload(wave_h, st); double* dlam_dd = upload(dlam_h, st);
   if (st == SPS_OK && cudaMalloc(&cssp, cs_n * sizeof(float)) != cudaSuccess) { st = SPS_ENOMEM; sps_set_error("cudaMalloc c_SSP failed"); }
   if (st == SPS_OK) {
     cudaMemset(cssp, 0, cs_n * sizeof(float));
     T.cssp = cssp;
     const int64_t warps = (int64_t)T.n_z * T.K;
-    cssp_build_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256>>>(T, cssp);
+    cssp_build_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256>>>(T, wave_dd, dlam_dd, d->z_min, (d->z_max - d->z_min) / (d->n_z - 1), cssp);
     sps_count_launch();
     st = sps_check_cuda(cudaDeviceSynchronize(), "c_SSP build");
   }
+  if (wave_dd) cudaFree(wave_dd);
+  if (dlam_dd) cudaFree(dlam_dd);
   if (st == SPS_OK) st = sps_exact_setup(t);
   if (st != SPS_OK) { sps_destroy_table(t); return st; }
   *out = t;
@@ -150,7 +175,7 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
 extern "C" sps_status sps_destroy_table(sps_table* t) {
   if (!t) return SPS_OK;
   TableDev& T = t->dev;
-  const void* ptrs[] = {T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
+  const void* ptrs[] = {T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
   for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
   sps_exact_teardown(t);
   sps_free_row_buffers(t);
@@ -162,9 +187,11 @@ extern "C" sps_status sps_table_cssp(const sps_table* t, float* host) {
   if (!t || !host) { sps_set_error("sps_table_cssp: null argument"); return SPS_EINVAL; }
   const TableDev& T = t->dev;
   const int E = T.n_Z * T.n_band;
-  std::vector<float> tmp((size_t)T.n_z * T.n_age * T.cs_stride);
+  std::vector<float> tmp((size_t)T.n_z * 2 * T.n_age * T.cs_stride);
   sps_status st = sps_check_cuda(cudaMemcpy(tmp.data(), T.cssp, tmp.size() * sizeof(float), cudaMemcpyDeviceToHost), "c_SSP D2H");
   if (st != SPS_OK) return st;
-  for (int64_t r = 0; r < (int64_t)T.n_z * T.n_age; ++r) memcpy(host + r * E, &tmp[r * T.cs_stride], sizeof(float) * E);
+  for (int64_t t2 = 0; t2 < T.n_z; ++t2)
+    for (int64_t i = 0; i < T.n_age; ++i)
+      memcpy(host + (t2 * T.n_age + i) * E, &tmp[((t2 * 2) * T.n_age + i) * T.cs_stride], sizeof(float) * E);
   return SPS_OK;
 }

@@ -1,0 +1,203 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (ctypes binding), against the float64
+oracle on the same seeded inputs.  Tolerances are BASELINE.json's north_star numbers as made precise
+in DESIGN.md: weights 1e-5 (inf-norm, relative to the row maximum) and 1e-4 elementwise where
+w > 1e-6 max; band fluxes 1e-4 relative; gradients 1e-3 relative to max(|g|, 1e-3 |g|_inf);
+first-20-leapfrog trajectories 1e-4; posterior mean/sd 0.05 sigma."""
+import numpy as np
+import pytest
+
+from oracle import sampler as S
+from oracle import sps_model as M
+from paper_2506_19919_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _sps():
+    import paper_2506_19919_b200 as sps
+    return sps
+
+
+def _dev(a, dtype=None):
+    return torch.tensor(np.asarray(a), dtype=dtype or torch.float32, device="cuda")
+
+
+def _rel(a, b):
+    return np.abs(a - b) / np.maximum(np.abs(b), 1e-300)
+
+
+def _grad_err(g, ref):
+    return np.abs(g - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(ref).max(1, keepdims=True))
+
+
+class Ctx:
+    def __init__(self, kind):
+        sps = _sps()
+        self.sps = sps
+        self.grid = W.make_grid(kind)
+        self.prior = W.make_prior()
+        self.P = self.prior.as_array()
+        self.ph = sps.PriorHandle(self.P)
+        self.table = sps.sps_create_table(self.grid)
+        self._cssp = None
+
+    def theta(self, n, seed, **kw):
+        thu = W.draw_theta_unbounded(self.prior, n, seed, **kw).astype(np.float32)
+        return thu.astype(np.float64), _dev(thu)
+
+    def cssp(self):
+        if self._cssp is None:
+            self._cssp = M.cssp_table(self.grid)
+        return self._cssp
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    return Ctx("tiny")
+
+
+@pytest.fixture(scope="module")
+def full():
+    return Ctx("full")
+
+
+def test_library_is_native():
+    sps = _sps()
+    from paper_2506_19919_b200 import binding
+    assert binding.lib().sps_version().decode().startswith("sps-b200")
+    n0 = sps.sps_launch_count()
+    sps.sps_philox_words(1, 0, 0, 0, 0, 8)
+    assert sps.sps_launch_count() == n0 + 1
+
+
+def test_philox_bit_exact():
+    sps = _sps()
+    seed = 0x1234567890ABCDEF
+    n = 1 << 18                                                   # 2^20 raw words
+    w = sps.sps_philox_words(seed, 5, 77, 3, 11, n).cpu().numpy().view(np.uint32)
+    idx = np.concatenate([np.arange(0, 64), np.random.default_rng(0).integers(0, n, 400), [n - 1]])
+    for i in idx:
+        assert tuple(int(x) for x in w[i]) == S.philox4x32((5 + int(i), 77, 3, 11), S.seed_key(seed))
+    # all words distinct enough: no stuck lanes
+    assert len(np.unique(w[:, 0])) > 0.999 * n
+
+
+@pytest.mark.parametrize("kind", ["tiny", "full"])
+def test_weights(kind, request):
+    cx = request.getfixturevalue(kind)
+    n = 777                                                        # several blocks and a ragged tail
+    thu, thd = cx.theta(n, 5, z_uniform=(0.1, 2.9))
+    th, _ = M.bound(thu, cx.P)
+    wa, wm, ms = (x.cpu().numpy().astype(np.float64) for x in cx.sps.sps_weights(cx.table, cx.ph, thd))
+    ow = M.weights(th, cx.grid)
+    for got, ref in ((wa, ow["a"]), (wm, ow["m"])):
+        mx = ref.max(1, keepdims=True)
+        assert (np.abs(got - ref) / mx).max() <= 1e-5
+        mask = ref > 1e-6 * mx
+        assert _rel(got, ref)[mask].max() <= 1e-4
+    assert _rel(ms, ow["Mn"]).max() <= 1e-5
+    # bounded-parameter entry point gives the same answer
+    wa2, _, _ = cx.sps.sps_weights(cx.table, None, _dev(th), unbounded=False)
+    assert np.abs(wa2.cpu().numpy() - wa).max() <= 2e-6
+
+
+def test_weights_edge_cases(tiny):
+    cx = tiny
+    th = M.bound(W.draw_theta_unbounded(cx.prior, 4, 3), cx.P)[0]
+    th[0, M.I_FB] = 0.0                           # no burst
+    th[1, M.I_FB] = 1.0; th[1, M.I_LTP] = 6.2; th[1, M.I_LTM] = 6.25   # burst inside one bin
+    th[2, M.I_SLZ] = 1e-3                         # delta-function MDF
+    th[3, M.I_Z] = 2.98; th[3, M.I_TAU] = 0.3; th[3, M.I_ALPHA] = 8.0; th[3, M.I_BETA] = 5.0   # sharpest SFH, youngest universe
+    wa, wm, ms = (x.cpu().numpy().astype(np.float64) for x in cx.sps.sps_weights(cx.table, None, _dev(th), unbounded=False))
+    ow = M.weights(th.astype(np.float32).astype(np.float64), cx.grid)
+    assert (np.abs(wa - ow["a"]) / ow["a"].max(1, keepdims=True)).max() <= 1e-5
+    assert np.abs(wm - ow["m"]).max() <= 1e-5
+    assert np.allclose(wa.sum(1), 1.0, atol=1e-5) and np.allclose(wm.sum(1), 1.0, atol=1e-5)
+    assert wa[1].max() > 0.999 and wm[2].max() > 0.999
+
+
+def test_empty_batch(tiny):
+    cx = tiny
+    e = torch.empty((0, 13), dtype=torch.float32, device="cuda")
+    wa, wm, ms = cx.sps.sps_weights(cx.table, cx.ph, e)
+    assert wa.shape == (0, cx.grid.n_age)
+    f = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, e)
+    assert f.shape == (0, cx.grid.n_band)
+
+
+@pytest.mark.parametrize("kind", ["tiny", "full"])
+def test_cssp_table(kind, request):
+    cx = request.getfixturevalue(kind)
+    c = cx.sps.sps_table_cssp(cx.table).astype(np.float64)
+    sel = np.unique(np.linspace(0, cx.grid.n_z - 1, 5).astype(int))
+    ref = M.cssp_table(cx.grid, M.z_grid(cx.grid)[sel])
+    mask = ref > 1e-6 * ref.max()
+    assert _rel(c[sel], ref)[mask].max() <= 1e-5
+
+
+@pytest.mark.parametrize("kind", ["tiny", "full"])
+def test_approx_flux_and_vjp(kind, request):
+    cx = request.getfixturevalue(kind)
+    n = 300
+    thu, thd = cx.theta(n, 15, z_uniform=(0.1, 2.9))
+    th, dth = M.bound(thu, cx.P)
+    of, J = M.photometry_approx(th, cx.grid, cx.cssp())
+    J = J * dth[:, None, :]
+    # the full Jacobian, one VJP per band (R20): no cross-band cancellation, so the north_star rule applies as is
+    for b in range(cx.grid.n_band):
+        fb = np.zeros((n, cx.grid.n_band), np.float32); fb[:, b] = 1.0
+        flux, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, thd, True, _dev(fb))
+        assert _grad_err(tb.cpu().numpy(), J[:, b, :]).max() <= 1e-3, b
+    assert _rel(flux.cpu().numpy(), of).max() <= 1e-4
+    # a random cotangent: terms cancel across bands, so the error is judged against the size of the terms
+    fb = np.random.default_rng(1).normal(size=(n, cx.grid.n_band)).astype(np.float32)
+    _, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, thd, True, _dev(fb))
+    ref = np.einsum("rb,rbp->rp", fb.astype(np.float64), J)
+    scale = np.einsum("rb,rbp->rp", np.abs(fb).astype(np.float64), np.abs(J))
+    assert (np.abs(tb.cpu().numpy() - ref) / np.maximum(scale, 1e-3 * scale.max(1, keepdims=True))).max() <= 1e-3
+    # forward-only call agrees with the fused one
+    f2 = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, thd)
+    assert torch.equal(f2, flux)
+
+
+def _observations(cx, n_gal, seed, path="approx", frac=(0.05, 0.10)):
+    truth_u, _ = cx.theta(n_gal, seed)
+    truth = M.bound(truth_u, cx.P)[0]
+    f = M.photometry_approx(truth, cx.grid, cx.cssp())[0] if path == "approx" else M.photometry_exact(truth, cx.grid, False)[0]
+    d, s = W.noisy_observations(f, seed + 1, *frac)
+    return truth_u, d.astype(np.float32), s.astype(np.float32)
+
+
+@pytest.mark.parametrize("kind", ["tiny", "full"])
+def test_loglike_grad_approx(kind, request):
+    cx = request.getfixturevalue(kind)
+    n_gal, n_chain = 40, 3
+    truth_u, d, s = _observations(cx, n_gal, 31)
+    thu = (np.repeat(truth_u, n_chain, 0) + 0.3 * np.random.default_rng(2).normal(size=(n_gal * n_chain, 13)) / cx.P[2]).astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+    olp, og, _ = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64),
+                                 "approx", cx.cssp())
+    assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4
+    assert _grad_err(g.cpu().numpy(), og).max() <= 1e-3
+
+
+def test_leapfrog_trajectory_approx(tiny):
+    cx = tiny
+    n = 16
+    truth_u, d, s = _observations(cx, n, 41, frac=(0.05, 0.05))
+    th0 = (truth_u + 0.2 * np.random.default_rng(3).normal(size=(n, 13)) / cx.P[2]).astype(np.float32)
+    p0 = np.random.default_rng(4).normal(size=(n, 13)).astype(np.float32)
+    # a stable step: the mass matrix is set to the scale 1/k of each unbounded parameter
+    eps = np.full(n, 0.01, np.float32); inv_m = np.tile((0.5 / cx.P[2]) ** 2, (n, 1)).astype(np.float32)
+    p0 = (p0 / np.sqrt(inv_m)).astype(np.float32)
+    traj, lpt = cx.sps.sps_leapfrog(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(th0), _dev(p0), _dev(eps), _dev(inv_m), _dev(d), _dev(s), 20)
+    f = lambda th: M.logp_and_grad(th, cx.grid, cx.P, d.astype(np.float64), s.astype(np.float64), "approx", cx.cssp())[:2]
+    lp0, g0 = f(th0.astype(np.float64))
+    _, _, _, _, ref = S.leapfrog(th0.astype(np.float64), p0.astype(np.float64), g0, eps.astype(np.float64), inv_m.astype(np.float64), f, 20, record=True)
+    traj = traj.cpu().numpy()
+    for k in range(20):
+        assert (np.abs(traj[k, :, 0] - ref[k][0]) / np.maximum(1.0, np.abs(ref[k][0]))).max() <= 1e-4, k
+        assert (np.abs(traj[k, :, 1] - ref[k][1]) / np.maximum(1.0, np.abs(ref[k][1]))).max() <= 1e-3, k
