@@ -201,3 +201,49 @@ def test_leapfrog_trajectory_approx(tiny):
     for k in range(20):
         assert (np.abs(traj[k, :, 0] - ref[k][0]) / np.maximum(1.0, np.abs(ref[k][0]))).max() <= 1e-4, k
         assert (np.abs(traj[k, :, 1] - ref[k][1]) / np.maximum(1.0, np.abs(ref[k][1]))).max() <= 1e-3, k
+
+
+# ---- a11/a12: HMC against the oracle under the shared counter-based RNG stream ------------------------
+def _run_both(cx, n_gal, n_chain, n_warmup, n_sample, n_leapfrog, eps0, seed, sampler="hmc", max_depth=5):
+    truth_u, d, s = _observations(cx, n_gal, 51, frac=(0.05, 0.05))
+    gal = np.repeat(np.arange(n_gal), n_chain)
+    out = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), sampler=cx.sps.SAMPLER_HMC if sampler == "hmc" else cx.sps.SAMPLER_NUTS,
+                             path=cx.sps.PATH_APPROX, n_chain=n_chain, n_warmup=n_warmup, n_sample=n_sample, n_leapfrog=n_leapfrog,
+                             max_depth=max_depth, eps0=eps0, seed=seed, keep_samples=True)
+    f = lambda th: M.logp_and_grad(th, cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), "approx", cx.cssp())[:2]
+    th0 = S.init_chains(cx.P, seed, np.arange(n_gal * n_chain), 13)
+    ref = S.run_chains(th0, f, seed, n_warmup, n_sample, eps0, sampler, n_leapfrog=n_leapfrog, max_depth=max_depth)
+    return {k: v.cpu().numpy() for k, v in out.items()}, ref
+
+
+def _coupled(got, ref, upto=None):
+    a, b = got["samples"][:, :upto], ref["samples"][:, :upto]
+    return (np.abs(a - b) / np.maximum(1.0, np.abs(b))).reshape(a.shape[0], -1).max(1)
+
+
+def test_hmc_config1_matches_oracle(tiny):
+    # BASELINE.json configs[0]: 8 galaxies x 4 chains, 200 HMC steps of 10 leapfrog steps, no warmup
+    got, ref = _run_both(tiny, 8, 4, 0, 200, 10, 0.004, seed=20250619)
+    assert _coupled(got, ref, 20).max() <= 1e-3                      # the first transitions agree for every chain
+    ok = _coupled(got, ref) <= 1e-2                                  # chains whose accept decisions never split
+    assert ok.mean() >= 0.85
+    mu_r, sd_r = ref["samples"].mean(1), ref["samples"].std(1, ddof=1)
+    assert (np.abs(got["mean"] - mu_r)[ok] <= 0.05 * sd_r[ok] + 1e-6).all()
+    assert (np.abs(got["sd"] - sd_r)[ok] <= 0.05 * sd_r[ok] + 1e-6).all()
+    assert np.abs(got["accept"] - ref["accept"])[ok].max() <= 0.02
+    assert (got["n_leapfrog"] == 2000).all()
+
+
+def test_hmc_warmup_adaptation_statistics(tiny):
+    # Warmup starts with large trial steps, so fp32 and fp64 trajectories decouple (chaotic dynamics):
+    # the adaptation is compared statistically (several results are correct; R14).
+    got, ref = _run_both(tiny, 4, 4, 150, 100, 8, 0.004, seed=7)
+    assert 0.6 < got["accept"].mean() < 0.98 and abs(got["accept"].mean() - ref["accept"].mean()) < 0.1
+    assert abs(np.log(np.median(got["eps"]) / np.median(ref["eps"]))) < 0.35
+    r = np.median(got["inv_mass"], 0) / np.median(ref["inv_mass"], 0)
+    assert np.all(np.abs(np.log(r)) < 0.9), r
+    # pooled per-galaxy posterior of the well-constrained direction (logM): within half a posterior sd
+    g_mu = got["samples"].reshape(4, -1, 13).mean(1); r_mu = ref["samples"].reshape(4, -1, 13).mean(1)
+    r_sd = ref["samples"].reshape(4, -1, 13).std(1)
+    assert np.all(np.abs(g_mu - r_mu)[:, 0] < 1.0 * r_sd[:, 0] + 0.02)
+    assert np.isfinite(got["rhat"]).all() and (got["n_leapfrog"] == 250 * 8).all()
