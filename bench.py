@@ -1,0 +1,305 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the SPS hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4_hmc|c3_approx|c2_exact]
+
+Default workload = BASELINE.json configs[3] ("c4_hmc"): full HMC on the approximate path, 10,000 synthetic
+galaxies x 4 chains x (500 warmup + 500 samples) x 16 leapfrog steps; metric = galaxy posteriors per GPU-minute.
+One "step" = one complete sps_hmc_run over the batch.  With N > 1 (torchrun) every rank runs the same number of
+galaxies (weak scaling; galaxies are independent, no data-path collective) and the value is the job aggregate.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SM_COUNT, FMA_PER_SM_CLK = 148, 128
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+# workload construction (synthetic, seeded)
+# ------------------------------------------------------------------------------------------------
+def make_hmc_inputs(sps, W, table, ph, prior, n_gal, seed, rank=0):
+    """True parameters drawn from the prior; observed fluxes = the library's own approximate-path photometry of the
+    truth with 5-10 % Gaussian noise (bench.py may not touch oracle/ outside the cpu_baseline leg)."""
+    import torch
+    thu = W.draw_theta_unbounded(prior, n_gal, seed + 1000 * rank).astype(np.float32)
+    f = sps.sps_photometry(table, ph, sps.PATH_APPROX, torch.tensor(thu, device="cuda")).cpu().numpy().astype(np.float64)
+    d, s = W.noisy_observations(f, seed + 7 + 1000 * rank, 0.05, 0.10)
+    return d.astype(np.float32), s.astype(np.float32)
+
+
+def run_ours(args):
+    import torch
+    import paper_2506_19919_b200 as sps
+    from paper_2506_19919_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", 0)); world = int(os.environ.get("WORLD_SIZE", 1)); local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = dict(W.CONFIGS[args.workload])
+    grid = W.make_grid(cfg["grid"]); prior = W.make_prior(); ph = sps.PriorHandle(prior.as_array())
+    table = sps.sps_create_table(grid)
+    peaks, peaks_src = _peaks()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
+
+    if args.workload == "c4_hmc":
+        n_gal = args.n_gal or cfg["n_gal"]
+        d, s = make_hmc_inputs(sps, W, table, ph, prior, n_gal, cfg["seed"], rank)
+        d_host = torch.from_numpy(d).pin_memory(); s_host = torch.from_numpy(s).pin_memory()
+        d_dev = d_host.cuda(); s_dev = s_host.cuda()
+        kw = dict(sampler=sps.SAMPLER_HMC, path=sps.PATH_APPROX, n_chain=cfg["n_chain"], n_warmup=args.n_warmup or cfg["n_warmup"],
+                  n_sample=args.n_sample or cfg["n_sample"], n_leapfrog=cfg["n_leapfrog"], eps0=0.01, seed=cfg["seed"])
+        evals_per_step = n_gal * cfg["n_chain"] * (kw["n_warmup"] + kw["n_sample"]) * cfg["n_leapfrog"]
+        units_per_step = n_gal                                                   # galaxy posteriors
+        step = lambda: sps.sps_hmc_run(table, ph, d_dev, s_dev, **kw)
+
+        def step_e2e():
+            dd = d_host.cuda(non_blocking=True); ss = s_host.cuda(non_blocking=True)
+            out = sps.sps_hmc_run(table, ph, dd, ss, **kw)
+            return out["mean"].cpu(), out["sd"].cpu(), out["rhat"].cpu()
+        h2d = d_host.numel() * 4 * 2
+        d2h = n_gal * cfg["n_chain"] * 13 * 4 * 2 + n_gal * 13 * 4
+        metric, unit, to_value = "galaxy posteriors/GPU-minute", "posteriors/min", lambda units, sec: 60.0 * units / sec
+        dom_kernel, rows_per_launch = "approx_contract", n_gal * cfg["n_chain"]
+    else:
+        n = args.n_rows or cfg["batch"]
+        path = sps.PATH_APPROX if args.workload == "c3_approx" else sps.PATH_EXACT
+        thu = W.draw_theta_unbounded(prior, n, cfg["seed"] + 1000 * rank, z_uniform=(0.1, 3.0)).astype(np.float32)
+        fb = np.random.default_rng(cfg["seed"]).normal(size=(n, grid.n_band)).astype(np.float32)
+        th_host = torch.from_numpy(thu).pin_memory(); fb_host = torch.from_numpy(fb).pin_memory()
+        th_dev = th_host.cuda(); fb_dev = fb_host.cuda()
+        evals_per_step = n; units_per_step = n
+        step = lambda: sps.sps_photometry(table, ph, path, th_dev, True, fb_dev)
+
+        def step_e2e():
+            a = th_host.cuda(non_blocking=True); b = fb_host.cuda(non_blocking=True)
+            fl, tb = sps.sps_photometry(table, ph, path, a, True, b)
+            return fl.cpu(), tb.cpu()
+        h2d = n * (13 + grid.n_band) * 4; d2h = n * (13 + grid.n_band) * 4
+        metric, unit, to_value = "flux+gradient evaluations/s", "evals/s", lambda units, sec: units / sec
+        dom_kernel, rows_per_launch = ("approx_contract" if path == sps.PATH_APPROX else "exact_fwd"), n
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    # ---- timed region 1: inputs resident in HBM ---------------------------------------------------
+    sps.sps_profile(True, 8)
+    launches0 = sps.sps_launch_count()
+    clocks = ClockSampler(local); clocks.start()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.fill_(1)                                                          # L2 flush between timed iterations
+        a.record(); step(); b.record()
+    barrier()
+    clk = clocks.stop()
+    dev_s = sum(a.elapsed_time(b) for a, b in ev) / 1e3
+    launches = sps.sps_launch_count() - launches0
+    prof = {k: sps.sps_profile_read(k) for k in ("prologue", "approx_contract", "epilogue", "exact_fwd", "exact_bwd")}
+    sps.sps_profile(False, 1)
+    # ---- timed region 2: end to end through the public API with host buffers -----------------------
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([dev_s, e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_s, e2e_s = t.tolist()
+    if rank != 0:
+        return
+    value = to_value(units_per_step * args.steps * world, dev_s)
+    out = {"metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32", "data": "synthetic (seeded stand-in SSP spectra, Gaussian filters, prior-drawn galaxies)",
+           "config": {"workload": args.workload, **{k: v for k, v in cfg.items() if k != "seed"},
+                      "n_gal_per_gpu": args.n_gal or cfg.get("n_gal"), "l2": "flushed between timed steps (256 MB write)"},
+           "loglike_grad_evals_per_s": evals_per_step * args.steps * world / dev_s,
+           "e2e": {"value": to_value(units_per_step * args.steps * world, e2e_s), "unit": unit, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h},
+           "gpu_launches": int(launches), "clocks": clk, "impl": "ours"}
+    out["roofline"] = roofline(prof, dom_kernel, rows_per_launch, grid, peaks, peaks_src)
+    out["kernel_ms"] = {k: {"avg_ms": (v[0] / v[1] if v[1] else None), "launches": v[2]} for k, v in prof.items() if v[2]}
+    if not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(args.workload, cfg, budget_s=args.cpu_budget)
+    print(json.dumps(out))
+
+
+def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src):
+    """Roofline of the dominant kernel.
+    approx_contract: FP32-FMA ("alu") bound: per row the forward + reverse pass over the two c_SSP arrays of its z cell
+    is 2 FMA per table word = 4 * n_age*n_Z*n_band flop ... no HBM stream: the table is L2/smem resident.
+    Peak = 148 SM x 128 FMA/clk x 2 flop x max SM clock (guide unit counts; clock from MEASURED_PEAKS.json)."""
+    ms, timed, allc = prof[kernel]
+    if not timed:
+        return {"bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None, "traffic": None}
+    avg_s = ms / timed / 1e3
+    if kernel == "approx_contract":
+        words = 2 * grid.n_age * grid.n_Z * grid.n_band
+        flop = 2.0 * 2.0 * words * rows_per_launch
+        peak = SM_COUNT * FMA_PER_SM_CLK * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        bound, note = "alu", f"fp32 FMA peak at {peaks.get('sm_max_mhz', 1965.0):.0f} MHz ({peaks_src})"
+    else:
+        K = grid.n_age * grid.n_Z
+        flop = 3.0 * 2.0 * K * grid.n_wave * rows_per_launch          # 3xTF32 issued flop over the unpadded columns
+        peak = 0.5 * float(peaks["bf16_tflops"])                       # TF32 = bf16 measured x nominal ratio 1.1/2.25
+        bound, note = "tensor", f"tf32 peak = 0.5 x bf16 burst ({peaks_src}); achieved counts the 3 split products"
+    ach = flop / avg_s / 1e12
+    return {"bound": bound, "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+            "traffic": None, "avg_launch_ms": 1e3 * avg_s, "timed_launches": timed, "launches": allc, "peak_note": note}
+
+
+def cpu_baseline(workload, cfg, budget_s=20.0):
+    """The float64 oracle, as it stands, timed on this box's host cores on a bounded sample of the same workload."""
+    from threadpoolctl import threadpool_limits
+    from oracle import sampler as S
+    from oracle import sps_model as M
+    from paper_2506_19919_b200 import workloads as W
+    grid = W.make_grid(cfg["grid"]); prior = W.make_prior(); P = prior.as_array()
+    with threadpool_limits(limits=1):
+        if workload == "c4_hmc":
+            cssp = M.cssp_table(grid, M.z_grid(grid))          # setup, untimed (as for the GPU)
+            n_gal, n_chain, L = 2, cfg["n_chain"], cfg["n_leapfrog"]
+            thu = W.draw_theta_unbounded(prior, n_gal, cfg["seed"])
+            f = M.photometry_approx(M.bound(thu, P)[0], grid, cssp)[0]
+            d, s = W.noisy_observations(f, cfg["seed"] + 7, 0.05, 0.10)
+            gal = np.repeat(np.arange(n_gal), n_chain)
+            fn = lambda th: M.logp_and_grad(th, grid, P, d[gal], s[gal], "approx", cssp)[:2]
+            th0 = S.init_chains(P, cfg["seed"], np.arange(n_gal * n_chain), 13)
+            n_tr, t0 = 0, time.perf_counter()
+            while time.perf_counter() - t0 < budget_s:
+                S.run_chains(th0, fn, cfg["seed"], 0, 2, 0.01, "hmc", n_leapfrog=L)
+                n_tr += 2
+            sec = time.perf_counter() - t0
+            evals = n_gal * n_chain * n_tr * L
+            per_post = n_chain * (cfg["n_warmup"] + cfg["n_sample"]) * L
+            return {"value": 60.0 * (evals / sec) / per_post, "unit": "posteriors/min", "cores": 1, "kind": "oracle",
+                    "sample": f"{n_gal} galaxies x {n_chain} chains x {n_tr} HMC transitions x {L} leapfrogs of the float64 numpy oracle "
+                              f"({evals} loglike+grad evals in {sec:.1f} s), scaled linearly to {per_post} evals per posterior",
+                    "loglike_grad_evals_per_s": evals / sec}
+        n = 8 if workload == "c2_exact" else 256
+        thu = W.draw_theta_unbounded(prior, n, cfg["seed"], z_uniform=(0.1, 3.0))
+        th = M.bound(thu, P)[0]
+        cssp = M.cssp_table(grid) if workload == "c3_approx" else None
+        done, t0 = 0, time.perf_counter()
+        while time.perf_counter() - t0 < budget_s:
+            (M.photometry_approx(th, grid, cssp) if workload == "c3_approx" else M.photometry_exact(th, grid))
+            done += n
+        sec = time.perf_counter() - t0
+        return {"value": done / sec, "unit": "evals/s", "cores": 1, "kind": "oracle",
+                "sample": f"{done} rows of the workload's parameter draws through the float64 numpy oracle (flux + full Jacobian)"}
+
+
+def run_reference(args):
+    """--impl reference: there is no reference implementation (the paper ships no code); for this tier the reference arm
+    is the oracle timed on the host cores."""
+    if int(os.environ.get("RANK", 0)) != 0:
+        return
+    from paper_2506_19919_b200 import workloads as W
+    cfg = dict(W.CONFIGS[args.workload])
+    per_step = max(5.0, min(30.0, 90.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        cpu_baseline(args.workload, cfg, budget_s=2.0)
+    t0 = time.perf_counter()
+    res = [cpu_baseline(args.workload, cfg, budget_s=per_step) for _ in range(args.steps)]
+    sec = time.perf_counter() - t0
+    v = float(np.mean([r["value"] for r in res]))
+    hmc = args.workload == "c4_hmc"
+    out = {"impl": "reference", "metric": "galaxy posteriors/GPU-minute" if hmc else "flux+gradient evaluations/s", "value": v,
+           "unit": res[0]["unit"], "n_gpus": int(os.environ.get("WORLD_SIZE", 1)), "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * sec / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": {"workload": args.workload, **{k: v2 for k, v2 in cfg.items() if k != "seed"}},
+           "cpu_baseline": {**res[0], "value": v}, "e2e": {"value": v, "unit": res[0]["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4_hmc", choices=["c4_hmc", "c3_approx", "c2_exact"])
+    ap.add_argument("--n-gal", type=int, default=0)
+    ap.add_argument("--n-rows", type=int, default=0)
+    ap.add_argument("--n-warmup", type=int, default=0)
+    ap.add_argument("--n-sample", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

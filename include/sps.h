@@ -149,6 +149,15 @@ sps_status sps_hmc_run(const sps_table* t, const sps_prior* prior, const sps_hmc
 sps_status sps_philox_words(uint64_t seed, uint32_t first_chain, uint32_t transition, uint32_t purpose,
                             uint32_t index, int64_t n, uint32_t* out_dev, void* stream);
 
+/* Per-kernel device timing for bench.py's roofline line.  sps_profile(1) makes the library bracket
+ * every `stride`-th launch of its main kernels with CUDA events on the launching stream;
+ * sps_profile_read(kernel_id, &total_ms, &timed_launches, &all_launches) synchronises, sums the recorded
+ * pairs for that kernel and clears them.  kernel_id: 0 prologue (weights), 1 approximate contraction,
+ * 2 epilogue (reverse of the weights + prior), 3 exact forward GEMM, 4 exact reverse GEMM. */
+enum { SPS_K_PROLOGUE = 0, SPS_K_APPROX = 1, SPS_K_EPILOGUE = 2, SPS_K_EXACT_FWD = 3, SPS_K_EXACT_BWD = 4, SPS_K_COUNT = 5 };
+sps_status sps_profile(int enable, int stride);
+sps_status sps_profile_read(int kernel_id, double* total_ms, int64_t* timed_launches, int64_t* all_launches);
+
 /* Number of kernels this library launched since load (for bench.py's gpu_launches). */
 int64_t sps_launch_count(void);
 

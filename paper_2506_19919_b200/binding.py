@@ -17,7 +17,7 @@ PATH_EXACT, PATH_APPROX = 0, 1
 SAMPLER_HMC, SAMPLER_NUTS = 0, 1
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
-           "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_launch_count",
+           "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
            "sps_last_error", "sps_version")
 
 
@@ -210,3 +210,17 @@ def sps_philox_words(seed, first_chain, transition, purpose, index, n):
 
 def sps_launch_count() -> int:
     return int(lib().sps_launch_count())
+
+
+KERNEL_IDS = {"prologue": 0, "approx_contract": 1, "epilogue": 2, "exact_fwd": 3, "exact_bwd": 4}
+
+
+def sps_profile(enable: bool, stride: int = 1):
+    _check(lib().sps_profile(int(enable), int(stride)), "sps_profile")
+
+
+def sps_profile_read(kernel: str):
+    """-> (total_ms over the timed launches, timed launches, all launches) since the last read."""
+    ms, n, a = C.c_double(), C.c_int64(), C.c_int64()
+    _check(lib().sps_profile_read(KERNEL_IDS[kernel], C.byref(ms), C.byref(n), C.byref(a)), "sps_profile_read")
+    return ms.value, n.value, a.value

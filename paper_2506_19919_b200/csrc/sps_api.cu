@@ -18,6 +18,41 @@ extern "C" int64_t sps_launch_count(void) { return g_launches.load(); }
 extern "C" const char* sps_last_error(void) { return g_err; }
 extern "C" const char* sps_version(void) { return "sps-b200 0.1 (sm_100a)"; }
 
+// ---- optional per-kernel event timing ---------------------------------------------------------
+#include <vector>
+struct ProfSlot { std::vector<cudaEvent_t> ev; int64_t launches = 0; bool open = false; };
+static ProfSlot g_prof[SPS_K_COUNT];
+static int g_prof_on = 0, g_prof_stride = 1;
+void sps_prof_begin(int id, cudaStream_t s) {
+  if (!g_prof_on) return;
+  ProfSlot& P = g_prof[id];
+  P.open = (P.launches++ % g_prof_stride) == 0 && P.ev.size() < 16384;
+  if (!P.open) return;
+  cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, s); P.ev.push_back(e);
+}
+void sps_prof_end(int id, cudaStream_t s) {
+  if (!g_prof_on) return;
+  ProfSlot& P = g_prof[id];
+  if (!P.open) return;
+  cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, s); P.ev.push_back(e); P.open = false;
+}
+extern "C" sps_status sps_profile(int enable, int stride) {
+  g_prof_on = enable; g_prof_stride = stride > 0 ? stride : 1;
+  for (auto& P : g_prof) { for (auto e : P.ev) cudaEventDestroy(e); P.ev.clear(); P.launches = 0; P.open = false; }
+  return SPS_OK;
+}
+extern "C" sps_status sps_profile_read(int id, double* total_ms, int64_t* timed, int64_t* all) {
+  if (id < 0 || id >= SPS_K_COUNT || !total_ms || !timed || !all) { sps_set_error("sps_profile_read: bad argument"); return SPS_EINVAL; }
+  cudaDeviceSynchronize();
+  ProfSlot& P = g_prof[id];
+  double tot = 0; int64_t n = 0;
+  for (size_t i = 0; i + 1 < P.ev.size(); i += 2) { float ms = 0; if (cudaEventElapsedTime(&ms, P.ev[i], P.ev[i + 1]) == cudaSuccess) { tot += ms; ++n; } }
+  *total_ms = tot; *timed = n; *all = P.launches;
+  for (auto e : P.ev) cudaEventDestroy(e);
+  P.ev.clear(); P.launches = 0;
+  return SPS_OK;
+}
+
 sps_status sps_check_cuda(cudaError_t e, const char* what) {
   if (e == cudaSuccess) return SPS_OK;
   sps_set_error("%s: %s", what, cudaGetErrorString(e));

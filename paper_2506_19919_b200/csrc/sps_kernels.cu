@@ -280,21 +280,27 @@ static inline unsigned blocks_for_rows(int64_t n) { return (unsigned)((n + WARPS
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      const int* rows, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
+  sps_prof_begin(SPS_K_PROLOGUE, s);
   prologue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
+  sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
 void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
+  sps_prof_begin(SPS_K_APPROX, s);
   approx_contract_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, n, rows, gal_of_row, obs_flux, obs_sigma,
                                                                            flux_bar, want_grad, B);
+  sps_prof_end(SPS_K_APPROX, s);
   sps_count_launch();
 }
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s) {
   if (n <= 0) return;
+  sps_prof_begin(SPS_K_EPILOGUE, s);
   epilogue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad);
+  sps_prof_end(SPS_K_EPILOGUE, s);
   sps_count_launch();
 }
 void launch_copy_weights(const TableDev& T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar, cudaStream_t s) {
