@@ -247,3 +247,46 @@ def test_hmc_warmup_adaptation_statistics(tiny):
     r_sd = ref["samples"].reshape(4, -1, 13).std(1)
     assert np.all(np.abs(g_mu - r_mu)[:, 0] < 1.0 * r_sd[:, 0] + 0.02)
     assert np.isfinite(got["rhat"]).all() and (got["n_leapfrog"] == 250 * 8).all()
+
+
+# ---- a6/a8/a10: exact path ---------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,n", [("tiny", 200), ("full", 24)])
+def test_exact_flux_and_jacobian(kind, n, request):
+    cx = request.getfixturevalue(kind)
+    thu, thd = cx.theta(n, 25, z_uniform=(0.1, 2.9))
+    th, dth = M.bound(thu, cx.P)
+    of, J = M.photometry_exact(th, cx.grid)
+    J = J * dth[:, None, :]
+    flux = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_EXACT, thd)
+    assert _rel(flux.cpu().numpy(), of).max() <= 1e-4
+    for b in range(cx.grid.n_band):
+        fb = np.zeros((n, cx.grid.n_band), np.float32); fb[:, b] = 1.0
+        f2, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_EXACT, thd, True, _dev(fb))
+        assert _grad_err(tb.cpu().numpy(), J[:, b, :]).max() <= 1e-3, b
+    assert _rel(f2.cpu().numpy(), of).max() <= 1e-4
+
+
+def test_exact_equals_approx_without_dust_on_z_nodes(full):
+    cx = full                                                       # Eq. 6 == Eq. 4 when F_att is constant
+    n = 64
+    thu, _ = cx.theta(n, 27)
+    th = M.bound(thu, cx.P)[0]
+    th[:, M.I_AV] = 0.0
+    th[:, M.I_Z] = M.z_grid(cx.grid)[np.random.default_rng(5).integers(3, 190, n)]
+    thd = _dev(th)
+    fe = cx.sps.sps_photometry(cx.table, None, cx.sps.PATH_EXACT, thd, unbounded=False).cpu().numpy()
+    fa = cx.sps.sps_photometry(cx.table, None, cx.sps.PATH_APPROX, thd, unbounded=False).cpu().numpy()
+    assert _rel(fe, fa).max() <= 2e-5
+
+
+@pytest.mark.parametrize("kind,n_gal", [("tiny", 40), ("full", 8)])
+def test_loglike_grad_exact(kind, n_gal, request):
+    cx = request.getfixturevalue(kind)
+    n_chain = 3
+    truth_u, d, s = _observations(cx, n_gal, 61, path="exact")
+    thu = (np.repeat(truth_u, n_chain, 0) + 0.3 * np.random.default_rng(2).normal(size=(n_gal * n_chain, 13)) / cx.P[2]).astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, cx.sps.PATH_EXACT, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+    olp, og, _ = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), "exact")
+    assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4
+    assert _grad_err(g.cpu().numpy(), og).max() <= 1e-3
