@@ -40,6 +40,12 @@ typedef enum {
 
 enum { SPS_PATH_EXACT = 0, SPS_PATH_APPROX = 1 };
 enum { SPS_SAMPLER_HMC = 0, SPS_SAMPLER_NUTS = 1 };
+/* Operand format of the exact path's tensor-core contractions (three split products a_lo b_hi + a_hi b_lo + a_hi b_hi,
+ * fp32 accumulation in TMEM).  BF16X3: ~2^-17 per product, 16 K-elements per accumulator update.  TF32X3: ~2^-21 per
+ * product but twice the operand bytes, half the MMA rate and twice the accumulator updates; since tcgen05 accumulation
+ * truncates (measured ~2.4e-8 relative per update) BF16X3 is both faster and, end to end, more accurate
+ * on this problem, hence the default. */
+enum { SPS_EXACT_BF16X3 = 0, SPS_EXACT_TF32X3 = 1 };
 
 typedef struct sps_table sps_table;      /* opaque; owns device memory */
 
@@ -55,6 +61,7 @@ typedef struct {
   double z_min, z_max;         /* uniform redshift grid of the c_SSP lookup table    */
   double H0, Om;               /* flat LCDM for t_obs(z) (R11)                       */
   double log10_mass_unit;      /* M_star is expressed in 10^this Msun so that fluxes are O(1)      */
+  int32_t exact_precision;     /* SPS_EXACT_BF16X3 (0, default) or SPS_EXACT_TF32X3                */
 } sps_table_desc;
 
 /* Per-parameter hyper-parameters, HOST arrays of SPS_NDIM doubles each.

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libsps_b200.so")
 NDIM = 13
 PATH_EXACT, PATH_APPROX = 0, 1
 SAMPLER_HMC, SAMPLER_NUTS = 0, 1
+EXACT_BF16X3, EXACT_TF32X3 = 0, 1
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
            "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
@@ -30,7 +31,7 @@ class _TableDesc(C.Structure):
                 ("log10_age_yr", C.POINTER(C.c_double)), ("log10_Z", C.POINTER(C.c_double)), ("wave_A", C.POINTER(C.c_double)),
                 ("ssp", C.POINTER(C.c_float)), ("filt_mu_A", C.POINTER(C.c_double)), ("filt_sigma_A", C.POINTER(C.c_double)),
                 ("z_min", C.c_double), ("z_max", C.c_double), ("H0", C.c_double), ("Om", C.c_double),
-                ("log10_mass_unit", C.c_double)]
+                ("log10_mass_unit", C.c_double), ("exact_precision", C.c_int32)]
 
 
 class _Prior(C.Structure):
@@ -103,7 +104,7 @@ class PriorHandle:
 class Table:
     """Owner of an sps_table handle."""
 
-    def __init__(self, grid):
+    def __init__(self, grid, exact_precision=0):
         self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z = grid.n_age, grid.n_Z, grid.n_wave, grid.n_band, grid.n_z
         keep = [_f64(grid.log10_age_yr), _f64(grid.log10_Z), _f64(grid.wave_A),
                 np.ascontiguousarray(grid.ssp, dtype=np.float32), _f64(grid.filt_mu_A), _f64(grid.filt_sigma_A)]
@@ -111,7 +112,8 @@ class Table:
         dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
         d = _TableDesc(self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z, dp(keep[0]), dp(keep[1]), dp(keep[2]),
                        keep[3].ctypes.data_as(C.POINTER(C.c_float)), dp(keep[4]), dp(keep[5]),
-                       float(grid.z_min), float(grid.z_max), float(grid.H0), float(grid.Om), float(grid.log10_mass_unit))
+                       float(grid.z_min), float(grid.z_max), float(grid.H0), float(grid.Om), float(grid.log10_mass_unit),
+                       int(exact_precision))
         h = C.c_void_p()
         _check(lib().sps_create_table(C.byref(d), C.byref(h)), "sps_create_table")
         self.handle = h
@@ -128,8 +130,8 @@ class Table:
             pass
 
 
-def sps_create_table(grid) -> Table:
-    return Table(grid)
+def sps_create_table(grid, exact_precision=EXACT_BF16X3) -> Table:
+    return Table(grid, exact_precision)
 
 
 def sps_table_cssp(table: Table) -> np.ndarray:

@@ -237,27 +237,50 @@ __global__ void exact_final_kernel(TableDev T, int64_t n, const int* __restrict_
   for (int j = 0; j < SPS_MAX_Z; ++j) { const float s = warp_sum(mb[j]); if (l == j) B.m_bar[row * ROW_M_STRIDE + j] = Mn * s; }
 }
 
+// ---- order the rows of a call by redshift (counting sort over ZSORT_BINS uniform bins of the table's z range) --------
+// The tensor-core kernels tile rows in groups of 128; rows of similar z share the wavelength range under the filters.
+#define ZSORT_BINS 1024
+__device__ __forceinline__ int zsort_bin(const TableDev& T, float z) {
+  const float u = (z - T.z_min) / (T.dz * (float)(T.n_z - 1));
+  return min(max((int)(u * ZSORT_BINS), 0), ZSORT_BINS - 1);
+}
+__global__ void zsort_hist_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) atomicAdd(&hist[zsort_bin(T, B.sc[rows ? rows[i] : i].z)], 1);
+}
+__global__ void __launch_bounds__(ZSORT_BINS) zsort_scan_kernel(int* __restrict__ hist) {      // hist -> exclusive offsets, in place (+ copy)
+  __shared__ int s[ZSORT_BINS];
+  const int t = threadIdx.x;
+  const int v = hist[t];
+  s[t] = v;
+  __syncthreads();
+  for (int o = 1; o < ZSORT_BINS; o <<= 1) { const int a = (t >= o) ? s[t - o] : 0; __syncthreads(); s[t] += a; __syncthreads(); }
+  hist[ZSORT_BINS + t] = s[t] - v;
+}
+__global__ void zsort_scatter_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ cursor, int* __restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int row = rows ? rows[i] : (int)i;
+  out[atomicAdd(&cursor[zsort_bin(T, B.sc[row].z)], 1)] = row;
+}
+
 // ---- host side ----------------------------------------------------------------------------------------
-sps_status sps_exact_tc_setup(sps_table* t);                       // sps_exact_tc.cu
-void sps_exact_tc_teardown(sps_table* t);
-sps_status sps_exact_tc_forward(sps_table* t, int64_t n, const int* rows, cudaStream_t s);
-sps_status sps_exact_tc_backward(sps_table* t, int64_t n, const int* rows, cudaStream_t s);
 
 static int g_force_simt = 0;
 extern "C" void sps_debug_force_simt(int on) { g_force_simt = on; }
 
-sps_status sps_exact_setup(sps_table* t) {
+sps_status sps_exact_setup(sps_table* t, int precision) {
   ExactState* X = new ExactState();
   memset(X, 0, sizeof(*X));
   X->ldw = (t->dev.K + 31) / 32 * 32;
   t->exact = X;
-  return sps_exact_tc_setup(t);
+  return sps_exact_tc_setup(t, precision);
 }
 
 static void exact_free_buffers(ExactState* X) {
-  void* ptrs[] = {X->W, X->Wbar, X->part, X->gbuf};
+  void* ptrs[] = {X->W, X->Wbar, X->part, X->gbuf, X->sorted, X->zhist};
   for (void* p : ptrs) if (p) cudaFree(p);
-  X->W = X->Wbar = X->part = X->gbuf = nullptr; X->cap = 0;
+  X->W = X->Wbar = X->part = X->gbuf = nullptr; X->sorted = X->zhist = nullptr; X->cap = 0;
 }
 
 void sps_exact_teardown(sps_table* t) {
@@ -267,7 +290,8 @@ void sps_exact_teardown(sps_table* t) {
   delete t->exact; t->exact = nullptr;
 }
 
-static sps_status exact_ensure(ExactState* X, int64_t n) {
+static sps_status exact_ensure(sps_table* t, int64_t n) {
+  ExactState* X = t->exact;
   const int64_t need = (n + 127) / 128 * 128;                      // whole row tiles for the tensor-core kernels
   if (X->cap >= need) return SPS_OK;
   cudaDeviceSynchronize();
@@ -276,20 +300,31 @@ static sps_status exact_ensure(ExactState* X, int64_t n) {
   if (e == cudaSuccess) e = cudaMalloc(&X->Wbar, need * X->ldw * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&X->part, need * 5 * SPS_MAX_BAND * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&X->gbuf, need * SPS_MAX_BAND * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&X->sorted, need * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&X->zhist, 2 * ZSORT_BINS * sizeof(int));
   if (e != cudaSuccess) { exact_free_buffers(X); return sps_check_cuda(e, "exact-path scratch allocation"); }
   cudaMemset(X->W, 0, need * X->ldw * sizeof(float));
   cudaMemset(X->gbuf, 0, need * SPS_MAX_BAND * sizeof(float));
   X->cap = need;
-  return SPS_OK;
+  return sps_exact_tc_ensure(t, need);
 }
 
 sps_status sps_exact_contract(sps_table* t, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
                               const float* obs_sigma, const float* flux_bar, bool want_grad, cudaStream_t s) {
   ExactState* X = t->exact;
   const TableDev& T = t->dev;
-  sps_status st = exact_ensure(X, n); if (st != SPS_OK) return st;
+  sps_status st = exact_ensure(t, n); if (st != SPS_OK) return st;
   const bool tc = X->use_tc && !g_force_simt;
-  exact_weights_kernel<<<(unsigned)n, 128, 0, s>>>(T, n, rows, t->rows, X->W, X->ldw); sps_count_launch();
+  if (tc) {                                                        // redshift-ordered row list for this call
+    cudaMemsetAsync(X->zhist, 0, 2 * ZSORT_BINS * sizeof(int), s);
+    const unsigned nb = (unsigned)((n + 255) / 256);
+    zsort_hist_kernel<<<nb, 256, 0, s>>>(T, n, rows, t->rows, X->zhist);
+    zsort_scan_kernel<<<1, ZSORT_BINS, 0, s>>>(X->zhist);
+    zsort_scatter_kernel<<<nb, 256, 0, s>>>(T, n, rows, t->rows, X->zhist + ZSORT_BINS, X->sorted);
+    sps_count_launch(3);
+    rows = X->sorted;
+  }
+  if (!tc) { exact_weights_kernel<<<(unsigned)n, 128, 0, s>>>(T, n, rows, t->rows, X->W, X->ldw); sps_count_launch(); }
   cudaMemsetAsync(X->part, 0, n * 5 * SPS_MAX_BAND * sizeof(float), s);
   sps_prof_begin(SPS_K_EXACT_FWD, s);
   if (tc) st = sps_exact_tc_forward(t, n, rows, s);

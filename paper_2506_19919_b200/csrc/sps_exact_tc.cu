@@ -1,6 +1,701 @@
-// sps_exact_tc.cu -- tcgen05 / TMA / TMEM kernels of the exact path.  [stub: filled in next]
+// sps_exact_tc.cu -- tcgen05 / TMA / TMEM kernels of the exact photometry path (a6, a10).
+//
+// Both contractions of the exact path are dense GEMMs with fp32 operands:
+//   forward   S[r,k]    = sum_c W[r,c]      L[c,k]      M = rows, N = wavelengths, K = n_age*n_Z
+//   reverse   Wbar[r,c] = sum_k SEDbar[r,k] L[c,k]      M = rows, N = n_age*n_Z,  K = wavelengths
+// They run on the 5th-generation tensor cores as three split products with fp32 accumulation in TMEM,
+//   x = x_hi + x_lo,   a b ~= a_lo b_hi + a_hi b_lo + a_hi b_hi,
+// in one of two operand formats chosen at table creation (sps_table_desc.exact_precision):
+//   SPS_EXACT_BF16X3 (default)  hi, lo as BF16 ( 8-bit significands): ~2^-17 per product, 16 K-elements per MMA;
+//   SPS_EXACT_TF32X3            hi, lo as TF32 (11-bit significands): ~2^-21 per product, twice the operand bytes, half
+//                               the MMA rate and twice the accumulator updates.
+// tcgen05 adds each MMA's partial dot product into the fp32 TMEM accumulator with truncation; measured here as a
+// relative bias of about -2.4e-8 per update (-7e-6 on S after the 252 updates of the BF16X3 forward pass, -1.2e-5 after
+// the 504 of TF32X3), so on this problem BF16X3 is the faster AND the more accurate of the two.
+// The SSP table is split once at table creation, in both majornesses; the row-side operands (W, SEDbar) are split by
+// the kernels that generate them.
+//
+// Work restriction (what makes the path fast): the rows of a call are ordered by redshift (counting sort, sps_exact.cu),
+// so the 128 rows of a row tile share a narrow z range and only the wavelength tiles under some filter's (5 sigma)
+// support at those redshifts are touched: forward items = (row tile, wavelength tile in range), reverse k loop =
+// wavelength blocks in range.  Everything outside contributes exactly zero to Eq. (4) and is never computed.
+//
+// One persistent CTA per SM, 320 threads, warp-specialised:
+//   warp 0      TMA producer: 128B-swizzled K-major tiles (A_hi, A_lo: 128 rows; B_hi, B_lo: BN rows; 128 B of K per
+//               row) into a 2-stage, 96 KB/stage shared-memory ring, mbarrier complete_tx
+//   warp 1      allocates 512 TMEM columns (two 256-column fp32 accumulators) and issues tcgen05.mma
+//               (cta_group::1, M = 128, N = BN, 32 B of K per instruction): 12 MMAs per k block
+//   warps 2-9   epilogue: tcgen05.ld of their 32 TMEM lanes (thread = row; two warps share a lane quarter and split
+//               the columns) while the MMA warp fills the other accumulator.
+//               forward: dust attenuation (Eq. A8-A9), redshifted Gaussian filters, trapezoid weight and the
+//               reduction over wavelength (Eq. 3-4) fused on the accumulators -- S never reaches HBM; flux and
+//               its four direct partials (A_V, delta, F_floor, z) per band stay in registers across the wavelength
+//               tiles of a row tile.   reverse: plain store of Wbar.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <algorithm>
+#include <cstring>
+#include <vector>
 #include "sps_exact.cuh"
-sps_status sps_exact_tc_setup(sps_table* t) { t->exact->use_tc = false; t->exact->tc = nullptr; return SPS_OK; }
-void sps_exact_tc_teardown(sps_table*) {}
-sps_status sps_exact_tc_forward(sps_table*, int64_t, const int*, cudaStream_t) { sps_set_error("tcgen05 path not built"); return SPS_EUNSUPPORTED; }
-sps_status sps_exact_tc_backward(sps_table*, int64_t, const int*, cudaStream_t) { sps_set_error("tcgen05 path not built"); return SPS_EUNSUPPORTED; }
+
+namespace {
+
+constexpr int BM = 128, BN_MAX = 256, STAGES = 2;
+constexpr int ROW_BYTES = 128;                                        // bytes of K per operand row per stage
+constexpr int A_TILE_BYTES = BM * ROW_BYTES;                          // 16 KB
+constexpr int B_TILE_BYTES = BN_MAX * ROW_BYTES;                      // 32 KB
+constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;      // 96 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int EPI_WARPS = 8;
+constexpr int NUM_THREADS = 64 + 32 * EPI_WARPS;
+constexpr int TMEM_COLS = 512;
+
+// operand formats
+template <int PREC> struct Op;
+template <> struct Op<SPS_EXACT_TF32X3> {
+  typedef float T;
+  static constexpr int BK = 32;                                      // elements per 128-byte row
+  static constexpr uint32_t FMT = 2;                                 // instruction-descriptor format code (TF32)
+  static __device__ __forceinline__ float rna(float v) { uint32_t u; asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v)); return __uint_as_float(u); }
+  static __device__ __forceinline__ void split(float v, T& hi, T& lo) { hi = rna(v); lo = rna(v - hi); }
+};
+template <> struct Op<SPS_EXACT_BF16X3> {
+  typedef __nv_bfloat16 T;
+  static constexpr int BK = 64;
+  static constexpr uint32_t FMT = 1;                                 // BF16
+  static __device__ __forceinline__ void split(float v, T& hi, T& lo) { hi = __float2bfloat16_rn(v); lo = __float2bfloat16_rn(v - __bfloat162float(hi)); }
+};
+
+struct FilterConsts {                 // x = lam (1+z) isg + nmu ; T_b = exp2(-x^2) for |x| <= 5 FILT_SCALE
+  float isg[SPS_MAX_BAND], nmu[SPS_MAX_BAND], dz[SPS_MAX_BAND], lo[SPS_MAX_BAND], hi[SPS_MAX_BAND];
+};
+
+struct TcState {
+  int prec, es, BK;                 // operand format, element size, elements per k block
+  void *LT_hi, *LT_lo;              // [n_wave_pad][Wld]    forward B operand (wavelength-major, K = ij contiguous)
+  void *Lc_hi, *Lc_lo;              // [nb*BNb][n_wave_pad] reverse B operand (ij-major, K = wavelength contiguous)
+  void *W_hi, *W_lo;                // [cap][Wld]           forward A operand
+  void *SB_hi, *SB_lo;              // [cap][n_wave_pad]    reverse A operand (SEDbar)
+  float4* wconst;                   // [n_wave_pad][2]      {lam, dlam, k0, drude}, {log2(lam/5500), -, -, -}
+  int* plan;                        // [4][plan_cap]: fwd item prefix, first wavelength tile, k-range begin / end (bytes/128)
+  int plan_cap;
+  CUtensorMap mLT_hi, mLT_lo, mLc_hi, mLc_lo, mW_hi, mW_lo, mSB_hi, mSB_lo;
+  FilterConsts fc;
+  int Kpad, Wld, nb, BNb;
+  int64_t cap;
+  int sm_count;
+};
+
+struct GemmArgs {
+  int64_t n;
+  int m_tiles, n_tiles, k_blocks, BN, BK;
+  const int* rows;
+  const int* plan; int plan_cap;
+  float* part;            // forward: [n][5][SPS_MAX_BAND] band sums (atomicAdd)
+  float* Wbar; int ldw;   // reverse
+};
+
+// ---- PTX wrappers ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  while (!ok) {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(map), "r"(bar), "r"(c_inner), "r"(c_outer) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+template <int PREC>
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  if (PREC == SPS_EXACT_BF16X3)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+  else
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// K-major operand tile with 128-byte rows, SWIZZLE_128B: 8-row atoms of 1024 B stacked along M/N (SBO = 1024)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
+  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(1024 >> 4) << 32;
+  d |= (uint64_t)1 << 46;            // descriptor version (sm_100)
+  d |= (uint64_t)2 << 61;            // SWIZZLE_128B
+  return d;
+}
+#define TMEM_LD8(taddr, v)                                                                                             \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"                               \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])        \
+               : "r"(taddr))
+#define TMEM_LD16(taddr, v)                                                                                            \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
+                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
+               : "r"(taddr))
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// exp(-x^2/2) = exp2(-(x * FILT_SCALE)^2)
+#define FILT_SCALE 0.84932180028801907f
+#define FILT_CUT (5.f * FILT_SCALE)
+
+#define FLUSH_PART()                                                                                  \
+  do {                                                                                                \
+    if (cur_m >= 0 && valid) {                                                                        \
+      float* p = G.part + r * 5 * SPS_MAX_BAND;                                                       \
+      _Pragma("unroll") for (int b = 0; b < SPS_MAX_BAND; ++b) {                                      \
+        if (b < T.n_band) {                                                                           \
+          if (s0[b] != 0.f) atomicAdd(p + b, s0[b]);                                                  \
+          if (s1[b] != 0.f) atomicAdd(p + SPS_MAX_BAND + b, s1[b]);                                   \
+          if (s2[b] != 0.f) atomicAdd(p + 2 * SPS_MAX_BAND + b, s2[b]);                               \
+          if (s3[b] != 0.f) atomicAdd(p + 3 * SPS_MAX_BAND + b, s3[b]);                               \
+          if (s4[b] != 0.f) atomicAdd(p + 4 * SPS_MAX_BAND + b, s4[b]);                               \
+        }                                                                                             \
+      }                                                                                               \
+    }                                                                                                 \
+    _Pragma("unroll") for (int b = 0; b < SPS_MAX_BAND; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f; \
+  } while (0)
+
+// Work items.  forward: item w -> (row tile m, wavelength tile nt) through the per-row-tile prefix plan[0][m] and
+// first tile plan[1][m]; reverse: w -> (m, w % n_tiles), k blocks plan[2][m] .. plan[3][m].
+struct ItemCursor {
+  const int* plan; int plan_cap, n_tiles, m;
+  template <int MODE> __device__ __forceinline__ void seek(int w, int& m_out, int& nt, int& kb_lo, int& kb_hi, int k_blocks) {
+    if (MODE == 0) {
+      while (w >= __ldg(plan + m + 1)) ++m;
+      m_out = m; nt = __ldg(plan + plan_cap + m) + (w - __ldg(plan + m)); kb_lo = 0; kb_hi = k_blocks;
+    } else {
+      m_out = w / n_tiles; nt = w - m_out * n_tiles;
+      kb_lo = __ldg(plan + 2 * plan_cap + m_out); kb_hi = __ldg(plan + 3 * plan_cap + m_out);
+    }
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+template <int MODE, int PREC>     // MODE 0: forward with the fused photometry epilogue, 1: reverse with a store epilogue
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constant__ CUtensorMap tmAl,
+                  const __grid_constant__ CUtensorMap tmBh, const __grid_constant__ CUtensorMap tmBl,
+                  TableDev T, RowBuffers B, GemmArgs G, FilterConsts FC, const float4* __restrict__ wconst) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  const uint32_t smem_base = smem_u32(smem);
+  const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+  // barriers: full[s] +0, empty[s] +16, tfull[b] +32, tempty[b] +48 ; tmem pointer +64
+  auto bar_full = [&](int s) { return bar_base + 8u * s; };
+  auto bar_empty = [&](int s) { return bar_base + 16u + 8u * s; };
+  auto bar_tfull = [&](int b) { return bar_base + 32u + 8u * b; };
+  auto bar_tempty = [&](int b) { return bar_base + 48u + 8u * b; };
+  volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + STAGES * STAGE_BYTES + 64);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int total = (MODE == 0) ? __ldg(G.plan + G.m_tiles) : G.m_tiles * G.n_tiles;
+  const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
+  const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
+  const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
+  ItemCursor cur; cur.plan = G.plan; cur.plan_cap = G.plan_cap; cur.n_tiles = G.n_tiles; cur.m = 0;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(bar_tfull(b), 1); mbar_init(bar_tempty(b), EPI_WARPS); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar_base + 64u), "r"(TMEM_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr;
+
+  if (warp == 0) {
+    // ===== TMA producer ==========================================================================
+    if (lane == 0) {
+      const uint32_t tx = 2u * A_TILE_BYTES + 2u * (uint32_t)G.BN * ROW_BYTES;
+      int stage = 0; uint32_t phase = 0;
+      for (int w = w_begin; w < w_end; ++w) {
+        int m, nt, kb_lo, kb_hi;
+        cur.seek<MODE>(w, m, nt, kb_lo, kb_hi, G.k_blocks);
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
+          mbar_wait(bar_empty(stage), phase ^ 1u);
+          const uint32_t sb = smem_base + stage * STAGE_BYTES;
+          mbar_expect_tx(bar_full(stage), tx);
+          tma_load_2d(sb, &tmAh, bar_full(stage), kb * G.BK, m * BM);
+          tma_load_2d(sb + A_TILE_BYTES, &tmAl, bar_full(stage), kb * G.BK, m * BM);
+          tma_load_2d(sb + 2 * A_TILE_BYTES, &tmBh, bar_full(stage), kb * G.BK, nt * G.BN);
+          tma_load_2d(sb + 2 * A_TILE_BYTES + B_TILE_BYTES, &tmBl, bar_full(stage), kb * G.BK, nt * G.BN);
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer ============================================================================
+    if (lane == 0) {
+      // instruction descriptor: D = F32, A and B in the operand format, both K-major, N = BN, M = 128
+      const uint32_t idesc = (1u << 4) | (Op<PREC>::FMT << 7) | (Op<PREC>::FMT << 10) | ((uint32_t)(G.BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      int stage = 0; uint32_t phase = 0; int buf = 0; uint32_t bphase = 0;
+      for (int w = w_begin; w < w_end; ++w) {
+        int m, nt, kb_lo, kb_hi;
+        cur.seek<MODE>(w, m, nt, kb_lo, kb_hi, G.k_blocks);
+        mbar_wait(bar_tempty(buf), bphase ^ 1u);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (uint32_t)buf * BN_MAX;
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
+          mbar_wait(bar_full(stage), phase);
+          tc_fence_after();
+          const uint32_t sb = smem_base + stage * STAGE_BYTES;
+#pragma unroll
+          for (int kk = 0; kk < ROW_BYTES / 32; ++kk) {
+            const uint64_t a_hi = umma_desc(sb + kk * 32), a_lo = umma_desc(sb + A_TILE_BYTES + kk * 32);
+            const uint64_t b_hi = umma_desc(sb + 2 * A_TILE_BYTES + kk * 32);
+            const uint64_t b_lo = umma_desc(sb + 2 * A_TILE_BYTES + B_TILE_BYTES + kk * 32);
+            tc_mma<PREC>(d_tmem, a_lo, b_hi, idesc, (kb > kb_lo || kk > 0) ? 1u : 0u);    // small terms first
+            tc_mma<PREC>(d_tmem, a_hi, b_lo, idesc, 1u);
+            tc_mma<PREC>(d_tmem, a_hi, b_hi, idesc, 1u);
+          }
+          tc_commit(bar_empty(stage));                      // frees the smem stage when these MMAs retire
+          if (kb == kb_hi - 1) tc_commit(bar_tfull(buf));
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+        buf ^= 1; if (buf == 0) bphase ^= 1u;
+      }
+    }
+  } else {
+    // ===== epilogue warps ==========================================================================
+    const int q = warp & 3;                                  // TMEM lane quarter this warp may read
+    const int half = (warp - 2) >> 2;                        // which half of the tile's columns
+    const int row_in_tile = q * 32 + lane;
+    int buf = 0; uint32_t bphase = 0;
+    if (MODE == 0) {
+      constexpr int COLS = BN_MAX / 2;
+      float s0[SPS_MAX_BAND], s1[SPS_MAX_BAND], s2[SPS_MAX_BAND], s3[SPS_MAX_BAND], s4[SPS_MAX_BAND];
+#pragma unroll
+      for (int b = 0; b < SPS_MAX_BAND; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f;
+      int cur_m = -1; int64_t r = 0; bool valid = false;
+      float zp = 1.f, AVs = 0.f, delta = 0.f, Ffl = 1.f, Eb = 0.85f, zp_min = 1.f, zp_max = 1.f;
+      for (int w = w_begin; w < w_end; ++w) {
+        int m, nt, kb_lo, kb_hi;
+        cur.seek<MODE>(w, m, nt, kb_lo, kb_hi, G.k_blocks);
+        if (m != cur_m) {
+          FLUSH_PART();
+          cur_m = m;
+          r = (int64_t)m * BM + row_in_tile;
+          valid = r < G.n;
+          zp = 1.f; AVs = 0.f; delta = 0.f; Ffl = 1.f;
+          if (valid) {
+            const RowScalars sc = B.sc[G.rows ? G.rows[r] : r];
+            zp = 1.f + sc.z; AVs = sc.AV * (1.f / 4.05f); delta = sc.delta; Ffl = sc.Ffloor;
+          }
+          Eb = 0.85f - 1.9f * delta;
+          float lo = valid ? zp : 1e30f, hi = valid ? zp : 0.f;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) { lo = fminf(lo, __shfl_xor_sync(FULL_MASK, lo, o)); hi = fmaxf(hi, __shfl_xor_sync(FULL_MASK, hi, o)); }
+          zp_min = lo; zp_max = hi;
+        }
+        const int n0 = nt * BN_MAX + half * COLS;
+        // bands whose (truncated) support can meet this warp's columns for some of its rows
+        unsigned mask = 0;
+        {
+          const float lam_lo = __ldg(&wconst[2 * n0].x) * zp_min * 0.999999f, lam_hi = __ldg(&wconst[2 * (n0 + COLS - 1)].x) * zp_max * 1.000001f;
+#pragma unroll
+          for (int b = 0; b < SPS_MAX_BAND; ++b)
+            if (b < T.n_band && lam_hi >= FC.lo[b] && lam_lo <= FC.hi[b]) mask |= 1u << b;
+        }
+        mbar_wait(bar_tfull(buf), bphase);
+        tc_fence_after();
+        if (mask != 0) {
+          const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * BN_MAX + half * COLS);
+          for (int c = 0; c < COLS / 8; ++c) {
+            uint32_t v[8];
+            TMEM_LD8(taddr + c * 8, v);
+            tmem_ld_wait();
+            float G0[8], G1[8], G2[8], G3[8], G4[8], lamz[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const int k = n0 + c * 8 + j;
+              const float4 c0 = __ldg(&wconst[2 * k]);
+              const float l2r = __ldg(&wconst[2 * k + 1].x);
+              const float lam = c0.x, dl = c0.y, k0 = c0.z, dr = c0.w;
+              // dust, Eq. (A8)-(A9) with the tabulated k0, Drude profile and log2(lam/lam_V) (R10)
+              const float pw = exp2f(delta * l2r);
+              const float br = fmaf(k0, pw, Eb * dr);
+              float A = AVs * br, A_av = br * (1.f / 4.05f), A_del = AVs * (k0 * pw * l2r * LN2F - 1.9f * dr);
+              if (!(A > 0.f)) { A = 0.f; A_av = 0.f; A_del = 0.f; }
+              const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+              const float dF = -(1.f - Ffl) * 0.4f * LN10F * Tt;
+              const float Sd = __uint_as_float(v[j]) * dl;
+              G0[j] = Sd * fmaf(1.f - Ffl, Tt, Ffl); G1[j] = Sd * dF * A_av; G2[j] = Sd * dF * A_del; G3[j] = Sd * (1.f - Tt);
+              G4[j] = G0[j] * lam; lamz[j] = lam * zp;
+            }
+#pragma unroll
+            for (int b = 0; b < SPS_MAX_BAND; ++b) {
+              if (mask & (1u << b)) {
+                const float isg = FC.isg[b], nmu = FC.nmu[b], dzf = FC.dz[b];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  const float x = fmaf(lamz[j], isg, nmu);
+                  const float Tb = (fabsf(x) <= FILT_CUT) ? exp2f(-x * x) : 0.f;
+                  s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
+                  s4[b] = fmaf(Tb * x, G4[j] * dzf, s4[b]);               // d/dz of T_b(lam (1+z)) = -T x' lam / sigma
+                }
+              }
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_tempty(buf));
+        buf ^= 1; if (buf == 0) bphase ^= 1u;
+      }
+      FLUSH_PART();
+    } else {
+      for (int w = w_begin; w < w_end; ++w) {
+        int m, nt, kb_lo, kb_hi;
+        cur.seek<MODE>(w, m, nt, kb_lo, kb_hi, G.k_blocks);
+        const int64_t r = (int64_t)m * BM + row_in_tile;
+        mbar_wait(bar_tfull(buf), bphase);
+        tc_fence_after();
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)buf * BN_MAX;
+        float* dst = G.Wbar + r * G.ldw + nt * G.BN;
+        for (int c = half; c < G.BN / 16; c += 2) {
+          uint32_t v[16];
+          TMEM_LD16(taddr + c * 16, v);
+          tmem_ld_wait();
+          if (r < G.n) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              reinterpret_cast<float4*>(dst + c * 16)[j] = make_float4(__uint_as_float(v[4 * j]), __uint_as_float(v[4 * j + 1]),
+                                                                      __uint_as_float(v[4 * j + 2]), __uint_as_float(v[4 * j + 3]));
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_tempty(buf));
+        buf ^= 1; if (buf == 0) bphase ^= 1u;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+  }
+}
+
+// ---- plan: per row tile, the wavelength range under some filter's support for the tile's redshifts -------------------
+// plan[0][m] = prefix of forward items, plan[1][m] = first wavelength tile, plan[2][m], plan[3][m] = k-block range (reverse)
+__global__ void __launch_bounds__(256) exact_plan_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
+                                                         int m_tiles, int BKe, int* __restrict__ plan, int plan_cap) {
+  __shared__ int cnt[1024];
+  float obs_lo = 1e30f, obs_hi = 0.f;
+  for (int b = 0; b < T.n_band; ++b) { obs_lo = fminf(obs_lo, FC.lo[b]); obs_hi = fmaxf(obs_hi, FC.hi[b]); }
+  for (int base = 0; base < m_tiles; base += 1024) {
+    for (int m = base + threadIdx.x; m < min(m_tiles, base + 1024); m += blockDim.x) {
+      float zmin = 1e30f, zmax = -1e30f;
+      const int64_t r1 = min(n, (int64_t)(m + 1) * BM);
+      for (int64_t r = (int64_t)m * BM; r < r1; ++r) { const float z = B.sc[rows ? rows[r] : r].z; zmin = fminf(zmin, z); zmax = fmaxf(zmax, z); }
+      const float lo = obs_lo / (1.f + zmax) * 0.99999f, hi = obs_hi / (1.f + zmin) * 1.00001f;
+      int a = 0, c = T.n_wave;
+      while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
+      int k_lo = max(a - 1, 0);
+      a = k_lo; c = T.n_wave;
+      while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= hi) a = mid + 1; else c = mid; }
+      int k_hi = min(a, T.n_wave - 1);                       // inclusive
+      if (k_hi < k_lo) k_hi = k_lo;
+      const int nt_lo = k_lo / BN_MAX, nt_hi = k_hi / BN_MAX + 1;
+      plan[plan_cap + m] = nt_lo;
+      plan[2 * plan_cap + m] = k_lo / BKe;
+      plan[3 * plan_cap + m] = k_hi / BKe + 1;
+      cnt[m - base] = nt_hi - nt_lo;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int acc = (base == 0) ? 0 : plan[base];
+      for (int m = base; m < min(m_tiles, base + 1024); ++m) { plan[m] = acc; acc += cnt[m - base]; }
+      plan[min(m_tiles, base + 1024)] = acc;
+    }
+    __syncthreads();
+  }
+}
+
+// ---- operand generation -----------------------------------------------------------------------------------------
+// forward B operand: LT[k][c] = L[c][k]  (one-time, at table creation)
+template <int PREC>
+__global__ void build_LT_kernel(TableDev T, int Wld, typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  __shared__ float tile[32][33];
+  const int k0 = blockIdx.x * 32, c0 = blockIdx.y * 32;
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    const int c = c0 + i, k = k0 + threadIdx.x;
+    tile[i][threadIdx.x] = (c < T.K && k < T.n_wave) ? T.ssp[(int64_t)c * T.n_wave_pad + k] : 0.f;
+  }
+  __syncthreads();
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    const int k = k0 + i, c = c0 + threadIdx.x;
+    if (k < T.n_wave_pad && c < Wld) Op<PREC>::split(tile[threadIdx.x][i], hi[(int64_t)k * Wld + c], lo[(int64_t)k * Wld + c]);
+  }
+}
+// reverse B operand: Lc[c][k] = L[c][k], zero rows for c >= K
+template <int PREC>
+__global__ void build_Lc_kernel(TableDev T, int rows, typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)rows * T.n_wave_pad) return;
+  const int c = (int)(idx / T.n_wave_pad), k = (int)(idx % T.n_wave_pad);
+  const float v = (c < T.K && k < T.n_wave) ? T.ssp[(int64_t)c * T.n_wave_pad + k] : 0.f;
+  Op<PREC>::split(v, hi[idx], lo[idx]);
+}
+__global__ void build_wconst_kernel(TableDev T, float4* __restrict__ wc) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= T.n_wave_pad) return;
+  wc[2 * k] = make_float4(T.wave[k], T.dlam[k], T.k0[k], T.drude[k]);
+  wc[2 * k + 1] = make_float4(T.l2r[k], 0.f, 0.f, 0.f);
+}
+
+// forward A operand: W[r][ij] = Mn a_i m_j (a5: Eq. 2 and M_star), split
+template <int PREC>
+__global__ void tc_weights_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, int Wld,
+                                  typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  const int64_t r = blockIdx.x;
+  const int64_t row = rows ? rows[r] : r;
+  const float Mn = B.sc[row].Mn;
+  for (int e = threadIdx.x; e < Wld; e += blockDim.x) {
+    float v = 0.f;
+    if (e < T.K) { const int i = e / T.n_Z, j = e - i * T.n_Z; v = Mn * B.a[row * ROW_A_STRIDE + i] * B.m[row * ROW_M_STRIDE + j]; }
+    Op<PREC>::split(v, hi[r * Wld + e], lo[r * Wld + e]);
+  }
+}
+
+// reverse A operand: SEDbar[r][k] = F_att(lam_k) dlam_k sum_b g_b T_b(lam_k (1+z))  (reverse of Eq. 3-4), split.
+// Only the k blocks of the row tile's plan range are written (the reverse GEMM reads nothing else).
+template <int PREC>
+__global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B,
+                                                        const float* __restrict__ gbuf, const float4* __restrict__ wconst,
+                                                        const int* __restrict__ plan, int plan_cap,
+                                                        typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  const int64_t r = blockIdx.x;
+  const int m = (int)(r / BM);
+  const int k_begin = plan[2 * plan_cap + m] * Op<PREC>::BK, k_end = plan[3 * plan_cap + m] * Op<PREC>::BK;
+  __shared__ float g_s[SPS_MAX_BAND];
+  __shared__ float sc_s[4];
+  if (threadIdx.x < SPS_MAX_BAND) g_s[threadIdx.x] = gbuf[r * SPS_MAX_BAND + threadIdx.x];
+  if (threadIdx.x == 32) {
+    const RowScalars sc = B.sc[rows ? rows[r] : r];
+    sc_s[0] = 1.f + sc.z; sc_s[1] = sc.AV; sc_s[2] = sc.delta; sc_s[3] = sc.Ffloor;
+  }
+  __syncthreads();
+  for (int k = k_begin + threadIdx.x; k < k_end; k += 256) {
+    const float4 c0 = __ldg(&wconst[2 * k]);
+    float v = 0.f;
+    if (c0.y > 0.f) {
+      const float lamz = c0.x * sc_s[0];
+      float tsum = 0.f;
+      for (int b = 0; b < T.n_band; ++b) {
+        const float x = (lamz - T.filt_mu[b]) / T.filt_sigma[b];
+        if (fabsf(x) <= 5.f) tsum += g_s[b] * expf(-0.5f * x * x);
+      }
+      if (tsum != 0.f) {
+        const float l2r = __ldg(&wconst[2 * k + 1].x);
+        const float delta = sc_s[2], Ffl = sc_s[3];
+        const float pw = exp2f(delta * l2r);
+        float A = sc_s[1] * (1.f / 4.05f) * (c0.z * pw + (0.85f - 1.9f * delta) * c0.w);
+        if (!(A > 0.f)) A = 0.f;
+        const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+        v = (Ffl + (1.f - Ffl) * Tt) * c0.y * tsum;
+      }
+    }
+    const int64_t o = r * T.n_wave_pad + k;
+    Op<PREC>::split(v, hi[o], lo[o]);
+  }
+}
+
+// ---- host side --------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+sps_status get_encoder() {
+  if (g_encode) return SPS_OK;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    sps_set_error("cuTensorMapEncodeTiled is not available from this driver");
+    return SPS_EUNSUPPORTED;
+  }
+  g_encode = (EncodeTiledFn)fn;
+  return SPS_OK;
+}
+
+// [rows][cols] row-major with pitch `ld` elements -> tiles of box_rows x 128 bytes, 128-byte swizzle
+sps_status make_map(const TcState* S, CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+  const cuuint64_t dims[2] = {cols, rows};
+  const cuuint64_t strides[1] = {ld * (uint64_t)S->es};
+  const cuuint32_t box[2] = {(cuuint32_t)S->BK, box_rows};
+  const cuuint32_t es[2] = {1, 1};
+  const CUresult r = g_encode(m, S->prec == SPS_EXACT_BF16X3 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                              const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { sps_set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return SPS_ECUDA; }
+  return SPS_OK;
+}
+
+void free_row_operands(TcState* S) {
+  void* ptrs[] = {S->W_hi, S->W_lo, S->SB_hi, S->SB_lo, S->plan};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  S->W_hi = S->W_lo = S->SB_hi = S->SB_lo = nullptr; S->plan = nullptr; S->cap = 0; S->plan_cap = 0;
+}
+
+template <int PREC>
+sps_status build_tables(const TableDev& T, TcState* S, size_t lc_rows) {
+  typedef typename Op<PREC>::T E;
+  const size_t lc_n = lc_rows * T.n_wave_pad;
+  build_LT_kernel<PREC><<<dim3((T.n_wave_pad + 31) / 32, (S->Wld + 31) / 32), dim3(32, 8)>>>(T, S->Wld, (E*)S->LT_hi, (E*)S->LT_lo);
+  build_Lc_kernel<PREC><<<(unsigned)((lc_n + 255) / 256), 256>>>(T, (int)lc_rows, (E*)S->Lc_hi, (E*)S->Lc_lo);
+  build_wconst_kernel<<<(T.n_wave_pad + 255) / 256, 256>>>(T, S->wconst);
+  sps_count_launch(3);
+  sps_status st = sps_check_cuda(cudaDeviceSynchronize(), "tensor-core operand build");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<1, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  return st;
+}
+
+template <int PREC>
+sps_status launch_forward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
+  typedef typename Op<PREC>::T E;
+  ExactState* X = t->exact; const TableDev& T = t->dev;
+  tc_weights_kernel<PREC><<<(unsigned)n, 128, 0, s>>>(T, n, rows, t->rows, S->Wld, (E*)S->W_hi, (E*)S->W_lo);
+  GemmArgs G; memset(&G, 0, sizeof(G));
+  G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = T.n_wave_pad / BN_MAX; G.k_blocks = S->Kpad / S->BK; G.BN = BN_MAX; G.BK = S->BK;
+  G.rows = rows; G.part = X->part; G.plan = S->plan; G.plan_cap = S->plan_cap;
+  exact_plan_kernel<<<1, 256, 0, s>>>(T, n, rows, t->rows, S->fc, G.m_tiles, S->BK, S->plan, S->plan_cap);
+  const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  exact_gemm_kernel<0, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+  sps_count_launch(3);
+  return sps_check_cuda(cudaGetLastError(), "exact forward (tcgen05) launch");
+}
+
+template <int PREC>
+sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
+  typedef typename Op<PREC>::T E;
+  ExactState* X = t->exact; const TableDev& T = t->dev;
+  tc_sedbar_kernel<PREC><<<(unsigned)n, 256, 0, s>>>(T, n, rows, t->rows, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
+  GemmArgs G; memset(&G, 0, sizeof(G));
+  G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = S->nb; G.k_blocks = T.n_wave_pad / S->BK; G.BN = S->BNb; G.BK = S->BK;
+  G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
+  const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  exact_gemm_kernel<1, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mSB_hi, S->mSB_lo, S->mLc_hi, S->mLc_lo, T, t->rows, G, S->fc, S->wconst);
+  sps_count_launch(2);
+  return sps_check_cuda(cudaGetLastError(), "exact reverse (tcgen05) launch");
+}
+
+}  // namespace
+
+static int g_disable_tc = 0;
+extern "C" void sps_debug_disable_tc(int on) { g_disable_tc = on; }
+
+sps_status sps_exact_tc_setup(sps_table* t, int precision) {
+  ExactState* X = t->exact;
+  X->use_tc = false; X->tc = nullptr;
+  if (g_disable_tc) return SPS_OK;
+  if (precision != SPS_EXACT_TF32X3 && precision != SPS_EXACT_BF16X3) { sps_set_error("exact_precision must be SPS_EXACT_TF32X3 or SPS_EXACT_BF16X3"); return SPS_EINVAL; }
+  sps_status st = get_encoder();
+  if (st != SPS_OK) return st;
+  const TableDev& T = t->dev;
+  TcState* S = new TcState();
+  memset(S, 0, sizeof(*S));
+  S->prec = precision; S->es = precision == SPS_EXACT_BF16X3 ? 2 : 4; S->BK = ROW_BYTES / S->es;
+  S->Kpad = (T.K + 63) / 64 * 64;
+  S->nb = (S->Kpad + BN_MAX - 1) / BN_MAX;
+  S->BNb = ((S->Kpad + S->nb - 1) / S->nb + 15) / 16 * 16;
+  S->Wld = (std::max(S->Kpad, S->nb * S->BNb) + 63) / 64 * 64;
+  int dev = 0; cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&S->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  for (int b = 0; b < SPS_MAX_BAND; ++b) {
+    const float mu = b < T.n_band ? T.filt_mu[b] : 1.f, sg = b < T.n_band ? T.filt_sigma[b] : 1.f;
+    S->fc.isg[b] = FILT_SCALE / sg; S->fc.nmu[b] = -mu * (FILT_SCALE / sg);
+    S->fc.dz[b] = -1.f / (sg * FILT_SCALE);
+    S->fc.lo[b] = mu - 5.f * sg; S->fc.hi[b] = mu + 5.f * sg;
+  }
+  const size_t lt_n = (size_t)T.n_wave_pad * S->Wld, lc_rows = (size_t)S->nb * S->BNb, lc_n = lc_rows * T.n_wave_pad;
+  cudaError_t e = cudaMalloc(&S->LT_hi, lt_n * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->LT_lo, lt_n * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->Lc_hi, lc_n * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->Lc_lo, lc_n * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->wconst, (size_t)T.n_wave_pad * 2 * sizeof(float4));
+  X->tc = S;
+  if (e != cudaSuccess) { sps_exact_tc_teardown(t); return sps_check_cuda(e, "tensor-core operand allocation"); }
+  st = precision == SPS_EXACT_BF16X3 ? build_tables<SPS_EXACT_BF16X3>(T, S, lc_rows) : build_tables<SPS_EXACT_TF32X3>(T, S, lc_rows);
+  if (st == SPS_OK) st = make_map(S, &S->mLT_hi, S->LT_hi, T.n_wave_pad, S->Wld, S->Wld, BN_MAX);
+  if (st == SPS_OK) st = make_map(S, &S->mLT_lo, S->LT_lo, T.n_wave_pad, S->Wld, S->Wld, BN_MAX);
+  if (st == SPS_OK) st = make_map(S, &S->mLc_hi, S->Lc_hi, lc_rows, T.n_wave_pad, T.n_wave_pad, S->BNb);
+  if (st == SPS_OK) st = make_map(S, &S->mLc_lo, S->Lc_lo, lc_rows, T.n_wave_pad, T.n_wave_pad, S->BNb);
+  if (st != SPS_OK) { sps_exact_tc_teardown(t); return st; }
+  X->ldw = S->Wld;
+  X->use_tc = true;
+  return SPS_OK;
+}
+
+void sps_exact_tc_teardown(sps_table* t) {
+  ExactState* X = t->exact;
+  if (!X || !X->tc) return;
+  TcState* S = (TcState*)X->tc;
+  free_row_operands(S);
+  void* ptrs[] = {S->LT_hi, S->LT_lo, S->Lc_hi, S->Lc_lo, S->wconst};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  delete S;
+  X->tc = nullptr; X->use_tc = false;
+}
+
+// row-side operand buffers for `cap` rows (cap is a multiple of 128); called when the exact scratch grows
+sps_status sps_exact_tc_ensure(sps_table* t, int64_t cap) {
+  ExactState* X = t->exact;
+  if (!X->use_tc) return SPS_OK;
+  TcState* S = (TcState*)X->tc;
+  if (S->cap >= cap) return SPS_OK;
+  free_row_operands(S);
+  const TableDev& T = t->dev;
+  const size_t wn = (size_t)cap * S->Wld, sn = (size_t)cap * T.n_wave_pad;
+  S->plan_cap = (int)(cap / BM) + 2;
+  cudaError_t e = cudaMalloc(&S->W_hi, wn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->W_lo, wn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->SB_hi, sn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->SB_lo, sn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&S->plan, (size_t)4 * S->plan_cap * sizeof(int));
+  if (e != cudaSuccess) { free_row_operands(S); return sps_check_cuda(e, "tensor-core row operand allocation"); }
+  cudaMemset(S->W_hi, 0, wn * S->es); cudaMemset(S->W_lo, 0, wn * S->es);
+  cudaMemset(S->SB_hi, 0, sn * S->es); cudaMemset(S->SB_lo, 0, sn * S->es);
+  S->cap = cap;
+  sps_status st = make_map(S, &S->mW_hi, S->W_hi, cap, S->Wld, S->Wld, BM);
+  if (st == SPS_OK) st = make_map(S, &S->mW_lo, S->W_lo, cap, S->Wld, S->Wld, BM);
+  if (st == SPS_OK) st = make_map(S, &S->mSB_hi, S->SB_hi, cap, T.n_wave_pad, T.n_wave_pad, BM);
+  if (st == SPS_OK) st = make_map(S, &S->mSB_lo, S->SB_lo, cap, T.n_wave_pad, T.n_wave_pad, BM);
+  return st;
+}
+
+sps_status sps_exact_tc_forward(sps_table* t, int64_t n, const int* rows, cudaStream_t s) {
+  TcState* S = (TcState*)t->exact->tc;
+  return S->prec == SPS_EXACT_BF16X3 ? launch_forward<SPS_EXACT_BF16X3>(t, S, n, rows, s) : launch_forward<SPS_EXACT_TF32X3>(t, S, n, rows, s);
+}
+
+sps_status sps_exact_tc_backward(sps_table* t, int64_t n, const int* rows, cudaStream_t s) {
+  TcState* S = (TcState*)t->exact->tc;
+  return S->prec == SPS_EXACT_BF16X3 ? launch_backward<SPS_EXACT_BF16X3>(t, S, n, rows, s) : launch_backward<SPS_EXACT_TF32X3>(t, S, n, rows, s);
+}

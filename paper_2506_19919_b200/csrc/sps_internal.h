@@ -18,7 +18,7 @@ void sps_free_row_buffers(sps_table* t);
 sps_status sps_prior_to_dev(const sps_prior* p, PriorDev& out);
 
 // exact path (sps_exact.cu)
-sps_status sps_exact_setup(sps_table* t);
+sps_status sps_exact_setup(sps_table* t, int precision);
 void sps_exact_teardown(sps_table* t);
 // flux + (optional) reverse pass over the SSP table for rows whose prologue has run:
 // fills B.flux, B.sc[*].logp_like and, if want_grad, B.a_bar, B.m_bar and the scalar bars.
