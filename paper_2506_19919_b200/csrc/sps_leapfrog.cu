@@ -15,19 +15,24 @@ sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n
   sps_status st = sps_check_cuda(cudaMalloc(&Q.gal_of_chain, Q.n * sizeof(int)), "gal_of_chain allocation");
   if (st != SPS_OK) return st;
   gal_of_chain_kernel<<<(unsigned)((Q.n + 255) / 256), 256>>>(Q.gal_of_chain, Q.n, cfg->n_chain); sps_count_launch();
+  st = sps_check_cuda(cudaMalloc(&Q.path_of_chain, Q.n), "path_of_chain allocation");
+  if (st != SPS_OK) return st;
   if (!path_of_gal_dev) {
     if (cfg->path != SPS_PATH_EXACT && cfg->path != SPS_PATH_APPROX) { sps_set_error("bad path"); return SPS_EINVAL; }
     Q.n_rows_path[cfg->path] = Q.n;
+    cudaMemset(Q.path_of_chain, cfg->path, Q.n);
     return SPS_OK;
   }
   std::vector<int32_t> pg(n_gal);
   st = sps_check_cuda(cudaMemcpy(pg.data(), path_of_gal_dev, n_gal * sizeof(int32_t), cudaMemcpyDeviceToHost), "path_of_gal D2H");
   if (st != SPS_OK) return st;
   std::vector<int> rows[2];
+  std::vector<unsigned char> pc(Q.n);
   for (int64_t g = 0; g < n_gal; ++g) {
     if (pg[g] != 0 && pg[g] != 1) { sps_set_error("path_of_gal[%lld] = %d is not 0/1", (long long)g, pg[g]); return SPS_EINVAL; }
-    for (int k = 0; k < cfg->n_chain; ++k) rows[pg[g]].push_back((int)(g * cfg->n_chain + k));
+    for (int k = 0; k < cfg->n_chain; ++k) { rows[pg[g]].push_back((int)(g * cfg->n_chain + k)); pc[g * cfg->n_chain + k] = (unsigned char)pg[g]; }
   }
+  cudaMemcpy(Q.path_of_chain, pc.data(), Q.n, cudaMemcpyHostToDevice);
   for (int p = 0; p < 2; ++p) {
     Q.n_rows_path[p] = (int64_t)rows[p].size();
     if (rows[p].empty()) continue;
@@ -40,6 +45,7 @@ sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n
 
 void hmc_problem_free(HmcProblem& Q) {
   if (Q.gal_of_chain) cudaFree(Q.gal_of_chain);
+  if (Q.path_of_chain) cudaFree(Q.path_of_chain);
   for (int p = 0; p < 2; ++p) if (Q.rows_path[p]) cudaFree(Q.rows_path[p]);
   memset(&Q, 0, sizeof(Q));
 }

@@ -29,6 +29,7 @@ struct AdaptFlags { int warmup, in_window, window_end, last_warmup, welford_n; f
 struct HmcProblem {
   int64_t n;                 // chains
   int* gal_of_chain;         // [n] device
+  unsigned char* path_of_chain;   // [n] device: photometry path of each chain
   int* rows_path[2];         // device index lists per path, or NULL = all rows
   int64_t n_rows_path[2];
   const float *obs_flux, *obs_sigma;

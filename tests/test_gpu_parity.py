@@ -266,6 +266,52 @@ def test_hmc_warmup_adaptation_statistics(tiny):
     assert np.isfinite(got["rhat"]).all() and (got["n_leapfrog"] == 250 * 8).all()
 
 
+# ---- a13: NUTS against the oracle under the shared counter-based RNG stream (R15) ------------------------------
+def test_nuts_matches_oracle(tiny):
+    # Several trees are "correct" once fp32 and fp64 decisions split, so what is unique is compared: while a chain
+    # stays coupled its states, tree sizes and accept statistics agree; the first transitions agree for every chain.
+    cx = tiny
+    n_gal, n_chain, n_sample, depth, eps0, seed = 4, 2, 25, 5, 0.004, 11
+    truth_u, d, s = _observations(cx, n_gal, 51, frac=(0.05, 0.05))
+    out = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), sampler=cx.sps.SAMPLER_NUTS, path=cx.sps.PATH_APPROX, n_chain=n_chain,
+                             n_warmup=0, n_sample=n_sample, max_depth=depth, eps0=eps0, seed=seed, keep_samples=True)
+    got = {k: v.cpu().numpy() for k, v in out.items()}
+    ref_s, ref_n, ref_a = [], [], []
+    for g in range(n_gal):                                           # the oracle's NUTS evaluates one chain at a time
+        ids = np.arange(g * n_chain, (g + 1) * n_chain)
+        f = lambda th, g=g: M.logp_and_grad(th, cx.grid, cx.P, d[g:g + 1].astype(np.float64), s[g:g + 1].astype(np.float64), "approx", cx.cssp())[:2]
+        r = S.run_chains(S.init_chains(cx.P, seed, ids, 13), f, seed, 0, n_sample, eps0, "nuts", max_depth=depth, chain_ids=ids)
+        ref_s.append(r["samples"]); ref_n.append(r["n_leapfrog_total"]); ref_a.append(r["accept"])
+    ref_s, ref_n, ref_a = np.concatenate(ref_s), np.concatenate(ref_n), np.concatenate(ref_a)
+    err = (np.abs(got["samples"] - ref_s) / np.maximum(1.0, np.abs(ref_s))).max(2)          # [chain, transition]
+    assert err[:, :5].max() <= 1e-3
+    coupled = err.max(1) <= 1e-2
+    assert coupled.mean() >= 0.75
+    assert (got["n_leapfrog"][coupled] == ref_n[coupled]).all()
+    assert np.abs(got["accept"] - ref_a)[coupled].max() <= 1e-3
+    assert (got["divergences"] == 0).all()
+
+
+def test_nuts_warmup_and_hmc_agree(tiny):
+    # HMC and NUTS give "very similar contours" on the same target.  Pooled over chains; loose (short runs).
+    cx = tiny
+    n_gal = 4
+    _, d, s = _observations(cx, n_gal, 51, frac=(0.05, 0.05))
+    res = {}
+    for name, smp, kw in (("nuts", cx.sps.SAMPLER_NUTS, dict(max_depth=6)), ("hmc", cx.sps.SAMPLER_HMC, dict(n_leapfrog=24))):
+        o = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), sampler=smp, path=cx.sps.PATH_APPROX, n_chain=16, n_warmup=300, n_sample=400,
+                               eps0=0.004, seed=5, keep_samples=True, **kw)
+        res[name] = {k: v.cpu().numpy() for k, v in o.items()}
+        assert np.isfinite(res[name]["samples"]).all()
+    a = res["nuts"]["accept"].mean()
+    assert 0.6 < a < 0.99
+    assert (res["nuts"]["n_leapfrog"] >= 700).all() and (res["nuts"]["n_leapfrog"] <= 700 * 63).all()
+    sn = res["nuts"]["samples"].reshape(n_gal, -1, 13); sh = res["hmc"]["samples"].reshape(n_gal, -1, 13)
+    sd = 0.5 * (sn.std(1) + sh.std(1))
+    # the well-constrained direction (logM) agrees within half a posterior sd between the samplers
+    assert (np.abs(sn.mean(1) - sh.mean(1))[:, 0] <= 0.5 * sd[:, 0] + 0.02).all()
+
+
 # ---- a6/a8/a10: exact path ---------------------------------------------------------------------------
 @pytest.mark.parametrize("kind,n", [("tiny", 200), ("full", 24)])
 def test_exact_flux_and_jacobian(kind, n, request, exact_kernels):
