@@ -72,7 +72,7 @@ sps_status sps_require_device() {
 
 void sps_free_row_buffers(sps_table* t) {
   RowBuffers& B = t->rows;
-  void* ptrs[] = {B.a, B.m, B.a_bar, B.m_bar, B.sc, B.flux};
+  void* ptrs[] = {B.a, B.m, B.a_bar, B.m_bar, B.sc, B.flux, B.part, B.order, B.bins};
   for (void* p : ptrs) if (p) cudaFree(p);
   B = RowBuffers();
 }
@@ -91,6 +91,9 @@ sps_status sps_ensure_row_buffers(sps_table* t, int64_t n) {
   al((void**)&B.m_bar, cap * ROW_M_STRIDE * sizeof(float));
   al((void**)&B.sc, cap * sizeof(RowScalars));
   al((void**)&B.flux, cap * SPS_MAX_BAND * sizeof(float));
+  al((void**)&B.part, cap * ROW_PARTS * ROW_A_STRIDE * sizeof(float));
+  al((void**)&B.order, cap * sizeof(int));
+  al((void**)&B.bins, 4 * (size_t)(t->dev.n_z + 1) * sizeof(int));
   if (e != cudaSuccess) { sps_free_row_buffers(t); return sps_check_cuda(e, "row scratch allocation"); }
   B.capacity = cap;
   return SPS_OK;
@@ -114,7 +117,7 @@ sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* thet
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
                     cudaStream_t s) {
   const TableDev& T = t->dev;
-  launch_prologue(T, P, theta, n, unbounded, rows, t->rows, s);
+  launch_prologue(T, P, theta, n, unbounded, want_grad, rows, t->rows, s);
   if (path == SPS_PATH_APPROX) {
     launch_approx_contract(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, t->rows, s);
   } else {
@@ -137,7 +140,7 @@ extern "C" sps_status sps_weights(const sps_table* tc, const sps_prior* prior, c
   PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
   st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
   cudaStream_t s = (cudaStream_t)stream;
-  launch_prologue(t->dev, P, theta, n, unbounded != 0, nullptr, t->rows, s);
+  launch_prologue(t->dev, P, theta, n, unbounded != 0, false, nullptr, t->rows, s);
   launch_copy_weights(t->dev, n, t->rows, w_age, w_met, mstar, s);
   return sps_check_cuda(cudaGetLastError(), "sps_weights launch");
 }

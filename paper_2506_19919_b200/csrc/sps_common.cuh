@@ -65,7 +65,8 @@ struct RowScalars {           // 16 floats
   float Mn_bar;               // d logL / d Mn
   float z_bar;                // direct d logL / d z (table interpolation + dust at lambda_eff/(1+z) or filter shift)
   float AV_bar, delta_bar, Ffloor_bar;
-  float pad0, pad1, pad2;
+  float Msum;                 // int_0^t_obs f dt for M_formed = 1 (Eq. A3), kept for the reverse pass
+  float pad1, pad2;
 };
 
 // ---------------------------------------------------------------------------------------------

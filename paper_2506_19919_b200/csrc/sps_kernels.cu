@@ -1,11 +1,11 @@
 // sps_kernels.cu -- prologue (a0-a5), approximate-photometry contraction (a7, a9, a10) and
-// epilogue (reverse of a0-a5 + prior) kernels.  One warp per parameter row.
+// epilogue (reverse of a0-a5 + prior) kernels.
 #include "sps_rows.cuh"
 
 #define WARPS_PER_BLOCK 8
 
 // ---------------------------------------------------------------------------------------------
-// Forward model of one row: everything a0-a5 needs, held per lane.
+// Forward model of one row (one warp per parameter row): everything a0-a5 needs, held per lane.
 // ---------------------------------------------------------------------------------------------
 struct RowFwd {
   float th[SPS_NDIM], dth[SPS_NDIM];
@@ -31,6 +31,9 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorDev& P
   met_bin(T, R.th[7], R.th[8], R.m, R.dm_lz, R.dm_s);
 }
 
+// a0-a5.  With WANT_GRAD the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
+// kept in B.part for the epilogue, which then has no quadrature to redo.
+template <bool WANT_GRAD>
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
                 const int* __restrict__ rows, RowBuffers B) {
@@ -39,12 +42,17 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
   RowFwd R;
-  row_forward<false>(T, P, theta + row * SPS_NDIM, unbounded, R);
+  row_forward<WANT_GRAD>(T, P, theta + row * SPS_NDIM, unbounded, R);
   const float Fb = R.th[4], inv_M = 1.f / R.Msum;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     const int i = l + 32 * q;
-    if (i < ROW_A_STRIDE) B.a[row * ROW_A_STRIDE + i] = (i < T.n_age) ? (1.f - Fb) * R.Q.dM[q] * inv_M + Fb * R.Bq.P[q] : 0.f;  // Eq. (A6)
+    B.a[row * ROW_A_STRIDE + i] = (i < T.n_age) ? (1.f - Fb) * R.Q.dM[q] * inv_M + Fb * R.Bq.P[q] : 0.f;  // Eq. (A6)
+    if (WANT_GRAD) {
+      float* p = B.part + row * (ROW_PARTS * ROW_A_STRIDE) + i;
+      p[0] = R.Q.dM[q]; p[ROW_A_STRIDE] = R.Q.g_tau[q]; p[2 * ROW_A_STRIDE] = R.Q.g_al[q];
+      p[3 * ROW_A_STRIDE] = R.Q.g_be[q]; p[4 * ROW_A_STRIDE] = R.Q.g_t[q];
+    }
   }
   if (l < ROW_M_STRIDE) B.m[row * ROW_M_STRIDE + l] = R.m;
   if (l == 0) {
@@ -56,142 +64,283 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     sc.z = z; sc.zbin = (int)zi; sc.zfrac = (z - (T.z_min + zi * T.dz)) * T.inv_dz;
     sc.AV = R.th[9]; sc.delta = R.th[10]; sc.Ffloor = R.th[11];
     sc.logp_like = 0.f; sc.Mn_bar = sc.z_bar = sc.AV_bar = sc.delta_bar = sc.Ffloor_bar = 0.f;
-    sc.pad0 = sc.pad1 = sc.pad2 = 0.f;
+    sc.Msum = R.Msum; sc.pad1 = sc.pad2 = 0.f;
     B.sc[row] = sc;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// a7 + a9 + a10: approximate photometry (Eq. 6) fused with the Gaussian likelihood
-// and the reverse pass over the c_SSP table.  v0: one warp per row, the two z-slices are read from
-// L2; lane l owns the entries e = 4l..4l+3 of a slice row (e = j*n_band + b).
-//   pass 1:  Q^(s)_e = sum_i a_i c^(s)[i][e]            (s = 0: c_t, s = 1: D_t = c_{t+1} - c_t)
-//   S^(s)_b = sum_j m_j Q^(s)_{jb};  flux_b = F_att,b Mn [S^(0)_b + f S^(1)_b]
-//   g_b = d logL / d flux_b = -(flux_b - d_b)/sigma_b^2   (or the caller's flux_bar)
-//   pass 2:  a_bar_i = sum_e [v^(0)_e c^(0)[i][e] + v^(1)_e c^(1)[i][e]],  v^(s)_e = g_b F_b Mn {1, f} m_j
+// Grouping of the rows of a call by z cell (counting sort): rows of one cell share the two c_SSP arrays c_t, D_t
+// (PAPER.md:87), so a CTA stages them in shared memory once for up to AC_ROWS_PER_CTA rows.
+// bins[0][.] histogram, bins[1][.] first position of each cell in `order`, bins[2][.] first CTA of each cell,
+// bins[3][.] scatter cursors.
 // ---------------------------------------------------------------------------------------------
-struct ApproxSmem {
-  float a[ROW_A_STRIDE];
-  float Q0[128], Q1[128];
-  float m[ROW_M_STRIDE], sbar[SPS_MAX_BAND];
-};
+#define AC_WARPS 8
+#define AC_R 8                                   // rows per warp, register-blocked
+#define AC_ROWS_PER_CTA (AC_WARPS * AC_R)
 
-__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
-approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ rows, const int* __restrict__ gal_of_row,
-                       const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
-                       const float* __restrict__ flux_bar, bool want_grad, RowBuffers B) {
-  __shared__ ApproxSmem smem_all[WARPS_PER_BLOCK];
-  const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
-  if (r >= n) return;
-  const int64_t row = rows ? rows[r] : r;
-  ApproxSmem& S = smem_all[threadIdx.x >> 5];
-  const int l = lane_id();
-  const int E = T.n_Z * T.n_band;
-  RowScalars sc = B.sc[row];
-#pragma unroll
-  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) S.a[l + 32 * q] = B.a[row * ROW_A_STRIDE + l + 32 * q];
-  if (l < ROW_M_STRIDE) S.m[l] = B.m[row * ROW_M_STRIDE + l];
-  __syncwarp();
-  const float* c0p = T.cssp + ((int64_t)sc.zbin * 2 * T.n_age) * T.cs_stride + 4 * l;     // c_t, then D_t
-  const float* c1p = c0p + (int64_t)T.n_age * T.cs_stride;
-  const bool act = 4 * l < T.cs_stride;
-  float4 q0 = make_float4(0, 0, 0, 0), q1 = make_float4(0, 0, 0, 0);
-  if (act) {
-#pragma unroll 4
-    for (int i = 0; i < T.n_age; ++i) {
-      const float4 c0 = __ldg(reinterpret_cast<const float4*>(c0p + (int64_t)i * T.cs_stride));
-      const float4 c1 = __ldg(reinterpret_cast<const float4*>(c1p + (int64_t)i * T.cs_stride));
-      const float ai = S.a[i];
-      q0.x += ai * c0.x; q0.y += ai * c0.y; q0.z += ai * c0.z; q0.w += ai * c0.w;
-      q1.x += ai * c1.x; q1.y += ai * c1.y; q1.z += ai * c1.z; q1.w += ai * c1.w;
+__global__ void approx_hist_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) atomicAdd(&hist[B.sc[rows ? rows[i] : i].zbin], 1);
+}
+__global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restrict__ bins) {
+  __shared__ int s_rows[1024], s_ctas[1024];
+  const int stride = nb + 2;
+  int* hist = bins; int* row_start = bins + stride; int* cta_start = bins + 2 * stride; int* cursor = bins + 3 * stride;
+  const int t = threadIdx.x;
+  int carry_r = 0, carry_c = 0;
+  for (int base = 0; base < nb; base += 1024) {
+    const int b = base + t;
+    const int cnt = b < nb ? hist[b] : 0, ctas = (cnt + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA;
+    s_rows[t] = cnt; s_ctas[t] = ctas;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+      const int a = t >= o ? s_rows[t - o] : 0, c = t >= o ? s_ctas[t - o] : 0;
+      __syncthreads();
+      s_rows[t] += a; s_ctas[t] += c;
+      __syncthreads();
     }
+    if (b < nb) { row_start[b] = carry_r + s_rows[t] - cnt; cursor[b] = carry_r + s_rows[t] - cnt; cta_start[b] = carry_c + s_ctas[t] - ctas; }
+    carry_r += s_rows[1023]; carry_c += s_ctas[1023];
+    __syncthreads();
   }
-  reinterpret_cast<float4*>(S.Q0)[l] = q0;
-  reinterpret_cast<float4*>(S.Q1)[l] = q1;
-  __syncwarp();
-  // per-band quantities on lanes b < n_band
-  const float f = sc.zfrac;
-  float S0 = 0.f, S1 = 0.f, F = 1.f, F_av = 0.f, F_del = 0.f, F_fl = 0.f, F_lam = 0.f, lam_r = 1.f, g = 0.f, flux = 0.f;
-  float chi2 = 0.f;
-  const bool isb = l < T.n_band;
-  if (isb) {
-    for (int j = 0; j < T.n_Z; ++j) { S0 += S.m[j] * S.Q0[j * T.n_band + l]; S1 += S.m[j] * S.Q1[j * T.n_band + l]; }
-    lam_r = T.lam_eff[l] / (1.f + sc.z);
-    dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
-    const float Sint = S0 + f * S1;
-    flux = F * sc.Mn * Sint;
-    B.flux[row * SPS_MAX_BAND + l] = flux;
-    if (flux_bar) g = flux_bar[row * T.n_band + l];
-    else {
-      const int64_t gal = gal_of_row ? gal_of_row[row] : row;
-      const float d = obs_flux[gal * T.n_band + l], sg = obs_sigma[gal * T.n_band + l];
-      const float rr = (flux - d) / sg;
-      chi2 = rr * rr;
-      g = -rr / sg;
-    }
-  }
-  chi2 = warp_sum(chi2);
-  if (!want_grad) {
-    if (l == 0) B.sc[row].logp_like = -0.5f * chi2;
-    return;
-  }
-  {
-    const float Sint = S0 + f * S1;
-    float Mn_bar = warp_sum(isb ? g * F * Sint : 0.f);
-    float z_bar = warp_sum(isb ? g * (F * sc.Mn * S1 * T.inv_dz + sc.Mn * Sint * F_lam * (-lam_r / (1.f + sc.z))) : 0.f);
-    float av_bar = warp_sum(isb ? g * sc.Mn * Sint * F_av : 0.f);
-    float del_bar = warp_sum(isb ? g * sc.Mn * Sint * F_del : 0.f);
-    float fl_bar = warp_sum(isb ? g * sc.Mn * Sint * F_fl : 0.f);
-    if (l == 0) {
-      sc.logp_like = -0.5f * chi2; sc.Mn_bar = Mn_bar; sc.z_bar = z_bar;
-      sc.AV_bar = av_bar; sc.delta_bar = del_bar; sc.Ffloor_bar = fl_bar;
-      B.sc[row] = sc;
-    }
-    if (isb) S.sbar[l] = g * F * sc.Mn;
-  }
-  __syncwarp();
-  // m_bar_j
-  if (l < ROW_M_STRIDE) {
-    float mb = 0.f;
-    if (l < T.n_Z)
-      for (int b = 0; b < T.n_band; ++b) mb += S.sbar[b] * (S.Q0[l * T.n_band + b] + f * S.Q1[l * T.n_band + b]);
-    B.m_bar[row * ROW_M_STRIDE + l] = mb;
-  }
-  // v quads
-  float v0[4], v1[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    const int e = 4 * l + k;
-    float v = 0.f;
-    if (e < E) { const int j = e / T.n_band, b = e - j * T.n_band; v = S.sbar[b] * S.m[j]; }
-    v0[k] = v; v1[k] = f * v;
-  }
-  // pass 2
-  float abar[SPS_AGE_PER_LANE] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-  for (int qq = 0; qq < SPS_AGE_PER_LANE; ++qq) {
-    const int i0 = 32 * qq;
-    float keep = 0.f;
-    const int i1 = min(32, T.n_age - i0);
-    for (int ii = 0; ii < i1; ++ii) {
-      float part = 0.f;
-      if (act) {
-        const float4 c0 = __ldg(reinterpret_cast<const float4*>(c0p + (int64_t)(i0 + ii) * T.cs_stride));
-        const float4 c1 = __ldg(reinterpret_cast<const float4*>(c1p + (int64_t)(i0 + ii) * T.cs_stride));
-        part = v0[0] * c0.x + v0[1] * c0.y + v0[2] * c0.z + v0[3] * c0.w + v1[0] * c1.x + v1[1] * c1.y + v1[2] * c1.z + v1[3] * c1.w;
-      }
-      part = warp_sum(part);
-      if (l == ii) keep = part;
-    }
-    abar[qq] = keep;
-  }
-#pragma unroll
-  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) B.a_bar[row * ROW_A_STRIDE + l + 32 * q] = abar[q];
+  if (t == 0) { row_start[nb] = carry_r; cta_start[nb] = carry_c; }
+}
+__global__ void approx_scatter_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ cursor, int* __restrict__ order) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int row = rows ? rows[i] : (int)i;
+  order[atomicAdd(&cursor[B.sc[row].zbin], 1)] = row;
 }
 
 // ---------------------------------------------------------------------------------------------
-// Reverse of a0-a5 (a10) + skew-normal prior (a9): one warp per row recomputes the quadratures with
-// their parameter partials and contracts them with a_bar, m_bar, Mn_bar and the direct bars.
+// a7 + a9 + a10: approximate photometry (Eq. 6) fused with the Gaussian likelihood and the reverse
+// pass over the c_SSP table.  One CTA per (z cell, chunk of 64 rows): the cell's two arrays c_t and D_t = c_{t+1} - c_t
+// (106 KB at full size) are staged in shared memory; each warp owns 8 rows and register-blocks over them, so every
+// table word read from shared memory feeds 8 FMAs (the 1 LDS : 2 FMA ratio of a row-at-a-time pass would leave the
+// kernel shared-memory bound at ~1/4 of the FMA rate).
+//   pass 1 (lane = 4 consecutive entries e = j*n_band + b of a table row):
+//            Q^(s)_r,e = sum_i a_r,i c^(s)[i][e]          s = 0: c_t, s = 1: D_t
+//   per row: S^(s)_b = sum_j m_j Q^(s)_{jb};  flux_b = F_att,b Mn [S^(0)_b + f S^(1)_b];  g_b = -(flux_b - d_b)/sigma_b^2
+//            (or the caller's flux_bar);  direct bars of Mn, z, A_V, delta, F_floor;  m_bar_j
+//   pass 2 (lane = age bins i = l, l+32, ...; table rows are an odd number of float4 apart: conflict free):
+//            a_bar_r,i = sum_e v_r,e (c_t[i][e] + f_r D_t[i][e]),   v_r,e = g_b F_b Mn m_j
+// ---------------------------------------------------------------------------------------------
+struct ACWarp {
+  float4 buf[128 * AC_R / 4];      // pass 1: a_T[i][r];  pass 2: v[e4][r] (float4 over 4 entries)
+  float Qs[2][128];
+  float ms[AC_R][ROW_M_STRIDE];
+  float sbar[SPS_MAX_BAND];
+  float4 sc[AC_R][4];              // RowScalars of the warp's rows, fetched before pass 1
+  float obs[AC_R][2][SPS_MAX_BAND];// (d_b, sigma_b) or (flux_bar_b, -) of the warp's rows
+};
+
+__global__ void __launch_bounds__(32 * AC_WARPS, 1)
+approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, const int* __restrict__ bins,
+                       const int* __restrict__ gal_of_row, const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
+                       const float* __restrict__ flux_bar, bool want_grad, RowBuffers B) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nb = T.n_z - 1, stride = nb + 2;
+  const int* row_start = bins + stride; const int* cta_start = bins + 2 * stride;
+  if ((int)blockIdx.x >= cta_start[nb]) return;
+  int lo = 0, hi = nb;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cta_start[mid] <= (int)blockIdx.x) lo = mid; else hi = mid; }
+  const int cell = lo;
+  const int r_begin = row_start[cell] + ((int)blockIdx.x - cta_start[cell]) * AC_ROWS_PER_CTA;
+  const int r_end = min(row_start[cell + 1], r_begin + AC_ROWS_PER_CTA);
+  const int cs4 = T.cs_stride >> 2;                         // float4 per table row (odd)
+  const int slice4 = T.n_age * cs4;                         // float4 per array
+  float4* s0 = reinterpret_cast<float4*>(smem_raw);
+  float4* s1 = s0 + slice4;
+  ACWarp* warps = reinterpret_cast<ACWarp*>(s0 + 2 * slice4 + 4);
+  // one thread streams the cell's two arrays (contiguous in HBM/L2) into shared memory with bulk async copies;
+  // meanwhile every warp stages its rows' weights
+  __shared__ __align__(8) unsigned long long load_bar;
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&load_bar);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const char* src = reinterpret_cast<const char*>(T.cssp + (int64_t)cell * 2 * T.n_age * T.cs_stride);
+    const uint32_t bytes = (uint32_t)(2 * slice4) * 16u;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s0);
+    for (uint32_t off = 0; off < bytes; off += 16384u) {
+      const uint32_t len = min(16384u, bytes - off);
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(dst + off), "l"(src + off), "r"(len), "r"(bar) : "memory");
+    }
+  }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  const int r0 = r_begin + w * AC_R;
+  if (r0 >= r_end) return;
+  ACWarp& S = warps[w];
+  int row[AC_R];
+#pragma unroll
+  for (int r = 0; r < AC_R; ++r) row[r] = (r0 + r < r_end) ? order[r0 + r] : -1;
+  // fetch everything the per-row band step needs now, so that its latency hides behind pass 1
+  {
+    const int rr = l >> 2, part = l & 3;                    // lane -> (row, quarter of its RowScalars)
+    const int rw = __shfl_sync(FULL_MASK, row[0], 0);       // (keeps row[] in registers: select by compile-time index below)
+    (void)rw;
+    int my_row = -1;
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) if (r == rr) my_row = row[r];
+    if (my_row >= 0) S.sc[rr][part] = reinterpret_cast<const float4*>(B.sc + my_row)[part];
+    if (l < T.n_band) {
+#pragma unroll
+      for (int r = 0; r < AC_R; ++r) {
+        if (row[r] < 0) continue;
+        if (flux_bar) S.obs[r][0][l] = flux_bar[(int64_t)row[r] * T.n_band + l];
+        else {
+          const int64_t gal = gal_of_row ? gal_of_row[row[r]] : row[r];
+          S.obs[r][0][l] = obs_flux[gal * T.n_band + l]; S.obs[r][1][l] = obs_sigma[gal * T.n_band + l];
+        }
+      }
+    }
+  }
+  // stage a (transposed: a_T[i][r]) and m
+  {
+    float* aT = reinterpret_cast<float*>(S.buf);
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) {
+#pragma unroll
+      for (int q = 0; q < SPS_AGE_PER_LANE; ++q) aT[(l + 32 * q) * AC_R + r] = row[r] >= 0 ? B.a[(int64_t)row[r] * ROW_A_STRIDE + l + 32 * q] : 0.f;
+      if (l < ROW_M_STRIDE) S.ms[r][l] = row[r] >= 0 ? B.m[(int64_t)row[r] * ROW_M_STRIDE + l] : 0.f;
+    }
+  }
+  __syncwarp();
+  {                                                         // wait for the table arrays
+    uint32_t ok = 0;
+    while (!ok)
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar) : "memory");
+  }
+  const bool act = l < cs4;
+  const int E = T.n_Z * T.n_band;
+  // ---- pass 1 ----
+  float4 q0[AC_R], q1[AC_R];
+#pragma unroll
+  for (int r = 0; r < AC_R; ++r) q0[r] = q1[r] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (act) {
+    const float4* c0p = s0 + l; const float4* c1p = s1 + l;
+#pragma unroll 2
+    for (int i = 0; i < T.n_age; ++i) {
+      const float4 c0 = c0p[i * cs4], c1 = c1p[i * cs4];
+      const float4 alo = S.buf[2 * i], ahi = S.buf[2 * i + 1];
+      const float a8[AC_R] = {alo.x, alo.y, alo.z, alo.w, ahi.x, ahi.y, ahi.z, ahi.w};
+#pragma unroll
+      for (int r = 0; r < AC_R; ++r) {
+        q0[r].x = fmaf(a8[r], c0.x, q0[r].x); q0[r].y = fmaf(a8[r], c0.y, q0[r].y); q0[r].z = fmaf(a8[r], c0.z, q0[r].z); q0[r].w = fmaf(a8[r], c0.w, q0[r].w);
+        q1[r].x = fmaf(a8[r], c1.x, q1[r].x); q1[r].y = fmaf(a8[r], c1.y, q1[r].y); q1[r].z = fmaf(a8[r], c1.z, q1[r].z); q1[r].w = fmaf(a8[r], c1.w, q1[r].w);
+      }
+    }
+  }
+  __syncwarp();                                             // a_T is dead: S.buf becomes the v buffer
+  // ---- per row: bands, likelihood, direct bars, m_bar, v ----
+  float f8[AC_R];
+#pragma unroll
+  for (int r = 0; r < AC_R; ++r) {
+    f8[r] = 0.f;
+    if (row[r] < 0) { if (act) S.buf[l * AC_R + r] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
+    reinterpret_cast<float4*>(S.Qs[0])[l] = q0[r];
+    reinterpret_cast<float4*>(S.Qs[1])[l] = q1[r];
+    __syncwarp();
+    RowScalars sc = *reinterpret_cast<const RowScalars*>(&S.sc[r][0]);
+    const float f = sc.zfrac;
+    f8[r] = f;
+    float S0 = 0.f, S1 = 0.f, F = 1.f, F_av = 0.f, F_del = 0.f, F_fl = 0.f, F_lam = 0.f, lam_r = 1.f, g = 0.f, flux = 0.f, chi2 = 0.f;
+    const bool isb = l < T.n_band;
+    if (isb) {
+      for (int j = 0; j < T.n_Z; ++j) { S0 = fmaf(S.ms[r][j], S.Qs[0][j * T.n_band + l], S0); S1 = fmaf(S.ms[r][j], S.Qs[1][j * T.n_band + l], S1); }
+      lam_r = T.lam_eff[l] / (1.f + sc.z);
+      dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
+      flux = F * sc.Mn * (S0 + f * S1);
+      B.flux[(int64_t)row[r] * SPS_MAX_BAND + l] = flux;
+      if (flux_bar) g = S.obs[r][0][l];
+      else {
+        const float d = S.obs[r][0][l], sg = S.obs[r][1][l];
+        const float rr = (flux - d) / sg;
+        chi2 = rr * rr;
+        g = -rr / sg;
+      }
+    }
+    chi2 = warp_sum(chi2);
+    if (!want_grad) {
+      if (l == 0) B.sc[row[r]].logp_like = -0.5f * chi2;
+      __syncwarp();
+      continue;
+    }
+    const float Sint = S0 + f * S1;
+    const float Mn_bar = warp_sum(isb ? g * F * Sint : 0.f);
+    const float z_bar = warp_sum(isb ? g * (F * sc.Mn * S1 * T.inv_dz + sc.Mn * Sint * F_lam * (-lam_r / (1.f + sc.z))) : 0.f);
+    const float av_bar = warp_sum(isb ? g * sc.Mn * Sint * F_av : 0.f);
+    const float del_bar = warp_sum(isb ? g * sc.Mn * Sint * F_del : 0.f);
+    const float fl_bar = warp_sum(isb ? g * sc.Mn * Sint * F_fl : 0.f);
+    if (l == 0) {
+      sc.logp_like = -0.5f * chi2; sc.Mn_bar = Mn_bar; sc.z_bar = z_bar;
+      sc.AV_bar = av_bar; sc.delta_bar = del_bar; sc.Ffloor_bar = fl_bar;
+      B.sc[row[r]] = sc;
+    }
+    if (isb) S.sbar[l] = g * F * sc.Mn;
+    __syncwarp();
+    if (l < ROW_M_STRIDE) {
+      float mb = 0.f;
+      if (l < T.n_Z)
+        for (int b = 0; b < T.n_band; ++b) mb = fmaf(S.sbar[b], S.Qs[0][l * T.n_band + b] + f * S.Qs[1][l * T.n_band + b], mb);
+      B.m_bar[(int64_t)row[r] * ROW_M_STRIDE + l] = mb;
+    }
+    if (act) {
+      float vv[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int e = 4 * l + k;
+        float v = 0.f;
+        if (e < E) { const int j = e / T.n_band, b = e - j * T.n_band; v = S.sbar[b] * S.ms[r][j]; }
+        vv[k] = v;
+      }
+      S.buf[l * AC_R + r] = make_float4(vv[0], vv[1], vv[2], vv[3]);
+    }
+    __syncwarp();
+  }
+  if (!want_grad) return;
+  __syncwarp();
+  // ---- pass 2 ----
+  float acc[SPS_AGE_PER_LANE][AC_R];
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q)
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) acc[q][r] = 0.f;
+  int irow[SPS_AGE_PER_LANE];
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) irow[q] = min(l + 32 * q, T.n_age - 1) * cs4;
+  for (int e4 = 0; e4 < cs4; ++e4) {
+    float4 v[AC_R];
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) v[r] = S.buf[e4 * AC_R + r];
+#pragma unroll
+    for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+      const float4 c0 = s0[irow[q] + e4], c1 = s1[irow[q] + e4];
+#pragma unroll
+      for (int r = 0; r < AC_R; ++r) {
+        const float tx = fmaf(f8[r], c1.x, c0.x), ty = fmaf(f8[r], c1.y, c0.y), tz = fmaf(f8[r], c1.z, c0.z), tw = fmaf(f8[r], c1.w, c0.w);
+        acc[q][r] = fmaf(v[r].x, tx, fmaf(v[r].y, ty, fmaf(v[r].z, tz, fmaf(v[r].w, tw, acc[q][r]))));
+      }
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < AC_R; ++r) {
+    if (row[r] < 0) continue;
+#pragma unroll
+    for (int q = 0; q < SPS_AGE_PER_LANE; ++q) B.a_bar[(int64_t)row[r] * ROW_A_STRIDE + l + 32 * q] = (l + 32 * q < T.n_age) ? acc[q][r] : 0.f;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Reverse of a0-a5 (a10) + skew-normal prior (a9): one warp per row contracts the stored per-bin partials (B.part)
+// with a_bar, m_bar, Mn_bar and the direct bars.  Only the cheap closed forms (C1, dt/dz, burst polynomial, MDF) are
+// re-evaluated; no quadrature is redone.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
 epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded, bool with_prior,
@@ -200,32 +349,48 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
-  RowFwd R;
-  row_forward<true>(T, P, theta + row * SPS_NDIM, unbounded, R);
   const RowScalars sc = B.sc[row];
-  const float Fb = R.th[4], inv_M = 1.f / R.Msum;
+  if (!grad) {                                               // log-posterior only
+    float lp = 0.f;
+    if (with_prior && l < SPS_NDIM) { float dlp; log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp); }
+    lp = warp_sum(lp);
+    if (l == 0 && logp) logp[row] = sc.logp_like + lp;
+    return;
+  }
+  float th[SPS_NDIM], dth[SPS_NDIM];
+  double zd_unused;
+  load_params<false>(theta + row * SPS_NDIM, unbounded, P, th, dth, zd_unused);
+  const float zp = 1.f + th[12];
+  const float dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp * zp * zp + T.OL));
+  BurstQuad Bq;
+  burst_bins(T, th[5], th[6], Bq);
+  float m_unused, dm_lz, dm_s;
+  met_bin(T, th[7], th[8], m_unused, dm_lz, dm_s);
+  const float Fb = th[4], inv_M = 1.f / sc.Msum, Mf = sc.Mn * inv_M;
+  const float* part = B.part + row * (ROW_PARTS * ROW_A_STRIDE);
   float abar[SPS_AGE_PER_LANE], Ps[SPS_AGE_PER_LANE];
   float s_fb = 0.f, s_pp = 0.f, s_ltp = 0.f, s_ltm = 0.f;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     abar[q] = B.a_bar[row * ROW_A_STRIDE + l + 32 * q];
-    Ps[q] = R.Q.dM[q] * inv_M;
-    s_fb += abar[q] * (R.Bq.P[q] - Ps[q]);             // dL/dF_burst           (Eq. A6)
+    Ps[q] = part[l + 32 * q] * inv_M;
+    s_fb += abar[q] * (Bq.P[q] - Ps[q]);                       // dL/dF_burst           (Eq. A6)
     s_pp += abar[q] * Ps[q];
-    s_ltp += abar[q] * R.Bq.d_ltp[q];
-    s_ltm += abar[q] * R.Bq.d_ltm[q];
+    s_ltp += abar[q] * Bq.d_ltp[q];
+    s_ltm += abar[q] * Bq.d_ltm[q];
   }
   s_fb = warp_sum(s_fb); s_pp = warp_sum(s_pp); s_ltp = warp_sum(s_ltp) * Fb; s_ltm = warp_sum(s_ltm) * Fb;
   // dL/d(dM_i) = (1-Fb)/Msum (a_bar_i - sum_k a_bar_k Ps_k) + Mn_bar * Mf
   float s_tau = 0.f, s_al = 0.f, s_be = 0.f, s_t = 0.f;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
-    const float dMb = (1.f - Fb) * inv_M * (abar[q] - s_pp) + sc.Mn_bar * R.Mf;
-    s_tau += dMb * R.Q.g_tau[q]; s_al += dMb * R.Q.g_al[q]; s_be += dMb * R.Q.g_be[q]; s_t += dMb * R.Q.g_t[q];
+    const float dMb = (l + 32 * q < T.n_age) ? (1.f - Fb) * inv_M * (abar[q] - s_pp) + sc.Mn_bar * Mf : 0.f;
+    const float* p = part + l + 32 * q;
+    s_tau += dMb * p[ROW_A_STRIDE]; s_al += dMb * p[2 * ROW_A_STRIDE]; s_be += dMb * p[3 * ROW_A_STRIDE]; s_t += dMb * p[4 * ROW_A_STRIDE];
   }
   s_tau = warp_sum(s_tau); s_al = warp_sum(s_al); s_be = warp_sum(s_be); s_t = warp_sum(s_t);
   const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
-  const float s_lz = warp_sum(mb * R.dm_lz), s_s = warp_sum(mb * R.dm_s);
+  const float s_lz = warp_sum(mb * dm_lz), s_s = warp_sum(mb * dm_s);
   float g = 0.f;
   switch (l) {
     case 0: g = sc.Mn_bar * sc.Mn * LN10F; break;
@@ -240,21 +405,21 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     case 9: g = sc.AV_bar; break;
     case 10: g = sc.delta_bar; break;
     case 11: g = sc.Ffloor_bar; break;
-    case 12: g = sc.z_bar + s_t * R.dt_dz; break;
+    case 12: g = sc.z_bar + s_t * dt_dz; break;
     default: break;
   }
   float lp = 0.f;
   if (l < SPS_NDIM) {
-    float dth = 1.f;
+    float d1 = 1.f;
 #pragma unroll
-    for (int p = 0; p < SPS_NDIM; ++p) if (p == l) dth = R.dth[p];
-    g *= dth;
+    for (int p = 0; p < SPS_NDIM; ++p) if (p == l) d1 = dth[p];
+    g *= d1;
     if (with_prior) {
       float dlp;
       log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp);
       g += dlp;
     }
-    if (grad) grad[row * SPS_NDIM + l] = g;
+    grad[row * SPS_NDIM + l] = g;
   }
   lp = warp_sum(lp);
   if (l == 0 && logp) logp[row] = sc.logp_like + lp;
@@ -277,23 +442,41 @@ __global__ void copy_flux_kernel(TableDev T, int64_t n, RowBuffers B, float* flu
 
 static inline unsigned blocks_for_rows(int64_t n) { return (unsigned)((n + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK); }
 
-void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
+void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
                      const int* rows, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
   sps_prof_begin(SPS_K_PROLOGUE, s);
-  prologue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
+  if (want_grad) prologue_kernel<true><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
+  else prologue_kernel<false><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
+
+static size_t approx_smem_bytes(const TableDev& T) {
+  return (size_t)2 * T.n_age * T.cs_stride * sizeof(float) + 64 + AC_WARPS * sizeof(ACWarp);
+}
+sps_status approx_contract_setup(const TableDev& T) {
+  if (T.n_z - 1 > 1 << 20) { sps_set_error("n_z too large"); return SPS_ESHAPE; }
+  return sps_check_cuda(cudaFuncSetAttribute(approx_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)approx_smem_bytes(T)),
+                        "approximate-path shared memory opt-in");
+}
+
 void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
+  const int nb = T.n_z - 1, stride = nb + 2;
+  const unsigned eb = (unsigned)((n + 255) / 256);
+  cudaMemsetAsync(B.bins, 0, stride * sizeof(int), s);
+  approx_hist_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins);
+  approx_plan_kernel<<<1, 1024, 0, s>>>(nb, B.bins);
+  approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
+  const unsigned grid = (unsigned)((n + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA + nb);
   sps_prof_begin(SPS_K_APPROX, s);
-  approx_contract_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, n, rows, gal_of_row, obs_flux, obs_sigma,
-                                                                           flux_bar, want_grad, B);
+  approx_contract_kernel<<<grid, 32 * AC_WARPS, approx_smem_bytes(T), s>>>(T, n, B.order, B.bins, gal_of_row, obs_flux, obs_sigma,
+                                                                         flux_bar, want_grad, B);
   sps_prof_end(SPS_K_APPROX, s);
-  sps_count_launch();
+  sps_count_launch(4);
 }
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s) {

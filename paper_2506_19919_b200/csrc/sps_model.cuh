@@ -11,6 +11,7 @@
 // ---- a0: Eq. (C1) PAPER.md:429 -----------------------------------------------------------------
 // Every lane returns all 13 bounded parameters (th) and d theta / d theta~ (dth).
 // The redshift (lane 12) is also returned in double: t_obs(z) - age cancels for the oldest bins.
+template <bool NEED_ZD = true>
 __device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PriorDev& pr,
                                             float th[SPS_NDIM], float dth[SPS_NDIM], double& z_d) {
   const int l = lane_id();
@@ -22,7 +23,7 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
     if (unbounded) {
       float s = 1.f / (1.f + expf(-pr.k[l] * (v - pr.x0[l])));
       float w = pr.y_hi[l] - pr.y_lo[l];
-      if (l == SPS_NDIM - 1) {
+      if (NEED_ZD && l == SPS_NDIM - 1) {
         const double sd = 1.0 / (1.0 + exp(-(double)pr.k[l] * ((double)v - (double)pr.x0[l])));
         vd = (double)pr.y_lo[l] + ((double)pr.y_hi[l] - (double)pr.y_lo[l]) * sd;
       }
@@ -30,7 +31,7 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
       d = w * pr.k[l] * s * (1.f - s);
     }
   }
-  z_d = __shfl_sync(FULL_MASK, vd, SPS_NDIM - 1);
+  z_d = NEED_ZD ? __shfl_sync(FULL_MASK, vd, SPS_NDIM - 1) : 0.0;
 #pragma unroll
   for (int p = 0; p < SPS_NDIM; ++p) {
     th[p] = __shfl_sync(FULL_MASK, v, p);

@@ -4,6 +4,7 @@
 #include "sps_model.cuh"
 
 // Work buffers for n rows (device memory owned by the library, grown on demand).
+#define ROW_PARTS 5
 struct RowBuffers {
   float* a;        // [n][ROW_A_STRIDE]  P_SFH (Eq. A6)
   float* m;        // [n][ROW_M_STRIDE]  P_met
@@ -11,15 +12,20 @@ struct RowBuffers {
   float* m_bar;    // [n][ROW_M_STRIDE]  d logL / d m_j
   RowScalars* sc;  // [n]
   float* flux;     // [n][SPS_MAX_BAND]  model band fluxes
+  float* part;     // [n][ROW_PARTS][ROW_A_STRIDE] per-bin dM and its partials (tau, alpha, beta, t_obs), written by the
+                   //                              gradient prologue and contracted with a_bar by the epilogue
+  int* order;      // [n]  rows of the current approximate-path call grouped by z cell
+  int* bins;       // [4][n_z + 1] histogram, row offsets, CTA offsets, cursors of that grouping
   int64_t capacity;
 };
 
 // kernels (sps_kernels.cu)
-void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
+void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
                      const int* rows, RowBuffers B, cudaStream_t s);
 void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);
+sps_status approx_contract_setup(const TableDev& T);
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s);
 void launch_copy_weights(const TableDev& T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar,

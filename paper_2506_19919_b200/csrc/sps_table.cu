@@ -166,6 +166,7 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   }
   if (wave_dd) cudaFree(wave_dd);
   if (dlam_dd) cudaFree(dlam_dd);
+  if (st == SPS_OK) st = approx_contract_setup(T);
   if (st == SPS_OK) st = sps_exact_setup(t, d->exact_precision);
   if (st != SPS_OK) { sps_destroy_table(t); return st; }
   *out = t;
