@@ -23,6 +23,7 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
+from paper_2506_19919_b200.sharding import aggregate_throughput, max_over_ranks, rank_seed  # noqa: E402
 
 SM_COUNT, FMA_PER_SM_CLK = 148, 128
 
@@ -79,9 +80,9 @@ def make_hmc_inputs(sps, W, table, ph, prior, n_gal, seed, rank=0):
     """True parameters drawn from the prior; observed fluxes = the library's own approximate-path photometry of the
     truth with 5-10 % Gaussian noise (bench.py may not touch oracle/ outside the cpu_baseline leg)."""
     import torch
-    thu = W.draw_theta_unbounded(prior, n_gal, seed + 1000 * rank).astype(np.float32)
+    thu = W.draw_theta_unbounded(prior, n_gal, rank_seed(seed, rank)).astype(np.float32)
     f = sps.sps_photometry(table, ph, sps.PATH_APPROX, torch.tensor(thu, device="cuda")).cpu().numpy().astype(np.float64)
-    d, s = W.noisy_observations(f, seed + 7 + 1000 * rank, 0.05, 0.10)
+    d, s = W.noisy_observations(f, rank_seed(seed, rank) + 7, 0.05, 0.10)
     return d.astype(np.float32), s.astype(np.float32)
 
 
@@ -124,7 +125,7 @@ def run_ours(args):
     else:
         n = args.n_rows or cfg["batch"]
         path = sps.PATH_APPROX if args.workload == "c3_approx" else sps.PATH_EXACT
-        thu = W.draw_theta_unbounded(prior, n, cfg["seed"] + 1000 * rank, z_uniform=(0.1, 3.0)).astype(np.float32)
+        thu = W.draw_theta_unbounded(prior, n, rank_seed(cfg["seed"], rank), z_uniform=(0.1, 3.0)).astype(np.float32)
         fb = np.random.default_rng(cfg["seed"]).normal(size=(n, grid.n_band)).astype(np.float32)
         th_host = torch.from_numpy(thu).pin_memory(); fb_host = torch.from_numpy(fb).pin_memory()
         th_dev = th_host.cuda(); fb_dev = fb_host.cuda()
@@ -169,34 +170,40 @@ def run_ours(args):
         step_e2e()
     barrier()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([dev_s, e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_s, e2e_s = t.tolist()
+    dev_s, e2e_s = max_over_ranks([dev_s, e2e_s], dist, device="cuda")
+    pairs = sps.sps_exact_last_work(table) if args.workload == "c2_exact" else 0
     if rank != 0:
         return
-    value = to_value(units_per_step * args.steps * world, dev_s)
+    value = to_value(aggregate_throughput(units_per_step * args.steps, world, dev_s), 1.0)
     out = {"metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f32", "data": "synthetic (seeded stand-in SSP spectra, Gaussian filters, prior-drawn galaxies)",
            "config": {"workload": args.workload, **{k: v for k, v in cfg.items() if k != "seed"},
                       "n_gal_per_gpu": args.n_gal or cfg.get("n_gal"), "l2": "flushed between timed steps (256 MB write)"},
            "loglike_grad_evals_per_s": evals_per_step * args.steps * world / dev_s,
-           "e2e": {"value": to_value(units_per_step * args.steps * world, e2e_s), "unit": unit, "h2d_bytes_per_step": h2d,
+           "e2e": {"value": to_value(aggregate_throughput(units_per_step * args.steps, world, e2e_s), 1.0), "unit": unit, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "clocks": clk, "impl": "ours"}
-    out["roofline"] = roofline(prof, dom_kernel, rows_per_launch, grid, peaks, peaks_src)
+    out["roofline"] = roofline(prof, dom_kernel, rows_per_launch, grid, peaks, peaks_src, pairs)
     out["kernel_ms"] = {k: {"avg_ms": (v[0] / v[1] if v[1] else None), "launches": v[2]} for k, v in prof.items() if v[2]}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, cfg, budget_s=args.cpu_budget)
     print(json.dumps(out))
 
 
-def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src):
-    """Roofline of the dominant kernel (DESIGN.md "Kernels and rooflines").
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
+# captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
+NCU_TRAFFIC = {}
+
+
+def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
+    """Roofline of the dominant kernel (DESIGN.md section 5).
     approx_contract: FP32-FMA ("alu") bound: per row the forward + reverse pass over the two c_SSP arrays of its z cell
-    is 2 FMA per table word = 4 * n_age*n_Z*n_band flop ... no HBM stream: the table is L2/smem resident.
-    Peak = 148 SM x 128 FMA/clk x 2 flop x max SM clock (guide unit counts; clock from MEASURED_PEAKS.json)."""
+    is 2 FMA per table word = 4 * n_age*n_Z*n_band flop per array pair; the table is L2/shared-memory resident, so there
+    is no HBM stream.  Peak = 148 SM x 128 FMA/clk x 2 flop x max SM clock (guide unit counts; clock from
+    MEASURED_PEAKS.json).
+    exact_fwd: tensor bound: 3 split products x 2 x n_age*n_Z flop per (row, wavelength) pair under some filter's support
+    (sps_exact_last_work: skipped and padded columns never count), against the measured bf16 burst peak (BF16X3)."""
     ms, timed, allc = prof[kernel]
     if not timed:
         return {"bound": "alu", "achieved": None, "peak": None, "unit": "TFLOP/s", "frac": None, "traffic": None}
@@ -208,12 +215,14 @@ def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src):
         bound, note = "alu", f"fp32 FMA peak at {peaks.get('sm_max_mhz', 1965.0):.0f} MHz ({peaks_src})"
     else:
         K = grid.n_age * grid.n_Z
-        flop = 3.0 * 2.0 * K * grid.n_wave * rows_per_launch          # 3xTF32 issued flop over the unpadded columns
-        peak = 0.5 * float(peaks["bf16_tflops"])                       # TF32 = bf16 measured x nominal ratio 1.1/2.25
-        bound, note = "tensor", f"tf32 peak = 0.5 x bf16 burst ({peaks_src}); achieved counts the 3 split products"
+        flop = 3.0 * 2.0 * K * float(pairs)
+        peak = float(peaks["bf16_tflops"])
+        bound, note = "tensor", (f"bf16 burst peak ({peaks_src}); achieved = 3 BF16 split products x 2 x {K} flop x {pairs} (row, wavelength) "
+                                 f"pairs under a filter's support = {pairs / max(1, rows_per_launch):.0f} of {grid.n_wave} wavelengths per row")
     ach = flop / avg_s / 1e12
     return {"bound": bound, "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-            "traffic": None, "avg_launch_ms": 1e3 * avg_s, "timed_launches": timed, "launches": allc, "peak_note": note}
+            "traffic": NCU_TRAFFIC.get((kernel, rows_per_launch)), "avg_launch_ms": 1e3 * avg_s, "timed_launches": timed, "launches": allc,
+            "peak_note": note}
 
 
 def cpu_baseline(workload, cfg, budget_s=20.0):

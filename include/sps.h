@@ -165,6 +165,11 @@ enum { SPS_K_PROLOGUE = 0, SPS_K_APPROX = 1, SPS_K_EPILOGUE = 2, SPS_K_EXACT_FWD
 sps_status sps_profile(int enable, int stride);
 sps_status sps_profile_read(int kernel_id, double* total_ms, int64_t* timed_launches, int64_t* all_launches);
 
+/* Algorithmic work of the last exact-path forward call on this table: the number of (row, wavelength) pairs that lie
+ * under some filter's 5-sigma support at the row's redshift (everything else contributes exactly zero to Eq. 4 and is
+ * skipped).  bench.py's tensor roofline counts 3 x 2 x n_age*n_Z flop per pair and pass.  Synchronises. */
+sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavelength_pairs);
+
 /* Number of kernels this library launched since load (for bench.py's gpu_launches). */
 int64_t sps_launch_count(void);
 

@@ -19,7 +19,7 @@ EXACT_BF16X3, EXACT_TF32X3 = 0, 1
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
            "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
-           "sps_last_error", "sps_version")
+           "sps_last_error", "sps_version", "sps_exact_last_work")
 
 
 class SpsError(RuntimeError):
@@ -208,6 +208,12 @@ def sps_philox_words(seed, first_chain, transition, purpose, index, n):
     _check(lib().sps_philox_words(C.c_uint64(seed), C.c_uint32(first_chain), C.c_uint32(transition), C.c_uint32(purpose),
                                   C.c_uint32(index), C.c_int64(n), _dptr(out), _stream()), "sps_philox_words")
     return out
+
+
+def sps_exact_last_work(table) -> int:
+    v = C.c_int64()
+    _check(lib().sps_exact_last_work(table.handle, C.byref(v)), "sps_exact_last_work")
+    return int(v.value)
 
 
 def sps_launch_count() -> int:

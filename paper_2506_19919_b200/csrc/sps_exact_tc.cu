@@ -77,6 +77,7 @@ struct TcState {
   void *W_hi, *W_lo;                // [cap][Wld]           forward A operand
   void *SB_hi, *SB_lo;              // [cap][n_wave_pad]    reverse A operand (SEDbar)
   float4* wconst;                   // [n_wave_pad][2]      {lam, dlam, k0, drude}, {log2(lam/5500), -, -, -}
+  unsigned long long* work;         // [1] (row, wavelength) pairs of the last forward call
   int* plan;                        // [4][plan_cap]: fwd item prefix, first wavelength tile, k-range begin / end (bytes/128)
   int plan_cap;
   CUtensorMap mLT_hi, mLT_lo, mLc_hi, mLc_lo, mW_hi, mW_lo, mSB_hi, mSB_lo;
@@ -403,7 +404,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
 // ---- plan: per row tile, the wavelength range under some filter's support for the tile's redshifts -------------------
 // plan[0][m] = prefix of forward items, plan[1][m] = first wavelength tile, plan[2][m], plan[3][m] = k-block range (reverse)
 __global__ void __launch_bounds__(256) exact_plan_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
-                                                         int m_tiles, int BKe, int* __restrict__ plan, int plan_cap) {
+                                                         int m_tiles, int BKe, int* __restrict__ plan, int plan_cap, unsigned long long* __restrict__ work) {
   __shared__ int cnt[1024];
   float obs_lo = 1e30f, obs_hi = 0.f;
   for (int b = 0; b < T.n_band; ++b) { obs_lo = fminf(obs_lo, FC.lo[b]); obs_hi = fmaxf(obs_hi, FC.hi[b]); }
@@ -411,7 +412,17 @@ __global__ void __launch_bounds__(256) exact_plan_kernel(TableDev T, int64_t n, 
     for (int m = base + threadIdx.x; m < min(m_tiles, base + 1024); m += blockDim.x) {
       float zmin = 1e30f, zmax = -1e30f;
       const int64_t r1 = min(n, (int64_t)(m + 1) * BM);
-      for (int64_t r = (int64_t)m * BM; r < r1; ++r) { const float z = B.sc[rows ? rows[r] : r].z; zmin = fminf(zmin, z); zmax = fmaxf(zmax, z); }
+      unsigned long long pairs = 0;                            // (row, wavelength) pairs under some filter: the algorithmic work
+      for (int64_t r = (int64_t)m * BM; r < r1; ++r) {
+        const float z = B.sc[rows ? rows[r] : r].z; zmin = fminf(zmin, z); zmax = fmaxf(zmax, z);
+        const float rlo = obs_lo / (1.f + z), rhi = obs_hi / (1.f + z);
+        int a = 0, c = T.n_wave;
+        while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < rlo) a = mid + 1; else c = mid; }
+        const int first = a; c = T.n_wave;
+        while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= rhi) a = mid + 1; else c = mid; }
+        pairs += (unsigned long long)(a - first);
+      }
+      atomicAdd(work, pairs);
       const float lo = obs_lo / (1.f + zmax) * 0.99999f, hi = obs_hi / (1.f + zmin) * 1.00001f;
       int a = 0, c = T.n_wave;
       while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
@@ -585,9 +596,12 @@ sps_status launch_forward(sps_table* t, TcState* S, int64_t n, const int* rows, 
   GemmArgs G; memset(&G, 0, sizeof(G));
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = T.n_wave_pad / BN_MAX; G.k_blocks = S->Kpad / S->BK; G.BN = BN_MAX; G.BK = S->BK;
   G.rows = rows; G.part = X->part; G.plan = S->plan; G.plan_cap = S->plan_cap;
-  exact_plan_kernel<<<1, 256, 0, s>>>(T, n, rows, t->rows, S->fc, G.m_tiles, S->BK, S->plan, S->plan_cap);
+  cudaMemsetAsync(S->work, 0, sizeof(unsigned long long), s);
+  exact_plan_kernel<<<1, 256, 0, s>>>(T, n, rows, t->rows, S->fc, G.m_tiles, S->BK, S->plan, S->plan_cap, S->work);
   const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  sps_prof_begin(SPS_K_EXACT_FWD, s);
   exact_gemm_kernel<0, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+  sps_prof_end(SPS_K_EXACT_FWD, s);
   sps_count_launch(3);
   return sps_check_cuda(cudaGetLastError(), "exact forward (tcgen05) launch");
 }
@@ -601,7 +615,9 @@ sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows,
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = S->nb; G.k_blocks = T.n_wave_pad / S->BK; G.BN = S->BNb; G.BK = S->BK;
   G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
   const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  sps_prof_begin(SPS_K_EXACT_BWD, s);
   exact_gemm_kernel<1, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mSB_hi, S->mSB_lo, S->mLc_hi, S->mLc_lo, T, t->rows, G, S->fc, S->wconst);
+  sps_prof_end(SPS_K_EXACT_BWD, s);
   sps_count_launch(2);
   return sps_check_cuda(cudaGetLastError(), "exact reverse (tcgen05) launch");
 }
@@ -640,6 +656,7 @@ sps_status sps_exact_tc_setup(sps_table* t, int precision) {
   if (e == cudaSuccess) e = cudaMalloc(&S->Lc_hi, lc_n * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&S->Lc_lo, lc_n * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&S->wconst, (size_t)T.n_wave_pad * 2 * sizeof(float4));
+  if (e == cudaSuccess) e = cudaMalloc(&S->work, sizeof(unsigned long long));
   X->tc = S;
   if (e != cudaSuccess) { sps_exact_tc_teardown(t); return sps_check_cuda(e, "tensor-core operand allocation"); }
   st = precision == SPS_EXACT_BF16X3 ? build_tables<SPS_EXACT_BF16X3>(T, S, lc_rows) : build_tables<SPS_EXACT_TF32X3>(T, S, lc_rows);
@@ -658,7 +675,7 @@ void sps_exact_tc_teardown(sps_table* t) {
   if (!X || !X->tc) return;
   TcState* S = (TcState*)X->tc;
   free_row_operands(S);
-  void* ptrs[] = {S->LT_hi, S->LT_lo, S->Lc_hi, S->Lc_lo, S->wconst};
+  void* ptrs[] = {S->LT_hi, S->LT_lo, S->Lc_hi, S->Lc_lo, S->wconst, S->work};
   for (void* p : ptrs) if (p) cudaFree(p);
   delete S;
   X->tc = nullptr; X->use_tc = false;
@@ -698,4 +715,14 @@ sps_status sps_exact_tc_forward(sps_table* t, int64_t n, const int* rows, cudaSt
 sps_status sps_exact_tc_backward(sps_table* t, int64_t n, const int* rows, cudaStream_t s) {
   TcState* S = (TcState*)t->exact->tc;
   return S->prec == SPS_EXACT_BF16X3 ? launch_backward<SPS_EXACT_BF16X3>(t, S, n, rows, s) : launch_backward<SPS_EXACT_TF32X3>(t, S, n, rows, s);
+}
+
+extern "C" sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavelength_pairs) {
+  if (!t || !row_wavelength_pairs) { sps_set_error("sps_exact_last_work: null argument"); return SPS_EINVAL; }
+  *row_wavelength_pairs = 0;
+  if (!t->exact || !t->exact->use_tc) return SPS_OK;
+  unsigned long long v = 0;
+  sps_status st = sps_check_cuda(cudaMemcpy(&v, ((TcState*)t->exact->tc)->work, sizeof(v), cudaMemcpyDeviceToHost), "sps_exact_last_work");
+  *row_wavelength_pairs = (int64_t)v;
+  return st;
 }

@@ -128,9 +128,10 @@ __global__ void approx_scatter_kernel(int64_t n, const int* __restrict__ rows, R
 // ---------------------------------------------------------------------------------------------
 struct ACWarp {
   float4 buf[128 * AC_R / 4];      // pass 1: a_T[i][r];  pass 2: v[e4][r] (float4 over 4 entries)
-  float Qs[2][128];
+  float Qs[AC_R][2][128];          // Q^(0), Q^(1) of the warp's rows after pass 1
   float ms[AC_R][ROW_M_STRIDE];
-  float sbar[SPS_MAX_BAND];
+  float sbar[AC_R][SPS_MAX_BAND];  // g_b F_b Mn
+  int rowid[AC_R];
   float4 sc[AC_R][4];              // RowScalars of the warp's rows, fetched before pass 1
   float obs[AC_R][2][SPS_MAX_BAND];// (d_b, sigma_b) or (flux_bar_b, -) of the warp's rows
 };
@@ -238,73 +239,87 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
     }
   }
   __syncwarp();                                             // a_T is dead: S.buf becomes the v buffer
-  // ---- per row: bands, likelihood, direct bars, m_bar, v ----
-  float f8[AC_R];
+  // ---- band step for the warp's 8 rows at once: lane = (row 2k + l/16, band l%16), four rounds ----
+  //      fluxes, likelihood, direct bars (16-lane reductions), then m_bar (lane = (row, j)) and v (lane = 4 entries)
 #pragma unroll
   for (int r = 0; r < AC_R; ++r) {
-    f8[r] = 0.f;
-    if (row[r] < 0) { if (act) S.buf[l * AC_R + r] = make_float4(0.f, 0.f, 0.f, 0.f); continue; }
-    reinterpret_cast<float4*>(S.Qs[0])[l] = q0[r];
-    reinterpret_cast<float4*>(S.Qs[1])[l] = q1[r];
-    __syncwarp();
-    RowScalars sc = *reinterpret_cast<const RowScalars*>(&S.sc[r][0]);
-    const float f = sc.zfrac;
-    f8[r] = f;
-    float S0 = 0.f, S1 = 0.f, F = 1.f, F_av = 0.f, F_del = 0.f, F_fl = 0.f, F_lam = 0.f, lam_r = 1.f, g = 0.f, flux = 0.f, chi2 = 0.f;
-    const bool isb = l < T.n_band;
-    if (isb) {
-      for (int j = 0; j < T.n_Z; ++j) { S0 = fmaf(S.ms[r][j], S.Qs[0][j * T.n_band + l], S0); S1 = fmaf(S.ms[r][j], S.Qs[1][j * T.n_band + l], S1); }
-      lam_r = T.lam_eff[l] / (1.f + sc.z);
-      dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
-      flux = F * sc.Mn * (S0 + f * S1);
-      B.flux[(int64_t)row[r] * SPS_MAX_BAND + l] = flux;
-      if (flux_bar) g = S.obs[r][0][l];
-      else {
-        const float d = S.obs[r][0][l], sg = S.obs[r][1][l];
-        const float rr = (flux - d) / sg;
-        chi2 = rr * rr;
-        g = -rr / sg;
+    if (act) { reinterpret_cast<float4*>(S.Qs[r][0])[l] = q0[r]; reinterpret_cast<float4*>(S.Qs[r][1])[l] = q1[r]; }
+    if (l == 0) S.rowid[r] = row[r];
+  }
+  __syncwarp();
+  {
+    const int b = l & 15, hl = l >> 4;
+    const bool isb = b < T.n_band;
+#pragma unroll 1
+    for (int k = 0; k < AC_R / 2; ++k) {
+      const int r = 2 * k + hl;
+      const int rw = S.rowid[r];
+      const RowScalars& sc = *reinterpret_cast<const RowScalars*>(&S.sc[r][0]);
+      const bool ok = isb && rw >= 0;
+      const float f = sc.zfrac, Mn = sc.Mn, zp = 1.f + sc.z;
+      float S0 = 0.f, S1 = 0.f, F = 1.f, F_av = 0.f, F_del = 0.f, F_fl = 0.f, F_lam = 0.f, lam_r = 1.f, g = 0.f, chi2 = 0.f;
+      if (ok) {
+        for (int j = 0; j < T.n_Z; ++j) { S0 = fmaf(S.ms[r][j], S.Qs[r][0][j * T.n_band + b], S0); S1 = fmaf(S.ms[r][j], S.Qs[r][1][j * T.n_band + b], S1); }
+        lam_r = T.lam_eff[b] / zp;
+        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
+        const float flux = F * Mn * (S0 + f * S1);
+        B.flux[(int64_t)rw * SPS_MAX_BAND + b] = flux;
+        if (flux_bar) g = S.obs[r][0][b];
+        else {
+          const float d = S.obs[r][0][b], sg = S.obs[r][1][b];
+          const float rr = (flux - d) / sg;
+          chi2 = rr * rr;
+          g = -rr / sg;
+        }
       }
-    }
-    chi2 = warp_sum(chi2);
-    if (!want_grad) {
-      if (l == 0) B.sc[row[r]].logp_like = -0.5f * chi2;
-      __syncwarp();
-      continue;
-    }
-    const float Sint = S0 + f * S1;
-    const float Mn_bar = warp_sum(isb ? g * F * Sint : 0.f);
-    const float z_bar = warp_sum(isb ? g * (F * sc.Mn * S1 * T.inv_dz + sc.Mn * Sint * F_lam * (-lam_r / (1.f + sc.z))) : 0.f);
-    const float av_bar = warp_sum(isb ? g * sc.Mn * Sint * F_av : 0.f);
-    const float del_bar = warp_sum(isb ? g * sc.Mn * Sint * F_del : 0.f);
-    const float fl_bar = warp_sum(isb ? g * sc.Mn * Sint * F_fl : 0.f);
-    if (l == 0) {
-      sc.logp_like = -0.5f * chi2; sc.Mn_bar = Mn_bar; sc.z_bar = z_bar;
-      sc.AV_bar = av_bar; sc.delta_bar = del_bar; sc.Ffloor_bar = fl_bar;
-      B.sc[row[r]] = sc;
-    }
-    if (isb) S.sbar[l] = g * F * sc.Mn;
-    __syncwarp();
-    if (l < ROW_M_STRIDE) {
-      float mb = 0.f;
-      if (l < T.n_Z)
-        for (int b = 0; b < T.n_band; ++b) mb = fmaf(S.sbar[b], S.Qs[0][l * T.n_band + b] + f * S.Qs[1][l * T.n_band + b], mb);
-      B.m_bar[(int64_t)row[r] * ROW_M_STRIDE + l] = mb;
-    }
-    if (act) {
-      float vv[4];
+      const float Sint = S0 + f * S1;
+      float v_mn = g * F * Sint, v_z = g * (F * Mn * S1 * T.inv_dz + Mn * Sint * F_lam * (-lam_r / zp));
+      float v_av = g * Mn * Sint * F_av, v_de = g * Mn * Sint * F_del, v_fl = g * Mn * Sint * F_fl;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int e = 4 * l + k;
-        float v = 0.f;
-        if (e < E) { const int j = e / T.n_band, b = e - j * T.n_band; v = S.sbar[b] * S.ms[r][j]; }
-        vv[k] = v;
+      for (int o = 8; o > 0; o >>= 1) {
+        chi2 += __shfl_xor_sync(FULL_MASK, chi2, o); v_mn += __shfl_xor_sync(FULL_MASK, v_mn, o); v_z += __shfl_xor_sync(FULL_MASK, v_z, o);
+        v_av += __shfl_xor_sync(FULL_MASK, v_av, o); v_de += __shfl_xor_sync(FULL_MASK, v_de, o); v_fl += __shfl_xor_sync(FULL_MASK, v_fl, o);
       }
-      S.buf[l * AC_R + r] = make_float4(vv[0], vv[1], vv[2], vv[3]);
+      if (b == 0 && rw >= 0) {
+        RowScalars* out = B.sc + rw;
+        out->logp_like = -0.5f * chi2;
+        if (want_grad) { out->Mn_bar = v_mn; out->z_bar = v_z; out->AV_bar = v_av; out->delta_bar = v_de; out->Ffloor_bar = v_fl; }
+      }
+      S.sbar[r][b] = ok ? g * F * Mn : 0.f;
     }
-    __syncwarp();
   }
   if (!want_grad) return;
+  __syncwarp();
+  {
+    const int j = l & 15, hl = l >> 4;
+#pragma unroll 1
+    for (int k = 0; k < AC_R / 2; ++k) {
+      const int r = 2 * k + hl;
+      const int rw = S.rowid[r];
+      if (rw < 0) continue;
+      const float f = reinterpret_cast<const RowScalars*>(&S.sc[r][0])->zfrac;
+      float mb = 0.f;
+      if (j < T.n_Z)
+        for (int b = 0; b < T.n_band; ++b) mb = fmaf(S.sbar[r][b], S.Qs[r][0][j * T.n_band + b] + f * S.Qs[r][1][j * T.n_band + b], mb);
+      B.m_bar[(int64_t)rw * ROW_M_STRIDE + j] = mb;
+    }
+  }
+  float f8[AC_R];
+  {
+    int ej[4], eb[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const int e = min(4 * l + k, E - 1); ej[k] = e / T.n_band; eb[k] = e - ej[k] * T.n_band; }
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) {
+      f8[r] = reinterpret_cast<const RowScalars*>(&S.sc[r][0])->zfrac;
+      if (act) {
+        float vv[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) vv[k] = (4 * l + k < E && row[r] >= 0) ? S.sbar[r][eb[k]] * S.ms[r][ej[k]] : 0.f;
+        S.buf[l * AC_R + r] = make_float4(vv[0], vv[1], vv[2], vv[3]);
+      }
+    }
+  }
   __syncwarp();
   // ---- pass 2 ----
   float acc[SPS_AGE_PER_LANE][AC_R];
