@@ -1,5 +1,6 @@
 // sps_kernels.cu -- prologue (a0-a5), approximate-photometry contraction (a7, a9, a10) and
 // epilogue (reverse of a0-a5 + prior) kernels.
+#include <algorithm>
 #include "sps_rows.cuh"
 
 #define WARPS_PER_BLOCK 8
@@ -136,48 +137,22 @@ struct ACWarp {
   float obs[AC_R][2][SPS_MAX_BAND];// (d_b, sigma_b) or (flux_bar_b, -) of the warp's rows
 };
 
-__global__ void __launch_bounds__(32 * AC_WARPS, 1)
-approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, const int* __restrict__ bins,
-                       const int* __restrict__ gal_of_row, const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
-                       const float* __restrict__ flux_bar, bool want_grad, RowBuffers B) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int nb = T.n_z - 1, stride = nb + 2;
-  const int* row_start = bins + stride; const int* cta_start = bins + 2 * stride;
-  if ((int)blockIdx.x >= cta_start[nb]) return;
-  int lo = 0, hi = nb;
-  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cta_start[mid] <= (int)blockIdx.x) lo = mid; else hi = mid; }
-  const int cell = lo;
-  const int r_begin = row_start[cell] + ((int)blockIdx.x - cta_start[cell]) * AC_ROWS_PER_CTA;
-  const int r_end = min(row_start[cell + 1], r_begin + AC_ROWS_PER_CTA);
-  const int cs4 = T.cs_stride >> 2;                         // float4 per table row (odd)
-  const int slice4 = T.n_age * cs4;                         // float4 per array
-  float4* s0 = reinterpret_cast<float4*>(smem_raw);
-  float4* s1 = s0 + slice4;
-  ACWarp* warps = reinterpret_cast<ACWarp*>(s0 + 2 * slice4 + 4);
-  // one thread streams the cell's two arrays (contiguous in HBM/L2) into shared memory with bulk async copies;
-  // meanwhile every warp stages its rows' weights
-  __shared__ __align__(8) unsigned long long load_bar;
-  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&load_bar);
-  if (threadIdx.x == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    const char* src = reinterpret_cast<const char*>(T.cssp + (int64_t)cell * 2 * T.n_age * T.cs_stride);
-    const uint32_t bytes = (uint32_t)(2 * slice4) * 16u;
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s0);
-    for (uint32_t off = 0; off < bytes; off += 16384u) {
-      const uint32_t len = min(16384u, bytes - off);
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(dst + off), "l"(src + off), "r"(len), "r"(bar) : "memory");
-    }
-  }
+__device__ __forceinline__ void ac_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  while (!ok)
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+}
+
+// One work item: up to 64 rows of one z cell; warp w owns rows r_begin + 8w .. + 7.
+__device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const float4* __restrict__ s0, const float4* __restrict__ s1,
+                                        int r_begin, int r_end, const int* __restrict__ order, const int* __restrict__ gal_of_row,
+                                        const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
+                                        const float* __restrict__ flux_bar, bool want_grad, const RowBuffers& B,
+                                        uint32_t bar, uint32_t parity, bool need_wait) {
   const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
   const int r0 = r_begin + w * AC_R;
-  if (r0 >= r_end) return;
-  ACWarp& S = warps[w];
+  const int cs4 = T.cs_stride >> 2;
+  if (r0 >= r_end) { if (need_wait) ac_wait(bar, parity); return; }
   int row[AC_R];
 #pragma unroll
   for (int r = 0; r < AC_R; ++r) row[r] = (r0 + r < r_end) ? order[r0 + r] : -1;
@@ -202,22 +177,23 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
       }
     }
   }
-  // stage a (transposed: a_T[i][r]) and m
+  // stage a (transposed: a_T[i][r], lane = age bin) and m
   {
-    float* aT = reinterpret_cast<float*>(S.buf);
 #pragma unroll
-    for (int r = 0; r < AC_R; ++r) {
+    for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+      float v[AC_R];
 #pragma unroll
-      for (int q = 0; q < SPS_AGE_PER_LANE; ++q) aT[(l + 32 * q) * AC_R + r] = row[r] >= 0 ? B.a[(int64_t)row[r] * ROW_A_STRIDE + l + 32 * q] : 0.f;
-      if (l < ROW_M_STRIDE) S.ms[r][l] = row[r] >= 0 ? B.m[(int64_t)row[r] * ROW_M_STRIDE + l] : 0.f;
+      for (int r = 0; r < AC_R; ++r) v[r] = row[r] >= 0 ? B.a[(int64_t)row[r] * ROW_A_STRIDE + l + 32 * q] : 0.f;
+      S.buf[2 * (l + 32 * q)] = make_float4(v[0], v[1], v[2], v[3]);
+      S.buf[2 * (l + 32 * q) + 1] = make_float4(v[4], v[5], v[6], v[7]);
+    }
+    if (l < ROW_M_STRIDE) {
+#pragma unroll
+      for (int r = 0; r < AC_R; ++r) S.ms[r][l] = row[r] >= 0 ? B.m[(int64_t)row[r] * ROW_M_STRIDE + l] : 0.f;
     }
   }
   __syncwarp();
-  {                                                         // wait for the table arrays
-    uint32_t ok = 0;
-    while (!ok)
-      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar) : "memory");
-  }
+  if (need_wait) ac_wait(bar, parity);
   const bool act = l < cs4;
   const int E = T.n_Z * T.n_band;
   // ---- pass 1 ----
@@ -352,6 +328,63 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
   }
 }
 
+// Persistent: one CTA per SM walks a contiguous range of the (cell-ordered) work items and reloads the two table
+// arrays only when the cell changes, so the 106 KB staging cost is paid ~once per cell per CTA instead of once per item.
+__global__ void __launch_bounds__(32 * AC_WARPS, 1)
+approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, const int* __restrict__ bins,
+                       const int* __restrict__ gal_of_row, const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
+                       const float* __restrict__ flux_bar, bool want_grad, RowBuffers B) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nb = T.n_z - 1, stride = nb + 2;
+  const int* row_start = bins + stride; const int* cta_start = bins + 2 * stride;
+  const int total = cta_start[nb];
+  const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
+  const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
+  const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
+  if (w_begin >= w_end) return;
+  const int cs4 = T.cs_stride >> 2;                         // float4 per table row (odd)
+  const int slice4 = T.n_age * cs4;                         // float4 per array
+  float4* s0 = reinterpret_cast<float4*>(smem_raw);
+  float4* s1 = s0 + slice4;
+  ACWarp* warps = reinterpret_cast<ACWarp*>(s0 + 2 * slice4 + 4);
+  __shared__ __align__(8) unsigned long long load_bar;
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&load_bar);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  int lo = 0, hi = nb;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cta_start[mid] <= w_begin) lo = mid; else hi = mid; }
+  int cell = lo, cur_cell = -1;
+  uint32_t parity = 1;                                      // flipped before each load: the first one completes phase 0
+  for (int w = w_begin; w < w_end; ++w) {
+    while (cta_start[cell + 1] <= w) ++cell;
+    const bool reload = cell != cur_cell;
+    if (reload) {
+      __syncthreads();                                      // every warp is done with the previous cell's arrays
+      parity ^= 1u;
+      cur_cell = cell;
+      if (threadIdx.x == 0) {
+        // one thread streams the cell's two arrays (contiguous in HBM/L2) into shared memory with bulk async copies
+        const char* src = reinterpret_cast<const char*>(T.cssp + (int64_t)cell * 2 * T.n_age * T.cs_stride);
+        const uint32_t bytes = (uint32_t)(2 * slice4) * 16u;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(s0);
+        for (uint32_t off = 0; off < bytes; off += 16384u) {
+          const uint32_t len = min(16384u, bytes - off);
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                       ::"r"(dst + off), "l"(src + off), "r"(len), "r"(bar) : "memory");
+        }
+      }
+    }
+    const int r_begin = row_start[cell] + (w - cta_start[cell]) * AC_ROWS_PER_CTA;
+    const int r_end = min(row_start[cell + 1], r_begin + AC_ROWS_PER_CTA);
+    ac_item(T, warps[threadIdx.x >> 5], s0, s1, r_begin, r_end, order, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, B, bar, parity, reload);
+    __syncwarp();
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Reverse of a0-a5 (a10) + skew-normal prior (a9): one warp per row contracts the stored per-bin partials (B.part)
 // with a_bar, m_bar, Mn_bar and the direct bars.  Only the cheap closed forms (C1, dt/dz, burst polynomial, MDF) are
@@ -372,6 +405,16 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     if (l == 0 && logp) logp[row] = sc.logp_like + lp;
     return;
   }
+  // all of the row's stored quantities are requested first: the kernel is a latency-bound stream over B.part
+  const float* part = B.part + row * (ROW_PARTS * ROW_A_STRIDE);
+  float abar[SPS_AGE_PER_LANE], pr[ROW_PARTS][SPS_AGE_PER_LANE];
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    abar[q] = B.a_bar[row * ROW_A_STRIDE + l + 32 * q];
+#pragma unroll
+    for (int k = 0; k < ROW_PARTS; ++k) pr[k][q] = part[k * ROW_A_STRIDE + l + 32 * q];
+  }
+  const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
   float th[SPS_NDIM], dth[SPS_NDIM];
   double zd_unused;
   load_params<false>(theta + row * SPS_NDIM, unbounded, P, th, dth, zd_unused);
@@ -382,13 +425,11 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
   float m_unused, dm_lz, dm_s;
   met_bin(T, th[7], th[8], m_unused, dm_lz, dm_s);
   const float Fb = th[4], inv_M = 1.f / sc.Msum, Mf = sc.Mn * inv_M;
-  const float* part = B.part + row * (ROW_PARTS * ROW_A_STRIDE);
-  float abar[SPS_AGE_PER_LANE], Ps[SPS_AGE_PER_LANE];
+  float Ps[SPS_AGE_PER_LANE];
   float s_fb = 0.f, s_pp = 0.f, s_ltp = 0.f, s_ltm = 0.f;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
-    abar[q] = B.a_bar[row * ROW_A_STRIDE + l + 32 * q];
-    Ps[q] = part[l + 32 * q] * inv_M;
+    Ps[q] = pr[0][q] * inv_M;
     s_fb += abar[q] * (Bq.P[q] - Ps[q]);                       // dL/dF_burst           (Eq. A6)
     s_pp += abar[q] * Ps[q];
     s_ltp += abar[q] * Bq.d_ltp[q];
@@ -400,11 +441,9 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     const float dMb = (l + 32 * q < T.n_age) ? (1.f - Fb) * inv_M * (abar[q] - s_pp) + sc.Mn_bar * Mf : 0.f;
-    const float* p = part + l + 32 * q;
-    s_tau += dMb * p[ROW_A_STRIDE]; s_al += dMb * p[2 * ROW_A_STRIDE]; s_be += dMb * p[3 * ROW_A_STRIDE]; s_t += dMb * p[4 * ROW_A_STRIDE];
+    s_tau += dMb * pr[1][q]; s_al += dMb * pr[2][q]; s_be += dMb * pr[3][q]; s_t += dMb * pr[4][q];
   }
   s_tau = warp_sum(s_tau); s_al = warp_sum(s_al); s_be = warp_sum(s_be); s_t = warp_sum(s_t);
-  const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
   const float s_lz = warp_sum(mb * dm_lz), s_s = warp_sum(mb * dm_s);
   float g = 0.f;
   switch (l) {
@@ -486,7 +525,9 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
   approx_hist_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins);
   approx_plan_kernel<<<1, 1024, 0, s>>>(nb, B.bins);
   approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
-  const unsigned grid = (unsigned)((n + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA + nb);
+  static int sm_count = 0;
+  if (!sm_count) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev); }
+  const unsigned grid = (unsigned)std::min<int64_t>(sm_count, (n + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA + nb);
   sps_prof_begin(SPS_K_APPROX, s);
   approx_contract_kernel<<<grid, 32 * AC_WARPS, approx_smem_bytes(T), s>>>(T, n, B.order, B.bins, gal_of_row, obs_flux, obs_sigma,
                                                                          flux_bar, want_grad, B);
