@@ -312,6 +312,27 @@ def test_nuts_warmup_and_hmc_agree(tiny):
     assert (np.abs(sn.mean(1) - sh.mean(1))[:, 0] <= 0.5 * sd[:, 0] + 0.02).all()
 
 
+def test_nuts_mixed_paths_config5_shape(tiny):
+    # BASELINE.json configs[4] in miniature: NUTS with the exact path on a subset of the galaxies and the approximate
+    # path on the rest (per-galaxy path mask).  Each galaxy's chains must reproduce the single-path run of that galaxy
+    # (same counter-based RNG streams: the result does not depend on how rows are grouped into launches).
+    cx = tiny
+    n_gal, n_chain = 6, 2
+    _, d, s = _observations(cx, n_gal, 71, frac=(0.05, 0.05))
+    mask = np.array([0, 1, 1, 0, 1, 1], np.int32)                      # 0 = exact, 1 = approximate
+    kw = dict(sampler=cx.sps.SAMPLER_NUTS, n_chain=n_chain, n_warmup=20, n_sample=20, max_depth=4, eps0=0.004, seed=3, keep_samples=True)
+    mixed = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path_of_gal=_dev(mask, torch.int32), **kw)
+    ms = mixed["samples"].cpu().numpy().reshape(n_gal, n_chain, 20, 13)
+    assert np.isfinite(ms).all()
+    for path in (0, 1):
+        single = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path=path, **kw)["samples"].cpu().numpy().reshape(n_gal, n_chain, 20, 13)
+        sel = mask == path
+        err = np.abs(ms[sel] - single[sel]) / np.maximum(1.0, np.abs(single[sel]))
+        assert err[:, :, :3].max() <= 1e-3                              # the first transitions agree tightly
+        assert np.median(err.reshape(sel.sum() * n_chain, -1).max(1)) <= 1e-2
+    assert (mixed["n_leapfrog"].cpu().numpy() >= 40).all()
+
+
 # ---- a6/a8/a10: exact path ---------------------------------------------------------------------------
 @pytest.mark.parametrize("kind,n", [("tiny", 200), ("full", 24)])
 def test_exact_flux_and_jacobian(kind, n, request, exact_kernels):
