@@ -76,8 +76,13 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 // bins[0][.] histogram, bins[1][.] first position of each cell in `order`, bins[2][.] first CTA of each cell,
 // bins[3][.] scatter cursors.
 // ---------------------------------------------------------------------------------------------
-#define AC_WARPS 8
-#define AC_R 8                                   // rows per warp, register-blocked
+#ifndef AC_WARPS
+#define AC_WARPS 16
+#endif
+#ifndef AC_R
+#define AC_R 4
+#endif
+//#define AC_R_DOC                                   // rows per warp, register-blocked
 #define AC_ROWS_PER_CTA (AC_WARPS * AC_R)
 
 __global__ void approx_hist_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
@@ -156,40 +161,43 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
   int row[AC_R];
 #pragma unroll
   for (int r = 0; r < AC_R; ++r) row[r] = (r0 + r < r_end) ? order[r0 + r] : -1;
-  // fetch everything the per-row band step needs now, so that its latency hides behind pass 1
+  // Request everything the item needs from global memory first (independent loads, all in flight together), then
+  // stage it: weights transposed (a_T[i][r], lane = age bin), m, RowScalars and observations of the 8 rows.
   {
-    const int rr = l >> 2, part = l & 3;                    // lane -> (row, quarter of its RowScalars)
-    const int rw = __shfl_sync(FULL_MASK, row[0], 0);       // (keeps row[] in registers: select by compile-time index below)
-    (void)rw;
-    int my_row = -1;
+    float av[SPS_AGE_PER_LANE][AC_R], mv[AC_R], o0[AC_R], o1[AC_R];
 #pragma unroll
-    for (int r = 0; r < AC_R; ++r) if (r == rr) my_row = row[r];
-    if (my_row >= 0) S.sc[rr][part] = reinterpret_cast<const float4*>(B.sc + my_row)[part];
-    if (l < T.n_band) {
+    for (int q = 0; q < SPS_AGE_PER_LANE; ++q)
 #pragma unroll
-      for (int r = 0; r < AC_R; ++r) {
-        if (row[r] < 0) continue;
-        if (flux_bar) S.obs[r][0][l] = flux_bar[(int64_t)row[r] * T.n_band + l];
+      for (int r = 0; r < AC_R; ++r) av[q][r] = row[r] >= 0 ? __ldg(B.a + (int64_t)row[r] * ROW_A_STRIDE + l + 32 * q) : 0.f;
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) {
+      mv[r] = (row[r] >= 0 && l < ROW_M_STRIDE) ? __ldg(B.m + (int64_t)row[r] * ROW_M_STRIDE + l) : 0.f;
+      o0[r] = o1[r] = 0.f;
+      if (row[r] >= 0 && l < T.n_band) {
+        if (flux_bar) o0[r] = __ldg(flux_bar + (int64_t)row[r] * T.n_band + l);
         else {
-          const int64_t gal = gal_of_row ? gal_of_row[row[r]] : row[r];
-          S.obs[r][0][l] = obs_flux[gal * T.n_band + l]; S.obs[r][1][l] = obs_sigma[gal * T.n_band + l];
+          const int64_t gal = gal_of_row ? __ldg(gal_of_row + row[r]) : row[r];
+          o0[r] = __ldg(obs_flux + gal * T.n_band + l); o1[r] = __ldg(obs_sigma + gal * T.n_band + l);
         }
       }
     }
-  }
-  // stage a (transposed: a_T[i][r], lane = age bin) and m
-  {
+    const int rr = l >> 2, part = l & 3;                    // lane -> (row, quarter of its RowScalars)
+    int my_row = -1;
+#pragma unroll
+    for (int r = 0; r < AC_R; ++r) if (r == rr) my_row = row[r];
+    float4 scv = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (my_row >= 0) scv = reinterpret_cast<const float4*>(B.sc + my_row)[part];
+    if (rr < AC_R) S.sc[rr][part] = scv;
 #pragma unroll
     for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
-      float v[AC_R];
 #pragma unroll
-      for (int r = 0; r < AC_R; ++r) v[r] = row[r] >= 0 ? B.a[(int64_t)row[r] * ROW_A_STRIDE + l + 32 * q] : 0.f;
-      S.buf[2 * (l + 32 * q)] = make_float4(v[0], v[1], v[2], v[3]);
-      S.buf[2 * (l + 32 * q) + 1] = make_float4(v[4], v[5], v[6], v[7]);
+      for (int h = 0; h < AC_R / 4; ++h)
+        S.buf[(AC_R / 4) * (l + 32 * q) + h] = make_float4(av[q][4 * h], av[q][4 * h + 1], av[q][4 * h + 2], av[q][4 * h + 3]);
     }
-    if (l < ROW_M_STRIDE) {
 #pragma unroll
-      for (int r = 0; r < AC_R; ++r) S.ms[r][l] = row[r] >= 0 ? B.m[(int64_t)row[r] * ROW_M_STRIDE + l] : 0.f;
+    for (int r = 0; r < AC_R; ++r) {
+      if (l < ROW_M_STRIDE) S.ms[r][l] = mv[r];
+      if (l < SPS_MAX_BAND) { S.obs[r][0][l] = o0[r]; S.obs[r][1][l] = o1[r]; }
     }
   }
   __syncwarp();
@@ -205,8 +213,12 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
 #pragma unroll 2
     for (int i = 0; i < T.n_age; ++i) {
       const float4 c0 = c0p[i * cs4], c1 = c1p[i * cs4];
-      const float4 alo = S.buf[2 * i], ahi = S.buf[2 * i + 1];
-      const float a8[AC_R] = {alo.x, alo.y, alo.z, alo.w, ahi.x, ahi.y, ahi.z, ahi.w};
+      float a8[AC_R];
+#pragma unroll
+      for (int h = 0; h < AC_R / 4; ++h) {
+        const float4 t4 = S.buf[(AC_R / 4) * i + h];
+        a8[4 * h] = t4.x; a8[4 * h + 1] = t4.y; a8[4 * h + 2] = t4.z; a8[4 * h + 3] = t4.w;
+      }
 #pragma unroll
       for (int r = 0; r < AC_R; ++r) {
         q0[r].x = fmaf(a8[r], c0.x, q0[r].x); q0[r].y = fmaf(a8[r], c0.y, q0[r].y); q0[r].z = fmaf(a8[r], c0.z, q0[r].z); q0[r].w = fmaf(a8[r], c0.w, q0[r].w);
