@@ -45,7 +45,8 @@ constexpr int ROW_BYTES = 128;                                        // bytes o
 constexpr int A_TILE_BYTES = BM * ROW_BYTES;                          // 16 KB
 constexpr int B_TILE_BYTES = BN_MAX * ROW_BYTES;                      // 32 KB
 constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;      // 96 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int CW_BYTES = 5 * BN_MAX * 4;                              // per-wavelength constants of the current tile (forward epilogue)
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256 + CW_BYTES;
 constexpr int EPI_WARPS = 8;
 constexpr int NUM_THREADS = 64 + 32 * EPI_WARPS;
 constexpr int TMEM_COLS = 512;
@@ -204,6 +205,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
   auto bar_tfull = [&](int b) { return bar_base + 32u + 8u * b; };
   auto bar_tempty = [&](int b) { return bar_base + 48u + 8u * b; };
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + STAGES * STAGE_BYTES + 64);
+  float* cw = reinterpret_cast<float*>(smem + STAGES * STAGE_BYTES + 256);   // [5][BN_MAX] lam, dlam, k0, drude, log2(lam/5500)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total = (MODE == 0) ? __ldg(G.plan + G.m_tiles) : G.m_tiles * G.n_tiles;
@@ -311,10 +313,19 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
           zp_min = lo; zp_max = hi;
         }
         const int n0 = nt * BN_MAX + half * COLS;
+        // the tile's per-wavelength constants go to shared memory once (coalesced), then are read as broadcasts
+        {
+          const int et = (int)threadIdx.x - 64;               // 0..255 over the epilogue warps = column of the tile
+          asm volatile("bar.sync 1, 256;" ::: "memory");     // every epilogue warp is done with the previous tile's constants
+          const float4 c0 = __ldg(&wconst[2 * (nt * BN_MAX + et)]);
+          const float l2 = __ldg(&wconst[2 * (nt * BN_MAX + et) + 1].x);
+          cw[et] = c0.x; cw[BN_MAX + et] = c0.y; cw[2 * BN_MAX + et] = c0.z; cw[3 * BN_MAX + et] = c0.w; cw[4 * BN_MAX + et] = l2;
+          asm volatile("bar.sync 1, 256;" ::: "memory");
+        }
         // bands whose (truncated) support can meet this warp's columns for some of its rows
         unsigned mask = 0;
         {
-          const float lam_lo = __ldg(&wconst[2 * n0].x) * zp_min * 0.999999f, lam_hi = __ldg(&wconst[2 * (n0 + COLS - 1)].x) * zp_max * 1.000001f;
+          const float lam_lo = cw[half * COLS] * zp_min * 0.999999f, lam_hi = cw[half * COLS + COLS - 1] * zp_max * 1.000001f;
 #pragma unroll
           for (int b = 0; b < SPS_MAX_BAND; ++b)
             if (b < T.n_band && lam_hi >= FC.lo[b] && lam_lo <= FC.hi[b]) mask |= 1u << b;
@@ -326,14 +337,24 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
           for (int c = 0; c < COLS / 8; ++c) {
             uint32_t v[8];
             TMEM_LD8(taddr + c * 8, v);
+            const int cb = half * COLS + c * 8;
+            float lam8[8], dl8[8], k08[8], dr8[8], l28[8];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const float4 a0 = *reinterpret_cast<const float4*>(cw + cb + 4 * h), a1 = *reinterpret_cast<const float4*>(cw + BN_MAX + cb + 4 * h);
+              const float4 a2 = *reinterpret_cast<const float4*>(cw + 2 * BN_MAX + cb + 4 * h), a3 = *reinterpret_cast<const float4*>(cw + 3 * BN_MAX + cb + 4 * h);
+              const float4 a4 = *reinterpret_cast<const float4*>(cw + 4 * BN_MAX + cb + 4 * h);
+              lam8[4 * h] = a0.x; lam8[4 * h + 1] = a0.y; lam8[4 * h + 2] = a0.z; lam8[4 * h + 3] = a0.w;
+              dl8[4 * h] = a1.x; dl8[4 * h + 1] = a1.y; dl8[4 * h + 2] = a1.z; dl8[4 * h + 3] = a1.w;
+              k08[4 * h] = a2.x; k08[4 * h + 1] = a2.y; k08[4 * h + 2] = a2.z; k08[4 * h + 3] = a2.w;
+              dr8[4 * h] = a3.x; dr8[4 * h + 1] = a3.y; dr8[4 * h + 2] = a3.z; dr8[4 * h + 3] = a3.w;
+              l28[4 * h] = a4.x; l28[4 * h + 1] = a4.y; l28[4 * h + 2] = a4.z; l28[4 * h + 3] = a4.w;
+            }
             tmem_ld_wait();
             float G0[8], G1[8], G2[8], G3[8], G4[8], lamz[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
-              const int k = n0 + c * 8 + j;
-              const float4 c0 = __ldg(&wconst[2 * k]);
-              const float l2r = __ldg(&wconst[2 * k + 1].x);
-              const float lam = c0.x, dl = c0.y, k0 = c0.z, dr = c0.w;
+              const float lam = lam8[j], dl = dl8[j], k0 = k08[j], dr = dr8[j], l2r = l28[j];
               // dust, Eq. (A8)-(A9) with the tabulated k0, Drude profile and log2(lam/lam_V) (R10)
               const float pw = exp2f(delta * l2r);
               const float br = fmaf(k0, pw, Eb * dr);
@@ -403,48 +424,56 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
 
 // ---- plan: per row tile, the wavelength range under some filter's support for the tile's redshifts -------------------
 // plan[0][m] = prefix of forward items, plan[1][m] = first wavelength tile, plan[2][m], plan[3][m] = k-block range (reverse)
-__global__ void __launch_bounds__(256) exact_plan_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
-                                                         int m_tiles, int BKe, int* __restrict__ plan, int plan_cap, unsigned long long* __restrict__ work) {
-  __shared__ int cnt[1024];
+// One CTA per row tile (thread = row): redshift range of the tile -> wavelength ranges; also counts the tile's
+// (row, wavelength) pairs under some filter's support (the algorithmic work reported by sps_exact_last_work).
+__global__ void __launch_bounds__(BM) exact_plan_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
+                                                        int BKe, int* __restrict__ plan, int plan_cap, unsigned long long* __restrict__ work) {
+  __shared__ float s_min[BM / 32], s_max[BM / 32];
+  __shared__ unsigned s_pairs[BM / 32];
+  const int m = blockIdx.x;
+  const int64_t r = (int64_t)m * BM + threadIdx.x;
   float obs_lo = 1e30f, obs_hi = 0.f;
   for (int b = 0; b < T.n_band; ++b) { obs_lo = fminf(obs_lo, FC.lo[b]); obs_hi = fmaxf(obs_hi, FC.hi[b]); }
-  for (int base = 0; base < m_tiles; base += 1024) {
-    for (int m = base + threadIdx.x; m < min(m_tiles, base + 1024); m += blockDim.x) {
-      float zmin = 1e30f, zmax = -1e30f;
-      const int64_t r1 = min(n, (int64_t)(m + 1) * BM);
-      unsigned long long pairs = 0;                            // (row, wavelength) pairs under some filter: the algorithmic work
-      for (int64_t r = (int64_t)m * BM; r < r1; ++r) {
-        const float z = B.sc[rows ? rows[r] : r].z; zmin = fminf(zmin, z); zmax = fmaxf(zmax, z);
-        const float rlo = obs_lo / (1.f + z), rhi = obs_hi / (1.f + z);
-        int a = 0, c = T.n_wave;
-        while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < rlo) a = mid + 1; else c = mid; }
-        const int first = a; c = T.n_wave;
-        while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= rhi) a = mid + 1; else c = mid; }
-        pairs += (unsigned long long)(a - first);
-      }
-      atomicAdd(work, pairs);
-      const float lo = obs_lo / (1.f + zmax) * 0.99999f, hi = obs_hi / (1.f + zmin) * 1.00001f;
-      int a = 0, c = T.n_wave;
-      while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
-      int k_lo = max(a - 1, 0);
-      a = k_lo; c = T.n_wave;
-      while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= hi) a = mid + 1; else c = mid; }
-      int k_hi = min(a, T.n_wave - 1);                       // inclusive
-      if (k_hi < k_lo) k_hi = k_lo;
-      const int nt_lo = k_lo / BN_MAX, nt_hi = k_hi / BN_MAX + 1;
-      plan[plan_cap + m] = nt_lo;
-      plan[2 * plan_cap + m] = k_lo / BKe;
-      plan[3 * plan_cap + m] = k_hi / BKe + 1;
-      cnt[m - base] = nt_hi - nt_lo;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      int acc = (base == 0) ? 0 : plan[base];
-      for (int m = base; m < min(m_tiles, base + 1024); ++m) { plan[m] = acc; acc += cnt[m - base]; }
-      plan[min(m_tiles, base + 1024)] = acc;
-    }
-    __syncthreads();
+  float zmin = 1e30f, zmax = -1e30f; unsigned pairs = 0;
+  if (r < n) {
+    const float z = B.sc[rows ? rows[r] : r].z; zmin = zmax = z;
+    const float rlo = obs_lo / (1.f + z), rhi = obs_hi / (1.f + z);
+    int a = 0, c = T.n_wave;
+    while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < rlo) a = mid + 1; else c = mid; }
+    const int first = a; c = T.n_wave;
+    while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= rhi) a = mid + 1; else c = mid; }
+    pairs = (unsigned)(a - first);
   }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    zmin = fminf(zmin, __shfl_xor_sync(FULL_MASK, zmin, o)); zmax = fmaxf(zmax, __shfl_xor_sync(FULL_MASK, zmax, o));
+    pairs += __shfl_xor_sync(FULL_MASK, pairs, o);
+  }
+  if ((threadIdx.x & 31) == 0) { s_min[threadIdx.x >> 5] = zmin; s_max[threadIdx.x >> 5] = zmax; s_pairs[threadIdx.x >> 5] = pairs; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long tot = 0;
+    for (int w = 0; w < BM / 32; ++w) { zmin = fminf(zmin, s_min[w]); zmax = fmaxf(zmax, s_max[w]); tot += s_pairs[w]; }
+    atomicAdd(work, tot);
+    const float lo = obs_lo / (1.f + zmax) * 0.99999f, hi = obs_hi / (1.f + zmin) * 1.00001f;
+    int a = 0, c = T.n_wave;
+    while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
+    const int k_lo = max(a - 1, 0);
+    a = k_lo; c = T.n_wave;
+    while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] <= hi) a = mid + 1; else c = mid; }
+    int k_hi = min(a, T.n_wave - 1);                         // inclusive
+    if (k_hi < k_lo) k_hi = k_lo;
+    plan[plan_cap + m] = k_lo / BN_MAX;
+    plan[2 * plan_cap + m] = k_lo / BKe;
+    plan[3 * plan_cap + m] = k_hi / BKe + 1;
+    plan[m] = k_hi / BN_MAX + 1 - k_lo / BN_MAX;             // number of wavelength tiles; exact_scan_kernel turns it into a prefix
+  }
+}
+__global__ void exact_scan_kernel(int m_tiles, int* __restrict__ plan) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  int acc = 0;
+  for (int m = 0; m < m_tiles; ++m) { const int c = plan[m]; plan[m] = acc; acc += c; }
+  plan[m_tiles] = acc;
 }
 
 // ---- operand generation -----------------------------------------------------------------------------------------
@@ -496,10 +525,11 @@ __global__ void tc_weights_kernel(TableDev T, int64_t n, const int* __restrict__
 // reverse A operand: SEDbar[r][k] = F_att(lam_k) dlam_k sum_b g_b T_b(lam_k (1+z))  (reverse of Eq. 3-4), split.
 // Only the k blocks of the row tile's plan range are written (the reverse GEMM reads nothing else).
 template <int PREC>
-__global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B,
+__global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
                                                         const float* __restrict__ gbuf, const float4* __restrict__ wconst,
                                                         const int* __restrict__ plan, int plan_cap,
                                                         typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  typedef typename Op<PREC>::T E;
   const int64_t r = blockIdx.x;
   const int m = (int)(r / BM);
   const int k_begin = plan[2 * plan_cap + m] * Op<PREC>::BK, k_end = plan[3 * plan_cap + m] * Op<PREC>::BK;
@@ -508,31 +538,43 @@ __global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, c
   if (threadIdx.x < SPS_MAX_BAND) g_s[threadIdx.x] = gbuf[r * SPS_MAX_BAND + threadIdx.x];
   if (threadIdx.x == 32) {
     const RowScalars sc = B.sc[rows ? rows[r] : r];
-    sc_s[0] = 1.f + sc.z; sc_s[1] = sc.AV; sc_s[2] = sc.delta; sc_s[3] = sc.Ffloor;
+    sc_s[0] = 1.f + sc.z; sc_s[1] = sc.AV * (1.f / 4.05f); sc_s[2] = sc.delta; sc_s[3] = sc.Ffloor;
   }
   __syncthreads();
-  for (int k = k_begin + threadIdx.x; k < k_end; k += 256) {
-    const float4 c0 = __ldg(&wconst[2 * k]);
-    float v = 0.f;
-    if (c0.y > 0.f) {
-      const float lamz = c0.x * sc_s[0];
-      float tsum = 0.f;
-      for (int b = 0; b < T.n_band; ++b) {
-        const float x = (lamz - T.filt_mu[b]) / T.filt_sigma[b];
-        if (fabsf(x) <= 5.f) tsum += g_s[b] * expf(-0.5f * x * x);
-      }
-      if (tsum != 0.f) {
-        const float l2r = __ldg(&wconst[2 * k + 1].x);
-        const float delta = sc_s[2], Ffl = sc_s[3];
-        const float pw = exp2f(delta * l2r);
-        float A = sc_s[1] * (1.f / 4.05f) * (c0.z * pw + (0.85f - 1.9f * delta) * c0.w);
-        if (!(A > 0.f)) A = 0.f;
-        const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
-        v = (Ffl + (1.f - Ffl) * Tt) * c0.y * tsum;
+  const float zp = sc_s[0], AVs = sc_s[1], delta = sc_s[2], Ffl = sc_s[3], Eb = 0.85f - 1.9f * delta;
+  for (int k = k_begin + 2 * threadIdx.x; k < k_end; k += 512) {              // two consecutive wavelengths per thread
+    float v[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const float4 c0 = __ldg(&wconst[2 * (k + u)]);
+      v[u] = 0.f;
+      if (c0.y > 0.f) {
+        const float lamz = c0.x * zp;
+        float tsum = 0.f;
+        for (int b = 0; b < T.n_band; ++b) {
+          const float x = fmaf(lamz, FC.isg[b], FC.nmu[b]);
+          if (fabsf(x) <= FILT_CUT) tsum = fmaf(g_s[b], exp2f(-x * x), tsum);
+        }
+        if (tsum != 0.f) {
+          const float l2r = __ldg(&wconst[2 * (k + u) + 1].x);
+          const float pw = exp2f(delta * l2r);
+          float A = AVs * fmaf(c0.z, pw, Eb * c0.w);
+          if (!(A > 0.f)) A = 0.f;
+          const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+          v[u] = fmaf(1.f - Ffl, Tt, Ffl) * c0.y * tsum;
+        }
       }
     }
     const int64_t o = r * T.n_wave_pad + k;
-    Op<PREC>::split(v, hi[o], lo[o]);
+    E h2[2], l2[2];
+    Op<PREC>::split(v[0], h2[0], l2[0]); Op<PREC>::split(v[1], h2[1], l2[1]);
+    if (sizeof(E) == 2) {
+      *reinterpret_cast<uint32_t*>(hi + o) = *reinterpret_cast<const uint32_t*>(h2);
+      *reinterpret_cast<uint32_t*>(lo + o) = *reinterpret_cast<const uint32_t*>(l2);
+    } else {
+      *reinterpret_cast<uint2*>(hi + o) = *reinterpret_cast<const uint2*>(h2);
+      *reinterpret_cast<uint2*>(lo + o) = *reinterpret_cast<const uint2*>(l2);
+    }
   }
 }
 
@@ -597,7 +639,8 @@ sps_status launch_forward(sps_table* t, TcState* S, int64_t n, const int* rows, 
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = T.n_wave_pad / BN_MAX; G.k_blocks = S->Kpad / S->BK; G.BN = BN_MAX; G.BK = S->BK;
   G.rows = rows; G.part = X->part; G.plan = S->plan; G.plan_cap = S->plan_cap;
   cudaMemsetAsync(S->work, 0, sizeof(unsigned long long), s);
-  exact_plan_kernel<<<1, 256, 0, s>>>(T, n, rows, t->rows, S->fc, G.m_tiles, S->BK, S->plan, S->plan_cap, S->work);
+  exact_plan_kernel<<<G.m_tiles, BM, 0, s>>>(T, n, rows, t->rows, S->fc, S->BK, S->plan, S->plan_cap, S->work);
+  exact_scan_kernel<<<1, 32, 0, s>>>(G.m_tiles, S->plan);
   const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_FWD, s);
   exact_gemm_kernel<0, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
@@ -610,7 +653,7 @@ template <int PREC>
 sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
   typedef typename Op<PREC>::T E;
   ExactState* X = t->exact; const TableDev& T = t->dev;
-  tc_sedbar_kernel<PREC><<<(unsigned)n, 256, 0, s>>>(T, n, rows, t->rows, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
+  tc_sedbar_kernel<PREC><<<(unsigned)n, 256, 0, s>>>(T, n, rows, t->rows, S->fc, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
   GemmArgs G; memset(&G, 0, sizeof(G));
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = S->nb; G.k_blocks = T.n_wave_pad / S->BK; G.BN = S->BNb; G.BK = S->BK;
   G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
