@@ -53,7 +53,7 @@ __device__ __forceinline__ void cosmic_time(const TableDev& T, double z_d, doubl
 __device__ __forceinline__ void sfr_node(float lx2, float alpha, float beta, float& f, float& q, float& fa, float& fb) {
   float xa = exp2f(fminf(alpha * lx2, 60.f));
   float xb = exp2f(fminf(-beta * lx2, 60.f));
-  f = __frcp_rn(xa + xb);
+  f = __fdividef(1.f, xa + xb);
   float f2 = f * f, lx = lx2 * LN2F;
   q = f2 * (alpha * xa - beta * xb);
   fa = -f2 * xa * lx;
@@ -62,7 +62,7 @@ __device__ __forceinline__ void sfr_node(float lx2, float alpha, float beta, flo
 __device__ __forceinline__ float sfr_value(float t, float tau, float alpha, float beta) {
   if (!(t > 0.f)) return 0.f;
   float lx2 = log2f(t / tau);
-  return __frcp_rn(exp2f(fminf(alpha * lx2, 60.f)) + exp2f(fminf(-beta * lx2, 60.f)));
+  return __fdividef(1.f, exp2f(fminf(alpha * lx2, 60.f)) + exp2f(fminf(-beta * lx2, 60.f)));
 }
 
 struct AgeQuad {                       // per lane: its (up to) 4 bins, for M_formed = 1
@@ -121,7 +121,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
           float t = t_mid + half * GL2_X[k], f, qq, fa, fb;
           sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
           s0 += f;
-          if (WANT_GRAD) { s1 += qq; s2 += fa; s3 += fb; s4 -= qq / t; }
+          if (WANT_GRAD) { s1 += qq; s2 += fa; s3 += fb; s4 -= __fdividef(qq, t); }
         }
       } else {
 #pragma unroll
@@ -129,30 +129,31 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
           float t = t_mid + half * GL4_X[k], f, qq, fa, fb, w = GL4_W[k];
           sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
           s0 += w * f;
-          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; s4 -= w * qq / t; }
+          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; s4 -= w * __fdividef(qq, t); }
         }
       }
       Q.dM[q] = half * s0;
       if (WANT_GRAD) { Q.g_tau[q] = half * s1 / tau; Q.g_al[q] = half * s2; Q.g_be[q] = half * s3; Q.g_t[q] = half * s4; }
     }
   }
-  // warp-cooperative bins
+  // warp-cooperative bins: 8-point Gauss-Legendre panels in v = ln t.
+  //  * the one bin that reaches t = 0 spans many panels: all 32 lanes share its nodes;
+  //  * the other old bins near t_obs need one or two panels each: four of them are integrated at once, 8 lanes per bin.
+  const float ln_tau = l2tau * LN2F;
+  const float w_target = fminf(fmaxf(6.5f / ab, 0.5f), 2.0f);
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     unsigned m = problem_mask[q];
-    while (m) {
-      const int src = __ffs(m) - 1;
-      m &= m - 1;
+    const unsigned mz = __ballot_sync(FULL_MASK, t_hi_q[q] > 0.f && !(t_lo_q[q] > 0.f)) & m;     // the bin touching t = 0
+    if (mz) {
+      const int src = __ffs(mz) - 1;
+      m &= ~mz;
       const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], src);
-      const float t_lo = __shfl_sync(FULL_MASK, t_lo_q[q], src);
       const float v_hi = logf(t_hi);
-      float v_lo = v_hi - 16.f / (beta + 1.f);
-      if (t_lo > 0.f) v_lo = fmaxf(v_lo, logf(t_lo));
-      const float dv = v_hi - v_lo;
-      const float w_target = fminf(fmaxf(6.5f / ab, 0.5f), 2.0f);
+      const float dv = 16.f / (beta + 1.f);
+      const float v_lo = v_hi - dv;
       const int n_pan = max(1, (int)ceilf(dv / w_target));
       const float wp = dv / (float)n_pan;
-      const float ln_tau = l2tau * LN2F;
       float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
       for (int n = l; n < n_pan * 8; n += 32) {
         const int pan = n >> 3, k = n & 7;
@@ -167,9 +168,52 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       if (WANT_GRAD) { s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3); }
       if (l == src) {
         Q.dM[q] = s0;
+        if (WANT_GRAD) { Q.g_tau[q] = s1 / tau; Q.g_al[q] = s2; Q.g_be[q] = s3; Q.g_t[q] = sfr_value(t_hi, tau, alpha, beta); }   // Leibniz, f(0) = 0
+      }
+    }
+    while (m) {
+      int srcs[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) { srcs[j] = m ? __ffs(m) - 1 : -1; m &= m - 1; }
+      const int sg = l >> 3, k = l & 7;
+      const int my_src = sg == 0 ? srcs[0] : (sg == 1 ? srcs[1] : (sg == 2 ? srcs[2] : srcs[3]));
+      const bool have = my_src >= 0;
+      const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], have ? my_src : 0);
+      const float t_lo = __shfl_sync(FULL_MASK, t_lo_q[q], have ? my_src : 0);
+      const float v_hi = logf(t_hi);
+      const float v_lo = fmaxf(v_hi - 16.f / (beta + 1.f), logf(t_lo));
+      const float dv = v_hi - v_lo;
+      int n_pan = have ? max(1, (int)ceilf(dv / w_target)) : 0;
+      const float wp = dv / (float)max(n_pan, 1);
+      int n_max = max(n_pan, __shfl_xor_sync(FULL_MASK, n_pan, 8));
+      n_max = max(n_max, __shfl_xor_sync(FULL_MASK, n_max, 16));
+      float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+      for (int pan = 0; pan < n_max; ++pan) {
+        if (pan < n_pan) {
+          const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
+          const float w = 0.5f * wp * GL8_W[k] * expf(v);
+          float f, qq, fa, fb;
+          sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
+          s0 += w * f;
+          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; }
+        }
+      }
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(FULL_MASK, s0, o);
+        if (WANT_GRAD) { s1 += __shfl_xor_sync(FULL_MASK, s1, o); s2 += __shfl_xor_sync(FULL_MASK, s2, o); s3 += __shfl_xor_sync(FULL_MASK, s3, o); }
+      }
+      // hand each result to the lane that owns the bin
+      const int rank = l == srcs[0] ? 0 : (l == srcs[1] ? 1 : (l == srcs[2] ? 2 : (l == srcs[3] ? 3 : -1)));
+      const int from = 8 * max(rank, 0);
+      const float r0 = __shfl_sync(FULL_MASK, s0, from);
+      float r1 = 0, r2 = 0, r3 = 0;
+      if (WANT_GRAD) { r1 = __shfl_sync(FULL_MASK, s1, from); r2 = __shfl_sync(FULL_MASK, s2, from); r3 = __shfl_sync(FULL_MASK, s3, from); }
+      if (rank >= 0) {
+        Q.dM[q] = r0;
         if (WANT_GRAD) {
-          Q.g_tau[q] = s1 / tau; Q.g_al[q] = s2; Q.g_be[q] = s3;
-          Q.g_t[q] = sfr_value(t_hi, tau, alpha, beta) - sfr_value(t_lo, tau, alpha, beta);   // Leibniz
+          Q.g_tau[q] = r1 / tau; Q.g_al[q] = r2; Q.g_be[q] = r3;
+          Q.g_t[q] = sfr_value(t_hi_q[q], tau, alpha, beta) - sfr_value(t_lo_q[q], tau, alpha, beta);   // Leibniz
         }
       }
     }
