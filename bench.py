@@ -193,7 +193,10 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
 # captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {
+    ("approx_contract", 40000): 49.0e6,   # profiles/r01_hmc_kernels_full.md: 47.69 MB read + 1.35 MB written (40,000 rows per launch)
+    ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
+}
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
