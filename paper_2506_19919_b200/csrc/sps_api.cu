@@ -117,7 +117,7 @@ sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* thet
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
                     cudaStream_t s) {
   const TableDev& T = t->dev;
-  launch_prologue(T, P, theta, n, unbounded, want_grad, rows, t->rows, s);
+  launch_prologue(T, P, theta, n, unbounded, want_grad, rows, t->rows, path == SPS_PATH_APPROX, s);
   if (path == SPS_PATH_APPROX) {
     launch_approx_contract(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, t->rows, s);
   } else {
@@ -140,7 +140,7 @@ extern "C" sps_status sps_weights(const sps_table* tc, const sps_prior* prior, c
   PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
   st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
   cudaStream_t s = (cudaStream_t)stream;
-  launch_prologue(t->dev, P, theta, n, unbounded != 0, false, nullptr, t->rows, s);
+  launch_prologue(t->dev, P, theta, n, unbounded != 0, false, nullptr, t->rows, false, s);
   launch_copy_weights(t->dev, n, t->rows, w_age, w_met, mstar, s);
   return sps_check_cuda(cudaGetLastError(), "sps_weights launch");
 }

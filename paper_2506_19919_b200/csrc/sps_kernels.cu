@@ -37,7 +37,7 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorDev& P
 template <bool WANT_GRAD>
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
-                const int* __restrict__ rows, RowBuffers B) {
+                const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
@@ -67,11 +67,12 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     sc.logp_like = 0.f; sc.Mn_bar = sc.z_bar = sc.AV_bar = sc.delta_bar = sc.Ffloor_bar = 0.f;
     sc.Msum = R.Msum; sc.pad1 = sc.pad2 = 0.f;
     B.sc[row] = sc;
+    if (hist) atomicAdd(&hist[sc.zbin], 1);                 // z-cell histogram for the approximate path's row grouping
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Grouping of the rows of a call by z cell (counting sort): rows of one cell share the two c_SSP arrays c_t, D_t
+// Grouping of the rows of a call by z cell (counting sort; the histogram is taken by the prologue): rows of one cell share the two c_SSP arrays c_t, D_t
 // (PAPER.md:87), so a CTA stages them in shared memory once for up to AC_ROWS_PER_CTA rows.
 // bins[0][.] histogram, bins[1][.] first position of each cell in `order`, bins[2][.] first CTA of each cell,
 // bins[3][.] scatter cursors.
@@ -85,10 +86,6 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 //#define AC_R_DOC                                   // rows per warp, register-blocked
 #define AC_ROWS_PER_CTA (AC_WARPS * AC_R)
 
-__global__ void approx_hist_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
-  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) atomicAdd(&hist[B.sc[rows ? rows[i] : i].zbin], 1);
-}
 __global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restrict__ bins) {
   __shared__ int s_rows[1024], s_ctas[1024];
   const int stride = nb + 2;
@@ -114,9 +111,16 @@ __global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restri
 }
 __global__ void approx_scatter_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int* __restrict__ cursor, int* __restrict__ order) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const int row = rows ? rows[i] : (int)i;
-  order[atomicAdd(&cursor[B.sc[row].zbin], 1)] = row;
+  const int lane = threadIdx.x & 31;
+  int row = -1, cell = -1 - lane;                            // idle lanes get distinct dummy keys
+  if (i < n) { row = rows ? rows[i] : (int)i; cell = B.sc[row].zbin; }
+  // chains of one galaxy sit in consecutive rows and mostly in one cell: one atomic per distinct cell per warp
+  const unsigned peers = __match_any_sync(FULL_MASK, cell);
+  const int leader = __ffs(peers) - 1;
+  int base = 0;
+  if (lane == leader && cell >= 0) base = atomicAdd(&cursor[cell], __popc(peers));
+  base = __shfl_sync(FULL_MASK, base, leader);
+  if (cell >= 0) order[base + __popc(peers & ((1u << lane) - 1u))] = row;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -509,11 +513,13 @@ __global__ void copy_flux_kernel(TableDev T, int64_t n, RowBuffers B, float* flu
 static inline unsigned blocks_for_rows(int64_t n) { return (unsigned)((n + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK); }
 
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, cudaStream_t s) {
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s) {
   if (n <= 0) return;
+  int* hist = nullptr;
+  if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, (T.n_z + 1) * sizeof(int), s); }
   sps_prof_begin(SPS_K_PROLOGUE, s);
-  if (want_grad) prologue_kernel<true><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
-  else prologue_kernel<false><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B);
+  if (want_grad) prologue_kernel<true><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
+  else prologue_kernel<false><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
@@ -533,8 +539,6 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
   if (n <= 0) return;
   const int nb = T.n_z - 1, stride = nb + 2;
   const unsigned eb = (unsigned)((n + 255) / 256);
-  cudaMemsetAsync(B.bins, 0, stride * sizeof(int), s);
-  approx_hist_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins);
   approx_plan_kernel<<<1, 1024, 0, s>>>(nb, B.bins);
   approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
   static int sm_count = 0;
@@ -544,7 +548,7 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
   approx_contract_kernel<<<grid, 32 * AC_WARPS, approx_smem_bytes(T), s>>>(T, n, B.order, B.bins, gal_of_row, obs_flux, obs_sigma,
                                                                          flux_bar, want_grad, B);
   sps_prof_end(SPS_K_APPROX, s);
-  sps_count_launch(4);
+  sps_count_launch(3);
 }
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s) {

@@ -21,7 +21,7 @@ struct RowBuffers {
 
 // kernels (sps_kernels.cu)
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, cudaStream_t s);
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s);
 void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);
