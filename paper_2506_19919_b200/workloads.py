@@ -195,6 +195,8 @@ def draw_theta_unbounded(prior: Prior, n: int, seed: int, z_uniform: tuple[float
     th = np.clip(th, prior.x0 - lim, prior.x0 + lim)
     if z_uniform is not None:
         zz = rng.uniform(z_uniform[0], z_uniform[1], n)
+        w = 1e-3 * (prior.y_hi[-1] - prior.y_lo[-1])             # U[0.1,3] reaches past the bound y_hi = 2.98: keep draws inside
+        zz = np.clip(zz, prior.y_lo[-1] + w, prior.y_hi[-1] - w)
         th[:, NDIM - 1] = _logit_inverse(zz, prior.y_lo[-1], prior.y_hi[-1], prior.k[-1], prior.x0[-1])
     return th
 

@@ -384,3 +384,66 @@ def test_loglike_grad_exact(kind, n_gal, request, exact_kernels):
     allow = eps_flux * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
     err = np.abs(g.cpu().numpy() - og) - allow
     assert (err / np.maximum(np.abs(og), floor * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled rows ---------------------------
+def test_full_size_approx_sampled(full):
+    # configs[2]: 2^20 rows through the approximate path, flux + VJP; 48 sampled rows against the oracle
+    cx = full
+    n = 1 << 20
+    thu = W.draw_theta_unbounded(cx.prior, n, W.CONFIGS["c3_approx"]["seed"], z_uniform=(0.1, 3.0)).astype(np.float32)
+    fb = np.random.default_rng(3).normal(size=(n, cx.grid.n_band)).astype(np.float32)
+    flux, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(thu), True, _dev(fb))
+    sel = np.random.default_rng(4).choice(n, 48, replace=False)
+    flux, tb = flux[_dev(sel, torch.int64)].cpu().numpy(), tb[_dev(sel, torch.int64)].cpu().numpy()
+    th, dth = M.bound(thu[sel].astype(np.float64), cx.P)
+    of, J = M.photometry_approx(th, cx.grid, cx.cssp())
+    J = J * dth[:, None, :]
+    assert _rel(flux, of).max() <= 1e-4
+    ref = np.einsum("rb,rbp->rp", fb[sel].astype(np.float64), J)
+    scale = np.einsum("rb,rbp->rp", np.abs(fb[sel]).astype(np.float64), np.abs(J))
+    assert (np.abs(tb - ref) / np.maximum(scale, 1e-3 * scale.max(1, keepdims=True))).max() <= 1e-3
+
+
+def test_full_size_exact_sampled(full):
+    # configs[1]: 8192 rows through the tensor-core exact path, flux + VJP; 12 sampled rows against the oracle
+    cx = full
+    n = 8192
+    thu = W.draw_theta_unbounded(cx.prior, n, W.CONFIGS["c2_exact"]["seed"], z_uniform=(0.1, 3.0)).astype(np.float32)
+    fb = np.random.default_rng(5).normal(size=(n, cx.grid.n_band)).astype(np.float32)
+    flux, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_EXACT, _dev(thu), True, _dev(fb))
+    assert cx.sps.sps_exact_last_work(cx.table) > 0.3 * n * cx.grid.n_wave      # the work restriction keeps ~40 % of the columns
+    sel = np.random.default_rng(6).choice(n, 12, replace=False)
+    flux, tb = flux.cpu().numpy()[sel], tb.cpu().numpy()[sel]
+    th, dth = M.bound(thu[sel].astype(np.float64), cx.P)
+    of, J = M.photometry_exact(th, cx.grid)
+    J = J * dth[:, None, :]
+    assert _rel(flux, of).max() <= 1e-4
+    ref = np.einsum("rb,rbp->rp", fb[sel].astype(np.float64), J)
+    scale = np.einsum("rb,rbp->rp", np.abs(fb[sel]).astype(np.float64), np.abs(J))
+    assert (np.abs(tb - ref) / np.maximum(scale, TC_FLOOR * scale.max(1, keepdims=True))).max() <= 1e-3
+
+
+def test_full_size_hmc_loglike_sampled(full):
+    # configs[3]'s launch: 10,000 galaxies x 4 chains = 40,000 rows of sps_loglike_grad on the approximate path
+    cx = full
+    n_gal, n_chain = 10000, 4
+    truth_u = W.draw_theta_unbounded(cx.prior, n_gal, W.CONFIGS["c4_hmc"]["seed"]).astype(np.float32)
+    f = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(truth_u)).cpu().numpy().astype(np.float64)
+    d, s = W.noisy_observations(f, 9, 0.05, 0.10)
+    d = d.astype(np.float32); s = s.astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    thu = (np.repeat(truth_u, n_chain, 0) + 0.2 * np.random.default_rng(8).normal(size=(n_gal * n_chain, 13)) / cx.P[2]).astype(np.float32)
+    lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+    sel = np.random.default_rng(10).choice(n_gal * n_chain, 64, replace=False)
+    olp, og, _ = M.logp_and_grad(thu[sel].astype(np.float64), cx.grid, cx.P, d[gal[sel]].astype(np.float64), s[gal[sel]].astype(np.float64),
+                                 "approx", cx.cssp())
+    assert (np.abs(lp.cpu().numpy()[sel] - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4
+    # Near the mode the likelihood gradient sum_b (d_b - f_b)/sigma_b^2 J_b is a difference of large terms: an fp32 flux
+    # error eps f_b enters as eps sum_b f_b/sigma_b^2 |J_b|; eps = 3e-6 is the fp32 rounding of a
+    # band flux (measured <= 2.5e-6), thirty times below north_star's flux tolerance.
+    th, dth = M.bound(thu[sel].astype(np.float64), cx.P)
+    of, J = M.photometry_approx(th, cx.grid, cx.cssp())
+    allow = 3e-6 * np.einsum("rb,rbp->rp", of / s[gal[sel]].astype(np.float64) ** 2, np.abs(J)) * dth
+    err = np.maximum(np.abs(g.cpu().numpy()[sel] - og) - allow, 0.0)
+    assert (err / np.maximum(np.abs(og), 1e-3 * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
