@@ -21,10 +21,10 @@
 // wavelength blocks in range.  Everything outside contributes exactly zero to Eq. (4) and is never computed.
 //
 // One persistent CTA per SM, 320 threads, warp-specialised:
-//   warp 0      TMA producer: 128B-swizzled K-major tiles (A_hi, A_lo: 128 rows; B_hi, B_lo: BN rows; 128 B of K per
-//               row) into a 2-stage, 96 KB/stage shared-memory ring, mbarrier complete_tx
+//   warp 0      TMA producer: 64B-swizzled K-major tiles (A_hi, A_lo: 128 rows; B_hi, B_lo: BN rows; 64 B of K per
+//               row) into a 4-stage, 48 KB/stage shared-memory ring, mbarrier complete_tx
 //   warp 1      allocates 512 TMEM columns (two 256-column fp32 accumulators) and issues tcgen05.mma
-//               (cta_group::1, M = 128, N = BN, 32 B of K per instruction): 12 MMAs per k block
+//               (cta_group::1, M = 128, N = BN, 32 B of K per instruction): 6 MMAs per k block
 //   warps 2-9   epilogue: tcgen05.ld of their 32 TMEM lanes (thread = row; two warps share a lane quarter and split
 //               the columns) while the MMA warp fills the other accumulator.
 //               forward: dust attenuation (Eq. A8-A9), redshifted Gaussian filters, trapezoid weight and the
@@ -40,11 +40,15 @@
 
 namespace {
 
-constexpr int BM = 128, BN_MAX = 256, STAGES = 2;
-constexpr int ROW_BYTES = 128;                                        // bytes of K per operand row per stage
-constexpr int A_TILE_BYTES = BM * ROW_BYTES;                          // 16 KB
-constexpr int B_TILE_BYTES = BN_MAX * ROW_BYTES;                      // 32 KB
-constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;      // 96 KB
+#ifndef TC_ROW_BYTES
+#define TC_ROW_BYTES 64
+#endif
+constexpr int BM = 128, BN_MAX = 256;
+constexpr int ROW_BYTES = TC_ROW_BYTES;                               // bytes of K per operand row per stage (= swizzle span)
+constexpr int STAGES = 256 / ROW_BYTES;                               // 192 KB of operand tiles in flight either way
+constexpr int A_TILE_BYTES = BM * ROW_BYTES;
+constexpr int B_TILE_BYTES = BN_MAX * ROW_BYTES;
+constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;      // 48 KB (64-byte rows) or 96 KB (128-byte rows)
 constexpr int CW_BYTES = 5 * BN_MAX * 4;                              // per-wavelength constants of the current tile (forward epilogue)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256 + CW_BYTES;
 constexpr int EPI_WARPS = 8;
@@ -55,14 +59,14 @@ constexpr int TMEM_COLS = 512;
 template <int PREC> struct Op;
 template <> struct Op<SPS_EXACT_TF32X3> {
   typedef float T;
-  static constexpr int BK = 32;                                      // elements per 128-byte row
+  static constexpr int BK = ROW_BYTES / 4;                           // elements per operand row of a k block
   static constexpr uint32_t FMT = 2;                                 // instruction-descriptor format code (TF32)
   static __device__ __forceinline__ float rna(float v) { uint32_t u; asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(u) : "f"(v)); return __uint_as_float(u); }
   static __device__ __forceinline__ void split(float v, T& hi, T& lo) { hi = rna(v); lo = rna(v - hi); }
 };
 template <> struct Op<SPS_EXACT_BF16X3> {
   typedef __nv_bfloat16 T;
-  static constexpr int BK = 64;
+  static constexpr int BK = ROW_BYTES / 2;
   static constexpr uint32_t FMT = 1;                                 // BF16
   static __device__ __forceinline__ void split(float v, T& hi, T& lo) { hi = __float2bfloat16_rn(v); lo = __float2bfloat16_rn(v - __bfloat162float(hi)); }
 };
@@ -133,13 +137,13 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
-// K-major operand tile with 128-byte rows, SWIZZLE_128B: 8-row atoms of 1024 B stacked along M/N (SBO = 1024)
+// K-major operand tile whose rows are one swizzle span (64 or 128 bytes): 8-row atoms stacked along M/N (SBO = 8 rows)
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
   d |= (uint64_t)1 << 16;
-  d |= (uint64_t)(1024 >> 4) << 32;
+  d |= (uint64_t)((8 * ROW_BYTES) >> 4) << 32;
   d |= (uint64_t)1 << 46;            // descriptor version (sm_100)
-  d |= (uint64_t)2 << 61;            // SWIZZLE_128B
+  d |= (uint64_t)(ROW_BYTES == 128 ? 2 : 4) << 61;   // SWIZZLE_128B / SWIZZLE_64B
   return d;
 }
 #define TMEM_LD8(taddr, v)                                                                                             \
@@ -199,12 +203,12 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   const uint32_t smem_base = smem_u32(smem);
   const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
-  // barriers: full[s] +0, empty[s] +16, tfull[b] +32, tempty[b] +48 ; tmem pointer +64
+  // barriers: full[s] +0, empty[s] +32, tfull[b] +64, tempty[b] +80 ; tmem pointer +96
   auto bar_full = [&](int s) { return bar_base + 8u * s; };
-  auto bar_empty = [&](int s) { return bar_base + 16u + 8u * s; };
-  auto bar_tfull = [&](int b) { return bar_base + 32u + 8u * b; };
-  auto bar_tempty = [&](int b) { return bar_base + 48u + 8u * b; };
-  volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + STAGES * STAGE_BYTES + 64);
+  auto bar_empty = [&](int s) { return bar_base + 32u + 8u * s; };
+  auto bar_tfull = [&](int b) { return bar_base + 64u + 8u * b; };
+  auto bar_tempty = [&](int b) { return bar_base + 80u + 8u * b; };
+  volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + STAGES * STAGE_BYTES + 96);
   float* cw = reinterpret_cast<float*>(smem + STAGES * STAGE_BYTES + 256);   // [5][BN_MAX] lam, dlam, k0, drude, log2(lam/5500)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -220,7 +224,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar_base + 64u), "r"(TMEM_COLS) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar_base + 96u), "r"(TMEM_COLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
@@ -604,7 +608,7 @@ sps_status make_map(const TcState* S, CUtensorMap* m, const void* base, uint64_t
   const cuuint32_t box[2] = {(cuuint32_t)S->BK, box_rows};
   const cuuint32_t es[2] = {1, 1};
   const CUresult r = g_encode(m, S->prec == SPS_EXACT_BF16X3 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
-                              const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, ROW_BYTES == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { sps_set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return SPS_ECUDA; }
   return SPS_OK;
