@@ -20,12 +20,12 @@
 // support at those redshifts are touched: forward items = (row tile, wavelength tile in range), reverse k loop =
 // wavelength blocks in range.  Everything outside contributes exactly zero to Eq. (4) and is never computed.
 //
-// One persistent CTA per SM, 320 threads, warp-specialised:
+// One persistent CTA per SM, 576 threads, warp-specialised:
 //   warp 0      TMA producer: 64B-swizzled K-major tiles (A_hi, A_lo: 128 rows; B_hi, B_lo: BN rows; 64 B of K per
 //               row) into a 4-stage, 48 KB/stage shared-memory ring, mbarrier complete_tx
 //   warp 1      allocates 512 TMEM columns (two 256-column fp32 accumulators) and issues tcgen05.mma
 //               (cta_group::1, M = 128, N = BN, 32 B of K per instruction): 6 MMAs per k block
-//   warps 2-9   epilogue: tcgen05.ld of their 32 TMEM lanes (thread = row; two warps share a lane quarter and split
+//   warps 2-17  epilogue: tcgen05.ld of their 32 TMEM lanes (thread = row; four warps share a lane quarter and split
 //               the columns) while the MMA warp fills the other accumulator.
 //               forward: dust attenuation (Eq. A8-A9), redshifted Gaussian filters, trapezoid weight and the
 //               reduction over wavelength (Eq. 3-4) fused on the accumulators -- S never reaches HBM; flux and
@@ -51,7 +51,11 @@ constexpr int B_TILE_BYTES = BN_MAX * ROW_BYTES;
 constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;      // 48 KB (64-byte rows) or 96 KB (128-byte rows)
 constexpr int CW_BYTES = 5 * BN_MAX * 4;                              // per-wavelength constants of the current tile (forward epilogue)
 constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256 + CW_BYTES;
-constexpr int EPI_WARPS = 8;
+#ifndef TC_EPI_WARPS
+#define TC_EPI_WARPS 16
+#endif
+constexpr int EPI_WARPS = TC_EPI_WARPS;                              // 4 TMEM lane quarters x EPI_PARTS column parts
+constexpr int EPI_PARTS = EPI_WARPS / 4;
 constexpr int NUM_THREADS = 64 + 32 * EPI_WARPS;
 constexpr int TMEM_COLS = 512;
 
@@ -150,6 +154,9 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"                               \
                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])        \
                : "r"(taddr))
+#define TMEM_LD4(taddr, v)                                                                                             \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"                                           \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(taddr))
 #define TMEM_LD16(taddr, v)                                                                                            \
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
                : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
@@ -165,7 +172,7 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
   do {                                                                                                \
     if (cur_m >= 0 && valid) {                                                                        \
       float* p = G.part + r * 5 * SPS_MAX_BAND;                                                       \
-      _Pragma("unroll") for (int b = 0; b < SPS_MAX_BAND; ++b) {                                      \
+      _Pragma("unroll") for (int b = 0; b < NB; ++b) {                                      \
         if (b < T.n_band) {                                                                           \
           if (s0[b] != 0.f) atomicAdd(p + b, s0[b]);                                                  \
           if (s1[b] != 0.f) atomicAdd(p + SPS_MAX_BAND + b, s1[b]);                                   \
@@ -175,7 +182,7 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
         }                                                                                             \
       }                                                                                               \
     }                                                                                                 \
-    _Pragma("unroll") for (int b = 0; b < SPS_MAX_BAND; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f; \
+    _Pragma("unroll") for (int b = 0; b < NB; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f; \
   } while (0)
 
 // Work items.  forward: item w -> (row tile m, wavelength tile nt) through the per-row-tile prefix plan[0][m] and
@@ -194,7 +201,7 @@ struct ItemCursor {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-template <int MODE, int PREC>     // MODE 0: forward with the fused photometry epilogue, 1: reverse with a store epilogue
+template <int MODE, int PREC, int NB>   // MODE 0: forward with the fused photometry epilogue (NB = compiled band slots), 1: reverse, store epilogue
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constant__ CUtensorMap tmAl,
                   const __grid_constant__ CUtensorMap tmBh, const __grid_constant__ CUtensorMap tmBl,
@@ -287,14 +294,14 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
   } else {
     // ===== epilogue warps ==========================================================================
     const int q = warp & 3;                                  // TMEM lane quarter this warp may read
-    const int half = (warp - 2) >> 2;                        // which half of the tile's columns
+    const int half = (warp - 2) >> 2;                        // which part of the tile's columns
     const int row_in_tile = q * 32 + lane;
     int buf = 0; uint32_t bphase = 0;
     if (MODE == 0) {
-      constexpr int COLS = BN_MAX / 2;
-      float s0[SPS_MAX_BAND], s1[SPS_MAX_BAND], s2[SPS_MAX_BAND], s3[SPS_MAX_BAND], s4[SPS_MAX_BAND];
+      constexpr int COLS = BN_MAX / EPI_PARTS;
+      float s0[NB], s1[NB], s2[NB], s3[NB], s4[NB];
 #pragma unroll
-      for (int b = 0; b < SPS_MAX_BAND; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f;
+      for (int b = 0; b < NB; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f;
       int cur_m = -1; int64_t r = 0; bool valid = false;
       float zp = 1.f, AVs = 0.f, delta = 0.f, Ffl = 1.f, Eb = 0.85f, zp_min = 1.f, zp_max = 1.f;
       for (int w = w_begin; w < w_end; ++w) {
@@ -320,31 +327,34 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
         // the tile's per-wavelength constants go to shared memory once (coalesced), then are read as broadcasts
         {
           const int et = (int)threadIdx.x - 64;               // 0..255 over the epilogue warps = column of the tile
-          asm volatile("bar.sync 1, 256;" ::: "memory");     // every epilogue warp is done with the previous tile's constants
-          const float4 c0 = __ldg(&wconst[2 * (nt * BN_MAX + et)]);
-          const float l2 = __ldg(&wconst[2 * (nt * BN_MAX + et) + 1].x);
-          cw[et] = c0.x; cw[BN_MAX + et] = c0.y; cw[2 * BN_MAX + et] = c0.z; cw[3 * BN_MAX + et] = c0.w; cw[4 * BN_MAX + et] = l2;
-          asm volatile("bar.sync 1, 256;" ::: "memory");
+          asm volatile("bar.sync 1, %0;" ::"n"(32 * EPI_WARPS) : "memory");   // every epilogue warp is done with the previous tile's constants
+          if (et < BN_MAX) {
+            const float4 c0 = __ldg(&wconst[2 * (nt * BN_MAX + et)]);
+            const float l2 = __ldg(&wconst[2 * (nt * BN_MAX + et) + 1].x);
+            cw[et] = c0.x; cw[BN_MAX + et] = c0.y; cw[2 * BN_MAX + et] = c0.z; cw[3 * BN_MAX + et] = c0.w; cw[4 * BN_MAX + et] = l2;
+          }
+          asm volatile("bar.sync 1, %0;" ::"n"(32 * EPI_WARPS) : "memory");
         }
         // bands whose (truncated) support can meet this warp's columns for some of its rows
         unsigned mask = 0;
         {
           const float lam_lo = cw[half * COLS] * zp_min * 0.999999f, lam_hi = cw[half * COLS + COLS - 1] * zp_max * 1.000001f;
 #pragma unroll
-          for (int b = 0; b < SPS_MAX_BAND; ++b)
+          for (int b = 0; b < NB; ++b)
             if (b < T.n_band && lam_hi >= FC.lo[b] && lam_lo <= FC.hi[b]) mask |= 1u << b;
         }
         mbar_wait(bar_tfull(buf), bphase);
         tc_fence_after();
         if (mask != 0) {
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * BN_MAX + half * COLS);
-          for (int c = 0; c < COLS / 8; ++c) {
-            uint32_t v[8];
-            TMEM_LD8(taddr + c * 8, v);
-            const int cb = half * COLS + c * 8;
-            float lam8[8], dl8[8], k08[8], dr8[8], l28[8];
+          constexpr int CH = EPI_WARPS > 8 ? 4 : 8;          // columns per step: fewer live registers with more warps
+          for (int c = 0; c < COLS / CH; ++c) {
+            uint32_t v[CH];
+            if (CH == 8) { TMEM_LD8(taddr + c * CH, v); } else { TMEM_LD4(taddr + c * CH, v); }
+            const int cb = half * COLS + c * CH;
+            float lam8[CH], dl8[CH], k08[CH], dr8[CH], l28[CH];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
+            for (int h = 0; h < CH / 4; ++h) {
               const float4 a0 = *reinterpret_cast<const float4*>(cw + cb + 4 * h), a1 = *reinterpret_cast<const float4*>(cw + BN_MAX + cb + 4 * h);
               const float4 a2 = *reinterpret_cast<const float4*>(cw + 2 * BN_MAX + cb + 4 * h), a3 = *reinterpret_cast<const float4*>(cw + 3 * BN_MAX + cb + 4 * h);
               const float4 a4 = *reinterpret_cast<const float4*>(cw + 4 * BN_MAX + cb + 4 * h);
@@ -355,9 +365,9 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
               l28[4 * h] = a4.x; l28[4 * h + 1] = a4.y; l28[4 * h + 2] = a4.z; l28[4 * h + 3] = a4.w;
             }
             tmem_ld_wait();
-            float G0[8], G1[8], G2[8], G3[8], G4[8], lamz[8];
+            float G0[CH], G1[CH], G2[CH], G3[CH], G4[CH], lamz[CH];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            for (int j = 0; j < CH; ++j) {
               const float lam = lam8[j], dl = dl8[j], k0 = k08[j], dr = dr8[j], l2r = l28[j];
               // dust, Eq. (A8)-(A9) with the tabulated k0, Drude profile and log2(lam/lam_V) (R10)
               const float pw = exp2f(delta * l2r);
@@ -371,11 +381,11 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
               G4[j] = G0[j] * lam; lamz[j] = lam * zp;
             }
 #pragma unroll
-            for (int b = 0; b < SPS_MAX_BAND; ++b) {
+            for (int b = 0; b < NB; ++b) {
               if (mask & (1u << b)) {
                 const float isg = FC.isg[b], nmu = FC.nmu[b], dzf = FC.dz[b];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < CH; ++j) {
                   const float x = fmaf(lamz[j], isg, nmu);
                   const float Tb = (fabsf(x) <= FILT_CUT) ? exp2f(-x * x) : 0.f;
                   s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
@@ -400,7 +410,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
         tc_fence_after();
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)buf * BN_MAX;
         float* dst = G.Wbar + r * G.ldw + nt * G.BN;
-        for (int c = half; c < G.BN / 16; c += 2) {
+        for (int c = half; c < G.BN / 16; c += EPI_PARTS) {
           uint32_t v[16];
           TMEM_LD16(taddr + c * 16, v);
           tmem_ld_wait();
@@ -629,8 +639,10 @@ sps_status build_tables(const TableDev& T, TcState* S, size_t lc_rows) {
   build_wconst_kernel<<<(T.n_wave_pad + 255) / 256, 256>>>(T, S->wconst);
   sps_count_launch(3);
   sps_status st = sps_check_cuda(cudaDeviceSynchronize(), "tensor-core operand build");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<1, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<1, PREC, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
   return st;
 }
 
@@ -647,7 +659,9 @@ sps_status launch_forward(sps_table* t, TcState* S, int64_t n, const int* rows, 
   exact_scan_kernel<<<1, 32, 0, s>>>(G.m_tiles, S->plan);
   const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_FWD, s);
-  exact_gemm_kernel<0, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+  if (T.n_band <= 4) exact_gemm_kernel<0, PREC, 4><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+  else if (T.n_band <= 10) exact_gemm_kernel<0, PREC, 10><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+  else exact_gemm_kernel<0, PREC, 16><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
   sps_prof_end(SPS_K_EXACT_FWD, s);
   sps_count_launch(3);
   return sps_check_cuda(cudaGetLastError(), "exact forward (tcgen05) launch");
@@ -663,7 +677,7 @@ sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows,
   G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
   const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_BWD, s);
-  exact_gemm_kernel<1, PREC><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mSB_hi, S->mSB_lo, S->mLc_hi, S->mLc_lo, T, t->rows, G, S->fc, S->wconst);
+  exact_gemm_kernel<1, PREC, 1><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mSB_hi, S->mSB_lo, S->mLc_hi, S->mLc_lo, T, t->rows, G, S->fc, S->wconst);
   sps_prof_end(SPS_K_EXACT_BWD, s);
   sps_count_launch(2);
   return sps_check_cuda(cudaGetLastError(), "exact reverse (tcgen05) launch");
