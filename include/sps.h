@@ -128,6 +128,13 @@ typedef struct {
   float   eps0;           /* initial step size                                                        */
   float   target_accept;  /* dual-averaging target (0.8)                                              */
   uint64_t seed;          /* Philox4x32-10 key (R16)                                                  */
+  /* Continuing chains (unconverged fits "require an additional ~N_steps"): the transition counter of the
+   * RNG streams starts at first_transition, and the adapted step sizes / inverse masses of an earlier run are taken
+   * instead of (eps0, unit mass) when the DEVICE arrays below are non-NULL.  With theta0 = the earlier run's theta_last,
+   * n_warmup = 0 and first_transition = transitions already done, a run continues exactly where it stopped. */
+  uint32_t first_transition;
+  const float* eps_in_dev;       /* [n_gal*n_chain]    or NULL */
+  const float* inv_mass_in_dev;  /* [n_gal*n_chain,13] or NULL */
 } sps_hmc_config;
 
 /* Per-chain summaries, DEVICE pointers, any may be NULL.  Chain index c = gal*n_chain + chain. */
@@ -140,6 +147,7 @@ typedef struct {
   int32_t* n_leapfrog;  /* [n_gal*n_chain]    total leapfrog steps taken                              */
   int32_t* divergences; /* [n_gal*n_chain]    divergent transitions in the sampling phase             */
   float* rhat;          /* [n_gal,13]         Gelman-Rubin statistic over the galaxy's chains */
+  float* theta_last;    /* [n_gal*n_chain,13] state of every chain after its last transition (to continue from)     */
 } sps_hmc_summary;
 
 /* sps_hmc_run: n_gal galaxies x n_chain chains of (n_warmup + n_sample) transitions.

@@ -41,11 +41,12 @@ class _Prior(C.Structure):
 class _HmcConfig(C.Structure):
     _fields_ = [("sampler", C.c_int32), ("path", C.c_int32), ("n_chain", C.c_int32), ("n_warmup", C.c_int32),
                 ("n_sample", C.c_int32), ("n_leapfrog", C.c_int32), ("max_depth", C.c_int32), ("eps0", C.c_float),
-                ("target_accept", C.c_float), ("seed", C.c_uint64)]
+                ("target_accept", C.c_float), ("seed", C.c_uint64),
+                ("first_transition", C.c_uint32), ("eps_in", C.c_void_p), ("inv_mass_in", C.c_void_p)]
 
 
 class _HmcSummary(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat")]
+    _fields_ = [(n, C.c_void_p) for n in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last")]
 
 
 _lib = None
@@ -182,7 +183,7 @@ def sps_leapfrog(table, prior, path, theta0, p0, eps, inv_mass, obs_flux, obs_si
 
 def sps_hmc_run(table, prior, obs_flux, obs_sigma, *, sampler=SAMPLER_HMC, path=PATH_APPROX, n_chain=4, n_warmup=500,
                 n_sample=500, n_leapfrog=16, max_depth=8, eps0=0.05, target_accept=0.8, seed=1, path_of_gal=None,
-                theta0=None, keep_samples=False):
+                theta0=None, keep_samples=False, first_transition=0, eps_in=None, inv_mass_in=None):
     import torch
     n_gal = obs_flux.shape[0]
     nc = n_gal * n_chain
@@ -190,11 +191,12 @@ def sps_hmc_run(table, prior, obs_flux, obs_sigma, *, sampler=SAMPLER_HMC, path=
     f32 = lambda *s: torch.zeros(s, dtype=torch.float32, device=dev)
     i32 = lambda *s: torch.zeros(s, dtype=torch.int32, device=dev)
     out = dict(mean=f32(nc, NDIM), sd=f32(nc, NDIM), accept=f32(nc), eps=f32(nc), inv_mass=f32(nc, NDIM),
-               n_leapfrog=i32(nc), divergences=i32(nc), rhat=f32(n_gal, NDIM))
+               n_leapfrog=i32(nc), divergences=i32(nc), rhat=f32(n_gal, NDIM), theta_last=f32(nc, NDIM))
     samples = f32(nc, n_sample, NDIM) if keep_samples else None
     cfg = _HmcConfig(int(sampler), int(path), int(n_chain), int(n_warmup), int(n_sample), int(n_leapfrog), int(max_depth),
-                     float(eps0), float(target_accept), int(seed))
-    summ = _HmcSummary(*[out[k].data_ptr() for k in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat")])
+                     float(eps0), float(target_accept), int(seed), int(first_transition),
+                     eps_in.data_ptr() if eps_in is not None else None, inv_mass_in.data_ptr() if inv_mass_in is not None else None)
+    summ = _HmcSummary(*[out[k].data_ptr() for k in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last")])
     _check(lib().sps_hmc_run(table.handle, prior.ref(), C.byref(cfg), _dptr(obs_flux), _dptr(obs_sigma), C.c_int64(n_gal),
                              _dptr(path_of_gal), _dptr(theta0), _dptr(samples), C.byref(summ), _stream()), "sps_hmc_run")
     if keep_samples:

@@ -29,7 +29,7 @@ struct NutsScalars {
   int* depth_hist;             // [NUTS_MAX_DEPTH + 1] tree depths of the sampling phase
 };
 
-struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; };
+struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; int first; };
 
 __device__ __forceinline__ AdaptFlags adapt_flags_dev(int it, const WarmupSched& S) {
   AdaptFlags A; A.warmup = it < S.n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == S.n_warmup); A.welford_n = 0;
@@ -98,14 +98,14 @@ __device__ __forceinline__ void begin_doubling(ChainState& C, NutsScalars& S, in
   }
 }
 
-__global__ void __launch_bounds__(256) nuts_begin_kernel(ChainState C, NutsScalars S, uint2 key) {
+__global__ void __launch_bounds__(256) nuts_begin_kernel(ChainState C, NutsScalars S, int first, uint2 key) {
   CHAIN_WARP_PROLOGUE(C.n);
   const bool act = l < SPS_NDIM;
   const int64_t o = c * SPS_NDIM + (act ? l : 0);
   if (l == 0) { S.it[c] = 0; S.done[c] = 0; }
-  begin_transition(C, S, c, l, act, o, 0, key);
+  begin_transition(C, S, c, l, act, o, first, key);
   __syncwarp();
-  begin_doubling(C, S, c, l, act, o, 0, 0, 0, key);
+  begin_doubling(C, S, c, l, act, o, first, 0, 0, key);
 }
 
 // One leaf per call for every live chain (see the header).  `live` lists the chains to advance (NULL: all).
@@ -119,6 +119,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
   const bool act = l < SPS_NDIM;
   const int64_t o = c * SPS_NDIM + (act ? l : 0);
   const int it = S.it[c], depth = S.depth[c], leaf = S.leaf[c];
+  const int tr = it + W.first;                               // transition index of the RNG streams (continued runs)
   int flags = S.flags[c];
   const bool fwd = flags & F_FWD;
   const float v = C.inv_mass[o], eps = C.eps[c], step = fwd ? eps : -eps;
@@ -138,7 +139,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
   else {
     logW_sub = logaddexpf_(logW_sub, -dH);
     rho_sub = (act ? vec(C, c, V_SRHO)[l] : 0.f) + p;
-    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)it, RNG_LEAF, (uint32_t)(depth * 65536 + leaf)), key).x);
+    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)tr, RNG_LEAF, (uint32_t)(depth * 65536 + leaf)), key).x);
     if (logf(u) + logW_sub < -dH) {                       // multinomial sampling inside the subtree
       if (act) { vec(C, c, V_SQ)[l] = q; vec(C, c, V_SG)[l] = g; }
       if (l == 0) S.sub_lp[c] = lp;
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     }
     // ---- subtree complete: biased progressive sampling across doublings, merge ----
     const float logW = S.logW[c];
-    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)it, RNG_SUBTREE, (uint32_t)depth), key).x);
+    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)tr, RNG_SUBTREE, (uint32_t)depth), key).x);
     if ((flags & F_HASSUB) && logf(u) < fminf(0.f, logW_sub - logW)) {
       if (act) { vec(C, c, V_PQ)[l] = vec(C, c, V_SQ)[l]; vec(C, c, V_PG)[l] = vec(C, c, V_SG)[l]; }
       if (l == 0) S.prop_lp[c] = S.sub_lp[c];
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     finish = uturn(rho, pl, pr, v, act) || new_depth >= max_depth;
     if (!finish) {
       __syncwarp();
-      begin_doubling(C, S, c, l, act, o, it, new_depth, flags, key);
+      begin_doubling(C, S, c, l, act, o, tr, new_depth, flags, key);
       return;
     }
   }
@@ -207,9 +208,9 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     return;
   }
   if (l == 0) S.it[c] = it1;
-  begin_transition(C, S, c, l, act, o, it1, key);
+  begin_transition(C, S, c, l, act, o, it1 + W.first, key);
   __syncwarp();
-  begin_doubling(C, S, c, l, act, o, it1, 0, 0, key);
+  begin_doubling(C, S, c, l, act, o, it1 + W.first, 0, 0, key);
 }
 
 // live-chain lists per photometry path after some chains have finished
@@ -244,13 +245,13 @@ sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, 
   {
     std::vector<int> ends; int lo, hi;
     warmup_schedule(cfg->n_warmup, ends, lo, hi);
-    W.n_warmup = cfg->n_warmup; W.n_sample = cfg->n_sample; W.slow_lo = lo; W.slow_hi = hi; W.target = cfg->target_accept;
+    W.n_warmup = cfg->n_warmup; W.n_sample = cfg->n_sample; W.slow_lo = lo; W.slow_hi = hi; W.target = cfg->target_accept; W.first = (int)cfg->first_transition;
     W.n_ends = (int)std::min<size_t>(ends.size(), 16);
     for (int k = 0; k < W.n_ends; ++k) W.ends[k] = ends[k];
   }
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
   const unsigned cb = (unsigned)((n * 32 + 255) / 256);
-  nuts_begin_kernel<<<cb, 256, 0, s>>>(C, S, key); sps_count_launch();
+  nuts_begin_kernel<<<cb, 256, 0, s>>>(C, S, (int)cfg->first_transition, key); sps_count_launch();
   // live lists: start from the problem's own per-path lists (NULL = all rows on one path)
   HmcProblem L = Q;
   const int* live = nullptr; int64_t n_live = n;

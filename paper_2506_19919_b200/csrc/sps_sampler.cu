@@ -27,19 +27,21 @@ extern "C" sps_status sps_philox_words(uint64_t seed, uint32_t first_chain, uint
 // ---------------------------------------------------------------------------------------------
 // chain initialisation (R17): theta~_0 = xi + 0.1 omega N(0,1) from (chain, transition 0, purpose 5)
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) chain_init_kernel(ChainState C, PriorDev P, const float* __restrict__ theta0, float eps0, uint2 key) {
+__global__ void __launch_bounds__(256) chain_init_kernel(ChainState C, PriorDev P, const float* __restrict__ theta0, float eps0, const float* __restrict__ eps_in,
+                                                         const float* __restrict__ inv_mass_in, uint2 key) {
   CHAIN_WARP_PROLOGUE(C.n);
   if (l < SPS_NDIM) {
     float v;
     if (theta0) v = theta0[c * SPS_NDIM + l];
     else v = P.xi[l] + 0.1f * P.omega[l] * chain_normal(key, (uint32_t)c, 0u, RNG_INIT, l);
     C.theta[c * SPS_NDIM + l] = v;
-    C.inv_mass[c * SPS_NDIM + l] = 1.f;
+    C.inv_mass[c * SPS_NDIM + l] = inv_mass_in ? inv_mass_in[c * SPS_NDIM + l] : 1.f;
     C.w_mean[c * SPS_NDIM + l] = 0.f; C.w_m2[c * SPS_NDIM + l] = 0.f;
     C.s_mean[c * SPS_NDIM + l] = 0.f; C.s_m2[c * SPS_NDIM + l] = 0.f;
   }
   if (l == 0) {
-    C.eps[c] = eps0; C.da_mu[c] = logf(10.f * eps0); C.da_hbar[c] = 0.f; C.da_logepsbar[c] = 0.f; C.da_m[c] = 0;
+    const float e0 = eps_in ? eps_in[c] : eps0;
+    C.eps[c] = e0; C.da_mu[c] = logf(10.f * e0); C.da_hbar[c] = 0.f; C.da_logepsbar[c] = 0.f; C.da_m[c] = 0;
     C.acc_sum[c] = 0.f; C.n_leapfrog[c] = 0; C.n_div[c] = 0;
   }
 }
@@ -115,6 +117,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain
     if (S.mean) S.mean[o] = mu;
     if (S.sd) S.sd[o] = sqrtf(var);
     if (S.inv_mass) S.inv_mass[o] = C.inv_mass[o];
+    if (S.theta_last) S.theta_last[o] = C.theta[o];
     if (l == 0) {
       if (S.accept) S.accept[c] = C.acc_sum[c] / (float)max(n_sample, 1);
       if (S.eps) S.eps[c] = C.eps[c];
@@ -226,7 +229,7 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
   st = chain_state_alloc(C, n, cfg->sampler == SPS_SAMPLER_NUTS ? NUTS_VECTORS : 0);
   if (st != SPS_OK) { hmc_problem_free(Q); return st; }
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
-  chain_init_kernel<<<chain_blocks(n), 256, 0, s>>>(C, P, theta0, cfg->eps0, key); sps_count_launch();
+  chain_init_kernel<<<chain_blocks(n), 256, 0, s>>>(C, P, theta0, cfg->eps0, cfg->eps_in_dev, cfg->inv_mass_in_dev, key); sps_count_launch();
   // logp / grad at the start: evaluate through the working buffers
   cudaMemcpyAsync(C.theta_w, C.theta, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
   st = eval_working(t, P, Q, C, s);
@@ -237,13 +240,13 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
     warmup_schedule(cfg->n_warmup, ends, slow_lo, slow_hi);
     const unsigned eb = (unsigned)((n * SPS_NDIM + 255) / 256);
     for (int it = 0; it < cfg->n_warmup + cfg->n_sample && st == SPS_OK; ++it) {
-      hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it, key); sps_count_launch();
+      hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key); sps_count_launch();
       for (int k = 0; k < cfg->n_leapfrog && st == SPS_OK; ++k) {
         st = eval_working(t, P, Q, C, s);
         if (k + 1 < cfg->n_leapfrog) { leapfrog_mid_kernel<<<eb, 256, 0, s>>>(C); sps_count_launch(); }
       }
       const AdaptFlags A = adapt_flags_for(it, cfg->n_warmup, ends, slow_lo, slow_hi, cfg->target_accept);
-      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it, key, cfg->n_leapfrog, A, samples, it - cfg->n_warmup, cfg->n_sample);
+      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key, cfg->n_leapfrog, A, samples, it - cfg->n_warmup, cfg->n_sample);
       sps_count_launch();
     }
   } else if (st == SPS_OK) {

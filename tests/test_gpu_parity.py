@@ -333,6 +333,28 @@ def test_nuts_mixed_paths_config5_shape(tiny):
     assert (mixed["n_leapfrog"].cpu().numpy() >= 40).all()
 
 
+# ---- continuing chains (unconverged fits "require an additional ~N_steps") ----------------------------
+@pytest.mark.parametrize("sampler", ["hmc", "nuts"])
+def test_continued_run_equals_one_long_run(tiny, sampler):
+    cx = tiny
+    n_gal = 4
+    _, d, s = _observations(cx, n_gal, 81, frac=(0.05, 0.05))
+    smp = cx.sps.SAMPLER_HMC if sampler == "hmc" else cx.sps.SAMPLER_NUTS
+    kw = dict(sampler=smp, path=cx.sps.PATH_APPROX, n_chain=3, n_leapfrog=6, max_depth=4, seed=13, keep_samples=True)
+    # adapt once, then sample 40 transitions in one go and as 20 + 20 from the returned state
+    warm = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), n_warmup=60, n_sample=1, eps0=0.004, **kw)
+    state = dict(theta0=warm["theta_last"], eps_in=warm["eps"], inv_mass_in=warm["inv_mass"])
+    full = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), n_warmup=0, n_sample=40, first_transition=61, **state, **kw)
+    a = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), n_warmup=0, n_sample=20, first_transition=61, **state, **kw)
+    b = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), n_warmup=0, n_sample=20, first_transition=81,
+                           theta0=a["theta_last"], eps_in=a["eps"], inv_mass_in=a["inv_mass"], **kw)
+    assert torch.equal(a["eps"], warm["eps"]) and torch.equal(a["inv_mass"], warm["inv_mass"])
+    assert torch.equal(full["samples"][:, :20], a["samples"])
+    assert torch.equal(full["samples"][:, 20:], b["samples"])
+    assert torch.equal(full["theta_last"], b["theta_last"])
+    assert torch.equal(full["theta_last"], full["samples"][:, -1])
+
+
 # ---- a6/a8/a10: exact path ---------------------------------------------------------------------------
 @pytest.mark.parametrize("kind,n", [("tiny", 200), ("full", 24)])
 def test_exact_flux_and_jacobian(kind, n, request, exact_kernels):

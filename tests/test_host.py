@@ -36,9 +36,9 @@ def test_struct_layouts_match_the_header():
     from paper_2506_19919_b200 import binding as b
     assert C.sizeof(b._TableDesc) == 5 * 4 + 4 + 6 * 8 + 5 * 8 + 8       # 5 int32 (+pad), 6 pointers, 5 doubles, int32 (+pad)
     assert C.sizeof(b._Prior) == 7 * 8
-    assert C.sizeof(b._HmcConfig) == 7 * 4 + 2 * 4 + 4 + 8                # 7 int32, 2 float, pad, uint64
+    assert C.sizeof(b._HmcConfig) == 7 * 4 + 2 * 4 + 4 + 8 + 4 + 4 + 2 * 8  # 7 int32, 2 float, pad, uint64, uint32, pad, 2 pointers
     assert b._HmcConfig.seed.offset == 40
-    assert C.sizeof(b._HmcSummary) == 8 * 8
+    assert C.sizeof(b._HmcSummary) == 9 * 8
 
 
 def test_no_cpu_fallback(lib):
