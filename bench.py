@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the SPS hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4_hmc|c3_approx|c2_exact]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4_hmc|c3_approx|c2_exact|c5_nuts]
 
 Default workload = BASELINE.json configs[3] ("c4_hmc"): full HMC on the approximate path, 10,000 synthetic
 galaxies x 4 chains x (500 warmup + 500 samples) x 16 leapfrog steps; metric = galaxy posteriors per GPU-minute.
@@ -103,16 +103,29 @@ def run_ours(args):
     peaks, peaks_src = _peaks()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
 
-    if args.workload == "c4_hmc":
+    if args.workload in ("c4_hmc", "c5_nuts"):
         n_gal = args.n_gal or cfg["n_gal"]
         d, s = make_hmc_inputs(sps, W, table, ph, prior, n_gal, cfg["seed"], rank)
         d_host = torch.from_numpy(d).pin_memory(); s_host = torch.from_numpy(s).pin_memory()
         d_dev = d_host.cuda(); s_dev = s_host.cuda()
         kw = dict(sampler=sps.SAMPLER_HMC, path=sps.PATH_APPROX, n_chain=cfg["n_chain"], n_warmup=args.n_warmup or cfg["n_warmup"],
-                  n_sample=args.n_sample or cfg["n_sample"], n_leapfrog=cfg["n_leapfrog"], eps0=0.01, seed=cfg["seed"])
-        evals_per_step = n_gal * cfg["n_chain"] * (kw["n_warmup"] + kw["n_sample"]) * cfg["n_leapfrog"]
+                  n_sample=args.n_sample or cfg["n_sample"], n_leapfrog=cfg.get("n_leapfrog", 0), eps0=0.01, seed=cfg["seed"])
+        evals_per_step = n_gal * cfg["n_chain"] * (kw["n_warmup"] + kw["n_sample"]) * cfg.get("n_leapfrog", 0)
+        if args.workload == "c5_nuts":
+            # BASELINE.json configs[4]: NUTS, tree depth <= 8, exact path on a seeded 10 % of the galaxies (their data come
+            # from the exact path), approximate path on the rest; evaluations are counted from the chains' leapfrog totals
+            mask = (np.random.default_rng(cfg["seed"]).random(n_gal) >= cfg["exact_fraction"]).astype(np.int32)      # 1 = approximate
+            thu_x = W.draw_theta_unbounded(prior, n_gal, rank_seed(cfg["seed"], rank)).astype(np.float32)[mask == 0]
+            fx = sps.sps_photometry(table, ph, sps.PATH_EXACT, torch.tensor(thu_x, device="cuda")).cpu().numpy().astype(np.float64)
+            dx, sx = W.noisy_observations(fx, cfg["seed"] + 11, 0.05, 0.10)
+            d[mask == 0] = dx; s[mask == 0] = sx
+            kw.update(sampler=sps.SAMPLER_NUTS, max_depth=cfg["max_depth"], path_of_gal=torch.tensor(mask, device="cuda"))
+            kw.pop("n_leapfrog")
         units_per_step = n_gal                                                   # galaxy posteriors
-        step = lambda: sps.sps_hmc_run(table, ph, d_dev, s_dev, **kw)
+        last = {}
+
+        def step():
+            last["out"] = sps.sps_hmc_run(table, ph, d_dev, s_dev, **kw)
 
         def step_e2e():
             dd = d_host.cuda(non_blocking=True); ss = s_host.cuda(non_blocking=True)
@@ -166,11 +179,19 @@ def run_ours(args):
     # ---- timed region 2: end to end through the public API with host buffers -----------------------
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(args.steps if not args.no_e2e else 0):
         step_e2e()
     barrier()
-    e2e_s = time.perf_counter() - t0
+    e2e_s = (time.perf_counter() - t0) if not args.no_e2e else float("inf")
     dev_s, e2e_s = max_over_ranks([dev_s, e2e_s], dist, device="cuda")
+    extra = {}
+    if args.workload == "c5_nuts":
+        o = last["out"]
+        evals_per_step = int(o["n_leapfrog"].sum().item())
+        extra = {"mean_leapfrogs_per_transition": evals_per_step / (n_gal * cfg["n_chain"] * (kw["n_warmup"] + kw["n_sample"])),
+                 "rhat_below_1p2": float((o["rhat"].max(1).values < 1.2).float().mean().item()), "divergences": int(o["divergences"].sum().item())}
+    elif args.workload == "c4_hmc":
+        extra = {"rhat_below_1p2": float((last["out"]["rhat"].max(1).values < 1.2).float().mean().item())}
     pairs = sps.sps_exact_last_work(table) if args.workload == "c2_exact" else 0
     if rank != 0:
         return
@@ -183,7 +204,7 @@ def run_ours(args):
            "loglike_grad_evals_per_s": evals_per_step * args.steps * world / dev_s,
            "e2e": {"value": to_value(aggregate_throughput(units_per_step * args.steps, world, e2e_s), 1.0), "unit": unit, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h},
-           "gpu_launches": int(launches), "clocks": clk, "impl": "ours"}
+           "gpu_launches": int(launches), "clocks": clk, "impl": "ours", **extra}
     out["roofline"] = roofline(prof, dom_kernel, rows_per_launch, grid, peaks, peaks_src, pairs)
     out["kernel_ms"] = {k: {"avg_ms": (v[0] / v[1] if v[1] else None), "launches": v[2]} for k, v in prof.items() if v[2]}
     if not args.no_cpu_baseline:
@@ -236,9 +257,9 @@ def cpu_baseline(workload, cfg, budget_s=20.0):
     from paper_2506_19919_b200 import workloads as W
     grid = W.make_grid(cfg["grid"]); prior = W.make_prior(); P = prior.as_array()
     with threadpool_limits(limits=1):
-        if workload == "c4_hmc":
+        if workload in ("c4_hmc", "c5_nuts"):
             cssp = M.cssp_table(grid, M.z_grid(grid))          # setup, untimed (as for the GPU)
-            n_gal, n_chain, L = 2, cfg["n_chain"], cfg["n_leapfrog"]
+            n_gal, n_chain, L = 2, cfg["n_chain"], cfg.get("n_leapfrog", 16)
             thu = W.draw_theta_unbounded(prior, n_gal, cfg["seed"])
             f = M.photometry_approx(M.bound(thu, P)[0], grid, cssp)[0]
             d, s = W.noisy_observations(f, cfg["seed"] + 7, 0.05, 0.10)
@@ -283,7 +304,7 @@ def run_reference(args):
     res = [cpu_baseline(args.workload, cfg, budget_s=per_step) for _ in range(args.steps)]
     sec = time.perf_counter() - t0
     v = float(np.mean([r["value"] for r in res]))
-    hmc = args.workload == "c4_hmc"
+    hmc = args.workload in ("c4_hmc", "c5_nuts")
     out = {"impl": "reference", "metric": "galaxy posteriors/GPU-minute" if hmc else "flux+gradient evaluations/s", "value": v,
            "unit": res[0]["unit"], "n_gpus": int(os.environ.get("WORLD_SIZE", 1)), "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": 1e3 * sec / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -299,13 +320,14 @@ def main():
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4_hmc", choices=["c4_hmc", "c3_approx", "c2_exact"])
+    ap.add_argument("--workload", default="c4_hmc", choices=["c4_hmc", "c3_approx", "c2_exact", "c5_nuts"])
     ap.add_argument("--n-gal", type=int, default=0)
     ap.add_argument("--n-rows", type=int, default=0)
     ap.add_argument("--n-warmup", type=int, default=0)
     ap.add_argument("--n-sample", type=int, default=0)
     ap.add_argument("--cpu-budget", type=float, default=20.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (side workloads only; the e2e value is then 0)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

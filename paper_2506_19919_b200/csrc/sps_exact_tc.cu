@@ -164,6 +164,9 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
                : "r"(taddr))
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// 2^x for the moderate arguments of the epilogues (|x| < 64): the bare SFU instruction, without exp2f's denormal-range fix-up
+__device__ __forceinline__ float ex2_fast(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 // exp(-x^2/2) = exp2(-(x * FILT_SCALE)^2)
 #define FILT_SCALE 0.84932180028801907f
 #define FILT_CUT (5.f * FILT_SCALE)
@@ -370,11 +373,11 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
             for (int j = 0; j < CH; ++j) {
               const float lam = lam8[j], dl = dl8[j], k0 = k08[j], dr = dr8[j], l2r = l28[j];
               // dust, Eq. (A8)-(A9) with the tabulated k0, Drude profile and log2(lam/lam_V) (R10)
-              const float pw = exp2f(delta * l2r);
+              const float pw = ex2_fast(delta * l2r);
               const float br = fmaf(k0, pw, Eb * dr);
               float A = AVs * br, A_av = br * (1.f / 4.05f), A_del = AVs * (k0 * pw * l2r * LN2F - 1.9f * dr);
               if (!(A > 0.f)) { A = 0.f; A_av = 0.f; A_del = 0.f; }
-              const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+              const float Tt = ex2_fast(-0.4f * 3.321928094887362f * A);
               const float dF = -(1.f - Ffl) * 0.4f * LN10F * Tt;
               const float Sd = __uint_as_float(v[j]) * dl;
               G0[j] = Sd * fmaf(1.f - Ffl, Tt, Ffl); G1[j] = Sd * dF * A_av; G2[j] = Sd * dF * A_del; G3[j] = Sd * (1.f - Tt);
@@ -387,7 +390,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
 #pragma unroll
                 for (int j = 0; j < CH; ++j) {
                   const float x = fmaf(lamz[j], isg, nmu);
-                  const float Tb = (fabsf(x) <= FILT_CUT) ? exp2f(-x * x) : 0.f;
+                  const float Tb = (fabsf(x) <= FILT_CUT) ? ex2_fast(-x * x) : 0.f;
                   s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
                   s4[b] = fmaf(Tb * x, G4[j] * dzf, s4[b]);               // d/dz of T_b(lam (1+z)) = -T x' lam / sigma
                 }
@@ -567,14 +570,14 @@ __global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, c
         float tsum = 0.f;
         for (int b = 0; b < T.n_band; ++b) {
           const float x = fmaf(lamz, FC.isg[b], FC.nmu[b]);
-          if (fabsf(x) <= FILT_CUT) tsum = fmaf(g_s[b], exp2f(-x * x), tsum);
+          if (fabsf(x) <= FILT_CUT) tsum = fmaf(g_s[b], ex2_fast(-x * x), tsum);
         }
         if (tsum != 0.f) {
           const float l2r = __ldg(&wconst[2 * (k + u) + 1].x);
-          const float pw = exp2f(delta * l2r);
+          const float pw = ex2_fast(delta * l2r);
           float A = AVs * fmaf(c0.z, pw, Eb * c0.w);
           if (!(A > 0.f)) A = 0.f;
-          const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
+          const float Tt = ex2_fast(-0.4f * 3.321928094887362f * A);
           v[u] = fmaf(1.f - Ffl, Tt, Ffl) * c0.y * tsum;
         }
       }
