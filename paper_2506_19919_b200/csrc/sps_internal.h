@@ -8,8 +8,7 @@ struct sps_table {
   TableDev dev;
   RowBuffers rows;         // scratch, grown on demand; a table must not be used from two host threads at once
   ExactState* exact;
-  void* hmc_scratch;
-  sps_table() : exact(nullptr), hmc_scratch(nullptr) { rows = RowBuffers(); }
+  sps_table() : exact(nullptr) { rows = RowBuffers(); }
 };
 
 sps_status sps_require_device();

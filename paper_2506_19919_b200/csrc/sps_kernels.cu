@@ -78,12 +78,11 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 // bins[3][.] scatter cursors.
 // ---------------------------------------------------------------------------------------------
 #ifndef AC_WARPS
-#define AC_WARPS 16
+#define AC_WARPS 16                              // warps per CTA
 #endif
 #ifndef AC_R
-#define AC_R 4
+#define AC_R 4                                    // rows per warp, register-blocked (4 or 8)
 #endif
-//#define AC_R_DOC                                   // rows per warp, register-blocked
 #define AC_ROWS_PER_CTA (AC_WARPS * AC_R)
 
 __global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restrict__ bins) {
@@ -126,8 +125,8 @@ __global__ void approx_scatter_kernel(int64_t n, const int* __restrict__ rows, R
 // ---------------------------------------------------------------------------------------------
 // a7 + a9 + a10: approximate photometry (Eq. 6) fused with the Gaussian likelihood and the reverse
 // pass over the c_SSP table.  One CTA per (z cell, chunk of 64 rows): the cell's two arrays c_t and D_t = c_{t+1} - c_t
-// (106 KB at full size) are staged in shared memory; each warp owns 8 rows and register-blocks over them, so every
-// table word read from shared memory feeds 8 FMAs (the 1 LDS : 2 FMA ratio of a row-at-a-time pass would leave the
+// (106 KB at full size) are staged in shared memory; each warp owns AC_R rows and register-blocks over them, so every
+// table word read from shared memory feeds AC_R FMAs (the 1 LDS : 2 FMA ratio of a row-at-a-time pass would leave the
 // kernel shared-memory bound at ~1/4 of the FMA rate).
 //   pass 1 (lane = 4 consecutive entries e = j*n_band + b of a table row):
 //            Q^(s)_r,e = sum_i a_r,i c^(s)[i][e]          s = 0: c_t, s = 1: D_t
@@ -152,7 +151,7 @@ __device__ __forceinline__ void ac_wait(uint32_t bar, uint32_t parity) {
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
 }
 
-// One work item: up to 64 rows of one z cell; warp w owns rows r_begin + 8w .. + 7.
+// One work item: up to AC_ROWS_PER_CTA rows of one z cell; warp w owns rows r_begin + AC_R w .. + AC_R - 1.
 __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const float4* __restrict__ s0, const float4* __restrict__ s1,
                                         int r_begin, int r_end, const int* __restrict__ order, const int* __restrict__ gal_of_row,
                                         const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
@@ -166,7 +165,7 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
 #pragma unroll
   for (int r = 0; r < AC_R; ++r) row[r] = (r0 + r < r_end) ? order[r0 + r] : -1;
   // Request everything the item needs from global memory first (independent loads, all in flight together), then
-  // stage it: weights transposed (a_T[i][r], lane = age bin), m, RowScalars and observations of the 8 rows.
+  // stage it: weights transposed (a_T[i][r], lane = age bin), m, RowScalars and observations of the warp's rows.
   {
     float av[SPS_AGE_PER_LANE][AC_R], mv[AC_R], o0[AC_R], o1[AC_R];
 #pragma unroll
@@ -231,7 +230,7 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
     }
   }
   __syncwarp();                                             // a_T is dead: S.buf becomes the v buffer
-  // ---- band step for the warp's 8 rows at once: lane = (row 2k + l/16, band l%16), four rounds ----
+  // ---- band step for the warp's rows: lane = (row 2k + l/16, band l%16), AC_R / 2 rounds ----
   //      fluxes, likelihood, direct bars (16-lane reductions), then m_bar (lane = (row, j)) and v (lane = 4 entries)
 #pragma unroll
   for (int r = 0; r < AC_R; ++r) {
