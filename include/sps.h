@@ -51,7 +51,8 @@ typedef struct sps_table sps_table;      /* opaque; owns device memory */
 
 /* Everything that is fixed before the analysis.  HOST pointers; copied. */
 typedef struct {
-  int32_t n_age, n_Z, n_wave, n_band, n_z;   /* n_age<=128, n_Z<=16, n_band<=16, n_z>=2           */
+  int32_t n_age, n_Z, n_wave, n_band, n_z;   /* n_age<=128, n_Z<=16, n_band<=16, n_z>=2; and       */
+                                             /* 8 n_age (n_Z n_band + 4) + 119 KB <= 227 KB (SPS_ESHAPE otherwise) */
   const double* log10_age_yr;  /* [n_age]  increasing                                              */
   const double* log10_Z;       /* [n_Z]    increasing, log10(Z/Zsun)                               */
   const double* wave_A;        /* [n_wave] strictly increasing rest-frame wavelength, Angstrom     */

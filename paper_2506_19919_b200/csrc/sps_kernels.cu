@@ -528,7 +528,14 @@ static size_t approx_smem_bytes(const TableDev& T) {
 }
 sps_status approx_contract_setup(const TableDev& T) {
   if (T.n_z - 1 > 1 << 20) { sps_set_error("n_z too large"); return SPS_ESHAPE; }
-  return sps_check_cuda(cudaFuncSetAttribute(approx_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)approx_smem_bytes(T)),
+  const size_t bytes = approx_smem_bytes(T);
+  if (bytes > 227 * 1024) {
+    sps_set_error("table too large for the approximate path: the two c_SSP arrays of a z cell (2 x n_age x n_Z*n_band floats = %zu bytes) "
+                  "plus %zu bytes of row staging must fit the 227 KB of shared memory of an SM", (size_t)2 * T.n_age * T.cs_stride * sizeof(float),
+                  bytes - (size_t)2 * T.n_age * T.cs_stride * sizeof(float));
+    return SPS_ESHAPE;
+  }
+  return sps_check_cuda(cudaFuncSetAttribute(approx_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
                         "approximate-path shared memory opt-in");
 }
 
