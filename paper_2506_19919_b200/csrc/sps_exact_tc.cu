@@ -181,7 +181,7 @@ __device__ __forceinline__ float ex2_fast(float x) { float y; asm("ex2.approx.ft
           if (s1[b] != 0.f) atomicAdd(p + SPS_MAX_BAND + b, s1[b]);                                   \
           if (s2[b] != 0.f) atomicAdd(p + 2 * SPS_MAX_BAND + b, s2[b]);                               \
           if (s3[b] != 0.f) atomicAdd(p + 3 * SPS_MAX_BAND + b, s3[b]);                               \
-          if (s4[b] != 0.f) atomicAdd(p + 4 * SPS_MAX_BAND + b, s4[b]);                               \
+          if (s4[b] != 0.f) atomicAdd(p + 4 * SPS_MAX_BAND + b, s4[b] * FC.dz[b]);                               \
         }                                                                                             \
       }                                                                                               \
     }                                                                                                 \
@@ -386,13 +386,13 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
               if (mask & (1u << b)) {
-                const float isg = FC.isg[b], nmu = FC.nmu[b], dzf = FC.dz[b];
+                const float isg = FC.isg[b], nmu = FC.nmu[b];
 #pragma unroll
                 for (int j = 0; j < CH; ++j) {
                   const float x = fmaf(lamz[j], isg, nmu);
                   const float Tb = (fabsf(x) <= FILT_CUT) ? ex2_fast(-x * x) : 0.f;
                   s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
-                  s4[b] = fmaf(Tb * x, G4[j] * dzf, s4[b]);               // d/dz of T_b(lam (1+z)) = -T x' lam / sigma
+                  s4[b] = fmaf(Tb * x, G4[j], s4[b]);   // d/dz of T_b(lam (1+z)) = -T x' lam / sigma: the band's factor FC.dz is applied at the flush
                 }
               }
             }
