@@ -251,20 +251,22 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
       float S0 = 0.f, S1 = 0.f, F = 1.f, F_av = 0.f, F_del = 0.f, F_fl = 0.f, F_lam = 0.f, lam_r = 1.f, g = 0.f, chi2 = 0.f;
       if (ok) {
         for (int j = 0; j < T.n_Z; ++j) { S0 = fmaf(S.ms[r][j], S.Qs[r][0][j * T.n_band + b], S0); S1 = fmaf(S.ms[r][j], S.Qs[r][1][j * T.n_band + b], S1); }
-        lam_r = T.lam_eff[b] / zp;
+        const float izp = __fdividef(1.f, zp);
+        lam_r = T.lam_eff[b] * izp;
         dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
         const float flux = F * Mn * (S0 + f * S1);
         B.flux[(int64_t)rw * SPS_MAX_BAND + b] = flux;
         if (flux_bar) g = S.obs[r][0][b];
         else {
           const float d = S.obs[r][0][b], sg = S.obs[r][1][b];
-          const float rr = (flux - d) / sg;
+          const float isg = __fdividef(1.f, sg);
+          const float rr = (flux - d) * isg;
           chi2 = rr * rr;
-          g = -rr / sg;
+          g = -rr * isg;
         }
       }
       const float Sint = S0 + f * S1;
-      float v_mn = g * F * Sint, v_z = g * (F * Mn * S1 * T.inv_dz + Mn * Sint * F_lam * (-lam_r / zp));
+      float v_mn = g * F * Sint, v_z = g * (F * Mn * S1 * T.inv_dz + Mn * Sint * F_lam * (-lam_r * __fdividef(1.f, zp)));
       float v_av = g * Mn * Sint * F_av, v_de = g * Mn * Sint * F_del, v_fl = g * Mn * Sint * F_fl;
 #pragma unroll
       for (int o = 8; o > 0; o >>= 1) {

@@ -275,7 +275,8 @@ __device__ __forceinline__ void met_bin(const TableDev& T, float lz, float s, fl
 #define CALZ_SWITCH_INV_UM 1.2809053864877329f
 __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float Ffl,
                                         float& F, float& F_av, float& F_del, float& F_fl, float& F_lam) {
-  const float u = 1.0e4f / lam;
+  const float ilam = __fdividef(1.f, lam);                  // one approximate reciprocal (1 ulp) serves every division by lambda
+  const float u = 1.0e4f * ilam;
   float k0, dk_du;
   if (u > CALZ_SWITCH_INV_UM) {
     k0 = 2.659f * (-2.156f + u * (1.509f + u * (-0.198f + u * 0.011f))) + 4.05f;
@@ -284,7 +285,7 @@ __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float 
     k0 = 2.659f * (-1.857f + 1.040f * u) + 4.05f;
     dk_du = 2.659f * 1.040f;
   }
-  float dk0 = dk_du * (-u / lam);
+  float dk0 = dk_du * (-u * ilam);
   if (!(k0 > 0.f)) { k0 = 0.f; dk0 = 0.f; }
   const float l0 = 2175.f, w = 350.f;
   const float n = (lam * w) * (lam * w);
@@ -292,7 +293,8 @@ __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float 
   const float den = dl * dl + n;
   const float dn = 2.f * lam * w * w;
   const float dd = 4.f * lam * dl + dn;
-  const float dr = n / den, ddr = (dn * den - n * dd) / (den * den);
+  const float iden = __fdividef(1.f, den);
+  const float dr = n * iden, ddr = (dn * den - n * dd) * iden * iden;
   const float l2r = log2f(lam * (1.f / 5500.f));
   const float pw = exp2f(delta * l2r);
   const float Eb = 0.85f - 1.9f * delta;
@@ -300,7 +302,7 @@ __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float 
   float A = AV * (1.f / 4.05f) * br;
   float A_av = br * (1.f / 4.05f);
   float A_del = AV * (1.f / 4.05f) * (k0 * pw * l2r * LN2F - 1.9f * dr);
-  float A_lam = AV * (1.f / 4.05f) * (dk0 * pw + k0 * delta * pw / lam + Eb * ddr);
+  float A_lam = AV * (1.f / 4.05f) * (dk0 * pw + k0 * delta * pw * ilam + Eb * ddr);
   if (!(A > 0.f)) { A = 0.f; A_av = A_del = A_lam = 0.f; }
   const float Tt = exp2f(-0.4f * 3.321928094887362f * A);
   const float dF_dA = -(1.f - Ffl) * 0.4f * LN10F * Tt;
