@@ -115,7 +115,7 @@ sps_status sps_prior_to_dev(const sps_prior* p, PriorDev& out) {
 sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* theta, int64_t n, bool unbounded,
                     bool with_prior, const int* rows, const int* gal_of_row, const float* obs_flux,
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
-                    cudaStream_t s) {
+                    cudaStream_t s, const LeapfrogFuse* lf) {
   const TableDev& T = t->dev;
   launch_prologue(T, P, theta, n, unbounded, want_grad, rows, t->rows, path == SPS_PATH_APPROX, s);
   if (path == SPS_PATH_APPROX) {
@@ -124,7 +124,8 @@ sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* thet
     sps_status st = sps_exact_contract(t, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, s);
     if (st != SPS_OK) return st;
   }
-  if (want_grad || logp) launch_epilogue(T, P, theta, n, unbounded, with_prior, rows, t->rows, logp, want_grad ? grad : nullptr, s);
+  if (want_grad || logp) launch_epilogue(T, P, theta, n, unbounded, with_prior, rows, t->rows, logp, want_grad ? grad : nullptr,
+                                           (lf && want_grad) ? *lf : LeapfrogFuse{nullptr, nullptr, nullptr, nullptr}, s);
   return sps_check_cuda(cudaGetLastError(), "sps_eval launch");
 }
 

@@ -28,4 +28,4 @@ sps_status sps_exact_contract(sps_table* t, int64_t n, const int* rows, const in
 sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* theta, int64_t n, bool unbounded,
                     bool with_prior, const int* rows, const int* gal_of_row, const float* obs_flux,
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
-                    cudaStream_t s);
+                    cudaStream_t s, const LeapfrogFuse* lf = nullptr);

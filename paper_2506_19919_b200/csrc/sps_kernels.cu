@@ -408,8 +408,8 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
 // re-evaluated; no quadrature is redone.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
-epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded, bool with_prior,
-                const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad) {
+epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbounded, bool with_prior,
+                const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad, LeapfrogFuse lf) {
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
@@ -491,6 +491,12 @@ epilogue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
       g += dlp;
     }
     grad[row * SPS_NDIM + l] = g;
+    if (lf.p_w) {                                            // fused leapfrog update (theta may alias lf.theta_w: read above, written here)
+      const int64_t o = row * SPS_NDIM + l;
+      const float e = lf.eps[row], pn = lf.p_w[o] + e * g;
+      lf.p_w[o] = pn;
+      lf.theta_w[o] += e * lf.inv_mass[o] * pn;
+    }
   }
   lp = warp_sum(lp);
   if (l == 0 && logp) logp[row] = sc.logp_like + lp;
@@ -559,10 +565,10 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
   sps_count_launch(3);
 }
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
-                     bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s) {
+                     bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s) {
   if (n <= 0) return;
   sps_prof_begin(SPS_K_EPILOGUE, s);
-  epilogue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad);
+  epilogue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad, lf);
   sps_prof_end(SPS_K_EPILOGUE, s);
   sps_count_launch();
 }

@@ -19,6 +19,10 @@ struct RowBuffers {
   int64_t capacity;
 };
 
+// Optional leapfrog update fused into the epilogue (HMC inner steps): after the gradient of a row is known,
+//   p += eps grad;  theta~ += eps invM p     (the two half kicks between consecutive evaluations merged)
+struct LeapfrogFuse { float* theta_w; float* p_w; const float* eps; const float* inv_mass; };
+
 // kernels (sps_kernels.cu)
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
                      const int* rows, RowBuffers B, bool with_hist, cudaStream_t s);
@@ -27,7 +31,7 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
                             bool want_grad, RowBuffers B, cudaStream_t s);
 sps_status approx_contract_setup(const TableDev& T);
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
-                     bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, cudaStream_t s);
+                     bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s);
 void launch_copy_weights(const TableDev& T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar,
                          cudaStream_t s);
 void launch_copy_flux(const TableDev& T, int64_t n, RowBuffers B, float* flux, cudaStream_t s);

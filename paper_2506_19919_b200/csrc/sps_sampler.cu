@@ -66,16 +66,7 @@ __global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, uint32_t t
   if (l == 0) C.H0[c] = -C.logp[c] + kin;
 }
 
-// between two gradient evaluations: p += eps * grad ; theta += eps * invM * p   (two half kicks merged)
-__global__ void __launch_bounds__(256) leapfrog_mid_kernel(ChainState C) {
-  const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (o >= C.n * SPS_NDIM) return;
-  const int64_t c = o / SPS_NDIM;
-  const float eps = C.eps[c];
-  const float p = C.p_w[o] + eps * C.grad_w[o];
-  C.p_w[o] = p;
-  C.theta_w[o] += eps * C.inv_mass[o] * p;
-}
+// (between two gradient evaluations the update p += eps grad; theta~ += eps invM p rides in the epilogue kernel: LeapfrogFuse)
 
 // end: last half kick, Metropolis test, warmup adaptation (R14), running summaries.
 __global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, uint32_t transition, uint2 key, int n_leapfrog, AdaptFlags A,
@@ -194,13 +185,14 @@ AdaptFlags adapt_flags_for(int it, int n_warmup, const std::vector<int>& ends, i
 
 static inline unsigned chain_blocks(int64_t n) { return (unsigned)((n * 32 + 255) / 256); }
 
-static sps_status eval_working(sps_table* t, const PriorDev& P, const HmcProblem& Q, ChainState& C, cudaStream_t s) {
+static sps_status eval_working(sps_table* t, const PriorDev& P, const HmcProblem& Q, ChainState& C, cudaStream_t s, bool fuse_leapfrog = false) {
+  const LeapfrogFuse lf = {C.theta_w, C.p_w, C.eps, C.inv_mass};
   // groups of rows per path: path_rows[0] exact, [1] approx (index lists) or all rows on one path
   sps_status st = SPS_OK;
   for (int path = 0; path < 2 && st == SPS_OK; ++path) {
     if (Q.n_rows_path[path] == 0) continue;
     st = sps_eval(t, P, path, C.theta_w, Q.n_rows_path[path], true, true, Q.rows_path[path], Q.gal_of_chain, Q.obs_flux,
-                  Q.obs_sigma, nullptr, true, C.logp_w, C.grad_w, s);
+                  Q.obs_sigma, nullptr, true, C.logp_w, C.grad_w, s, fuse_leapfrog ? &lf : nullptr);
   }
   return st;
 }
@@ -238,12 +230,10 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
   if (st == SPS_OK && cfg->sampler == SPS_SAMPLER_HMC) {
     std::vector<int> ends; int slow_lo, slow_hi;
     warmup_schedule(cfg->n_warmup, ends, slow_lo, slow_hi);
-    const unsigned eb = (unsigned)((n * SPS_NDIM + 255) / 256);
     for (int it = 0; it < cfg->n_warmup + cfg->n_sample && st == SPS_OK; ++it) {
       hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key); sps_count_launch();
       for (int k = 0; k < cfg->n_leapfrog && st == SPS_OK; ++k) {
-        st = eval_working(t, P, Q, C, s);
-        if (k + 1 < cfg->n_leapfrog) { leapfrog_mid_kernel<<<eb, 256, 0, s>>>(C); sps_count_launch(); }
+        st = eval_working(t, P, Q, C, s, k + 1 < cfg->n_leapfrog);    // inner steps: the leapfrog update rides in the epilogue
       }
       const AdaptFlags A = adapt_flags_for(it, cfg->n_warmup, ends, slow_lo, slow_hi, cfg->target_accept);
       hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key, cfg->n_leapfrog, A, samples, it - cfg->n_warmup, cfg->n_sample);
