@@ -125,7 +125,7 @@ def gaussian_filters(centres_A, lam_over_fwhm):
 
 
 def make_grid(kind: str, seed: int | None = None) -> Grid:
-    """kind = 'tiny' (BASELINE.json configs[0]: 20 x 4 x 500, 3 filters) or
+    """kind = 'tiny' (BASELINE.json configs[0]: 20 x 4 x 500, 3 filters), 'odd' (33 x 5 x 777, 12 filters: test shapes) or
     'full' (configs[1..4]: 107 x 12 x 5994, 10 filters, 200-point z grid)."""
     if kind == "tiny":
         seed = SEED0 if seed is None else seed
@@ -141,6 +141,14 @@ def make_grid(kind: str, seed: int | None = None) -> Grid:
         wave = np.geomspace(250.0, 5.0e4, 5994)
         mu, sg = gaussian_filters(np.geomspace(3300.0, 11000.0, 10), np.geomspace(3.4, 25.5, 10))
         n_z = 200
+    elif kind == "odd":
+        # awkward sizes for the parity tests (not a BASELINE config): nothing is a multiple of a tile, 12 bands
+        seed = SEED0 + 2 if seed is None else seed
+        la = np.linspace(5.5, 10.2, 33)
+        lz = np.linspace(-2.2, 0.4, 5)
+        wave = np.geomspace(400.0, 4.0e4, 777)
+        mu, sg = gaussian_filters(np.geomspace(3500.0, 10500.0, 12), np.geomspace(4.0, 12.0, 12))
+        n_z = 9
     else:
         raise ValueError(kind)
     ssp = make_ssp_spectra(la, lz, wave, seed)

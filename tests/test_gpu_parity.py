@@ -80,6 +80,11 @@ def full():
     return Ctx("full")
 
 
+@pytest.fixture(scope="module")
+def odd():
+    return Ctx("odd")
+
+
 def test_library_is_native():
     sps = _sps()
     from paper_2506_19919_b200 import binding
@@ -483,3 +488,26 @@ def test_approximation_error_falls_with_filter_resolution(full):
     med = np.median(np.abs(2.5 * np.log10(fa / fe)), axis=0)
     assert np.all(np.diff(med) < 0)
     assert med[0] < 3e-2 and med[-1] < 3e-4 and np.all(med[6:] < 1e-3)
+
+
+# ---- awkward table shape: 33 ages x 5 Z x 777 wavelengths x 12 bands, 9 z nodes (nothing a multiple of a tile) ----------
+def test_odd_shape_both_paths(odd, exact_kernels):
+    cx = odd
+    floor = exact_kernels
+    n_gal, n_chain = 37, 3
+    truth_u, d, s = _observations(cx, n_gal, 91)
+    thu = (np.repeat(truth_u, n_chain, 0) + 0.3 * np.random.default_rng(2).normal(size=(n_gal * n_chain, 13)) / cx.P[2]).astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    th, dth = M.bound(thu.astype(np.float64), cx.P)
+    for path, name, fl in ((cx.sps.PATH_APPROX, "approx", 1e-3), (cx.sps.PATH_EXACT, "exact", floor)):
+        flux = cx.sps.sps_photometry(cx.table, cx.ph, path, _dev(thu)).cpu().numpy()
+        of = (M.photometry_approx(th, cx.grid, cx.cssp())[0] if name == "approx" else M.photometry_exact(th, cx.grid, False)[0])
+        assert _rel(flux, of).max() <= 1e-4, name
+        lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, path, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+        olp, og, _ = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), name, cx.cssp())
+        assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4, name
+        J = (M.photometry_approx(th, cx.grid, cx.cssp())[1] if name == "approx" else M.photometry_exact(th, cx.grid)[1])
+        eps_flux = 2e-5 if fl == TC_FLOOR else 3e-6
+        allow = eps_flux * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
+        err = np.maximum(np.abs(g.cpu().numpy() - og) - allow, 0.0)
+        assert (err / np.maximum(np.abs(og), fl * np.abs(og).max(1, keepdims=True))).max() <= 1e-3, name
