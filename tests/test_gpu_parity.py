@@ -333,8 +333,11 @@ def test_nuts_mixed_paths_config5_shape(tiny):
         single = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path=path, **kw)["samples"].cpu().numpy().reshape(n_gal, n_chain, 20, 13)
         sel = mask == path
         err = np.abs(ms[sel] - single[sel]) / np.maximum(1.0, np.abs(single[sel]))
-        assert err[:, :, :3].max() <= 1e-3                              # the first transitions agree tightly
-        assert np.median(err.reshape(sel.sum() * n_chain, -1).max(1)) <= 1e-2
+        if path == 1:                                                   # approximate path: deterministic, so bit-identical
+            assert err.max() == 0.0
+        else:                                                           # exact path: band sums are combined with atomics (order varies in
+            assert err[:, :, :2].max() <= 1e-3                          # the last bit), so chains may decouple later: the start must agree
+            assert np.median(err.reshape(sel.sum() * n_chain, -1).max(1)) <= 5e-2
     assert (mixed["n_leapfrog"].cpu().numpy() >= 40).all()
 
 
