@@ -36,6 +36,7 @@ void sps_prof_end(int id, cudaStream_t s) {
   if (!P.open) return;
   cudaEvent_t e; cudaEventCreate(&e); cudaEventRecord(e, s); P.ev.push_back(e); P.open = false;
 }
+bool sps_prof_enabled() { return g_prof_on != 0; }
 extern "C" sps_status sps_profile(int enable, int stride) {
   g_prof_on = enable; g_prof_stride = stride > 0 ? stride : 1;
   for (auto& P : g_prof) { for (auto e : P.ev) cudaEventDestroy(e); P.ev.clear(); P.launches = 0; P.open = false; }

@@ -83,6 +83,7 @@ __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 // launch counter (host side)
 extern "C" int64_t sps_launch_count(void);
 void sps_count_launch(int n = 1);
+bool sps_prof_enabled();
 void sps_prof_begin(int id, cudaStream_t s);
 void sps_prof_end(int id, cudaStream_t s);
 void sps_set_error(const char* fmt, ...);

@@ -29,23 +29,6 @@ struct NutsScalars {
   int* depth_hist;             // [NUTS_MAX_DEPTH + 1] tree depths of the sampling phase
 };
 
-struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; int first; };
-
-__device__ __forceinline__ AdaptFlags adapt_flags_dev(int it, const WarmupSched& S) {
-  AdaptFlags A; A.warmup = it < S.n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == S.n_warmup); A.welford_n = 0;
-  A.target = S.target;
-  if (A.warmup && it >= S.slow_lo && it < S.slow_hi) {
-    A.in_window = 1;
-    int start = S.slow_lo;
-    for (int k = 0; k < S.n_ends; ++k) {
-      const int e = S.ends[k];
-      if (it < e) { A.welford_n = it - start + 1; A.window_end = (it + 1 == e); break; }
-      start = e;
-    }
-  }
-  return A;
-}
-
 __device__ __forceinline__ float logaddexpf_(float a, float b) {
   const float hi = fmaxf(a, b), lo = fminf(a, b);
   if (hi == -INFINITY) return -INFINITY;
@@ -225,7 +208,6 @@ __global__ void nuts_compact_kernel(int64_t n, const int* __restrict__ done, con
 
 }  // namespace
 
-void warmup_schedule(int W, std::vector<int>& ends, int& slow_lo, int& slow_hi);    // sps_sampler.cu
 
 sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples, cudaStream_t s) {
   const int64_t n = C.n;
@@ -241,14 +223,7 @@ sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, 
   S.n_done = ibase + 6 * n; S.depth_hist = ibase + 6 * n + 4;
   int* counts = ibase + 6 * n + 4 + NUTS_MAX_DEPTH + 1;
   cudaMemsetAsync(ibase, 0, (6 * n + 4 + NUTS_MAX_DEPTH + 1 + 4) * sizeof(int), s);
-  WarmupSched W; memset(&W, 0, sizeof(W));
-  {
-    std::vector<int> ends; int lo, hi;
-    warmup_schedule(cfg->n_warmup, ends, lo, hi);
-    W.n_warmup = cfg->n_warmup; W.n_sample = cfg->n_sample; W.slow_lo = lo; W.slow_hi = hi; W.target = cfg->target_accept; W.first = (int)cfg->first_transition;
-    W.n_ends = (int)std::min<size_t>(ends.size(), 16);
-    for (int k = 0; k < W.n_ends; ++k) W.ends[k] = ends[k];
-  }
+  const WarmupSched W = make_warmup_sched(cfg);
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
   const unsigned cb = (unsigned)((n * 32 + 255) / 256);
   nuts_begin_kernel<<<cb, 256, 0, s>>>(C, S, (int)cfg->first_transition, key); sps_count_launch();

@@ -50,8 +50,14 @@ __global__ void __launch_bounds__(256) chain_init_kernel(ChainState C, PriorDev 
 // HMC transition (R-step 13).  Draw order: 13 normals (purpose 0), one uniform (purpose 1).
 // begin: p = N / sqrt(invM); H0 = -logP + 1/2 sum invM p^2; first half kick and drift.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, uint32_t transition, uint2 key) {
+__global__ void hmc_ctl_kernel(HmcCtl* ctl, WarmupSched W) {      // next transition: counter and adaptation flags
+  const int it = ctl->it + 1;
+  ctl->it = it; ctl->sample_index = it - W.n_warmup; ctl->A = adapt_flags_dev(it, W);
+}
+
+__global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, const HmcCtl* __restrict__ ctl, uint32_t first, uint2 key) {
   CHAIN_WARP_PROLOGUE(C.n);
+  const uint32_t transition = (uint32_t)ctl->it + first;
   float kin = 0.f;
   if (l < SPS_NDIM) {
     const int64_t o = c * SPS_NDIM + l;
@@ -69,9 +75,12 @@ __global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, uint32_t t
 // (between two gradient evaluations the update p += eps grad; theta~ += eps invM p rides in the epilogue kernel: LeapfrogFuse)
 
 // end: last half kick, Metropolis test, warmup adaptation (R14), running summaries.
-__global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, uint32_t transition, uint2 key, int n_leapfrog, AdaptFlags A,
-                                                      float* __restrict__ samples, int sample_index, int n_sample) {
+__global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, const HmcCtl* __restrict__ ctl, uint32_t first, uint2 key, int n_leapfrog,
+                                                      float* __restrict__ samples, int n_sample) {
   CHAIN_WARP_PROLOGUE(C.n);
+  const uint32_t transition = (uint32_t)ctl->it + first;
+  const AdaptFlags A = ctl->A;
+  const int sample_index = ctl->sample_index;
   const int64_t o = c * SPS_NDIM + (l < SPS_NDIM ? l : 0);
   const bool act = l < SPS_NDIM;
   const float v = C.inv_mass[o], eps = C.eps[c];
@@ -172,15 +181,15 @@ void warmup_schedule(int W, std::vector<int>& ends, int& slow_lo, int& slow_hi) 
   slow_lo = init; slow_hi = stop;
 }
 
-AdaptFlags adapt_flags_for(int it, int n_warmup, const std::vector<int>& ends, int slow_lo, int slow_hi, float target) {
-  AdaptFlags A; A.warmup = it < n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == n_warmup); A.welford_n = 0;
-  A.target = target;
-  if (A.warmup && it >= slow_lo && it < slow_hi) {
-    A.in_window = 1;
-    int start = slow_lo;
-    for (int e : ends) { if (it < e) { A.welford_n = it - start + 1; A.window_end = (it + 1 == e); break; } start = e; }
-  }
-  return A;
+WarmupSched make_warmup_sched(const sps_hmc_config* cfg) {
+  WarmupSched W; memset(&W, 0, sizeof(W));
+  std::vector<int> ends; int lo, hi;
+  warmup_schedule(cfg->n_warmup, ends, lo, hi);
+  W.n_warmup = cfg->n_warmup; W.n_sample = cfg->n_sample; W.slow_lo = lo; W.slow_hi = hi; W.target = cfg->target_accept;
+  W.first = (int)cfg->first_transition;
+  W.n_ends = (int)std::min<size_t>(ends.size(), 16);
+  for (int k = 0; k < W.n_ends; ++k) W.ends[k] = ends[k];
+  return W;
 }
 
 static inline unsigned chain_blocks(int64_t n) { return (unsigned)((n * 32 + 255) / 256); }
@@ -202,6 +211,9 @@ sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n
 void hmc_problem_free(HmcProblem& Q);
 sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples, cudaStream_t s);
 
+static int g_no_graph = 0;
+extern "C" void sps_debug_no_graph(int on) { g_no_graph = on; }
+
 extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, const sps_hmc_config* cfg, const float* obs_flux,
                                   const float* obs_sigma, int64_t n_gal, const int32_t* path_of_gal, const float* theta0,
                                   float* samples, const sps_hmc_summary* summary, void* stream) {
@@ -213,6 +225,13 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
   if (n_gal == 0) return SPS_OK;
   sps_table* t = const_cast<sps_table*>(tc);
   cudaStream_t s = (cudaStream_t)stream;
+  if (!s) {
+    // The legacy default stream cannot be captured into a graph: the run (which synchronises before returning anyway)
+    // goes on a stream of the library's own, after everything already queued on the caller's stream.
+    static cudaStream_t own = nullptr;
+    if (!own && cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking) != cudaSuccess) { own = nullptr; cudaGetLastError(); }
+    if (own) { cudaStreamSynchronize(nullptr); s = own; }
+  }
   PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
   const int64_t n = n_gal * cfg->n_chain;
   st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
@@ -221,6 +240,7 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
   st = chain_state_alloc(C, n, cfg->sampler == SPS_SAMPLER_NUTS ? NUTS_VECTORS : 0);
   if (st != SPS_OK) { hmc_problem_free(Q); return st; }
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
+  cudaDeviceSynchronize();                                   // the set-up above ran on the default stream
   chain_init_kernel<<<chain_blocks(n), 256, 0, s>>>(C, P, theta0, cfg->eps0, cfg->eps_in_dev, cfg->inv_mass_in_dev, key); sps_count_launch();
   // logp / grad at the start: evaluate through the working buffers
   cudaMemcpyAsync(C.theta_w, C.theta, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
@@ -228,17 +248,46 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
   cudaMemcpyAsync(C.grad, C.grad_w, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
   cudaMemcpyAsync(C.logp, C.logp_w, n * sizeof(float), cudaMemcpyDeviceToDevice, s);
   if (st == SPS_OK && cfg->sampler == SPS_SAMPLER_HMC) {
-    std::vector<int> ends; int slow_lo, slow_hi;
-    warmup_schedule(cfg->n_warmup, ends, slow_lo, slow_hi);
-    for (int it = 0; it < cfg->n_warmup + cfg->n_sample && st == SPS_OK; ++it) {
-      hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key); sps_count_launch();
-      for (int k = 0; k < cfg->n_leapfrog && st == SPS_OK; ++k) {
-        st = eval_working(t, P, Q, C, s, k + 1 < cfg->n_leapfrog);    // inner steps: the leapfrog update rides in the epilogue
-      }
-      const AdaptFlags A = adapt_flags_for(it, cfg->n_warmup, ends, slow_lo, slow_hi, cfg->target_accept);
-      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, (uint32_t)it + cfg->first_transition, key, cfg->n_leapfrog, A, samples, it - cfg->n_warmup, cfg->n_sample);
+    // One transition = control update, momentum draw, n_leapfrog evaluations (each five launches), accept/adapt.  Every
+    // launch argument is the same from one transition to the next (the counter lives in device memory), so the
+    // sequence is captured once in a CUDA graph and replayed: small batches are launch-latency bound.
+    // Plain launches are used when per-kernel profiling is on, on the legacy default stream, or if capture fails.
+    const WarmupSched W = make_warmup_sched(cfg);
+    const int n_tr = cfg->n_warmup + cfg->n_sample;
+    HmcCtl* ctl = nullptr;
+    st = sps_check_cuda(cudaMalloc(&ctl, sizeof(HmcCtl)), "HMC control block");
+    if (st == SPS_OK) cudaMemsetAsync(ctl, 0xff, sizeof(int), s);          // it = -1
+    auto enqueue_transition = [&]() -> sps_status {
+      hmc_ctl_kernel<<<1, 1, 0, s>>>(ctl, W);
+      hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, ctl, cfg->first_transition, key);
+      sps_count_launch(2);
+      sps_status e = SPS_OK;
+      for (int k = 0; k < cfg->n_leapfrog && e == SPS_OK; ++k) e = eval_working(t, P, Q, C, s, k + 1 < cfg->n_leapfrog);
+      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, ctl, cfg->first_transition, key, cfg->n_leapfrog, samples, cfg->n_sample);
       sps_count_launch();
+      return e;
+    };
+    cudaGraphExec_t exec = nullptr;
+    int64_t per_graph = 0;
+    if (st == SPS_OK && n_tr > 2 && s != nullptr && !sps_prof_enabled() && !g_no_graph) {
+      const int64_t c0 = sps_launch_count();
+      cudaGraph_t graph = nullptr;
+      if (cudaStreamBeginCapture(s, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+        const sps_status e = enqueue_transition();
+        const cudaError_t ce = cudaStreamEndCapture(s, &graph);
+        if (e == SPS_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+        if (graph) cudaGraphDestroy(graph);
+      }
+      cudaGetLastError();
+      per_graph = sps_launch_count() - c0;                                 // launches one replay stands for
+      sps_count_launch(-(int)per_graph);                                   // (capturing launched nothing)
     }
+    for (int it = 0; it < n_tr && st == SPS_OK; ++it) {
+      if (exec) { st = sps_check_cuda(cudaGraphLaunch(exec, s), "HMC transition graph"); sps_count_launch((int)per_graph); }
+      else st = enqueue_transition();
+    }
+    if (exec) { cudaStreamSynchronize(s); cudaGraphExecDestroy(exec); }
+    if (ctl) { cudaStreamSynchronize(s); cudaFree(ctl); }
   } else if (st == SPS_OK) {
     st = nuts_run(t, P, cfg, Q, C, samples, s);
   }

@@ -26,6 +26,31 @@ struct ChainState {
 
 struct AdaptFlags { int warmup, in_window, window_end, last_warmup, welford_n; float target; };
 
+// Warmup windows (R14) in a form kernels can evaluate: slow windows end at ends[0..n_ends) inside [slow_lo, slow_hi).
+// `first` = transition index of the RNG streams at local transition 0 (continued runs).
+struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; int first; };
+
+__device__ __forceinline__ AdaptFlags adapt_flags_dev(int it, const WarmupSched& S) {
+  AdaptFlags A; A.warmup = it < S.n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == S.n_warmup); A.welford_n = 0;
+  A.target = S.target;
+  if (A.warmup && it >= S.slow_lo && it < S.slow_hi) {
+    A.in_window = 1;
+    int start = S.slow_lo;
+    for (int k = 0; k < S.n_ends; ++k) {
+      const int e = S.ends[k];
+      if (it < e) { A.welford_n = it - start + 1; A.window_end = (it + 1 == e); break; }
+      start = e;
+    }
+  }
+  return A;
+}
+
+// Per-run control block in device memory: the transition counter and its adaptation flags are advanced on the device,
+// so that one HMC transition is a self-contained sequence of launches (capturable in a CUDA graph and replayed).
+struct HmcCtl { int it; int sample_index; AdaptFlags A; };
+
+WarmupSched make_warmup_sched(const sps_hmc_config* cfg);            // sps_sampler.cu
+
 struct HmcProblem {
   int64_t n;                 // chains
   int* gal_of_chain;         // [n] device
