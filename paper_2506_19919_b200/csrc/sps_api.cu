@@ -120,7 +120,10 @@ sps_status sps_eval(sps_table* t, const PriorDev& P, int path, const float* thet
   const TableDev& T = t->dev;
   launch_prologue(T, P, theta, n, unbounded, want_grad, rows, t->rows, path == SPS_PATH_APPROX, s);
   if (path == SPS_PATH_APPROX) {
-    launch_approx_contract(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, t->rows, s);
+    if (sps_approx_tc_active(t)) {
+      sps_status st = sps_approx_tc_contract(t, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, s);
+      if (st != SPS_OK) return st;
+    } else launch_approx_contract(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, t->rows, s);
   } else {
     sps_status st = sps_exact_contract(t, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, s);
     if (st != SPS_OK) return st;

@@ -1,0 +1,594 @@
+// sps_approx_tc.cu -- tensor-core formulation of the approximate-photometry contraction (a7 + a9 + a10).
+//
+// After the rows of a call are grouped by z cell, Eq. (6) and its reverse are two small GEMMs per cell:
+//   pass 1   P[r, e]     = sum_i a[r, i] C[i, e]          e = s*128 + (j n_band + b),  s = 0: c_t, s = 1: D_t = c_{t+1} - c_t
+//   pass 2   a_bar[r, i] = sum_e V[r, e] C[i, e]          V[r, e] = g_b F_b M m_j {1, f_r}
+// One persistent CTA per SM works on 128-row tiles of one cell:
+//   warps 0-3  thread = row: split the row's weights a (fp32) into FP16 hi + lo and write them into shared memory in the
+//              128-byte-swizzled K-major operand layout; after pass 1 read P from TMEM (tcgen05.ld), do the band step (dust at
+//              lambda_eff/(1+z), fluxes, likelihood, the direct bars, m_bar), generate V (split, swizzled) for pass 2, and at the
+//              end store a_bar from TMEM
+//   warp 4     one thread: TMA loads of the cell's table operands (FP16 hi + lo, both majornesses, built at table creation)
+//              and the tcgen05.mma issue (three split products a_lo c_hi + a_hi c_lo + a_hi c_hi, fp32 accumulation in TMEM)
+// P and a_bar never leave TMEM / registers; the table operands are L2 resident (51 MB for 199 cells).
+// FP16 rather than BF16 split: two FP16 terms carry 22 significant bits (BF16: 16), which the reverse pass needs -- the epilogue
+// contracts a_bar with partials that cancel to ~1e-3 of their size.  Operands are scaled by powers of two into the FP16 range:
+// a_i <= 1 by 2^14, the table arrays by one scale each (largest |c_t|, |D_t| -> [2^13, 2^14)), V by a per-row scale.
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include "sps_internal.h"
+
+namespace {
+
+constexpr int TM = 128;                         // rows per tile
+constexpr int KB = 64;                          // fp16 elements per 128-byte operand row (one k block)
+constexpr int NE = 256;                         // table entries per cell as GEMM dimension: [0,128) c_t, [128,256) D_t
+constexpr int NA = 128;                         // ages as GEMM dimension
+constexpr int TILE_A = TM * 128;                // 16 KB: 128 rows x 128 B
+constexpr int REG_AV = 4 * TILE_A;              // 64 KB: A (hi, lo) x 2 k blocks; later V (hi, lo) x 2 k blocks of a phase
+constexpr int REG_B = 128 * 1024;               // pass 1: 2 k blocks x (hi 32 KB + lo 32 KB); pass 2: 4 k blocks x (hi 16 KB + lo 16 KB)
+constexpr int SMEM_TC = REG_AV + REG_B + 1024 + 256 + 512;
+constexpr int THREADS_TC = 160;
+constexpr float H_TOP = 16384.f;                // operands are scaled so that their largest magnitude sits just below 2^14 before the FP16 split
+
+// band counts the kernel is instantiated for (other tables use the SIMT kernel of sps_kernels.cu)
+#define SPS_APPROX_TC_BANDS(X) X(3) X(10) X(12)
+
+struct ApproxTc {
+  __half *C1_hi, *C1_lo;      // [n_cells * 256][128]  pass-1 B operand: row = (cell, entry), K = age contiguous
+  __half *C2_hi, *C2_lo;      // [n_cells * 128][256]  pass-2 B operand: row = (cell, age),   K = entry contiguous
+  CUtensorMap m1_hi, m1_lo, m2_hi, m2_lo;
+  float* Cm;                         // [n_cells][128] power of two >= max_e |c_t[i][e]| of each (cell, age): a_i Cm_i and c_t / Cm_i are what is split
+  float sD;                          // power of two: D_t sD / Cm_i <= 1 everywhere
+  int sm_count;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok = 0;
+  while (!ok)
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(map), "r"(bar), "r"(c_inner), "r"(c_outer) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) { asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory"); }
+__device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+               ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// K-major operand tile, 128-byte rows, SWIZZLE_128B: 8-row atoms of 1024 B stacked along M/N
+__device__ __forceinline__ uint64_t desc_sw128(uint32_t saddr) {
+  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(1024 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+// byte offset of the 16-byte chunk `c` (0..7) of row r in a 128-byte-swizzled tile (what TMA writes and tcgen05 reads)
+__device__ __forceinline__ uint32_t sw128_off(int r, int c) { return (uint32_t)((r >> 3) * 1024 + (r & 7) * 128 + ((c ^ (r & 7)) << 4)); }
+#define TLD16(taddr, v)                                                                                                \
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
+                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
+               : "r"(taddr))
+__device__ __forceinline__ void tld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ void split8(const float* v, uint4& hi, uint4& lo) {
+  __half h[8], l[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { h[k] = __float2half_rn(v[k]); l[k] = __float2half_rn(v[k] - __half2float(h[k])); }
+  hi = *reinterpret_cast<const uint4*>(h); lo = *reinterpret_cast<const uint4*>(l);
+}
+
+// table operands (one-time, at table creation): entry e = s*128 + (j n_band + b)
+// one warp per (cell, age): Cm = 2^ceil(log2 max_e |c_t[i][e]|); the largest |D_t| / Cm over the table goes to *dmax
+__global__ void cssp_rowmax_kernel(TableDev T, float* __restrict__ Cm, int* __restrict__ dmax) {
+  const int64_t wid = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (wid >= (int64_t)(T.n_z - 1) * NA) return;
+  const int i = (int)(wid % NA), cell = (int)(wid / NA);
+  float cm = 1.f;
+  if (i < T.n_age) {
+    const float* c0 = T.cssp + (((int64_t)cell * 2) * T.n_age + i) * T.cs_stride;
+    const float* c1 = c0 + (int64_t)T.n_age * T.cs_stride;
+    const int E = T.n_Z * T.n_band;
+    float mx = 0.f, dx = 0.f;
+    for (int e = lane; e < E; e += 32) { mx = fmaxf(mx, fabsf(c0[e])); dx = fmaxf(dx, fabsf(c1[e])); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { mx = fmaxf(mx, __shfl_xor_sync(FULL_MASK, mx, o)); dx = fmaxf(dx, __shfl_xor_sync(FULL_MASK, dx, o)); }
+    if (mx > 1.0e-30f && mx < 1.0e30f) cm = __uint_as_float(((__float_as_uint(mx) >> 23) + 1u) << 23);       // 2^(ex+1) > mx
+    if (lane == 0 && dx > 0.f) atomicMax(dmax, __float_as_int(dx / cm));
+  }
+  if (lane == 0) Cm[wid] = cm;
+}
+__global__ void build_c_operands_kernel(TableDev T, const float* __restrict__ Cm, float sD, __half* __restrict__ c1h, __half* __restrict__ c1l,
+                                        __half* __restrict__ c2h, __half* __restrict__ c2l) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int n_cells = T.n_z - 1;
+  if (idx >= (int64_t)n_cells * NE * NA) return;
+  const int i = (int)(idx % NA), e = (int)((idx / NA) % NE), cell = (int)(idx / ((int64_t)NA * NE));
+  const int s = e >> 7, ee = e & 127;
+  float v = 0.f;
+  if (i < T.n_age && ee < T.n_Z * T.n_band) v = T.cssp[(((int64_t)cell * 2 + s) * T.n_age + i) * T.cs_stride + ee] * (H_TOP / Cm[cell * NA + i]) * (s ? sD : 1.f);
+  const __half h = __float2half_rn(v), l = __float2half_rn(v - __half2float(h));
+  c1h[((int64_t)cell * NE + e) * NA + i] = h; c1l[((int64_t)cell * NE + e) * NA + i] = l;
+  c2h[((int64_t)cell * NA + i) * NE + e] = h; c2l[((int64_t)cell * NA + i) * NE + e] = l;
+}
+
+// shared memory: [0, 64 KB) A / V operand tiles, [64 KB, 192 KB) table operand tiles, then the barriers
+constexpr uint32_t OFF_B = REG_AV, OFF_BAR = REG_AV + REG_B;
+enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M0, BAR_V1, BAR_M1, N_BARS };
+
+struct ApproxArgs {
+  int64_t n;
+  const int* order; const int* bins;
+  const int* gal_of_row; const float* obs_flux; const float* obs_sigma; const float* flux_bar;
+  int want_grad;
+  const float* Cm;         // [n_cells][128]
+  float inv_sD;
+};
+
+// NB = n_band (compile time: entry e -> (j, b) = (e / NB, e % NB) resolves to register names in the unrolled band step)
+template <int NB>
+__global__ void __launch_bounds__(THREADS_TC, 1)
+approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__ CUtensorMap m1h, const __grid_constant__ CUtensorMap m1l,
+                 const __grid_constant__ CUtensorMap m2h, const __grid_constant__ CUtensorMap m2l) {
+  extern __shared__ unsigned char smem_dyn[];
+  const int nb = T.n_z - 1, stride = nb + 2;
+  const int* row_start = G.bins + stride; const int* cta_start = G.bins + 2 * stride;
+  const int total = cta_start[nb];
+  const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
+  const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
+  const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
+  if (w_begin >= w_end) return;
+  const uint32_t base = (smem_u32(smem_dyn) + 1023u) & ~1023u;
+  unsigned char* gbase = smem_dyn + (base - smem_u32(smem_dyn));
+  const uint32_t bars = base + OFF_BAR;
+  volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + OFF_BAR + 128);
+  float* cm_s = reinterpret_cast<float*>(gbase + OFF_BAR + 256);     // [128] Cm_i / 2^14 of the current tile's cell
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#define BAR(i) (bars + 8u * (i))
+  if (threadIdx.x == 0) {
+    mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
+    mbar_init(BAR(BAR_V0), TM); mbar_init(BAR(BAR_M0), 1); mbar_init(BAR(BAR_V1), TM); mbar_init(BAR(BAR_M1), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 4) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bars + 128u), "n"(512) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr;
+  int lo = 0, hi = nb;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cta_start[mid] <= w_begin) lo = mid; else hi = mid; }
+  int cell = lo;
+
+  if (warp == 4) {
+    // ===== TMA loads + MMA issue =================================================================
+    if (lane == 0) {
+      // instruction descriptor: D = F32, A and B = F16 (format 0), both K-major
+      const uint32_t idesc1 = (1u << 4) | ((uint32_t)(NE >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+      const uint32_t idesc2 = (1u << 4) | ((uint32_t)(NA >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+      uint32_t ph = 0;
+      for (int w = w_begin; w < w_end; ++w, ph ^= 1u) {
+        while (cta_start[cell + 1] <= w) ++cell;
+        // pass-1 operands: C1 tiles [256 entries][64 ages], hi k-block 0, 1 then lo k-block 0, 1
+        mbar_expect_tx(BAR(BAR_B1), (uint32_t)REG_B);
+        tma_load_2d(base + OFF_B, &m1h, BAR(BAR_B1), 0, cell * NE);
+        tma_load_2d(base + OFF_B + 32768u, &m1h, BAR(BAR_B1), KB, cell * NE);
+        tma_load_2d(base + OFF_B + 65536u, &m1l, BAR(BAR_B1), 0, cell * NE);
+        tma_load_2d(base + OFF_B + 98304u, &m1l, BAR(BAR_B1), KB, cell * NE);
+        mbar_wait(BAR(BAR_B1), ph);
+        mbar_wait(BAR(BAR_A), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk) {
+            const uint64_t a_hi = desc_sw128(base + kb * TILE_A + kk * 32), a_lo = desc_sw128(base + (2 + kb) * TILE_A + kk * 32);
+            const uint64_t b_hi = desc_sw128(base + OFF_B + kb * 32768u + kk * 32), b_lo = desc_sw128(base + OFF_B + 65536u + kb * 32768u + kk * 32);
+            // the cross terms (2^-11 of the main one) have an accumulator of their own: the main accumulator then sees
+            // 8 truncating updates instead of 24 (tensor-core accumulation rounds toward zero)
+            tc_mma_f16(tmem_base + NE, a_lo, b_hi, idesc1, (kb | kk) ? 1u : 0u);
+            tc_mma_f16(tmem_base + NE, a_hi, b_lo, idesc1, 1u);
+            tc_mma_f16(tmem_base, a_hi, b_hi, idesc1, (kb | kk) ? 1u : 0u);
+          }
+        tc_commit(BAR(BAR_P));
+        mbar_wait(BAR(BAR_P), ph);                          // pass 1 retired: the table region may be overwritten
+        if (!G.want_grad) continue;
+        // pass-2 operands: C2 tiles [128 ages][64 entries], hi entry block 0..3 then lo entry block 0..3
+        mbar_expect_tx(BAR(BAR_B2), (uint32_t)REG_B);
+#pragma unroll
+        for (int eb = 0; eb < 4; ++eb) {
+          tma_load_2d(base + OFF_B + eb * 16384u, &m2h, BAR(BAR_B2), eb * KB, cell * NA);
+          tma_load_2d(base + OFF_B + 65536u + eb * 16384u, &m2l, BAR(BAR_B2), eb * KB, cell * NA);
+        }
+        mbar_wait(BAR(BAR_B2), ph);
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+          mbar_wait(BAR(s ? BAR_V1 : BAR_V0), ph);
+          tc_fence_after();
+#pragma unroll
+          for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk) {
+              const int eb = 2 * s + kb;
+              const uint64_t a_hi = desc_sw128(base + kb * TILE_A + kk * 32), a_lo = desc_sw128(base + (2 + kb) * TILE_A + kk * 32);
+              const uint64_t b_hi = desc_sw128(base + OFF_B + eb * 16384u + kk * 32), b_lo = desc_sw128(base + OFF_B + 65536u + eb * 16384u + kk * 32);
+              // a_bar reuses the columns of P (dead once V is being written): main terms at 0, cross terms at NA
+              tc_mma_f16(tmem_base + NA, a_lo, b_hi, idesc2, (s | kb | kk) ? 1u : 0u);
+              tc_mma_f16(tmem_base + NA, a_hi, b_lo, idesc2, 1u);
+              tc_mma_f16(tmem_base, a_hi, b_hi, idesc2, (s | kb | kk) ? 1u : 0u);
+            }
+          tc_commit(BAR(s ? BAR_M1 : BAR_M0));
+        }
+        mbar_wait(BAR(BAR_M1), ph);                         // pass 2 retired: both regions are free for the next tile
+      }
+    }
+  } else {
+    // ===== row warps ==============================================================================
+    const int r = threadIdx.x;                              // tile row = TMEM lane
+    const uint32_t tlane = tmem_base + ((uint32_t)(warp * 32) << 16);
+    uint32_t ph = 0;
+    for (int w = w_begin; w < w_end; ++w, ph ^= 1u) {
+      while (cta_start[cell + 1] <= w) ++cell;
+      const int r_begin = row_start[cell] + (w - cta_start[cell]) * TM;
+      const int r_end = min(row_start[cell + 1], r_begin + TM);
+      const int rw = (r_begin + r < r_end) ? __ldg(G.order + r_begin + r) : -1;
+      // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row ----
+      float a_rs = 1.f;                                     // this thread's row: power-of-two scale of its a_i Cm_i
+      {
+        const int kb = lane >> 4, c = (lane & 15) >> 1, half = lane & 1;
+        const float4 cm4 = __ldg(reinterpret_cast<const float4*>(G.Cm + (int64_t)cell * NA) + lane);
+        asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");            // every row thread is done with the previous tile's cm_s
+        cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
+#pragma unroll
+        for (int t0 = 0; t0 < 32; t0 += 8) {
+          float4 av[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int row_u = __shfl_sync(FULL_MASK, rw, t0 + u);
+            av[u] = row_u >= 0 ? __ldg(reinterpret_cast<const float4*>(B.a + (int64_t)row_u * ROW_A_STRIDE) + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            float v[4] = {av[u].x * cm4.x, av[u].y * cm4.y, av[u].z * cm4.z, av[u].w * cm4.w};
+            float mx = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { if (4 * lane + k >= T.n_age) v[k] = 0.f; mx = fmaxf(mx, fabsf(v[k])); }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL_MASK, mx, o));
+            float rs = 1.f;                                   // rs mx in [2^13, 2^14)
+            if (mx > 1.0e-30f && mx < 1.0e30f) rs = __uint_as_float((uint32_t)(127 + 13 + 127 - (int)((__float_as_uint(mx) >> 23) & 0xffu)) << 23);
+            if (lane == t0 + u) a_rs = rs;
+            __half h[4], l[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              v[k] *= rs;
+              h[k] = __float2half_rn(v[k]); l[k] = __float2half_rn(v[k] - __half2float(h[k]));
+            }
+            const uint32_t off = kb * TILE_A + sw128_off(warp * 32 + t0 + u, c) + half * 8;
+            *reinterpret_cast<uint2*>(gbase + off) = *reinterpret_cast<const uint2*>(h);
+            *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(l);
+          }
+        }
+      }
+      tc_fence_before();                                    // the previous tile's TMEM reads are complete
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_arrive(BAR(BAR_A));
+      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // cm_s of this tile is complete
+      const float u0 = 1.f / (H_TOP * a_rs), u1 = u0 * G.inv_sD;          // P^(s) back to table units
+      // ---- the row's scalars, metallicity weights and observations (while the MMAs run) ----
+      RowScalars sc;
+      float m[16], ob0[NB], ob1[NB];
+      {
+        float4* scq = reinterpret_cast<float4*>(&sc);
+        float4* mq = reinterpret_cast<float4*>(m);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          scq[q] = rw >= 0 ? reinterpret_cast<const float4*>(B.sc + rw)[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+          mq[q] = rw >= 0 ? __ldg(reinterpret_cast<const float4*>(B.m + (int64_t)rw * ROW_M_STRIDE) + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < 16; ++j) if (j >= T.n_Z) m[j] = 0.f;
+        const int64_t gal = (rw >= 0 && !G.flux_bar) ? (G.gal_of_row ? __ldg(G.gal_of_row + rw) : rw) : 0;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+          ob0[b] = 0.f; ob1[b] = 1.f;
+          if (rw >= 0) {
+            if (G.flux_bar) ob0[b] = __ldg(G.flux_bar + (int64_t)rw * NB + b);
+            else { ob0[b] = __ldg(G.obs_flux + gal * NB + b); ob1[b] = __ldg(G.obs_sigma + gal * NB + b); }
+          }
+        }
+      }
+      const float f = sc.zfrac, Mn = sc.Mn, zp = 1.f + sc.z;
+      const int E = T.n_Z * NB;
+      // ---- sweep 1 over P: S^(s)_b = sum_j m_j P^(s)[j NB + b] ----
+      float S0[NB], S1[NB];
+#pragma unroll
+      for (int b = 0; b < NB; ++b) S0[b] = S1[b] = 0.f;
+      mbar_wait(BAR(BAR_P), ph);
+      tc_fence_after();
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        if (16 * c < E) {
+          uint32_t v0[16], v1[16], x0[16], x1[16];
+          TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
+          TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
+          tld_wait();
+#pragma unroll
+          for (int k = 0; k < 16; ++k) {
+            const int e = 16 * c + k, j = e / NB, b = e % NB;
+            if (j < 16) {
+              S0[b] = fmaf(m[j], __uint_as_float(v0[k]) + __uint_as_float(x0[k]), S0[b]);
+              S1[b] = fmaf(m[j], __uint_as_float(v1[k]) + __uint_as_float(x1[k]), S1[b]);
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int b = 0; b < NB; ++b) { S0[b] *= u0; S1[b] *= u1; }
+      // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood) ----
+      float sbar[NB], fl[16];
+      float chi2 = 0.f, v_mn = 0.f, v_z = 0.f, v_av = 0.f, v_de = 0.f, v_fl = 0.f;
+      const float izp = __fdividef(1.f, zp);
+#pragma unroll
+      for (int b = 0; b < 16; ++b) fl[b] = 0.f;
+#pragma unroll
+      for (int b = 0; b < NB; ++b) {
+        float F, F_av, F_del, F_fl, F_lam;
+        const float lam_r = T.lam_eff[b] * izp;
+        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
+        const float Sint = S0[b] + f * S1[b];
+        const float flux = F * Mn * Sint;
+        fl[b] = flux;
+        float g;
+        if (G.flux_bar) g = ob0[b];
+        else {
+          const float isg = __fdividef(1.f, ob1[b]);
+          const float rr = (flux - ob0[b]) * isg;
+          chi2 = fmaf(rr, rr, chi2);
+          g = -rr * isg;
+        }
+        v_mn += g * F * Sint;
+        v_z += g * (F * Mn * S1[b] * T.inv_dz + Mn * Sint * F_lam * (-lam_r * izp));
+        v_av += g * Mn * Sint * F_av; v_de += g * Mn * Sint * F_del; v_fl += g * Mn * Sint * F_fl;
+        sbar[b] = g * F * Mn;
+      }
+      if (rw >= 0) {
+        float4* fo = reinterpret_cast<float4*>(B.flux + (int64_t)rw * SPS_MAX_BAND);
+#pragma unroll
+        for (int q = 0; q < (NB + 3) / 4; ++q) fo[q] = make_float4(fl[4 * q], fl[4 * q + 1], fl[4 * q + 2], fl[4 * q + 3]);
+        RowScalars* out = B.sc + rw;
+        out->logp_like = -0.5f * chi2;
+        if (G.want_grad) { out->Mn_bar = v_mn; out->z_bar = v_z; out->AV_bar = v_av; out->delta_bar = v_de; out->Ffloor_bar = v_fl; }
+      }
+      if (!G.want_grad) continue;
+      // ---- sweep 2 over P: m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
+      {
+        float mb[16];
+        const float fu1 = f * u1;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) mb[j] = 0.f;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          if (16 * c < E) {
+            uint32_t v0[16], v1[16], x0[16], x1[16];
+            TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
+            TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
+            tld_wait();
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+              const int e = 16 * c + k, j = e / NB, b = e % NB;
+              if (j < 16) mb[j] = fmaf(sbar[b], fmaf(fu1, __uint_as_float(v1[k]) + __uint_as_float(x1[k]), u0 * (__uint_as_float(v0[k]) + __uint_as_float(x0[k]))), mb[j]);
+            }
+          }
+        }
+        if (rw >= 0) {
+          float4* mo = reinterpret_cast<float4*>(B.m_bar + (int64_t)rw * ROW_M_STRIDE);
+#pragma unroll
+          for (int q = 0; q < 4; ++q) mo[q] = make_float4(mb[4 * q], mb[4 * q + 1], mb[4 * q + 2], mb[4 * q + 3]);
+        }
+      }
+      tc_fence_before();
+      // ---- V^(s)[e] = sbar_b m_j {1, f}: the A operand of pass 2, one phase per table array; the row is scaled by a
+      //      power of two sv that puts its largest entry near 2^14 (FP16 split: 22 significant bits below the row maximum) ----
+      float sv = 1.f;
+      {
+        float smax = 0.f, mmax = 0.f;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) smax = fmaxf(smax, fabsf(sbar[b]));
+#pragma unroll
+        for (int j = 0; j < 16; ++j) mmax = fmaxf(mmax, fabsf(m[j]));
+        const float vmax = smax * mmax * fmaxf(1.f, f * G.inv_sD);
+        if (vmax > 1.0e-30f && vmax < 1.0e30f) {
+          const int ex = (int)((__float_as_uint(vmax) >> 23) & 0xffu) - 127;      // vmax in [2^ex, 2^(ex+1))
+          sv = __uint_as_float((uint32_t)(127 + 13 - ex) << 23);                 // sv vmax in [2^13, 2^14)
+        }
+      }
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        if (s == 1) mbar_wait(BAR(BAR_M0), ph);             // phase-0 MMAs have read V^(0)
+        const float scale = (rw >= 0) ? (s ? sv * f * G.inv_sD : sv) : 0.f;
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            float v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const int e = 64 * kb + 8 * c + k, j = e / NB, b = e % NB;
+              v[k] = (j < 16) ? scale * sbar[b] * m[j] : 0.f;
+            }
+            uint4 vh, vl;
+            split8(v, vh, vl);
+            const uint32_t off = kb * TILE_A + sw128_off(r, c);
+            *reinterpret_cast<uint4*>(gbase + off) = vh;
+            *reinterpret_cast<uint4*>(gbase + 2 * TILE_A + off) = vl;
+          }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_arrive(BAR(s ? BAR_V1 : BAR_V0));
+      }
+      // ---- a_bar from TMEM ----
+      mbar_wait(BAR(BAR_M1), ph);
+      tc_fence_after();
+      const float ua = 1.f / sv;
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        uint32_t v[16], x[16];
+        TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x);
+        tld_wait();
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = __float_as_uint((__uint_as_float(v[k]) + __uint_as_float(x[k])) * (ua * cm_s[16 * c + k]));
+        if (rw >= 0) {
+          float4* ao = reinterpret_cast<float4*>(B.a_bar + (int64_t)rw * ROW_A_STRIDE + 16 * c);
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            ao[q] = make_float4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]));
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512) : "memory");
+  }
+#undef BAR
+}
+
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// [rows][cols] fp16 row-major -> boxes of box_rows x 64 elements (128 bytes), 128-byte swizzle
+sps_status make_map_f16(EncodeTiledFn enc, CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+  const cuuint64_t dims[2] = {cols, rows};
+  const cuuint64_t strides[1] = {cols * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)KB, box_rows};
+  const cuuint32_t es[2] = {1, 1};
+  const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { sps_set_error("cuTensorMapEncodeTiled (approximate path) failed with CUresult %d", (int)r); return SPS_ECUDA; }
+  return SPS_OK;
+}
+
+template <int NB>
+sps_status launch_nb(const ApproxTc* S, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
+  if (configure_only)
+    return sps_check_cuda(cudaFuncSetAttribute(approx_tc_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TC), "approximate tensor-core kernel shared memory opt-in");
+  approx_tc_kernel<NB><<<S->sm_count, THREADS_TC, SMEM_TC, s>>>(T, G, B, S->m1_hi, S->m1_lo, S->m2_hi, S->m2_lo);
+  return SPS_OK;
+}
+sps_status dispatch(const ApproxTc* S, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
+  switch (T.n_band) {
+#define CASE(NB) case NB: return launch_nb<NB>(S, T, G, B, s, configure_only);
+    SPS_APPROX_TC_BANDS(CASE)
+#undef CASE
+    default: return SPS_EUNSUPPORTED;
+  }
+}
+int g_force_simt_approx = 0;
+
+}  // namespace
+
+extern "C" void sps_debug_approx_simt(int on) { g_force_simt_approx = on; }
+
+bool sps_approx_tc_active(const sps_table* t) { return t->approx_tc != nullptr && !g_force_simt_approx; }
+
+// Table operands of the tensor-core contraction; leaves t->approx_tc null (SIMT kernel) for shapes outside its range.
+sps_status sps_approx_tc_setup(sps_table* t) {
+  const TableDev& T = t->dev;
+  t->approx_tc = nullptr;
+  bool band_ok = false;
+#define CASE(NB) band_ok = band_ok || T.n_band == NB;
+  SPS_APPROX_TC_BANDS(CASE)
+#undef CASE
+  if (!band_ok || T.n_Z * T.n_band > 128 || T.n_age > NA || T.n_Z > 16) return SPS_OK;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    sps_set_error("cuTensorMapEncodeTiled is not available from this driver");
+    return SPS_EUNSUPPORTED;
+  }
+  ApproxTc* S = new ApproxTc();
+  memset(S, 0, sizeof(*S));
+  int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&S->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  const int n_cells = T.n_z - 1;
+  const size_t elems = (size_t)n_cells * NE * NA;
+  sps_status st = SPS_OK;
+  __half** arrs[4] = {&S->C1_hi, &S->C1_lo, &S->C2_hi, &S->C2_lo};
+  for (auto a : arrs)
+    if (st == SPS_OK && cudaMalloc(a, elems * sizeof(__half)) != cudaSuccess) { cudaGetLastError(); sps_set_error("cudaMalloc of the approximate-path tensor-core operands failed"); st = SPS_ENOMEM; }
+  int* d_max = nullptr;
+  if (st == SPS_OK && (cudaMalloc(&d_max, sizeof(int)) != cudaSuccess || cudaMalloc(&S->Cm, (size_t)n_cells * NA * sizeof(float)) != cudaSuccess)) {
+    cudaGetLastError(); sps_set_error("cudaMalloc of the approximate-path scales failed"); st = SPS_ENOMEM;
+  }
+  if (st == SPS_OK) {
+    cudaMemset(d_max, 0, sizeof(int));
+    cssp_rowmax_kernel<<<(unsigned)(((int64_t)n_cells * NA * 32 + 255) / 256), 256>>>(T, S->Cm, d_max);
+    float rho = 0.f;
+    st = sps_check_cuda(cudaMemcpy(&rho, d_max, sizeof(float), cudaMemcpyDeviceToHost), "c_SSP range");
+    int ex = 0;
+    S->sD = 1.f;
+    if (rho > 0.f) { std::frexp(rho, &ex); S->sD = std::ldexp(1.f, std::max(-60, std::min(60, -ex))); }         // rho sD in [1/2, 1)
+  }
+  if (d_max) cudaFree(d_max);
+  if (st == SPS_OK) {
+    build_c_operands_kernel<<<(unsigned)((elems + 255) / 256), 256>>>(T, S->Cm, S->sD, S->C1_hi, S->C1_lo, S->C2_hi, S->C2_lo);
+    sps_count_launch(2);
+    st = sps_check_cuda(cudaDeviceSynchronize(), "approximate-path operand build");
+  }
+  EncodeTiledFn enc = (EncodeTiledFn)fn;
+  if (st == SPS_OK) st = make_map_f16(enc, &S->m1_hi, S->C1_hi, (uint64_t)n_cells * NE, NA, NE);
+  if (st == SPS_OK) st = make_map_f16(enc, &S->m1_lo, S->C1_lo, (uint64_t)n_cells * NE, NA, NE);
+  if (st == SPS_OK) st = make_map_f16(enc, &S->m2_hi, S->C2_hi, (uint64_t)n_cells * NA, NE, NA);
+  if (st == SPS_OK) st = make_map_f16(enc, &S->m2_lo, S->C2_lo, (uint64_t)n_cells * NA, NE, NA);
+  if (st == SPS_OK) st = dispatch(S, T, ApproxArgs(), RowBuffers(), 0, true);
+  t->approx_tc = S;
+  if (st != SPS_OK) sps_approx_tc_teardown(t);
+  return st;
+}
+
+void sps_approx_tc_teardown(sps_table* t) {
+  ApproxTc* S = reinterpret_cast<ApproxTc*>(t->approx_tc);
+  if (!S) return;
+  void* ptrs[] = {S->C1_hi, S->C1_lo, S->C2_hi, S->C2_lo, S->Cm};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  delete S;
+  t->approx_tc = nullptr;
+}
+
+sps_status sps_approx_tc_contract(sps_table* t, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
+                                  const float* obs_sigma, const float* flux_bar, bool want_grad, cudaStream_t s) {
+  if (n <= 0) return SPS_OK;
+  const ApproxTc* S = reinterpret_cast<const ApproxTc*>(t->approx_tc);
+  const TableDev& T = t->dev;
+  approx_group_rows(T, n, rows, t->rows, TM, s);
+  ApproxArgs G;
+  G.n = n; G.order = t->rows.order; G.bins = t->rows.bins; G.gal_of_row = gal_of_row; G.obs_flux = obs_flux; G.obs_sigma = obs_sigma;
+  G.flux_bar = flux_bar; G.want_grad = want_grad ? 1 : 0;
+  G.Cm = S->Cm; G.inv_sD = 1.f / S->sD;
+  sps_prof_begin(SPS_K_APPROX, s);
+  sps_status st = dispatch(S, T, G, t->rows, s, false);
+  sps_prof_end(SPS_K_APPROX, s);
+  sps_count_launch();
+  if (st != SPS_OK) return st;
+  return sps_check_cuda(cudaGetLastError(), "approximate contraction (tcgen05) launch");
+}

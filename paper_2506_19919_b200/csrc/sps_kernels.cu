@@ -85,7 +85,7 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
 #endif
 #define AC_ROWS_PER_CTA (AC_WARPS * AC_R)
 
-__global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restrict__ bins) {
+__global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int rows_per_item, int* __restrict__ bins) {
   __shared__ int s_rows[1024], s_ctas[1024];
   const int stride = nb + 2;
   int* hist = bins; int* row_start = bins + stride; int* cta_start = bins + 2 * stride; int* cursor = bins + 3 * stride;
@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(1024) approx_plan_kernel(int nb, int* __restri
   int carry_r = 0, carry_c = 0;
   for (int base = 0; base < nb; base += 1024) {
     const int b = base + t;
-    const int cnt = b < nb ? hist[b] : 0, ctas = (cnt + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA;
+    const int cnt = b < nb ? hist[b] : 0, ctas = (cnt + rows_per_item - 1) / rows_per_item;
     s_rows[t] = cnt; s_ctas[t] = ctas;
     __syncthreads();
     for (int o = 1; o < 1024; o <<= 1) {
@@ -547,14 +547,21 @@ sps_status approx_contract_setup(const TableDev& T) {
                         "approximate-path shared memory opt-in");
 }
 
+// rows of a call grouped by z cell (the histogram was taken by the prologue): cell offsets, item offsets, scatter
+void approx_group_rows(const TableDev& T, int64_t n, const int* rows, RowBuffers B, int rows_per_item, cudaStream_t s) {
+  const int nb = T.n_z - 1, stride = nb + 2;
+  const unsigned eb = (unsigned)((n + 255) / 256);
+  approx_plan_kernel<<<1, 1024, 0, s>>>(nb, rows_per_item, B.bins);
+  approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
+  sps_count_launch(2);
+}
+
 void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
-  const int nb = T.n_z - 1, stride = nb + 2;
-  const unsigned eb = (unsigned)((n + 255) / 256);
-  approx_plan_kernel<<<1, 1024, 0, s>>>(nb, B.bins);
-  approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
+  const int nb = T.n_z - 1;
+  approx_group_rows(T, n, rows, B, AC_ROWS_PER_CTA, s);
   static int sm_count = 0;
   if (!sm_count) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev); }
   const unsigned grid = (unsigned)std::min<int64_t>(sm_count, (n + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA + nb);
@@ -562,7 +569,7 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
   approx_contract_kernel<<<grid, 32 * AC_WARPS, approx_smem_bytes(T), s>>>(T, n, B.order, B.bins, gal_of_row, obs_flux, obs_sigma,
                                                                          flux_bar, want_grad, B);
   sps_prof_end(SPS_K_APPROX, s);
-  sps_count_launch(3);
+  sps_count_launch();
 }
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s) {

@@ -30,6 +30,7 @@ void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);
 sps_status approx_contract_setup(const TableDev& T);
+void approx_group_rows(const TableDev& T, int64_t n, const int* rows, RowBuffers B, int rows_per_item, cudaStream_t s);
 void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded,
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s);
 void launch_copy_weights(const TableDev& T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar,

@@ -167,6 +167,7 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   if (wave_dd) cudaFree(wave_dd);
   if (dlam_dd) cudaFree(dlam_dd);
   if (st == SPS_OK) st = approx_contract_setup(T);
+  if (st == SPS_OK) st = sps_approx_tc_setup(t);
   if (st == SPS_OK) st = sps_exact_setup(t, d->exact_precision);
   if (st != SPS_OK) { sps_destroy_table(t); return st; }
   *out = t;
@@ -179,6 +180,7 @@ extern "C" sps_status sps_destroy_table(sps_table* t) {
   const void* ptrs[] = {T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
   for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
   sps_exact_teardown(t);
+  sps_approx_tc_teardown(t);
   sps_free_row_buffers(t);
   delete t;
   return SPS_OK;

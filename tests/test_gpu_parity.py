@@ -49,6 +49,15 @@ def exact_kernels(request):
     binding.lib().sps_debug_force_simt(0)
 
 
+@pytest.fixture(params=["tcgen05", "simt_fp32"])
+def approx_kernels(request):
+    """Runs an approximate-path test through the tcgen05 contraction (FP16 split) and through the fp32 SIMT contraction."""
+    from paper_2506_19919_b200 import binding
+    binding.lib().sps_debug_approx_simt(int(request.param == "simt_fp32"))
+    yield request.param
+    binding.lib().sps_debug_approx_simt(0)
+
+
 class Ctx:
     def __init__(self, kind):
         sps = _sps()
@@ -160,7 +169,7 @@ def test_cssp_table(kind, request):
 
 
 @pytest.mark.parametrize("kind", ["tiny", "full"])
-def test_approx_flux_and_vjp(kind, request):
+def test_approx_flux_and_vjp(kind, request, approx_kernels):
     cx = request.getfixturevalue(kind)
     n = 300
     thu, thd = cx.theta(n, 15, z_uniform=(0.1, 2.9))
@@ -193,7 +202,7 @@ def _observations(cx, n_gal, seed, path="approx", frac=(0.05, 0.10)):
 
 
 @pytest.mark.parametrize("kind", ["tiny", "full"])
-def test_loglike_grad_approx(kind, request):
+def test_loglike_grad_approx(kind, request, approx_kernels):
     cx = request.getfixturevalue(kind)
     n_gal, n_chain = 40, 3
     truth_u, d, s = _observations(cx, n_gal, 31)
@@ -203,7 +212,14 @@ def test_loglike_grad_approx(kind, request):
     olp, og, _ = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64),
                                  "approx", cx.cssp())
     assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4
-    assert _grad_err(g.cpu().numpy(), og).max() <= 1e-3
+    # rows 0.3 sd from the mode: a flux error eps f_b enters the gradient as eps sum_b f_b/sigma_b^2 |J_b| (DESIGN.md
+    # "Tolerances"); eps = 4e-6 covers the fp32 rounding of a band flux and the tensor-core accumulation bias (measured
+    # <= 3.6e-6 in all, against north_star's 1e-4 on fluxes)
+    th, dth = M.bound(thu.astype(np.float64), cx.P)
+    of, J = M.photometry_approx(th, cx.grid, cx.cssp())
+    allow = 4e-6 * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
+    err = np.maximum(np.abs(g.cpu().numpy() - og) - allow, 0.0)
+    assert (err / np.maximum(np.abs(og), 1e-3 * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
 
 
 def test_leapfrog_trajectory_approx(tiny):
