@@ -130,6 +130,13 @@ __global__ void build_c_operands_kernel(TableDev T, const float* __restrict__ Cm
 constexpr uint32_t OFF_B = REG_AV, OFF_BAR = REG_AV + REG_B;
 enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M0, BAR_V1, BAR_M1, N_BARS };
 
+#ifdef SPS_ATC_TIMING
+__device__ long long g_atc_t[16];
+#define TSTAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { const long long t_now = clock64(); g_atc_t[i] += t_now - t_prev; t_prev = t_now; } } while (0)
+#else
+#define TSTAMP(i)
+#endif
+
 struct ApproxArgs {
   int64_t n;
   const int* order; const int* bins;
@@ -248,50 +255,12 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       const int r_begin = row_start[cell] + (w - cta_start[cell]) * TM;
       const int r_end = min(row_start[cell + 1], r_begin + TM);
       const int rw = (r_begin + r < r_end) ? __ldg(G.order + r_begin + r) : -1;
-      // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row ----
-      float a_rs = 1.f;                                     // this thread's row: power-of-two scale of its a_i Cm_i
-      {
-        const int kb = lane >> 4, c = (lane & 15) >> 1, half = lane & 1;
-        const float4 cm4 = __ldg(reinterpret_cast<const float4*>(G.Cm + (int64_t)cell * NA) + lane);
-        asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");            // every row thread is done with the previous tile's cm_s
-        cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
-#pragma unroll
-        for (int t0 = 0; t0 < 32; t0 += 8) {
-          float4 av[8];
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const int row_u = __shfl_sync(FULL_MASK, rw, t0 + u);
-            av[u] = row_u >= 0 ? __ldg(reinterpret_cast<const float4*>(B.a + (int64_t)row_u * ROW_A_STRIDE) + lane) : make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            float v[4] = {av[u].x * cm4.x, av[u].y * cm4.y, av[u].z * cm4.z, av[u].w * cm4.w};
-            float mx = 0.f;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { if (4 * lane + k >= T.n_age) v[k] = 0.f; mx = fmaxf(mx, fabsf(v[k])); }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL_MASK, mx, o));
-            float rs = 1.f;                                   // rs mx in [2^13, 2^14)
-            if (mx > 1.0e-30f && mx < 1.0e30f) rs = __uint_as_float((uint32_t)(127 + 13 + 127 - (int)((__float_as_uint(mx) >> 23) & 0xffu)) << 23);
-            if (lane == t0 + u) a_rs = rs;
-            __half h[4], l[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              v[k] *= rs;
-              h[k] = __float2half_rn(v[k]); l[k] = __float2half_rn(v[k] - __half2float(h[k]));
-            }
-            const uint32_t off = kb * TILE_A + sw128_off(warp * 32 + t0 + u, c) + half * 8;
-            *reinterpret_cast<uint2*>(gbase + off) = *reinterpret_cast<const uint2*>(h);
-            *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(l);
-          }
-        }
-      }
-      tc_fence_before();                                    // the previous tile's TMEM reads are complete
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_arrive(BAR(BAR_A));
-      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // cm_s of this tile is complete
-      const float u0 = 1.f / (H_TOP * a_rs), u1 = u0 * G.inv_sD;          // P^(s) back to table units
-      // ---- the row's scalars, metallicity weights and observations (while the MMAs run) ----
+      const int n_rows = r_end - r_begin;
+#ifdef SPS_ATC_TIMING
+      long long t_prev = clock64();
+#endif
+      const int next_row = (w + 1 < w_end && r_end + r < G.n) ? __ldg(G.order + r_end + r) : -1;
+      // ---- the row's scalars, metallicity weights and observations (requested first: in flight while a is staged) ----
       RowScalars sc;
       float m[16], ob0[NB], ob1[NB];
       {
@@ -314,14 +283,65 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           }
         }
       }
+      // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row ----
+      float a_rs = 1.f;                                     // this thread's row: power-of-two scale of its a_i Cm_i
+      {
+        const int kb = lane >> 4, c = (lane & 15) >> 1, half = lane & 1;
+        const float4 cm4 = __ldg(reinterpret_cast<const float4*>(G.Cm + (int64_t)cell * NA) + lane);
+        asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");            // every row thread is done with the previous tile's cm_s
+        cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
+#pragma unroll 1
+        for (int t0 = 0; t0 < 32; t0 += 16) {
+          float4 av[16];
+#pragma unroll
+          for (int u = 0; u < 16; ++u) {
+            const int row_u = __shfl_sync(FULL_MASK, rw, t0 + u);                // rows past the tile's end: any valid row, zeroed below
+            av[u] = __ldg(reinterpret_cast<const float4*>(B.a + (int64_t)max(row_u, 0) * ROW_A_STRIDE) + lane);
+          }
+#pragma unroll
+          for (int u = 0; u < 16; ++u) {
+            float v[4] = {av[u].x * cm4.x, av[u].y * cm4.y, av[u].z * cm4.z, av[u].w * cm4.w};
+            float mx = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { if (4 * lane + k >= T.n_age || t0 + u >= n_rows - warp * 32) v[k] = 0.f; mx = fmaxf(mx, fabsf(v[k])); }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL_MASK, mx, o));
+            float rs = 1.f;                                   // rs mx in [2^13, 2^14)
+            if (mx > 1.0e-30f && mx < 1.0e30f) rs = __uint_as_float((uint32_t)(127 + 13 + 127 - (int)((__float_as_uint(mx) >> 23) & 0xffu)) << 23);
+            if (lane == t0 + u) a_rs = rs;
+            __half h[4], l[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              v[k] *= rs;
+              h[k] = __float2half_rn(v[k]); l[k] = __float2half_rn(v[k] - __half2float(h[k]));
+            }
+            const uint32_t off = kb * TILE_A + sw128_off(warp * 32 + t0 + u, c) + half * 8;
+            *reinterpret_cast<uint2*>(gbase + off) = *reinterpret_cast<const uint2*>(h);
+            *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(l);
+          }
+        }
+      }
+      if (next_row >= 0) {                                  // the next tile's weights start their way into L2 (its rows follow in `order`)
+        const char* np_ = reinterpret_cast<const char*>(B.a + (int64_t)next_row * ROW_A_STRIDE);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(np_ + 128 * q));
+      }
+      tc_fence_before();                                    // the previous tile's TMEM reads are complete
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_arrive(BAR(BAR_A));
+      TSTAMP(0);
+      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // cm_s of this tile is complete
+      const float u0 = 1.f / (H_TOP * a_rs), u1 = u0 * G.inv_sD;          // P^(s) back to table units
       const float f = sc.zfrac, Mn = sc.Mn, zp = 1.f + sc.z;
       const int E = T.n_Z * NB;
       // ---- sweep 1 over P: S^(s)_b = sum_j m_j P^(s)[j NB + b] ----
       float S0[NB], S1[NB];
 #pragma unroll
       for (int b = 0; b < NB; ++b) S0[b] = S1[b] = 0.f;
+      TSTAMP(1);
       mbar_wait(BAR(BAR_P), ph);
       tc_fence_after();
+      TSTAMP(2);
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         if (16 * c < E) {
@@ -339,45 +359,48 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           }
         }
       }
+      // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood).  A rolled loop over the
+      //      bands keeps the kernel inside the instruction cache; its per-band inputs and sbar_b sit in a per-thread scratch
+      //      column of the A / V region (pass 1 has retired, V is written later) ----
+      TSTAMP(3);
+      float* scr = reinterpret_cast<float*>(gbase) + r;     // scr[slot * TM]: slots 0-15 S^(0), 16-31 S^(1), 32-47 / 48-63 observations, 64-79 sbar
 #pragma unroll
-      for (int b = 0; b < NB; ++b) { S0[b] *= u0; S1[b] *= u1; }
-      // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood) ----
-      float sbar[NB], fl[16];
+      for (int b = 0; b < NB; ++b) { scr[b * TM] = S0[b] * u0; scr[(16 + b) * TM] = S1[b] * u1; scr[(32 + b) * TM] = ob0[b]; scr[(48 + b) * TM] = ob1[b]; }
       float chi2 = 0.f, v_mn = 0.f, v_z = 0.f, v_av = 0.f, v_de = 0.f, v_fl = 0.f;
       const float izp = __fdividef(1.f, zp);
-#pragma unroll
-      for (int b = 0; b < 16; ++b) fl[b] = 0.f;
-#pragma unroll
+      float* fo = B.flux + (int64_t)max(rw, 0) * SPS_MAX_BAND;
+#pragma unroll 2
       for (int b = 0; b < NB; ++b) {
         float F, F_av, F_del, F_fl, F_lam;
         const float lam_r = T.lam_eff[b] * izp;
         dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
-        const float Sint = S0[b] + f * S1[b];
+        const float s1 = scr[(16 + b) * TM];
+        const float Sint = scr[b * TM] + f * s1;
         const float flux = F * Mn * Sint;
-        fl[b] = flux;
-        float g;
-        if (G.flux_bar) g = ob0[b];
-        else {
-          const float isg = __fdividef(1.f, ob1[b]);
-          const float rr = (flux - ob0[b]) * isg;
+        if (rw >= 0) fo[b] = flux;
+        float g = scr[(32 + b) * TM];
+        if (!G.flux_bar) {
+          const float isg = __fdividef(1.f, scr[(48 + b) * TM]);
+          const float rr = (flux - g) * isg;
           chi2 = fmaf(rr, rr, chi2);
           g = -rr * isg;
         }
         v_mn += g * F * Sint;
-        v_z += g * (F * Mn * S1[b] * T.inv_dz + Mn * Sint * F_lam * (-lam_r * izp));
+        v_z += g * (F * Mn * s1 * T.inv_dz + Mn * Sint * F_lam * (-lam_r * izp));
         v_av += g * Mn * Sint * F_av; v_de += g * Mn * Sint * F_del; v_fl += g * Mn * Sint * F_fl;
-        sbar[b] = g * F * Mn;
+        scr[(64 + b) * TM] = g * F * Mn;
       }
       if (rw >= 0) {
-        float4* fo = reinterpret_cast<float4*>(B.flux + (int64_t)rw * SPS_MAX_BAND);
-#pragma unroll
-        for (int q = 0; q < (NB + 3) / 4; ++q) fo[q] = make_float4(fl[4 * q], fl[4 * q + 1], fl[4 * q + 2], fl[4 * q + 3]);
         RowScalars* out = B.sc + rw;
         out->logp_like = -0.5f * chi2;
         if (G.want_grad) { out->Mn_bar = v_mn; out->z_bar = v_z; out->AV_bar = v_av; out->delta_bar = v_de; out->Ffloor_bar = v_fl; }
       }
+      TSTAMP(4);
       if (!G.want_grad) continue;
       // ---- sweep 2 over P: m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
+      float sbar[NB];
+#pragma unroll
+      for (int b = 0; b < NB; ++b) sbar[b] = scr[(64 + b) * TM];
       {
         float mb[16];
         const float fu1 = f * u1;
@@ -403,6 +426,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           for (int q = 0; q < 4; ++q) mo[q] = make_float4(mb[4 * q], mb[4 * q + 1], mb[4 * q + 2], mb[4 * q + 3]);
         }
       }
+      TSTAMP(5);
       tc_fence_before();
       // ---- V^(s)[e] = sbar_b m_j {1, f}: the A operand of pass 2, one phase per table array; the row is scaled by a
       //      power of two sv that puts its largest entry near 2^14 (FP16 split: 22 significant bits below the row maximum) ----
@@ -419,9 +443,10 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           sv = __uint_as_float((uint32_t)(127 + 13 - ex) << 23);                 // sv vmax in [2^13, 2^14)
         }
       }
-#pragma unroll
+      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // every thread has read its scratch column: V may overwrite it
+#pragma unroll 1
       for (int s = 0; s < 2; ++s) {
-        if (s == 1) mbar_wait(BAR(BAR_M0), ph);             // phase-0 MMAs have read V^(0)
+        if (s == 1) { TSTAMP(7); mbar_wait(BAR(BAR_M0), ph); TSTAMP(8); }             // phase-0 MMAs have read V^(0)
         const float scale = (rw >= 0) ? (s ? sv * f * G.inv_sD : sv) : 0.f;
 #pragma unroll
         for (int kb = 0; kb < 2; ++kb)
@@ -442,24 +467,38 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         mbar_arrive(BAR(s ? BAR_V1 : BAR_V0));
       }
+      TSTAMP(9);
       // ---- a_bar from TMEM ----
       mbar_wait(BAR(BAR_M1), ph);
       tc_fence_after();
+      TSTAMP(10);
+      // thread = row reads its TMEM lane and parks the scaled values in the (free) A / V region, 16-byte chunks XOR-swizzled
+      // by the row; then each warp writes its 32 rows to global memory 512 contiguous bytes at a time
       const float ua = 1.f / sv;
-#pragma unroll
+      float4* stage = reinterpret_cast<float4*>(gbase);                   // [TM][32] float4
+#pragma unroll 1
       for (int c = 0; c < 8; ++c) {
         uint32_t v[16], x[16];
         TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x);
         tld_wait();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = __float_as_uint((__uint_as_float(v[k]) + __uint_as_float(x[k])) * (ua * cm_s[16 * c + k]));
-        if (rw >= 0) {
-          float4* ao = reinterpret_cast<float4*>(B.a_bar + (int64_t)rw * ROW_A_STRIDE + 16 * c);
-#pragma unroll
-          for (int q = 0; q < 4; ++q)
-            ao[q] = make_float4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), __uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]));
+        for (int q = 0; q < 4; ++q) {
+          float4 o;
+          o.x = (__uint_as_float(v[4 * q]) + __uint_as_float(x[4 * q])) * (ua * cm_s[16 * c + 4 * q]);
+          o.y = (__uint_as_float(v[4 * q + 1]) + __uint_as_float(x[4 * q + 1])) * (ua * cm_s[16 * c + 4 * q + 1]);
+          o.z = (__uint_as_float(v[4 * q + 2]) + __uint_as_float(x[4 * q + 2])) * (ua * cm_s[16 * c + 4 * q + 2]);
+          o.w = (__uint_as_float(v[4 * q + 3]) + __uint_as_float(x[4 * q + 3])) * (ua * cm_s[16 * c + 4 * q + 3]);
+          stage[r * 32 + ((4 * c + q) ^ (r & 7))] = o;
         }
       }
+      __syncwarp();                                                       // a warp stores the rows its own threads parked
+#pragma unroll 4
+      for (int t = 0; t < 32; ++t) {
+        const int row_t = __shfl_sync(FULL_MASK, rw, t);
+        const int rr = warp * 32 + t;
+        if (row_t >= 0) reinterpret_cast<float4*>(B.a_bar + (int64_t)row_t * ROW_A_STRIDE)[lane] = stage[rr * 32 + (lane ^ (rr & 7))];
+      }
+      TSTAMP(11);
     }
   }
   tc_fence_before();
@@ -508,6 +547,12 @@ int g_force_simt_approx = 0;
 }  // namespace
 
 extern "C" void sps_debug_approx_simt(int on) { g_force_simt_approx = on; }
+#ifdef SPS_ATC_TIMING
+extern "C" void sps_debug_atc_timing(long long* out16, int reset) {
+  cudaMemcpyFromSymbol(out16, g_atc_t, sizeof(long long) * 16);
+  if (reset) { long long z[16] = {0}; cudaMemcpyToSymbol(g_atc_t, z, sizeof(z)); }
+}
+#endif
 
 bool sps_approx_tc_active(const sps_table* t) { return t->approx_tc != nullptr && !g_force_simt_approx; }
 
