@@ -30,8 +30,10 @@ constexpr int NA = 128;                         // ages as GEMM dimension
 constexpr int TILE_A = TM * 128;                // 16 KB: 128 rows x 128 B
 constexpr int REG_AV = 4 * TILE_A;              // 64 KB: A (hi, lo) x 2 k blocks; later V (hi, lo) x 2 k blocks of a phase
 constexpr int REG_B = 128 * 1024;               // pass 1: 2 k blocks x (hi 32 KB + lo 32 KB); pass 2: 4 k blocks x (hi 16 KB + lo 16 KB)
-constexpr int SMEM_TC = REG_AV + REG_B + 1024 + 256 + 512;
-constexpr int THREADS_TC = 160;
+constexpr int OFF_EXTRA = REG_AV + REG_B + 256;     // cm_s[128], rs_s[128], red_s[6][128], mb_s[16][128] floats
+constexpr int BINS_S = 2048;                     // ints of shared memory for the cell offsets (row_start, cta_start)
+constexpr int SMEM_TC = OFF_EXTRA + (2 + 6 + 16) * 128 * 4 + BINS_S * 4 + 1024;
+constexpr int THREADS_TC = 288;                 // 8 row warps + the TMA / MMA warp
 constexpr float H_TOP = 16384.f;                // operands are scaled so that their largest magnitude sits just below 2^14 before the FP16 split
 
 // band counts the kernel is instantiated for (other tables use the SIMT kernel of sps_kernels.cu)
@@ -153,8 +155,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
                  const __grid_constant__ CUtensorMap m2h, const __grid_constant__ CUtensorMap m2l) {
   extern __shared__ unsigned char smem_dyn[];
   const int nb = T.n_z - 1, stride = nb + 2;
-  const int* row_start = G.bins + stride; const int* cta_start = G.bins + 2 * stride;
-  const int total = cta_start[nb];
+  const int* row_start_g = G.bins + stride; const int* cta_start_g = G.bins + 2 * stride;
+  const int total = cta_start_g[nb];
   const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
   const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
   const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
@@ -163,15 +165,23 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
   unsigned char* gbase = smem_dyn + (base - smem_u32(smem_dyn));
   const uint32_t bars = base + OFF_BAR;
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(gbase + OFF_BAR + 128);
-  float* cm_s = reinterpret_cast<float*>(gbase + OFF_BAR + 256);     // [128] Cm_i / 2^14 of the current tile's cell
+  float* cm_s = reinterpret_cast<float*>(gbase + OFF_EXTRA);         // [128] Cm_i / 2^14 of the current tile's cell
+  float* rs_s = cm_s + 128;                                          // [128] power-of-two scale of each tile row's a_i Cm_i
+  float* red_s = rs_s + 128;                                         // [6][128] band-loop partial sums of the h = 1 threads
+  float* mb_s = red_s + 6 * 128;                                     // [16][128] partial m_bar of the h = 1 threads
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #define BAR(i) (bars + 8u * (i))
+  // cell offsets of the call in shared memory when they fit (they are walked once per tile by every thread)
+  int* bins_s = reinterpret_cast<int*>(gbase + OFF_EXTRA + (2 + 6 + 16) * 128 * 4);
+  for (int i = threadIdx.x; i <= nb; i += blockDim.x) { bins_s[i] = row_start_g[i]; bins_s[nb + 1 + i] = cta_start_g[i]; }
+  const int* row_start = bins_s;
+  const int* cta_start = bins_s + nb + 1;
   if (threadIdx.x == 0) {
-    mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
-    mbar_init(BAR(BAR_V0), TM); mbar_init(BAR(BAR_M0), 1); mbar_init(BAR(BAR_V1), TM); mbar_init(BAR(BAR_M1), 1);
+    mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), 2 * TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
+    mbar_init(BAR(BAR_V0), 2 * TM); mbar_init(BAR(BAR_M0), 1); mbar_init(BAR(BAR_V1), 2 * TM); mbar_init(BAR(BAR_M1), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 4) {
+  if (warp == 8) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bars + 128u), "n"(512) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
@@ -183,7 +193,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
   while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (cta_start[mid] <= w_begin) lo = mid; else hi = mid; }
   int cell = lo;
 
-  if (warp == 4) {
+  if (warp == 8) {
     // ===== TMA loads + MMA issue =================================================================
     if (lane == 0) {
       // instruction descriptor: D = F32, A and B = F16 (format 0), both K-major
@@ -246,23 +256,43 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       }
     }
   } else {
-    // ===== row warps ==============================================================================
-    const int r = threadIdx.x;                              // tile row = TMEM lane
-    const uint32_t tlane = tmem_base + ((uint32_t)(warp * 32) << 16);
+    // ===== row warps: two threads per tile row.  Warps w and w + 4 share TMEM lane quarter w & 3; h = w >> 2 picks the
+    //       thread's share of every phase (P chunks, bands, V k-block, a_bar columns) ===================================
+    const int h = warp >> 2;
+    const int r = (warp & 3) * 32 + lane;                   // tile row = TMEM lane
+    const uint32_t tlane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
     uint32_t ph = 0;
+    // The row index and galaxy of a tile row are fetched one tile ahead (dependent loads order -> gal_of_row off the critical path).
+    int rw_next, gal_next = 0;
+    {
+      while (cta_start[cell + 1] <= w_begin) ++cell;
+      const int rb = row_start[cell] + (w_begin - cta_start[cell]) * TM;
+      rw_next = (rb + r < min(row_start[cell + 1], rb + TM)) ? __ldg(G.order + rb + r) : -1;
+      if (rw_next >= 0 && !G.flux_bar) gal_next = G.gal_of_row ? __ldg(G.gal_of_row + rw_next) : rw_next;
+    }
     for (int w = w_begin; w < w_end; ++w, ph ^= 1u) {
       while (cta_start[cell + 1] <= w) ++cell;
       const int r_begin = row_start[cell] + (w - cta_start[cell]) * TM;
       const int r_end = min(row_start[cell + 1], r_begin + TM);
-      const int rw = (r_begin + r < r_end) ? __ldg(G.order + r_begin + r) : -1;
+      const int rw = rw_next;
+      const int64_t gal = gal_next;
       const int n_rows = r_end - r_begin;
 #ifdef SPS_ATC_TIMING
       long long t_prev = clock64();
 #endif
-      const int next_row = (w + 1 < w_end && r_end + r < G.n) ? __ldg(G.order + r_end + r) : -1;
-      // ---- the row's scalars, metallicity weights and observations (requested first: in flight while a is staged) ----
+      // the next tile's rows follow this tile's in `order`
+      int r_end_next = r_end;
+      if (w + 1 < w_end) {
+        int cn = cell;
+        while (cta_start[cn + 1] <= w + 1) ++cn;
+        r_end_next = min(row_start[cn + 1], r_end + TM);
+      }
+      rw_next = (r_end + r < r_end_next) ? __ldg(G.order + r_end + r) : -1;
+      gal_next = 0;
+      // ---- the row's scalars, metallicity weights and this thread's bands of the observations (requested first: in
+      //      flight while a is staged) ----
       RowScalars sc;
-      float m[16], ob0[NB], ob1[NB];
+      float m[16], ob0[(NB + 1) / 2], ob1[(NB + 1) / 2];
       {
         float4* scq = reinterpret_cast<float4*>(&sc);
         float4* mq = reinterpret_cast<float4*>(m);
@@ -273,68 +303,71 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         }
 #pragma unroll
         for (int j = 0; j < 16; ++j) if (j >= T.n_Z) m[j] = 0.f;
-        const int64_t gal = (rw >= 0 && !G.flux_bar) ? (G.gal_of_row ? __ldg(G.gal_of_row + rw) : rw) : 0;
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-          ob0[b] = 0.f; ob1[b] = 1.f;
+        for (int k = 0; k < (NB + 1) / 2; ++k) {
+          const int b = min(h + 2 * k, NB - 1);
+          ob0[k] = 0.f; ob1[k] = 1.f;
           if (rw >= 0) {
-            if (G.flux_bar) ob0[b] = __ldg(G.flux_bar + (int64_t)rw * NB + b);
-            else { ob0[b] = __ldg(G.obs_flux + gal * NB + b); ob1[b] = __ldg(G.obs_sigma + gal * NB + b); }
+            if (G.flux_bar) ob0[k] = __ldg(G.flux_bar + (int64_t)rw * NB + b);
+            else { ob0[k] = __ldg(G.obs_flux + gal * NB + b); ob1[k] = __ldg(G.obs_sigma + gal * NB + b); }
           }
         }
       }
-      // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row ----
-      float a_rs = 1.f;                                     // this thread's row: power-of-two scale of its a_i Cm_i
+      // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row; warp (q, h) stages rows
+      //      32 q + 16 h .. + 15 ----
       {
         const int kb = lane >> 4, c = (lane & 15) >> 1, half = lane & 1;
         const float4 cm4 = __ldg(reinterpret_cast<const float4*>(G.Cm + (int64_t)cell * NA) + lane);
-        asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");            // every row thread is done with the previous tile's cm_s
-        cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
-#pragma unroll 1
-        for (int t0 = 0; t0 < 32; t0 += 16) {
-          float4 av[16];
+        TSTAMP(12);
+        asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");        // every row thread is done with the previous tile's shared arrays
+        TSTAMP(13);
+        if (h == 0) cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
+        float4 av[16];
 #pragma unroll
-          for (int u = 0; u < 16; ++u) {
-            const int row_u = __shfl_sync(FULL_MASK, rw, t0 + u);                // rows past the tile's end: any valid row, zeroed below
-            av[u] = __ldg(reinterpret_cast<const float4*>(B.a + (int64_t)max(row_u, 0) * ROW_A_STRIDE) + lane);
+        for (int u = 0; u < 16; ++u) {
+          const int row_u = __shfl_sync(FULL_MASK, rw, 16 * h + u);                // rows past the tile's end: any valid row, zeroed below
+          av[u] = __ldg(reinterpret_cast<const float4*>(B.a + (int64_t)max(row_u, 0) * ROW_A_STRIDE) + lane);
+        }
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+          const int tr = (warp & 3) * 32 + 16 * h + u;       // tile row being staged
+          float v[4] = {av[u].x * cm4.x, av[u].y * cm4.y, av[u].z * cm4.z, av[u].w * cm4.w};
+          float mx = 0.f;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) { if (4 * lane + k >= T.n_age || tr >= n_rows) v[k] = 0.f; mx = fmaxf(mx, fabsf(v[k])); }
+          mx = __uint_as_float(__reduce_max_sync(FULL_MASK, __float_as_uint(mx)));
+          float rs = 1.f;                                   // rs mx in [2^13, 2^14)
+          if (mx > 1.0e-30f && mx < 1.0e30f) rs = __uint_as_float((uint32_t)(127 + 13 + 127 - (int)((__float_as_uint(mx) >> 23) & 0xffu)) << 23);
+          if (lane == u) rs_s[tr] = rs;
+          __half hh[4], ll[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            v[k] *= rs;
+            hh[k] = __float2half_rn(v[k]); ll[k] = __float2half_rn(v[k] - __half2float(hh[k]));
           }
-#pragma unroll
-          for (int u = 0; u < 16; ++u) {
-            float v[4] = {av[u].x * cm4.x, av[u].y * cm4.y, av[u].z * cm4.z, av[u].w * cm4.w};
-            float mx = 0.f;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) { if (4 * lane + k >= T.n_age || t0 + u >= n_rows - warp * 32) v[k] = 0.f; mx = fmaxf(mx, fabsf(v[k])); }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL_MASK, mx, o));
-            float rs = 1.f;                                   // rs mx in [2^13, 2^14)
-            if (mx > 1.0e-30f && mx < 1.0e30f) rs = __uint_as_float((uint32_t)(127 + 13 + 127 - (int)((__float_as_uint(mx) >> 23) & 0xffu)) << 23);
-            if (lane == t0 + u) a_rs = rs;
-            __half h[4], l[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              v[k] *= rs;
-              h[k] = __float2half_rn(v[k]); l[k] = __float2half_rn(v[k] - __half2float(h[k]));
-            }
-            const uint32_t off = kb * TILE_A + sw128_off(warp * 32 + t0 + u, c) + half * 8;
-            *reinterpret_cast<uint2*>(gbase + off) = *reinterpret_cast<const uint2*>(h);
-            *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(l);
-          }
+          const uint32_t off = kb * TILE_A + sw128_off(tr, c) + half * 8;
+          *reinterpret_cast<uint2*>(gbase + off) = *reinterpret_cast<const uint2*>(hh);
+          *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(ll);
         }
       }
-      if (next_row >= 0) {                                  // the next tile's weights start their way into L2 (its rows follow in `order`)
-        const char* np_ = reinterpret_cast<const char*>(B.a + (int64_t)next_row * ROW_A_STRIDE);
+      TSTAMP(14);
+      if (rw_next >= 0) {                                   // the next tile's weights start their way into L2
+        if (h == 0) {
+          const char* np_ = reinterpret_cast<const char*>(B.a + (int64_t)rw_next * ROW_A_STRIDE);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(np_ + 128 * q));
+          for (int q = 0; q < 4; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(np_ + 128 * q));
+        }
+        if (!G.flux_bar) gal_next = G.gal_of_row ? __ldg(G.gal_of_row + rw_next) : rw_next;
       }
       tc_fence_before();                                    // the previous tile's TMEM reads are complete
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_arrive(BAR(BAR_A));
       TSTAMP(0);
-      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // cm_s of this tile is complete
-      const float u0 = 1.f / (H_TOP * a_rs), u1 = u0 * G.inv_sD;          // P^(s) back to table units
+      asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");            // cm_s and rs_s of this tile are complete
+      const float u0 = 1.f / (H_TOP * rs_s[r]), u1 = u0 * G.inv_sD;       // P^(s) back to table units
       const float f = sc.zfrac, Mn = sc.Mn, zp = 1.f + sc.z;
       const int E = T.n_Z * NB;
-      // ---- sweep 1 over P: S^(s)_b = sum_j m_j P^(s)[j NB + b] ----
+      // ---- sweep 1 over P (this thread's chunks): S^(s)_b = sum_j m_j P^(s)[j NB + b] ----
       float S0[NB], S1[NB];
 #pragma unroll
       for (int b = 0; b < NB; ++b) S0[b] = S1[b] = 0.f;
@@ -344,7 +377,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       TSTAMP(2);
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
-        if (16 * c < E) {
+        if ((c & 1) == h && 16 * c < E) {
           uint32_t v0[16], v1[16], x0[16], x1[16];
           TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
           TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
@@ -359,28 +392,34 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           }
         }
       }
-      // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood).  A rolled loop over the
-      //      bands keeps the kernel inside the instruction cache; its per-band inputs and sbar_b sit in a per-thread scratch
-      //      column of the A / V region (pass 1 has retired, V is written later) ----
       TSTAMP(3);
-      float* scr = reinterpret_cast<float*>(gbase) + r;     // scr[slot * TM]: slots 0-15 S^(0), 16-31 S^(1), 32-47 / 48-63 observations, 64-79 sbar
+      // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood).  A rolled loop over this
+      //      thread's bands keeps the kernel inside the instruction cache; per-band inputs and sbar_b sit in a scratch column
+      //      of the A / V region (pass 1 has retired, V is written later).
+      //      scr[slot * TM]: slots 0-15 / 16-31 partial S^(0) of h = 0 / 1, 32-47 / 48-63 partial S^(1), 64-79 / 80-95
+      //      observations, 96-111 sbar ----
+      float* scr = reinterpret_cast<float*>(gbase) + r;
 #pragma unroll
-      for (int b = 0; b < NB; ++b) { scr[b * TM] = S0[b] * u0; scr[(16 + b) * TM] = S1[b] * u1; scr[(32 + b) * TM] = ob0[b]; scr[(48 + b) * TM] = ob1[b]; }
+      for (int b = 0; b < NB; ++b) { scr[(16 * h + b) * TM] = S0[b] * u0; scr[(32 + 16 * h + b) * TM] = S1[b] * u1; }
+#pragma unroll
+      for (int k = 0; k < (NB + 1) / 2; ++k)
+        if (h + 2 * k < NB) { scr[(64 + h + 2 * k) * TM] = ob0[k]; scr[(80 + h + 2 * k) * TM] = ob1[k]; }
+      asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");
       float chi2 = 0.f, v_mn = 0.f, v_z = 0.f, v_av = 0.f, v_de = 0.f, v_fl = 0.f;
       const float izp = __fdividef(1.f, zp);
       float* fo = B.flux + (int64_t)max(rw, 0) * SPS_MAX_BAND;
-#pragma unroll 2
-      for (int b = 0; b < NB; ++b) {
+#pragma unroll 1
+      for (int b = h; b < NB; b += 2) {
         float F, F_av, F_del, F_fl, F_lam;
         const float lam_r = T.lam_eff[b] * izp;
         dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
-        const float s1 = scr[(16 + b) * TM];
-        const float Sint = scr[b * TM] + f * s1;
+        const float s1 = scr[(32 + b) * TM] + scr[(48 + b) * TM];
+        const float Sint = (scr[b * TM] + scr[(16 + b) * TM]) + f * s1;
         const float flux = F * Mn * Sint;
         if (rw >= 0) fo[b] = flux;
-        float g = scr[(32 + b) * TM];
+        float g = scr[(64 + b) * TM];
         if (!G.flux_bar) {
-          const float isg = __fdividef(1.f, scr[(48 + b) * TM]);
+          const float isg = __fdividef(1.f, scr[(80 + b) * TM]);
           const float rr = (flux - g) * isg;
           chi2 = fmaf(rr, rr, chi2);
           g = -rr * isg;
@@ -388,27 +427,32 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         v_mn += g * F * Sint;
         v_z += g * (F * Mn * s1 * T.inv_dz + Mn * Sint * F_lam * (-lam_r * izp));
         v_av += g * Mn * Sint * F_av; v_de += g * Mn * Sint * F_del; v_fl += g * Mn * Sint * F_fl;
-        scr[(64 + b) * TM] = g * F * Mn;
+        scr[(96 + b) * TM] = g * F * Mn;
       }
-      if (rw >= 0) {
+      if (h == 1) { red_s[r] = chi2; red_s[TM + r] = v_mn; red_s[2 * TM + r] = v_z; red_s[3 * TM + r] = v_av; red_s[4 * TM + r] = v_de; red_s[5 * TM + r] = v_fl; }
+      asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");
+      if (h == 0 && rw >= 0) {
         RowScalars* out = B.sc + rw;
-        out->logp_like = -0.5f * chi2;
-        if (G.want_grad) { out->Mn_bar = v_mn; out->z_bar = v_z; out->AV_bar = v_av; out->delta_bar = v_de; out->Ffloor_bar = v_fl; }
+        out->logp_like = -0.5f * (chi2 + red_s[r]);
+        if (G.want_grad) {
+          out->Mn_bar = v_mn + red_s[TM + r]; out->z_bar = v_z + red_s[2 * TM + r]; out->AV_bar = v_av + red_s[3 * TM + r];
+          out->delta_bar = v_de + red_s[4 * TM + r]; out->Ffloor_bar = v_fl + red_s[5 * TM + r];
+        }
       }
       TSTAMP(4);
       if (!G.want_grad) continue;
-      // ---- sweep 2 over P: m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
+      // ---- sweep 2 over P (this thread's chunks): m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
       float sbar[NB];
 #pragma unroll
-      for (int b = 0; b < NB; ++b) sbar[b] = scr[(64 + b) * TM];
+      for (int b = 0; b < NB; ++b) sbar[b] = scr[(96 + b) * TM];
+      float mb[16];
       {
-        float mb[16];
         const float fu1 = f * u1;
 #pragma unroll
         for (int j = 0; j < 16; ++j) mb[j] = 0.f;
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
-          if (16 * c < E) {
+          if ((c & 1) == h && 16 * c < E) {
             uint32_t v0[16], v1[16], x0[16], x1[16];
             TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
             TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
@@ -420,16 +464,22 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
             }
           }
         }
-        if (rw >= 0) {
-          float4* mo = reinterpret_cast<float4*>(B.m_bar + (int64_t)rw * ROW_M_STRIDE);
+        if (h == 1) {
 #pragma unroll
-          for (int q = 0; q < 4; ++q) mo[q] = make_float4(mb[4 * q], mb[4 * q + 1], mb[4 * q + 2], mb[4 * q + 3]);
+          for (int j = 0; j < 16; ++j) mb_s[j * TM + r] = mb[j];
         }
       }
       TSTAMP(5);
       tc_fence_before();
-      // ---- V^(s)[e] = sbar_b m_j {1, f}: the A operand of pass 2, one phase per table array; the row is scaled by a
-      //      power of two sv that puts its largest entry near 2^14 (FP16 split: 22 significant bits below the row maximum) ----
+      asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");            // partial m_bar parked; every thread has read its scratch: V may overwrite it
+      if (h == 0 && rw >= 0) {
+        float4* mo = reinterpret_cast<float4*>(B.m_bar + (int64_t)rw * ROW_M_STRIDE);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          mo[q] = make_float4(mb[4 * q] + mb_s[(4 * q) * TM + r], mb[4 * q + 1] + mb_s[(4 * q + 1) * TM + r], mb[4 * q + 2] + mb_s[(4 * q + 2) * TM + r], mb[4 * q + 3] + mb_s[(4 * q + 3) * TM + r]);
+      }
+      // ---- V^(s)[e] = sbar_b m_j {1, f}: the A operand of pass 2, one phase per table array, this thread's k block (64
+      //      entries); the row is scaled by a power of two sv that puts its largest entry near 2^14 ----
       float sv = 1.f;
       {
         float smax = 0.f, mmax = 0.f;
@@ -443,41 +493,55 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           sv = __uint_as_float((uint32_t)(127 + 13 - ex) << 23);                 // sv vmax in [2^13, 2^14)
         }
       }
-      asm volatile("bar.sync 1, %0;" ::"n"(TM) : "memory");                // every thread has read its scratch column: V may overwrite it
 #pragma unroll 1
       for (int s = 0; s < 2; ++s) {
-        if (s == 1) { TSTAMP(7); mbar_wait(BAR(BAR_M0), ph); TSTAMP(8); }             // phase-0 MMAs have read V^(0)
+        if (s == 1) { TSTAMP(7); mbar_wait(BAR(BAR_M0), ph); TSTAMP(8); }   // phase-0 MMAs have read V^(0)
         const float scale = (rw >= 0) ? (s ? sv * f * G.inv_sD : sv) : 0.f;
-#pragma unroll
-        for (int kb = 0; kb < 2; ++kb)
+        if (h == 0) {
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
             float v[8];
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-              const int e = 64 * kb + 8 * c + k, j = e / NB, b = e % NB;
+              const int e = 8 * c + k, j = e / NB, b = e % NB;
               v[k] = (j < 16) ? scale * sbar[b] * m[j] : 0.f;
             }
             uint4 vh, vl;
             split8(v, vh, vl);
-            const uint32_t off = kb * TILE_A + sw128_off(r, c);
+            const uint32_t off = sw128_off(r, c);
             *reinterpret_cast<uint4*>(gbase + off) = vh;
             *reinterpret_cast<uint4*>(gbase + 2 * TILE_A + off) = vl;
           }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            float v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const int e = 64 + 8 * c + k, j = e / NB, b = e % NB;
+              v[k] = (j < 16) ? scale * sbar[b] * m[j] : 0.f;
+            }
+            uint4 vh, vl;
+            split8(v, vh, vl);
+            const uint32_t off = TILE_A + sw128_off(r, c);
+            *reinterpret_cast<uint4*>(gbase + off) = vh;
+            *reinterpret_cast<uint4*>(gbase + 2 * TILE_A + off) = vl;
+          }
+        }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         mbar_arrive(BAR(s ? BAR_V1 : BAR_V0));
       }
       TSTAMP(9);
-      // ---- a_bar from TMEM ----
+      // ---- a_bar from TMEM (main + cross-term accumulators), this thread's 64 columns ----
       mbar_wait(BAR(BAR_M1), ph);
       tc_fence_after();
       TSTAMP(10);
-      // thread = row reads its TMEM lane and parks the scaled values in the (free) A / V region, 16-byte chunks XOR-swizzled
-      // by the row; then each warp writes its 32 rows to global memory 512 contiguous bytes at a time
+      // thread = (row, half of the ages) reads its TMEM lane and parks the scaled values in the (free) A / V region, 16-byte
+      // chunks XOR-swizzled by the row; then each warp writes 16 rows to global memory 512 contiguous bytes at a time
       const float ua = 1.f / sv;
       float4* stage = reinterpret_cast<float4*>(gbase);                   // [TM][32] float4
 #pragma unroll 1
-      for (int c = 0; c < 8; ++c) {
+      for (int c = 4 * h; c < 4 * h + 4; ++c) {
         uint32_t v[16], x[16];
         TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x);
         tld_wait();
@@ -491,11 +555,12 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           stage[r * 32 + ((4 * c + q) ^ (r & 7))] = o;
         }
       }
-      __syncwarp();                                                       // a warp stores the rows its own threads parked
+      tc_fence_before();
+      asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");
 #pragma unroll 4
-      for (int t = 0; t < 32; ++t) {
-        const int row_t = __shfl_sync(FULL_MASK, rw, t);
-        const int rr = warp * 32 + t;
+      for (int t = 0; t < 16; ++t) {
+        const int row_t = __shfl_sync(FULL_MASK, rw, 16 * h + t);
+        const int rr = (warp & 3) * 32 + 16 * h + t;
         if (row_t >= 0) reinterpret_cast<float4*>(B.a_bar + (int64_t)row_t * ROW_A_STRIDE)[lane] = stage[rr * 32 + (lane ^ (rr & 7))];
       }
       TSTAMP(11);
@@ -503,7 +568,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 4) {
+  if (warp == 8) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512) : "memory");
   }
@@ -564,7 +629,7 @@ sps_status sps_approx_tc_setup(sps_table* t) {
 #define CASE(NB) band_ok = band_ok || T.n_band == NB;
   SPS_APPROX_TC_BANDS(CASE)
 #undef CASE
-  if (!band_ok || T.n_Z * T.n_band > 128 || T.n_age > NA || T.n_Z > 16) return SPS_OK;
+  if (!band_ok || T.n_Z * T.n_band > 128 || T.n_age > NA || T.n_Z > 16 || 2 * T.n_z > BINS_S) return SPS_OK;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qr;
   if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
