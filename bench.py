@@ -25,7 +25,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 from paper_2506_19919_b200.sharding import aggregate_throughput, max_over_ranks, rank_seed  # noqa: E402
 
-SM_COUNT, FMA_PER_SM_CLK = 148, 128
 
 
 def _peaks():
@@ -215,17 +214,17 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
 # captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("approx_contract", 40000): 49.0e6,   # profiles/r01_hmc_kernels_full.md: 47.69 MB read + 1.35 MB written (40,000 rows per launch)
+    ("approx_contract", 40000): 87.3e6,   # profiles/r01_hmc_kernels_full.md: 80.41 MB read + 6.94 MB written (40,000 rows per launch)
     ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
 }
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
     """Roofline of the dominant kernel.
-    approx_contract: FP32-FMA ("alu") bound: per row the forward + reverse pass over the two c_SSP arrays of its z cell
-    is 2 FMA per table word = 4 * n_age*n_Z*n_band flop per array pair; the table is L2/shared-memory resident, so there
-    is no HBM stream.  Peak = 148 SM x 128 FMA/clk x 2 flop x max SM clock (guide unit counts; clock from
-    MEASURED_PEAKS.json).
+    approx_contract: tensor bound (tcgen05 kernel, FP16 two-term split): per row the forward + reverse pass over the two
+    c_SSP arrays of its z cell is 2 MAC per table word = 4 * 2 n_age*n_Z*n_band flop, times the 3 split products, against the
+    measured bf16 burst peak (FP16 runs at the same rate); the table operands are L2 resident, so there is no HBM stream.
+    (The fp32 SIMT kernel that serves other table shapes is FMA-pipe bound: DESIGN.md 5.2.)
     exact_fwd: tensor bound: 3 split products x 2 x n_age*n_Z flop per (row, wavelength) pair under some filter's support
     (sps_exact_last_work: skipped and padded columns never count), against the measured bf16 burst peak (BF16X3)."""
     ms, timed, allc = prof[kernel]
@@ -234,9 +233,10 @@ def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
     avg_s = ms / timed / 1e3
     if kernel == "approx_contract":
         words = 2 * grid.n_age * grid.n_Z * grid.n_band
-        flop = 2.0 * 2.0 * words * rows_per_launch
-        peak = SM_COUNT * FMA_PER_SM_CLK * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
-        bound, note = "alu", f"fp32 FMA peak at {peaks.get('sm_max_mhz', 1965.0):.0f} MHz ({peaks_src})"
+        flop = 3.0 * 2.0 * 2.0 * words * rows_per_launch
+        peak = float(peaks["bf16_tflops"])
+        bound, note = "tensor", (f"bf16 burst peak ({peaks_src}; FP16 operands, same rate); achieved = 3 FP16 split products x 2 passes x 2 x "
+                                 f"{words} table words per row; the kernel is bound by its per-row staging / band step, not by the tensor pipe (DESIGN.md 5.2)")
     else:
         K = grid.n_age * grid.n_Z
         flop = 3.0 * 2.0 * K * float(pairs)
