@@ -4,6 +4,12 @@
 #include "sps_rows.cuh"
 
 #define WARPS_PER_BLOCK 8
+#ifndef PRO_MIN_BLOCKS
+#define PRO_MIN_BLOCKS 4                        // resident blocks per SM the prologue / epilogue are compiled for
+#endif
+#ifndef EPI_MIN_BLOCKS
+#define EPI_MIN_BLOCKS 3
+#endif
 
 // ---------------------------------------------------------------------------------------------
 // Forward model of one row (one warp per parameter row): everything a0-a5 needs, held per lane.
@@ -35,7 +41,7 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorDev& P
 // a0-a5.  With WANT_GRAD the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
 // kept in B.part for the epilogue, which then has no quadrature to redo.
 template <bool WANT_GRAD>
-__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
+__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, PRO_MIN_BLOCKS)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
@@ -407,7 +413,7 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
 // with a_bar, m_bar, Mn_bar and the direct bars.  Only the cheap closed forms (C1, dt/dz, burst polynomial, MDF) are
 // re-evaluated; no quadrature is redone.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK)
+__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, EPI_MIN_BLOCKS)
 epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbounded, bool with_prior,
                 const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad, LeapfrogFuse lf) {
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
