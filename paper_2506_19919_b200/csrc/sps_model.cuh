@@ -252,20 +252,21 @@ __device__ __forceinline__ void burst_bins(const TableDev& T, float ltp, float l
 // ---- a4: lognormal MDF PAPER.md:378 (R9).  Lane j < n_Z owns metallicity bin j. -------------------
 __device__ __forceinline__ void met_bin(const TableDev& T, float lz, float s, float& m, float& d_lz, float& d_s) {
   const int j = lane_id();
+  const float inv_s = 1.f / s;
+  const bool has_lo = j > 0 && j < T.n_Z, has_hi = j < T.n_Z - 1;
+  // lane k < n_Z - 1 evaluates bin edge k once (erfc of |u| and the normal density); bin j takes its lower edge from lane j - 1
+  const float ub = has_hi ? (T.g_mid[j] - lz) * inv_s : 1e30f;
+  const float r2 = 0.7071067811865476f, c = 0.3989422804014327f;
+  const float eb = has_hi ? erfcf(fabsf(ub) * r2) : 0.f;
+  const float pb = has_hi ? c * expf(-0.5f * ub * ub) : 0.f;
+  float ua = __shfl_up_sync(FULL_MASK, ub, 1), ea = __shfl_up_sync(FULL_MASK, eb, 1), pa = __shfl_up_sync(FULL_MASK, pb, 1);
+  if (!has_lo) { ua = -1e30f; ea = 0.f; pa = 0.f; }
   m = d_lz = d_s = 0.f;
   if (j < T.n_Z) {
-    const float inv_s = 1.f / s;
-    const bool has_lo = j > 0, has_hi = j < T.n_Z - 1;
-    float ua = has_lo ? (T.g_mid[j - 1] - lz) * inv_s : -1e30f;
-    float ub = has_hi ? (T.g_mid[j] - lz) * inv_s : 1e30f;
-    const float r2 = 0.7071067811865476f;
     // normal-CDF difference through the tail that keeps relative accuracy
-    if (ua > 0.f) m = 0.5f * (erfcf(ua * r2) - (has_hi ? erfcf(ub * r2) : 0.f));
-    else if (ub < 0.f) m = 0.5f * (erfcf(-ub * r2) - (has_lo ? erfcf(-ua * r2) : 0.f));
-    else m = 1.f - 0.5f * ((has_hi ? erfcf(ub * r2) : 0.f) + (has_lo ? erfcf(-ua * r2) : 0.f));
-    const float c = 0.3989422804014327f;
-    float pa = has_lo ? c * expf(-0.5f * ua * ua) : 0.f;
-    float pb = has_hi ? c * expf(-0.5f * ub * ub) : 0.f;
+    if (ua > 0.f) m = 0.5f * (ea - eb);
+    else if (ub < 0.f) m = 0.5f * (eb - ea);
+    else m = 1.f - 0.5f * (eb + ea);
     d_lz = -(pb - pa) * inv_s;
     d_s = -(pb * (has_hi ? ub : 0.f) - pa * (has_lo ? ua : 0.f)) * inv_s;
   }
