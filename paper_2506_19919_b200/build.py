@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsps_b200.so")
 SOURCES = ["sps_api.cu", "sps_table.cu", "sps_kernels.cu", "sps_approx_tc.cu", "sps_exact.cu", "sps_exact_tc.cu", "sps_sampler.cu", "sps_leapfrog.cu", "sps_nuts.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-              "--expt-relaxed-constexpr", "-Xptxas", "-v"]
+              "--expt-relaxed-constexpr", "-use_fast_math", "-Xptxas", "-v"]
 
 
 def _stale() -> bool:

@@ -429,6 +429,11 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
     return;
   }
   // all of the row's stored quantities are requested first: the kernel is a latency-bound stream over B.part
+  float lf_eps = 0.f, lf_p = 0.f, lf_im = 0.f, lf_th = 0.f;     // operands of the fused leapfrog update, in flight from the start
+  if (lf.p_w && l < SPS_NDIM) {
+    const int64_t o = row * SPS_NDIM + l;
+    lf_eps = lf.eps[row]; lf_p = lf.p_w[o]; lf_im = lf.inv_mass[o]; lf_th = lf.theta_w[o];
+  }
   const float* part = B.part + row * (ROW_PARTS * ROW_A_STRIDE);
   float abar[SPS_AGE_PER_LANE], pr[ROW_PARTS][SPS_AGE_PER_LANE];
 #pragma unroll
@@ -438,6 +443,9 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
     for (int k = 0; k < ROW_PARTS; ++k) pr[k][q] = part[k * ROW_A_STRIDE + l + 32 * q];
   }
   const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
+  // the prior term (a9) depends on the row's parameters only: evaluated while the loads above are in flight
+  float lp = 0.f, dlp = 0.f;
+  if (with_prior && l < SPS_NDIM) log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp);
   float th[SPS_NDIM], dth[SPS_NDIM];
   double zd_unused;
   load_params<false>(theta + row * SPS_NDIM, unbounded, P, th, dth, zd_unused);
@@ -485,23 +493,17 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
     case 12: g = sc.z_bar + s_t * dt_dz; break;
     default: break;
   }
-  float lp = 0.f;
   if (l < SPS_NDIM) {
     float d1 = 1.f;
 #pragma unroll
     for (int p = 0; p < SPS_NDIM; ++p) if (p == l) d1 = dth[p];
-    g *= d1;
-    if (with_prior) {
-      float dlp;
-      log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp);
-      g += dlp;
-    }
+    g = g * d1 + dlp;
     grad[row * SPS_NDIM + l] = g;
     if (lf.p_w) {                                            // fused leapfrog update (theta may alias lf.theta_w: read above, written here)
       const int64_t o = row * SPS_NDIM + l;
-      const float e = lf.eps[row], pn = lf.p_w[o] + e * g;
+      const float pn = lf_p + lf_eps * g;
       lf.p_w[o] = pn;
-      lf.theta_w[o] += e * lf.inv_mass[o] * pn;
+      lf.theta_w[o] = lf_th + lf_eps * lf_im * pn;
     }
   }
   lp = warp_sum(lp);

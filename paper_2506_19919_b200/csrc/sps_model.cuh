@@ -61,7 +61,7 @@ __device__ __forceinline__ void sfr_node(float lx2, float alpha, float beta, flo
 }
 __device__ __forceinline__ float sfr_value(float t, float tau, float alpha, float beta) {
   if (!(t > 0.f)) return 0.f;
-  float lx2 = log2f(t / tau);
+  float lx2 = __log2f(t / tau);
   return __fdividef(1.f, exp2f(fminf(alpha * lx2, 60.f)) + exp2f(fminf(-beta * lx2, 60.f)));
 }
 
@@ -88,7 +88,7 @@ __device__ __constant__ float GL8_W[8] = {0.1012285362903763f, 0.222381034453374
 template <bool WANT_GRAD>
 __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, float tau, float alpha, float beta, AgeQuad& Q) {
   const int l = lane_id();
-  const float l2tau = log2f(tau);
+  const float l2tau = __log2f(tau);
   const float ab = alpha + beta;
   unsigned problem_mask[SPS_AGE_PER_LANE];
   float t_lo_q[SPS_AGE_PER_LANE], t_hi_q[SPS_AGE_PER_LANE];
@@ -119,7 +119,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           float t = t_mid + half * GL2_X[k], f, qq, fa, fb;
-          sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
+          sfr_node(__log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
           s0 += f;
           if (WANT_GRAD) { s1 += qq; s2 += fa; s3 += fb; s4 -= __fdividef(qq, t); }
         }
@@ -127,7 +127,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
           float t = t_mid + half * GL4_X[k], f, qq, fa, fb, w = GL4_W[k];
-          sfr_node(log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
+          sfr_node(__log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
           s0 += w * f;
           if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; s4 -= w * __fdividef(qq, t); }
         }
@@ -149,7 +149,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       const int src = __ffs(mz) - 1;
       m &= ~mz;
       const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], src);
-      const float v_hi = logf(t_hi);
+      const float v_hi = __logf(t_hi);
       const float dv = 16.f / (beta + 1.f);
       const float v_lo = v_hi - dv;
       const int n_pan = max(1, (int)ceilf(dv / w_target));
@@ -158,7 +158,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       for (int n = l; n < n_pan * 8; n += 32) {
         const int pan = n >> 3, k = n & 7;
         const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
-        const float w = 0.5f * wp * GL8_W[k] * expf(v);        // dt = t dv
+        const float w = 0.5f * wp * GL8_W[k] * __expf(v);        // dt = t dv
         float f, qq, fa, fb;
         sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
         s0 += w * f;
@@ -180,8 +180,8 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       const bool have = my_src >= 0;
       const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], have ? my_src : 0);
       const float t_lo = __shfl_sync(FULL_MASK, t_lo_q[q], have ? my_src : 0);
-      const float v_hi = logf(t_hi);
-      const float v_lo = fmaxf(v_hi - 16.f / (beta + 1.f), logf(t_lo));
+      const float v_hi = __logf(t_hi);
+      const float v_lo = fmaxf(v_hi - 16.f / (beta + 1.f), __logf(t_lo));
       const float dv = v_hi - v_lo;
       int n_pan = have ? max(1, (int)ceilf(dv / w_target)) : 0;
       const float wp = dv / (float)max(n_pan, 1);
@@ -191,7 +191,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       for (int pan = 0; pan < n_max; ++pan) {
         if (pan < n_pan) {
           const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
-          const float w = 0.5f * wp * GL8_W[k] * expf(v);
+          const float w = 0.5f * wp * GL8_W[k] * __expf(v);
           float f, qq, fa, fb;
           sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
           s0 += w * f;
