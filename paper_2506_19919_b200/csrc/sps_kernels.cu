@@ -128,6 +128,59 @@ __global__ void approx_scatter_kernel(int64_t n, const int* __restrict__ rows, R
   if (cell >= 0) order[base + __popc(peers & ((1u << lane) - 1u))] = row;
 }
 
+// The same with the cell offsets computed in place (n_z - 1 <= 1024): every block scans the histogram itself (4 cells per
+// thread), block 0 publishes the row / item offsets for the contraction kernel, and the scatter cursors start at zero
+// (cleared together with the histogram before the prologue).  One launch instead of two.
+__global__ void __launch_bounds__(256) approx_scan_scatter_kernel(int64_t n, const int* __restrict__ rows, RowBuffers B, int nb,
+                                                                  int rows_per_item, int* __restrict__ bins, int* __restrict__ order) {
+  __shared__ int s_row[1024];
+  __shared__ int s_wr[8], s_wc[8];
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5, stride = nb + 2;
+  int hq[4], cq[4], sum_r = 0, sum_c = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int b = 4 * t + k;
+    hq[k] = b < nb ? bins[b] : 0;
+    cq[k] = (hq[k] + rows_per_item - 1) / rows_per_item;
+    sum_r += hq[k]; sum_c += cq[k];
+  }
+  int inc_r = sum_r, inc_c = sum_c;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int a = __shfl_up_sync(FULL_MASK, inc_r, o), c = __shfl_up_sync(FULL_MASK, inc_c, o);
+    if (lane >= o) { inc_r += a; inc_c += c; }
+  }
+  if (lane == 31) { s_wr[wid] = inc_r; s_wc[wid] = inc_c; }
+  __syncthreads();
+  int base_r = inc_r - sum_r, base_c = inc_c - sum_c, tot_r = 0, tot_c = 0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    if (w < wid) { base_r += s_wr[w]; base_c += s_wc[w]; }
+    tot_r += s_wr[w]; tot_c += s_wc[w];
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int b = 4 * t + k;
+    if (b < nb) {
+      s_row[b] = base_r;
+      if (blockIdx.x == 0) { bins[stride + b] = base_r; bins[2 * stride + b] = base_c; }
+    }
+    base_r += hq[k]; base_c += cq[k];
+  }
+  if (blockIdx.x == 0 && t == 0) { bins[stride + nb] = tot_r; bins[2 * stride + nb] = tot_c; }
+  __syncthreads();
+  int* cursor = bins + 3 * stride;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int row = -1, cell = -1 - lane;                            // idle lanes get distinct dummy keys
+  if (i < n) { row = rows ? rows[i] : (int)i; cell = B.sc[row].zbin; }
+  const unsigned peers = __match_any_sync(FULL_MASK, cell);
+  const int leader = __ffs(peers) - 1;
+  int base = 0;
+  if (lane == leader && cell >= 0) base = s_row[cell] + atomicAdd(&cursor[cell], __popc(peers));
+  base = __shfl_sync(FULL_MASK, base, leader);
+  if (cell >= 0) order[base + __popc(peers & ((1u << lane) - 1u))] = row;
+}
+
 // ---------------------------------------------------------------------------------------------
 // a7 + a9 + a10: approximate photometry (Eq. 6) fused with the Gaussian likelihood and the reverse
 // pass over the c_SSP table.  One CTA per (z cell, chunk of 64 rows): the cell's two arrays c_t and D_t = c_{t+1} - c_t
@@ -531,7 +584,7 @@ void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, i
                      const int* rows, RowBuffers B, bool with_hist, cudaStream_t s) {
   if (n <= 0) return;
   int* hist = nullptr;
-  if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, (T.n_z + 1) * sizeof(int), s); }
+  if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
   sps_prof_begin(SPS_K_PROLOGUE, s);
   if (want_grad) prologue_kernel<true><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
   else prologue_kernel<false><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
@@ -559,6 +612,11 @@ sps_status approx_contract_setup(const TableDev& T) {
 void approx_group_rows(const TableDev& T, int64_t n, const int* rows, RowBuffers B, int rows_per_item, cudaStream_t s) {
   const int nb = T.n_z - 1, stride = nb + 2;
   const unsigned eb = (unsigned)((n + 255) / 256);
+  if (nb <= 1024) {
+    approx_scan_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, nb, rows_per_item, B.bins, B.order);
+    sps_count_launch();
+    return;
+  }
   approx_plan_kernel<<<1, 1024, 0, s>>>(nb, rows_per_item, B.bins);
   approx_scatter_kernel<<<eb, 256, 0, s>>>(n, rows, B, B.bins + 3 * stride, B.order);
   sps_count_launch(2);
