@@ -130,7 +130,7 @@ __global__ void build_c_operands_kernel(TableDev T, const float* __restrict__ Cm
 
 // shared memory: [0, 64 KB) A / V operand tiles, [64 KB, 192 KB) table operand tiles, then the barriers
 constexpr uint32_t OFF_B = REG_AV, OFF_BAR = REG_AV + REG_B;
-enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M0, BAR_V1, BAR_M1, N_BARS };
+enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M1, N_BARS };
 
 #ifdef SPS_ATC_TIMING
 __device__ long long g_atc_t[16];
@@ -178,7 +178,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
   const int* cta_start = bins_s + nb + 1;
   if (threadIdx.x == 0) {
     mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), 2 * TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
-    mbar_init(BAR(BAR_V0), 2 * TM); mbar_init(BAR(BAR_M0), 1); mbar_init(BAR(BAR_V1), 2 * TM); mbar_init(BAR(BAR_M1), 1);
+    mbar_init(BAR(BAR_V0), 2 * TM); mbar_init(BAR(BAR_M1), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 8) {
@@ -234,10 +234,13 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           tma_load_2d(base + OFF_B + 65536u + eb * 16384u, &m2l, BAR(BAR_B2), eb * KB, cell * NA);
         }
         mbar_wait(BAR(BAR_B2), ph);
+        mbar_wait(BAR(BAR_V0), ph);
+        tc_fence_after();
+        // Both table arrays are contracted with the same operand V (the row's factor f on the D_t part is applied when the
+        // accumulators are read): acc^(s) = sum_e V[e] C^(s)[i][e].  The accumulators reuse the columns of P (dead once V is
+        // being written): s = 0 main / cross terms at columns 0 / NA, s = 1 at 2 NA / 3 NA.
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-          mbar_wait(BAR(s ? BAR_V1 : BAR_V0), ph);
-          tc_fence_after();
+        for (int s = 0; s < 2; ++s)
 #pragma unroll
           for (int kb = 0; kb < 2; ++kb)
 #pragma unroll
@@ -245,13 +248,11 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
               const int eb = 2 * s + kb;
               const uint64_t a_hi = desc_sw128(base + kb * TILE_A + kk * 32), a_lo = desc_sw128(base + (2 + kb) * TILE_A + kk * 32);
               const uint64_t b_hi = desc_sw128(base + OFF_B + eb * 16384u + kk * 32), b_lo = desc_sw128(base + OFF_B + 65536u + eb * 16384u + kk * 32);
-              // a_bar reuses the columns of P (dead once V is being written): main terms at 0, cross terms at NA
-              tc_mma_f16(tmem_base + NA, a_lo, b_hi, idesc2, (s | kb | kk) ? 1u : 0u);
-              tc_mma_f16(tmem_base + NA, a_hi, b_lo, idesc2, 1u);
-              tc_mma_f16(tmem_base, a_hi, b_hi, idesc2, (s | kb | kk) ? 1u : 0u);
+              tc_mma_f16(tmem_base + (2 * s + 1) * NA, a_lo, b_hi, idesc2, (kb | kk) ? 1u : 0u);
+              tc_mma_f16(tmem_base + (2 * s + 1) * NA, a_hi, b_lo, idesc2, 1u);
+              tc_mma_f16(tmem_base + 2 * s * NA, a_hi, b_hi, idesc2, (kb | kk) ? 1u : 0u);
             }
-          tc_commit(BAR(s ? BAR_M1 : BAR_M0));
-        }
+        tc_commit(BAR(BAR_M1));
         mbar_wait(BAR(BAR_M1), ph);                         // pass 2 retired: both regions are free for the next tile
       }
     }
@@ -478,8 +479,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         for (int q = 0; q < 4; ++q)
           mo[q] = make_float4(mb[4 * q] + mb_s[(4 * q) * TM + r], mb[4 * q + 1] + mb_s[(4 * q + 1) * TM + r], mb[4 * q + 2] + mb_s[(4 * q + 2) * TM + r], mb[4 * q + 3] + mb_s[(4 * q + 3) * TM + r]);
       }
-      // ---- V^(s)[e] = sbar_b m_j {1, f}: the A operand of pass 2, one phase per table array, this thread's k block (64
-      //      entries); the row is scaled by a power of two sv that puts its largest entry near 2^14 ----
+      // ---- V[e] = sbar_b m_j: the A operand of pass 2 (both table arrays), this thread's k block (64 entries); the row is
+      //      scaled by a power of two sv that puts its largest entry near 2^14 ----
       float sv = 1.f;
       {
         float smax = 0.f, mmax = 0.f;
@@ -487,16 +488,14 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         for (int b = 0; b < NB; ++b) smax = fmaxf(smax, fabsf(sbar[b]));
 #pragma unroll
         for (int j = 0; j < 16; ++j) mmax = fmaxf(mmax, fabsf(m[j]));
-        const float vmax = smax * mmax * fmaxf(1.f, f * G.inv_sD);
+        const float vmax = smax * mmax;
         if (vmax > 1.0e-30f && vmax < 1.0e30f) {
           const int ex = (int)((__float_as_uint(vmax) >> 23) & 0xffu) - 127;      // vmax in [2^ex, 2^(ex+1))
           sv = __uint_as_float((uint32_t)(127 + 13 - ex) << 23);                 // sv vmax in [2^13, 2^14)
         }
       }
-#pragma unroll 1
-      for (int s = 0; s < 2; ++s) {
-        if (s == 1) { TSTAMP(7); mbar_wait(BAR(BAR_M0), ph); TSTAMP(8); }   // phase-0 MMAs have read V^(0)
-        const float scale = (rw >= 0) ? (s ? sv * f * G.inv_sD : sv) : 0.f;
+      {
+        const float scale = (rw >= 0) ? sv : 0.f;
         if (h == 0) {
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
@@ -529,7 +528,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_arrive(BAR(s ? BAR_V1 : BAR_V0));
+        mbar_arrive(BAR(BAR_V0));
       }
       TSTAMP(9);
       // ---- a_bar from TMEM (main + cross-term accumulators), this thread's 64 columns ----
@@ -538,20 +537,23 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       TSTAMP(10);
       // thread = (row, half of the ages) reads its TMEM lane and parks the scaled values in the (free) A / V region, 16-byte
       // chunks XOR-swizzled by the row; then each warp writes 16 rows to global memory 512 contiguous bytes at a time
-      const float ua = 1.f / sv;
+      const float ua = 1.f / sv, fa = f * G.inv_sD;      // a_bar_i = (acc^(0)_i + f / sD acc^(1)_i) Cm_i / (2^14 sv)
       float4* stage = reinterpret_cast<float4*>(gbase);                   // [TM][32] float4
 #pragma unroll 1
       for (int c = 4 * h; c < 4 * h + 4; ++c) {
-        uint32_t v[16], x[16];
-        TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x);
+        uint32_t v[16], x[16], v1[16], x1[16];
+        TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x); TLD16(tlane + 2 * NA + 16 * c, v1); TLD16(tlane + 3 * NA + 16 * c, x1);
         tld_wait();
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+          v[k] = __float_as_uint(fmaf(fa, __uint_as_float(v1[k]) + __uint_as_float(x1[k]), __uint_as_float(v[k]) + __uint_as_float(x[k])));
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           float4 o;
-          o.x = (__uint_as_float(v[4 * q]) + __uint_as_float(x[4 * q])) * (ua * cm_s[16 * c + 4 * q]);
-          o.y = (__uint_as_float(v[4 * q + 1]) + __uint_as_float(x[4 * q + 1])) * (ua * cm_s[16 * c + 4 * q + 1]);
-          o.z = (__uint_as_float(v[4 * q + 2]) + __uint_as_float(x[4 * q + 2])) * (ua * cm_s[16 * c + 4 * q + 2]);
-          o.w = (__uint_as_float(v[4 * q + 3]) + __uint_as_float(x[4 * q + 3])) * (ua * cm_s[16 * c + 4 * q + 3]);
+          o.x = __uint_as_float(v[4 * q]) * (ua * cm_s[16 * c + 4 * q]);
+          o.y = __uint_as_float(v[4 * q + 1]) * (ua * cm_s[16 * c + 4 * q + 1]);
+          o.z = __uint_as_float(v[4 * q + 2]) * (ua * cm_s[16 * c + 4 * q + 2]);
+          o.w = __uint_as_float(v[4 * q + 3]) * (ua * cm_s[16 * c + 4 * q + 3]);
           stage[r * 32 + ((4 * c + q) ^ (r & 7))] = o;
         }
       }
