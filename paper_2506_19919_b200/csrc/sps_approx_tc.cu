@@ -271,6 +271,29 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       rw_next = (rb + r < min(row_start[cell + 1], rb + TM)) ? __ldg(G.order + rb + r) : -1;
       if (rw_next >= 0 && !G.flux_bar) gal_next = G.gal_of_row ? __ldg(G.gal_of_row + rw_next) : rw_next;
     }
+    RowScalars sc_n;
+    float m_n[16], ob0_n[(NB + 1) / 2], ob1_n[(NB + 1) / 2];
+    auto load_row = [&](int rw, int64_t gal) {
+      float4* scq = reinterpret_cast<float4*>(&sc_n);
+      float4* mq = reinterpret_cast<float4*>(m_n);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        scq[q] = rw >= 0 ? reinterpret_cast<const float4*>(B.sc + rw)[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+        mq[q] = rw >= 0 ? __ldg(reinterpret_cast<const float4*>(B.m + (int64_t)rw * ROW_M_STRIDE) + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int j = 0; j < 16; ++j) if (j >= T.n_Z) m_n[j] = 0.f;
+#pragma unroll
+      for (int k = 0; k < (NB + 1) / 2; ++k) {
+        const int b = min(h + 2 * k, NB - 1);
+        ob0_n[k] = 0.f; ob1_n[k] = 1.f;
+        if (rw >= 0) {
+          if (G.flux_bar) ob0_n[k] = __ldg(G.flux_bar + (int64_t)rw * NB + b);
+          else { ob0_n[k] = __ldg(G.obs_flux + gal * NB + b); ob1_n[k] = __ldg(G.obs_sigma + gal * NB + b); }
+        }
+      }
+    };
+    load_row(rw_next, gal_next);
     for (int w = w_begin; w < w_end; ++w, ph ^= 1u) {
       while (cta_start[cell + 1] <= w) ++cell;
       const int r_begin = row_start[cell] + (w - cta_start[cell]) * TM;
@@ -290,30 +313,14 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       }
       rw_next = (r_end + r < r_end_next) ? __ldg(G.order + r_end + r) : -1;
       gal_next = 0;
-      // ---- the row's scalars, metallicity weights and this thread's bands of the observations (requested first: in
-      //      flight while a is staged) ----
-      RowScalars sc;
+      // ---- the row's scalars, metallicity weights and this thread's bands of the observations: requested during the
+      //      previous tile (before its wait for pass 2) ----
+      const RowScalars sc = sc_n;
       float m[16], ob0[(NB + 1) / 2], ob1[(NB + 1) / 2];
-      {
-        float4* scq = reinterpret_cast<float4*>(&sc);
-        float4* mq = reinterpret_cast<float4*>(m);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          scq[q] = rw >= 0 ? reinterpret_cast<const float4*>(B.sc + rw)[q] : make_float4(0.f, 0.f, 0.f, 0.f);
-          mq[q] = rw >= 0 ? __ldg(reinterpret_cast<const float4*>(B.m + (int64_t)rw * ROW_M_STRIDE) + q) : make_float4(0.f, 0.f, 0.f, 0.f);
-        }
+      for (int j = 0; j < 16; ++j) m[j] = m_n[j];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) if (j >= T.n_Z) m[j] = 0.f;
-#pragma unroll
-        for (int k = 0; k < (NB + 1) / 2; ++k) {
-          const int b = min(h + 2 * k, NB - 1);
-          ob0[k] = 0.f; ob1[k] = 1.f;
-          if (rw >= 0) {
-            if (G.flux_bar) ob0[k] = __ldg(G.flux_bar + (int64_t)rw * NB + b);
-            else { ob0[k] = __ldg(G.obs_flux + gal * NB + b); ob1[k] = __ldg(G.obs_sigma + gal * NB + b); }
-          }
-        }
-      }
+      for (int k = 0; k < (NB + 1) / 2; ++k) { ob0[k] = ob0_n[k]; ob1[k] = ob1_n[k]; }
       // ---- stage a (split, swizzled): warp-cooperative, lane = 4 consecutive ages of one row; warp (q, h) stages rows
       //      32 q + 16 h .. + 15 ----
       {
@@ -441,7 +448,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         }
       }
       TSTAMP(4);
-      if (!G.want_grad) continue;
+      if (!G.want_grad) { if (w + 1 < w_end) load_row(rw_next, gal_next); continue; }
       // ---- sweep 2 over P (this thread's chunks): m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
       float sbar[NB];
 #pragma unroll
@@ -532,6 +539,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       }
       TSTAMP(9);
       // ---- a_bar from TMEM (main + cross-term accumulators), this thread's 64 columns ----
+      if (w + 1 < w_end) load_row(rw_next, gal_next);       // the next tile's row inputs travel while pass 2 runs
       mbar_wait(BAR(BAR_M1), ph);
       tc_fence_after();
       TSTAMP(10);
