@@ -214,7 +214,7 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
 # captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("approx_contract", 40000): 84.9e6,   # profiles/r01_hmc_kernels_full.md: 79.89 MB read + 5.02 MB written (40,000 rows per launch)
+    ("approx_contract", 40000): 85.1e6,   # profiles/r01_hmc_kernels_full.md: 79.62 MB read + 5.51 MB written (40,000 rows per launch)
     ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
 }
 
