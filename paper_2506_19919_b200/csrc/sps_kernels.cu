@@ -604,7 +604,13 @@ sps_status approx_contract_setup(const TableDev& T) {
                   bytes - (size_t)2 * T.n_age * T.cs_stride * sizeof(float));
     return SPS_ESHAPE;
   }
-  return sps_check_cuda(cudaFuncSetAttribute(approx_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
+  // the opt-in is per kernel, not per table: ask for the device maximum so that tables of different sizes can coexist
+  int dev = 0, optin = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  cudaFuncAttributes fa;
+  if (cudaFuncGetAttributes(&fa, approx_contract_kernel) == cudaSuccess) optin -= (int)fa.sharedSizeBytes; else cudaGetLastError();
+  return sps_check_cuda(cudaFuncSetAttribute(approx_contract_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max((int)bytes, optin)),
                         "approximate-path shared memory opt-in");
 }
 
