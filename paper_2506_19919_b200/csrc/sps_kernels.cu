@@ -24,7 +24,7 @@ struct RowFwd {
 };
 
 template <bool WANT_GRAD>
-__device__ __forceinline__ void row_forward(const TableDev& T, const PriorDev& P, const float* __restrict__ row,
+__device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& P, const float* __restrict__ row,
                                             bool unbounded, RowFwd& R) {
   load_params(row, unbounded, P, R.th, R.dth, R.z_d);
   cosmic_time(T, R.z_d, R.t_obs_d, R.dt_dz);
@@ -44,12 +44,14 @@ template <bool WANT_GRAD>
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, PRO_MIN_BLOCKS)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
+  __shared__ float s_prior[7 * SPS_NDIM];
+  const PriorView PV = stage_prior(P, s_prior);
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
   RowFwd R;
-  row_forward<WANT_GRAD>(T, P, theta + row * SPS_NDIM, unbounded, R);
+  row_forward<WANT_GRAD>(T, PV, theta + row * SPS_NDIM, unbounded, R);
   const float Fb = R.th[4], inv_M = 1.f / R.Msum;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
@@ -469,6 +471,8 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
 __global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, EPI_MIN_BLOCKS)
 epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbounded, bool with_prior,
                 const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad, LeapfrogFuse lf) {
+  __shared__ float s_prior[7 * SPS_NDIM];
+  const PriorView PV = stage_prior(P, s_prior);
   const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
@@ -476,7 +480,7 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
   const RowScalars sc = B.sc[row];
   if (!grad) {                                               // log-posterior only
     float lp = 0.f;
-    if (with_prior && l < SPS_NDIM) { float dlp; log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp); }
+    if (with_prior && l < SPS_NDIM) { float dlp; log_skew_normal(theta[row * SPS_NDIM + l], PV.xi[l], PV.omega[l], PV.skew[l], lp, dlp); }
     lp = warp_sum(lp);
     if (l == 0 && logp) logp[row] = sc.logp_like + lp;
     return;
@@ -498,10 +502,10 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
   const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
   // the prior term (a9) depends on the row's parameters only: evaluated while the loads above are in flight
   float lp = 0.f, dlp = 0.f;
-  if (with_prior && l < SPS_NDIM) log_skew_normal(theta[row * SPS_NDIM + l], P.xi[l], P.omega[l], P.skew[l], lp, dlp);
+  if (with_prior && l < SPS_NDIM) log_skew_normal(theta[row * SPS_NDIM + l], PV.xi[l], PV.omega[l], PV.skew[l], lp, dlp);
   float th[SPS_NDIM], dth[SPS_NDIM];
   double zd_unused;
-  load_params<false>(theta + row * SPS_NDIM, unbounded, P, th, dth, zd_unused);
+  load_params<false>(theta + row * SPS_NDIM, unbounded, PV, th, dth, zd_unused);
   const float zp = 1.f + th[12];
   const float dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp * zp * zp + T.OL));
   BurstQuad Bq;

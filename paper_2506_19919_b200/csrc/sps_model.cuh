@@ -11,8 +11,19 @@
 // ---- a0: Eq. (C1) PAPER.md:429 -----------------------------------------------------------------
 // Every lane returns all 13 bounded parameters (th) and d theta / d theta~ (dth).
 // The redshift (lane 12) is also returned in double: t_obs(z) - age cancels for the oldest bins.
-template <bool NEED_ZD = true>
-__device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PriorDev& pr,
+// The prior / bounds arrays of a launch, staged once per block in shared memory: lanes index them by parameter, and a
+// lane-indexed read of the kernel-parameter (constant) bank is replayed once per distinct address.
+struct PriorView { const float *y_lo, *y_hi, *k, *x0, *xi, *omega, *skew; };
+__device__ __forceinline__ PriorView stage_prior(const PriorDev& P, float* s_prior) {
+  static_assert(sizeof(PriorDev) == 7 * SPS_NDIM * sizeof(float), "PriorDev is seven float[SPS_NDIM] arrays");
+  if (threadIdx.x < 7 * SPS_NDIM) s_prior[threadIdx.x] = reinterpret_cast<const float*>(&P)[threadIdx.x];
+  __syncthreads();
+  return PriorView{s_prior, s_prior + SPS_NDIM, s_prior + 2 * SPS_NDIM, s_prior + 3 * SPS_NDIM, s_prior + 4 * SPS_NDIM,
+                   s_prior + 5 * SPS_NDIM, s_prior + 6 * SPS_NDIM};
+}
+
+template <bool NEED_ZD = true, class PR = PriorDev>
+__device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PR& pr,
                                             float th[SPS_NDIM], float dth[SPS_NDIM], double& z_d) {
   const int l = lane_id();
   float v = 0.f, d = 1.f;
