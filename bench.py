@@ -205,6 +205,7 @@ def run_ours(args):
                    "d2h_bytes_per_step": d2h},
            "gpu_launches": int(launches), "clocks": clk, "impl": "ours", **extra}
     out["roofline"] = roofline(prof, dom_kernel, rows_per_launch, grid, peaks, peaks_src, pairs)
+    out["roofline_step"] = [r for r in (row_kernel_roofline(prof, k, rows_per_launch, grid, peaks, peaks_src, args.workload in ("c4_hmc", "c5_nuts")) for k in ("prologue", "epilogue")) if r]
     out["kernel_ms"] = {k: {"avg_ms": (v[0] / v[1] if v[1] else None), "launches": v[2]} for k, v in prof.items() if v[2]}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, cfg, budget_s=args.cpu_budget)
@@ -217,6 +218,41 @@ NCU_TRAFFIC = {
     ("approx_contract", 40000): 85.1e6,   # profiles/r01_hmc_kernels_full.md: 79.62 MB read + 5.51 MB written (40,000 rows per launch)
     ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
 }
+
+
+# warp instructions per row of the two row kernels, from the committed ncu --set full capture (smsp__inst_executed.sum over
+# 40,000 rows, profiles/r01_hmc_kernels_full.md): the prologue's work is transcendental-heavy quadrature, not a byte stream.
+NCU_WARP_INST_PER_ROW = {"prologue": 67137647 / 40000.0, "epilogue": 43276400 / 40000.0}
+NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 70.6e6, ("epilogue", 40000): 139.7e6}   # same capture: dram read + written per launch
+
+
+def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, fused_leapfrog):
+    """The other kernels of an evaluation, reported beside the contraction's roofline.
+    prologue (a0-a5): instruction-issue bound ("alu"): achieved = ncu's warp instructions per row x rows per launch / the live
+    launch time, against 148 SMs x 4 schedulers x the maximum SM clock (one warp instruction per scheduler per clock).  The
+    instruction count is this implementation's, not an algorithmic minimum: the fraction says how busy the issue slots are.
+    epilogue (a10 reverse of a0-a5 + the fused leapfrog update): an HBM stream: algorithmic bytes per row = the five stored
+    per-bin vectors and a_bar (n_age words each), m_bar (n_Z), the 64-byte row scalars, theta, the leapfrog operands
+    (p, theta, inverse mass, eps; sampler workloads only) in; grad, logp, p, theta out; against the measured HBM copy bandwidth."""
+    ms, timed, allc = prof[kernel]
+    if not timed:
+        return None
+    avg_s = ms / timed / 1e3
+    base = {"kernel": kernel, "avg_launch_ms": 1e3 * avg_s, "timed_launches": timed, "launches": allc,
+            "traffic": NCU_TRAFFIC_ROW_KERNELS.get((kernel, rows_per_launch))}
+    if kernel == "prologue":
+        clock_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+        peak = 148 * 4 * clock_hz / 1e9
+        ach = NCU_WARP_INST_PER_ROW[kernel] * rows_per_launch / avg_s / 1e9
+        return {**base, "bound": "alu", "achieved": ach, "peak": peak, "unit": "G warp-inst/s", "frac": ach / peak,
+                "peak_note": f"issue-slot peak = 148 SM x 4 schedulers x {clock_hz / 1e6:.0f} MHz ({peaks_src} clock); achieved = "
+                             f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (ncu, profiles/r01_hmc_kernels_full.md)"}
+    bytes_row = 4 * (6 * grid.n_age + grid.n_Z + 16 + 13 + 13 + 1 + ((3 * 13 + 1) + 2 * 13 if fused_leapfrog else 0))
+    ach = bytes_row * rows_per_launch / avg_s / 1e9
+    peak = float(peaks["hbm_gbs"])
+    return {**base, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "peak_note": f"HBM copy bandwidth ({peaks_src}); achieved = {bytes_row} algorithmic bytes per row; the kernel also issues "
+                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 61 % busy in the ncu capture)"}
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
