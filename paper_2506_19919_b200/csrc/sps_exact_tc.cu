@@ -541,11 +541,16 @@ __global__ void tc_weights_kernel(TableDev T, int64_t n, const int* __restrict__
 
 // reverse A operand: SEDbar[r][k] = F_att(lam_k) dlam_k sum_b g_b T_b(lam_k (1+z))  (reverse of Eq. 3-4), split.
 // Only the k blocks of the row tile's plan range are written (the reverse GEMM reads nothing else).
+// One block per row; per pass a warp owns 256 consecutive wavelengths (a thread: four pairs 64 apart, so loads and stores
+// stay coalesced): the bands whose 5-sigma support meets the warp's span at the row's redshift are found once per pass,
+// warp-uniformly (the filters overlap little, so two to four of them), and only those are evaluated.  The kernel is
+// instruction-issue bound (a per-element loop over all bands cost 148 instructions per element).
+constexpr int SB_G = 4, SB_THREADS = 128, SB_SPAN = 64 * SB_G;
 template <int PREC>
-__global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
-                                                        const float* __restrict__ gbuf, const float4* __restrict__ wconst,
-                                                        const int* __restrict__ plan, int plan_cap,
-                                                        typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+__global__ void __launch_bounds__(SB_THREADS) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
+                                                               const float* __restrict__ gbuf, const float4* __restrict__ wconst,
+                                                               const int* __restrict__ plan, int plan_cap,
+                                                               typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
   typedef typename Op<PREC>::T E;
   const int64_t r = blockIdx.x;
   const int m = (int)(r / BM);
@@ -559,38 +564,58 @@ __global__ void __launch_bounds__(256) tc_sedbar_kernel(TableDev T, int64_t n, c
   }
   __syncthreads();
   const float zp = sc_s[0], AVs = sc_s[1], delta = sc_s[2], Ffl = sc_s[3], Eb = 0.85f - 1.9f * delta;
-  for (int k = k_begin + 2 * threadIdx.x; k < k_end; k += 512) {              // two consecutive wavelengths per thread
-    float v[2];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int kb = k_begin + SB_SPAN * warp; kb < k_end; kb += SB_SPAN * (SB_THREADS / 32)) {
+    float4 c0[2 * SB_G];
+    float tsum[2 * SB_G], lamz[2 * SB_G];
+    float mx = 0.f;
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
-      const float4 c0 = __ldg(&wconst[2 * (k + u)]);
-      v[u] = 0.f;
-      if (c0.y > 0.f) {
-        const float lamz = c0.x * zp;
-        float tsum = 0.f;
-        for (int b = 0; b < T.n_band; ++b) {
-          const float x = fmaf(lamz, FC.isg[b], FC.nmu[b]);
-          if (fabsf(x) <= FILT_CUT) tsum = fmaf(g_s[b], ex2_fast(-x * x), tsum);
-        }
-        if (tsum != 0.f) {
-          const float l2r = __ldg(&wconst[2 * (k + u) + 1].x);
-          const float pw = ex2_fast(delta * l2r);
-          float A = AVs * fmaf(c0.z, pw, Eb * c0.w);
-          if (!(A > 0.f)) A = 0.f;
-          const float Tt = ex2_fast(-0.4f * 3.321928094887362f * A);
-          v[u] = fmaf(1.f - Ffl, Tt, Ffl) * c0.y * tsum;
+    for (int e = 0; e < 2 * SB_G; ++e) {
+      const int k = kb + 64 * (e >> 1) + 2 * lane + (e & 1);
+      c0[e] = (k < k_end) ? __ldg(&wconst[2 * k]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      lamz[e] = c0[e].x * zp; tsum[e] = 0.f;
+      mx = fmaxf(mx, lamz[e]);                              // padded columns carry no wavelength: take the largest
+    }
+    const float lam_lo = __shfl_sync(FULL_MASK, lamz[0], 0) * 0.99999f;
+    const float lam_hi = __uint_as_float(__reduce_max_sync(FULL_MASK, __float_as_uint(mx))) * 1.00001f;
+    for (int b = 0; b < T.n_band; ++b) {
+      if (lam_hi >= FC.lo[b] && lam_lo <= FC.hi[b]) {
+        const float isg = FC.isg[b], nmu = FC.nmu[b], g = g_s[b];
+#pragma unroll
+        for (int e = 0; e < 2 * SB_G; ++e) {
+          const float x = fmaf(lamz[e], isg, nmu);
+          if (fabsf(x) <= FILT_CUT) tsum[e] = fmaf(g, ex2_fast(-x * x), tsum[e]);
         }
       }
     }
-    const int64_t o = r * T.n_wave_pad + k;
-    E h2[2], l2[2];
-    Op<PREC>::split(v[0], h2[0], l2[0]); Op<PREC>::split(v[1], h2[1], l2[1]);
-    if (sizeof(E) == 2) {
-      *reinterpret_cast<uint32_t*>(hi + o) = *reinterpret_cast<const uint32_t*>(h2);
-      *reinterpret_cast<uint32_t*>(lo + o) = *reinterpret_cast<const uint32_t*>(l2);
-    } else {
-      *reinterpret_cast<uint2*>(hi + o) = *reinterpret_cast<const uint2*>(h2);
-      *reinterpret_cast<uint2*>(lo + o) = *reinterpret_cast<const uint2*>(l2);
+#pragma unroll
+    for (int q = 0; q < SB_G; ++q) {
+      const int k = kb + 64 * q + 2 * lane;
+      E h2[2], l2[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int e = 2 * q + u;
+        float v = 0.f;
+        if (c0[e].y > 0.f && tsum[e] != 0.f) {
+          const float l2r = __ldg(&wconst[2 * (k + u) + 1].x);
+          const float pw = ex2_fast(delta * l2r);
+          float A = AVs * fmaf(c0[e].z, pw, Eb * c0[e].w);
+          if (!(A > 0.f)) A = 0.f;
+          const float Tt = ex2_fast(-0.4f * 3.321928094887362f * A);
+          v = fmaf(1.f - Ffl, Tt, Ffl) * c0[e].y * tsum[e];
+        }
+        Op<PREC>::split(v, h2[u], l2[u]);
+      }
+      if (k < k_end) {
+        const int64_t o = r * T.n_wave_pad + k;
+        if (sizeof(E) == 2) {
+          *reinterpret_cast<uint32_t*>(hi + o) = *reinterpret_cast<const uint32_t*>(h2);
+          *reinterpret_cast<uint32_t*>(lo + o) = *reinterpret_cast<const uint32_t*>(l2);
+        } else {
+          *reinterpret_cast<uint2*>(hi + o) = *reinterpret_cast<const uint2*>(h2);
+          *reinterpret_cast<uint2*>(lo + o) = *reinterpret_cast<const uint2*>(l2);
+        }
+      }
     }
   }
 }
@@ -674,7 +699,7 @@ template <int PREC>
 sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
   typedef typename Op<PREC>::T E;
   ExactState* X = t->exact; const TableDev& T = t->dev;
-  tc_sedbar_kernel<PREC><<<(unsigned)n, 256, 0, s>>>(T, n, rows, t->rows, S->fc, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
+  tc_sedbar_kernel<PREC><<<(unsigned)n, SB_THREADS, 0, s>>>(T, n, rows, t->rows, S->fc, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
   GemmArgs G; memset(&G, 0, sizeof(G));
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = S->nb; G.k_blocks = T.n_wave_pad / S->BK; G.BN = S->BNb; G.BK = S->BK;
   G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
