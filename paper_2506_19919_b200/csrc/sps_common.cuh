@@ -80,6 +80,30 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
 
+// Warp sums of N = 4 or 8 per-lane values at once: every exchange step halves the number of values a lane carries
+// (N + log2(32) - 1 shuffles instead of 5 N).  On return lane l holds the complete sum of value
+// k(l) = 4 b4 + 2 b3 + b2 (N = 8) or 2 b4 + b3 (N = 4), b_i = bit i of l: value k is held by lane warp_multi_holder<N>(k).
+template <int N> __device__ __forceinline__ float warp_sum_multi(float (&v)[N]) {
+  static_assert(N == 4 || N == 8, "4 or 8 values");
+  const int l = threadIdx.x & 31;
+  int o = 16;
+#pragma unroll
+  for (int n = N / 2; n >= 1; n >>= 1, o >>= 1) {
+    const bool up = (l & o) != 0;
+#pragma unroll
+    for (int k = 0; k < n; ++k) {
+      const float send = up ? v[k] : v[k + n], keep = up ? v[k + n] : v[k];
+      v[k] = keep + __shfl_xor_sync(FULL_MASK, send, o);
+    }
+  }
+#pragma unroll
+  for (; o > 0; o >>= 1) v[0] += __shfl_xor_sync(FULL_MASK, v[0], o);
+  return v[0];
+}
+template <int N> __device__ __forceinline__ constexpr int warp_multi_holder(int k) {
+  return N == 8 ? 16 * ((k >> 2) & 1) + 8 * ((k >> 1) & 1) + 4 * (k & 1) : 16 * ((k >> 1) & 1) + 8 * (k & 1);
+}
+
 // launch counter (host side)
 extern "C" int64_t sps_launch_count(void);
 void sps_count_launch(int n = 1);

@@ -1,6 +1,7 @@
 // sps_kernels.cu -- prologue (a0-a5), approximate-photometry contraction (a7, a9, a10) and
 // epilogue (reverse of a0-a5 + prior) kernels.
 #include <algorithm>
+#include <cstddef>
 #include "sps_rows.cuh"
 
 #define WARPS_PER_BLOCK 8
@@ -500,60 +501,62 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
     for (int k = 0; k < ROW_PARTS; ++k) pr[k][q] = part[k * ROW_A_STRIDE + l + 32 * q];
   }
   const float mb = (l < ROW_M_STRIDE) ? B.m_bar[row * ROW_M_STRIDE + l] : 0.f;
+  // the direct bar of this lane's parameter, straight from the row's scalars (lane 0: Mn_bar, 9-11: dust bars, 12: z_bar)
+  const int fld = l < 16 ? (int)((0x9CBA000000008ull >> (4 * l)) & 15ull) : 0;   // nibble l = the field of RowScalars lane l needs
+  static_assert(offsetof(RowScalars, Mn_bar) == 32 && offsetof(RowScalars, z_bar) == 36 && offsetof(RowScalars, AV_bar) == 40 &&
+                offsetof(RowScalars, Ffloor_bar) == 48, "RowScalars layout");
+  const float direct = reinterpret_cast<const float*>(B.sc + row)[fld];
   // the prior term (a9) depends on the row's parameters only: evaluated while the loads above are in flight
   float lp = 0.f, dlp = 0.f;
   if (with_prior && l < SPS_NDIM) log_skew_normal(theta[row * SPS_NDIM + l], PV.xi[l], PV.omega[l], PV.skew[l], lp, dlp);
-  float th[SPS_NDIM], dth[SPS_NDIM];
-  double zd_unused;
-  load_params<false>(theta + row * SPS_NDIM, unbounded, PV, th, dth, zd_unused);
-  const float zp = 1.f + th[12];
+  float th_l, d1;                                             // lane p: bounded parameter p and d theta_p / d theta~_p
+  load_param_lane(theta + row * SPS_NDIM, unbounded, PV, th_l, d1);
+  const float Fb = __shfl_sync(FULL_MASK, th_l, 4), ltp = __shfl_sync(FULL_MASK, th_l, 5), ltm = __shfl_sync(FULL_MASK, th_l, 6);
+  const float lz = __shfl_sync(FULL_MASK, th_l, 7), slz = __shfl_sync(FULL_MASK, th_l, 8);
+  const float zp = 1.f + __shfl_sync(FULL_MASK, th_l, 12);
   const float dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp * zp * zp + T.OL));
   BurstQuad Bq;
-  burst_bins(T, th[5], th[6], Bq);
+  burst_bins(T, ltp, ltm, Bq);
   float m_unused, dm_lz, dm_s;
-  met_bin(T, th[7], th[8], m_unused, dm_lz, dm_s);
-  const float Fb = th[4], inv_M = 1.f / sc.Msum, Mf = sc.Mn * inv_M;
+  met_bin(T, lz, slz, m_unused, dm_lz, dm_s);
+  const float inv_M = 1.f / sc.Msum, Mf = sc.Mn * inv_M;
   float Ps[SPS_AGE_PER_LANE];
-  float s_fb = 0.f, s_pp = 0.f, s_ltp = 0.f, s_ltm = 0.f;
+  // round 1 of warp sums: {dL/dF_burst (Eq. A6), sum a_bar P_smooth, burst-time sums}
+  float r1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     Ps[q] = pr[0][q] * inv_M;
-    s_fb += abar[q] * (Bq.P[q] - Ps[q]);                       // dL/dF_burst           (Eq. A6)
-    s_pp += abar[q] * Ps[q];
-    s_ltp += abar[q] * Bq.d_ltp[q];
-    s_ltm += abar[q] * Bq.d_ltm[q];
+    r1[0] += abar[q] * (Bq.P[q] - Ps[q]);
+    r1[1] += abar[q] * Ps[q];
+    r1[2] += abar[q] * Bq.d_ltp[q];
+    r1[3] += abar[q] * Bq.d_ltm[q];
   }
-  s_fb = warp_sum(s_fb); s_pp = warp_sum(s_pp); s_ltp = warp_sum(s_ltp) * Fb; s_ltm = warp_sum(s_ltm) * Fb;
+  const float R1 = warp_sum_multi<4>(r1);
+  const float s_pp = __shfl_sync(FULL_MASK, R1, warp_multi_holder<4>(1));
   // dL/d(dM_i) = (1-Fb)/Msum (a_bar_i - sum_k a_bar_k Ps_k) + Mn_bar * Mf
-  float s_tau = 0.f, s_al = 0.f, s_be = 0.f, s_t = 0.f;
+  // round 2: {tau, alpha, beta, t_obs sums; MDF sums; prior}
+  float r2[8] = {0.f, 0.f, 0.f, 0.f, mb * dm_lz, mb * dm_s, lp, 0.f};
+  const float c1 = (1.f - Fb) * inv_M, c2 = sc.Mn_bar * Mf;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
-    const float dMb = (l + 32 * q < T.n_age) ? (1.f - Fb) * inv_M * (abar[q] - s_pp) + sc.Mn_bar * Mf : 0.f;
-    s_tau += dMb * pr[1][q]; s_al += dMb * pr[2][q]; s_be += dMb * pr[3][q]; s_t += dMb * pr[4][q];
+    const float dMb = (l + 32 * q < T.n_age) ? fmaf(c1, abar[q] - s_pp, c2) : 0.f;
+    r2[0] += dMb * pr[1][q]; r2[1] += dMb * pr[2][q]; r2[2] += dMb * pr[3][q]; r2[3] += dMb * pr[4][q];
   }
-  s_tau = warp_sum(s_tau); s_al = warp_sum(s_al); s_be = warp_sum(s_be); s_t = warp_sum(s_t);
-  const float s_lz = warp_sum(mb * dm_lz), s_s = warp_sum(mb * dm_s);
-  float g = 0.f;
-  switch (l) {
-    case 0: g = sc.Mn_bar * sc.Mn * LN10F; break;
-    case 1: g = s_tau; break;
-    case 2: g = s_al; break;
-    case 3: g = s_be; break;
-    case 4: g = s_fb; break;
-    case 5: g = s_ltp; break;
-    case 6: g = s_ltm; break;
-    case 7: g = s_lz; break;
-    case 8: g = s_s; break;
-    case 9: g = sc.AV_bar; break;
-    case 10: g = sc.delta_bar; break;
-    case 11: g = sc.Ffloor_bar; break;
-    case 12: g = sc.z_bar + s_t * dt_dz; break;
-    default: break;
-  }
+  const float R2 = warp_sum_multi<8>(r2);
+  // lane p fetches the sum its gradient component needs.  Round 2 holders: value k in lane 16 b2(k) + 8 b1(k) + 4 b0(k):
+  // lane 1 <- tau (k 0), 2 <- alpha (1), 3 <- beta (2), 12 <- t_obs (3), 7 <- logZ (4), 8 <- sigma_logZ (5), 0 <- prior (6).
+  // Round 1 holders: lane 4 <- F_burst (k 0: lane 0), 5 <- logT_peak (k 2: lane 16), 6 <- logT_max (k 3: lane 24).
+  const int k2 = l < 16 ? (int)((0x3000540002106ull >> (4 * l)) & 15ull) : 0;      // nibble l = the round-2 value lane l needs
+  const int k1 = l < 16 ? (int)((0x3200000ull >> (4 * l)) & 15ull) : 0;            // nibble l = the round-1 value lane l needs
+  const float g2 = __shfl_sync(FULL_MASK, R2, warp_multi_holder<8>(k2));
+  const float g1 = __shfl_sync(FULL_MASK, R1, warp_multi_holder<4>(k1));
+  float g = g2;                                              // lanes 1, 2, 3, 7, 8
+  if (l == 0) g = direct * sc.Mn * LN10F;
+  else if (l == 4) g = g1;
+  else if (l == 5 || l == 6) g = g1 * Fb;
+  else if (l >= 9 && l <= 11) g = direct;
+  else if (l == 12) g = fmaf(g2, dt_dz, direct);
   if (l < SPS_NDIM) {
-    float d1 = 1.f;
-#pragma unroll
-    for (int p = 0; p < SPS_NDIM; ++p) if (p == l) d1 = dth[p];
     g = g * d1 + dlp;
     grad[row * SPS_NDIM + l] = g;
     if (lf.p_w) {                                            // fused leapfrog update (theta may alias lf.theta_w: read above, written here)
@@ -563,8 +566,7 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
       lf.theta_w[o] = lf_th + lf_eps * lf_im * pn;
     }
   }
-  lp = warp_sum(lp);
-  if (l == 0 && logp) logp[row] = sc.logp_like + lp;
+  if (l == 0 && logp) logp[row] = sc.logp_like + g2;         // lane 0's fetch is the prior sum
 }
 
 __global__ void copy_weights_kernel(TableDev T, int64_t n, RowBuffers B, float* w_age, float* w_met, float* mstar) {

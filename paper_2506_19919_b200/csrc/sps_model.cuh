@@ -50,6 +50,22 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
   }
 }
 
+// The same for lane p < SPS_NDIM only: its own bounded parameter and slope (no broadcast; the reverse pass needs six of them).
+template <class PR>
+__device__ __forceinline__ void load_param_lane(const float* __restrict__ row, bool unbounded, const PR& pr, float& v, float& d) {
+  const int l = lane_id();
+  v = 0.f; d = 1.f;
+  if (l < SPS_NDIM) {
+    v = row[l];
+    if (unbounded) {
+      const float s = 1.f / (1.f + expf(-pr.k[l] * (v - pr.x0[l])));
+      const float w = pr.y_hi[l] - pr.y_lo[l];
+      v = pr.y_lo[l] + w * s;
+      d = w * pr.k[l] * s * (1.f - s);
+    }
+  }
+}
+
 // ---- a1: age of the universe (R11), Gyr, and dt/dz ------------------------------------------------
 __device__ __forceinline__ void cosmic_time(const TableDev& T, double z_d, double& t_d, float& dt_dz) {
   const double zpd = 1.0 + z_d;
@@ -241,22 +257,34 @@ struct BurstQuad { float P[SPS_AGE_PER_LANE], d_ltp[SPS_AGE_PER_LANE], d_ltm[SPS
 __device__ __forceinline__ void burst_bins(const TableDev& T, float ltp, float ltm, BurstQuad& B) {
   const int l = lane_id();
   const float inv_s3 = 1.f / (ltm - ltp);
+  // Every bin edge is evaluated once, by the lane that owns the bin above it: y clipped to [-1, 1] and the density there
+  // (zero at the clips); a bin takes its upper edge from the owner of the next bin (lane + 1, or lane 0's next slot).
+  // Slots past the grid sit at the upper clip, so their bins come out as zero without a branch.
+  float y[SPS_AGE_PER_LANE + 1], p[SPS_AGE_PER_LANE + 1];
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     const int i = l + 32 * q;
-    B.P[q] = B.d_ltp[q] = B.d_ltm[q] = 0.f;
-    if (i < T.n_age) {
-      float ya = fminf(fmaxf((T.e_edge[i] - ltp) * inv_s3, -1.f), 1.f);
-      float yb = fminf(fmaxf((T.e_edge[i + 1] - ltp) * inv_s3, -1.f), 1.f);
-      float half = 0.5f * (yb - ya), mid = 0.5f * (yb + ya), s = 0.f;
+    const float e = (i <= T.n_age) ? T.e_edge[i] : 1e30f;
+    y[q] = fminf(fmaxf((e - ltp) * inv_s3, -1.f), 1.f);
+    p[q] = tri_pdf_y(y[q]);
+  }
+  y[SPS_AGE_PER_LANE] = 1.f; p[SPS_AGE_PER_LANE] = 0.f;
+  const float x1 = 0.8611363115940526f, x2 = 0.3399810435848563f, w1 = 0.3478548451374538f, w2 = 0.6521451548625461f;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) s += GL4_W[k] * tri_pdf_y(mid + half * GL4_X[k]);
-      B.P[q] = half * s;
-      float pa = tri_pdf_y(ya), pb = tri_pdf_y(yb);           // zero at the clips
-      // dy/dlogT_peak = (y-1)/s3, dy/dlogT_max = -y/s3
-      B.d_ltp[q] = (pb * (yb - 1.f) - pa * (ya - 1.f)) * inv_s3;
-      B.d_ltm[q] = (-pb * yb + pa * ya) * inv_s3;
-    }
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    float yb = __shfl_down_sync(FULL_MASK, y[q], 1), pb = __shfl_down_sync(FULL_MASK, p[q], 1);
+    const float y0 = __shfl_sync(FULL_MASK, y[q + 1], 0), p0 = __shfl_sync(FULL_MASK, p[q + 1], 0);
+    if (l == 31) { yb = y0; pb = p0; }
+    const float ya = y[q], pa = p[q];
+    const float half = 0.5f * (yb - ya), mid = 0.5f * (yb + ya), h1 = half * x1, h2 = half * x2;
+    // 4-point Gauss-Legendre on the symmetric node pairs mid +- h1, mid +- h2
+    float u1 = fmaf(-(mid - h1), mid - h1, 1.f), u2 = fmaf(-(mid + h1), mid + h1, 1.f);
+    float u3 = fmaf(-(mid - h2), mid - h2, 1.f), u4 = fmaf(-(mid + h2), mid + h2, 1.f);
+    const float s = w1 * (u1 * u1 * u1 + u2 * u2 * u2) + w2 * (u3 * u3 * u3 + u4 * u4 * u4);
+    B.P[q] = (35.f / 32.f) * half * s;
+    // dy/dlogT_peak = (y-1)/s3, dy/dlogT_max = -y/s3
+    B.d_ltp[q] = (pb * (yb - 1.f) - pa * (ya - 1.f)) * inv_s3;
+    B.d_ltm[q] = (-pb * yb + pa * ya) * inv_s3;
   }
 }
 
