@@ -215,15 +215,15 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
 # captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("approx_contract", 40000): 85.1e6,   # profiles/r01_hmc_kernels_full.md: 79.62 MB read + 5.51 MB written (40,000 rows per launch)
+    ("approx_contract", 40000): 85.2e6,   # profiles/r01_hmc_kernels_full.md: 79.82 MB read + 5.33 MB written (40,000 rows per launch)
     ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
 }
 
 
 # warp instructions per row of the two row kernels, from the committed ncu --set full capture (smsp__inst_executed.sum over
 # 40,000 rows, profiles/r01_hmc_kernels_full.md): the prologue's work is transcendental-heavy quadrature, not a byte stream.
-NCU_WARP_INST_PER_ROW = {"prologue": 67137647 / 40000.0, "epilogue": 43276400 / 40000.0}
-NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 70.6e6, ("epilogue", 40000): 139.7e6}   # same capture: dram read + written per launch
+NCU_WARP_INST_PER_ROW = {"prologue": 65137994 / 40000.0, "epilogue": 28996415 / 40000.0}
+NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 70.7e6, ("epilogue", 40000): 140.0e6}   # same capture: dram read + written per launch
 
 
 def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, fused_leapfrog):
@@ -252,7 +252,7 @@ def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, f
     peak = float(peaks["hbm_gbs"])
     return {**base, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
             "peak_note": f"HBM copy bandwidth ({peaks_src}); achieved = {bytes_row} algorithmic bytes per row; the kernel also issues "
-                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 61 % busy in the ncu capture)"}
+                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 64 % busy in the ncu capture)"}
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
