@@ -43,6 +43,12 @@ struct TableDev {
   // cosmology (R11): t = t_pref * asinh(t_arg * (1+z)^-1.5)  [Gyr];  H0 in 1/Gyr
   float t_pref, t_arg, H0_gyr, Om, OL;
   double t_pref_d, t_arg_d;
+  // the same function as piecewise degree-5 polynomials in double over the z grid's range (tz_n intervals, local variable
+  // u in [-1, 1], coefficients c0..c5; interpolated at Chebyshev nodes at table creation: relative error < 1e-15), so that a
+  // row costs five double FMAs instead of a double-precision asinh; outside the range the closed form is evaluated
+  const double* tz_coef;    // [tz_n][6] or null
+  double tz_lo, tz_inv_h;
+  int tz_n;
   float log10_mass_unit;
 };
 

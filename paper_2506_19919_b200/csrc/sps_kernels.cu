@@ -16,7 +16,7 @@
 // Forward model of one row (one warp per parameter row): everything a0-a5 needs, held per lane.
 // ---------------------------------------------------------------------------------------------
 struct RowFwd {
-  float th[SPS_NDIM], dth[SPS_NDIM];
+  float th[SPS_NDIM];
   double t_obs_d, z_d;
   float dt_dz, Msum, Mf;
   AgeQuad Q;
@@ -27,7 +27,7 @@ struct RowFwd {
 template <bool WANT_GRAD>
 __device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& P, const float* __restrict__ row,
                                             bool unbounded, RowFwd& R) {
-  load_params(row, unbounded, P, R.th, R.dth, R.z_d);
+  load_params(row, unbounded, P, R.th, R.z_d);
   cosmic_time(T, R.z_d, R.t_obs_d, R.dt_dz);
   smooth_bins<WANT_GRAD>(T, R.t_obs_d, R.th[1], R.th[2], R.th[3], R.Q);
   float s = 0.f;

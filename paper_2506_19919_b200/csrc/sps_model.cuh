@@ -9,7 +9,7 @@
 #define LN10F 2.3025850929940457f
 
 // ---- a0: Eq. (C1) PAPER.md:429 -----------------------------------------------------------------
-// Every lane returns all 13 bounded parameters (th) and d theta / d theta~ (dth).
+// Every lane returns all 13 bounded parameters (th); the slopes d theta / d theta~ are lane-local (load_param_lane).
 // The redshift (lane 12) is also returned in double: t_obs(z) - age cancels for the oldest bins.
 // The prior / bounds arrays of a launch, staged once per block in shared memory: lanes index them by parameter, and a
 // lane-indexed read of the kernel-parameter (constant) bank is replayed once per distinct address.
@@ -24,9 +24,9 @@ __device__ __forceinline__ PriorView stage_prior(const PriorDev& P, float* s_pri
 
 template <bool NEED_ZD = true, class PR = PriorDev>
 __device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PR& pr,
-                                            float th[SPS_NDIM], float dth[SPS_NDIM], double& z_d) {
+                                            float th[SPS_NDIM], double& z_d) {
   const int l = lane_id();
-  float v = 0.f, d = 1.f;
+  float v = 0.f;
   double vd = 0.0;
   if (l < SPS_NDIM) {
     v = row[l];
@@ -39,15 +39,11 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
         vd = (double)pr.y_lo[l] + ((double)pr.y_hi[l] - (double)pr.y_lo[l]) * sd;
       }
       v = pr.y_lo[l] + w * s;
-      d = w * pr.k[l] * s * (1.f - s);
     }
   }
   z_d = NEED_ZD ? __shfl_sync(FULL_MASK, vd, SPS_NDIM - 1) : 0.0;
 #pragma unroll
-  for (int p = 0; p < SPS_NDIM; ++p) {
-    th[p] = __shfl_sync(FULL_MASK, v, p);
-    dth[p] = __shfl_sync(FULL_MASK, d, p);
-  }
+  for (int p = 0; p < SPS_NDIM; ++p) th[p] = __shfl_sync(FULL_MASK, v, p);
 }
 
 // The same for lane p < SPS_NDIM only: its own bounded parameter and slope (no broadcast; the reverse pass needs six of them).
@@ -69,7 +65,15 @@ __device__ __forceinline__ void load_param_lane(const float* __restrict__ row, b
 // ---- a1: age of the universe (R11), Gyr, and dt/dz ------------------------------------------------
 __device__ __forceinline__ void cosmic_time(const TableDev& T, double z_d, double& t_d, float& dt_dz) {
   const double zpd = 1.0 + z_d;
-  t_d = T.t_pref_d * asinh(T.t_arg_d * rsqrt(zpd * zpd * zpd));
+  const double sz = (z_d - T.tz_lo) * T.tz_inv_h;
+  if (T.tz_coef != nullptr && sz >= 0.0 && sz < (double)T.tz_n) {            // every lane of the warp holds the same z
+    const int iz = (int)sz;
+    const double u = 2.0 * (sz - (double)iz) - 1.0;
+    const double* c = T.tz_coef + 6 * iz;
+    t_d = fma(fma(fma(fma(fma(c[5], u, c[4]), u, c[3]), u, c[2]), u, c[1]), u, c[0]);
+  } else {
+    t_d = T.t_pref_d * asinh(T.t_arg_d * rsqrt(zpd * zpd * zpd));
+  }
   const float zp = (float)zpd, zp3 = zp * zp * zp;
   dt_dz = -1.f / (zp * T.H0_gyr * sqrtf(T.Om * zp3 + T.OL));
 }

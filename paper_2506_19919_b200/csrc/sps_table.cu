@@ -140,10 +140,43 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   T.t_pref = (float)T.t_pref_d; T.t_arg = (float)T.t_arg_d;
   T.H0_gyr = (float)(1.0 / inv_H0); T.Om = (float)d->Om; T.OL = (float)OL;
   T.log10_mass_unit = (float)d->log10_mass_unit;
+  // t_obs(z) (R11) as piecewise degree-5 polynomials over [z_min, z_max]: interpolation of the closed form at the six
+  // Chebyshev nodes of each interval (6 x 6 Vandermonde system in long double)
+  T.tz_coef = nullptr; T.tz_n = 0; T.tz_lo = 0.0; T.tz_inv_h = 0.0;
+  std::vector<double> tz;
+  if (d->z_max > d->z_min) {
+    const int N = 256;
+    const double h = (d->z_max - d->z_min) / N;
+    tz.resize((size_t)N * 6);
+    long double un[6];
+    for (int k = 0; k < 6; ++k) un[k] = cosl((2 * k + 1) * 3.14159265358979323846264338327950288L / 12.0L);
+    for (int i = 0; i < N; ++i) {
+      long double A[6][7];
+      for (int k = 0; k < 6; ++k) {
+        long double pw = 1.0L;
+        for (int c = 0; c < 6; ++c) { A[k][c] = pw; pw *= un[k]; }
+        const double z = d->z_min + (i + 0.5) * h + 0.5 * h * (double)un[k];
+        A[k][6] = (long double)(T.t_pref_d * asinh(T.t_arg_d * pow(1.0 + z, -1.5)));
+      }
+      for (int c = 0; c < 6; ++c) {                          // Gauss-Jordan with partial pivoting
+        int piv = c;
+        for (int r = c + 1; r < 6; ++r) if (fabsl(A[r][c]) > fabsl(A[piv][c])) piv = r;
+        for (int k = 0; k < 7; ++k) std::swap(A[c][k], A[piv][k]);
+        for (int r = 0; r < 6; ++r) {
+          if (r == c) continue;
+          const long double f = A[r][c] / A[c][c];
+          for (int k = c; k < 7; ++k) A[r][k] -= f * A[c][k];
+        }
+      }
+      for (int c = 0; c < 6; ++c) tz[(size_t)i * 6 + c] = (double)(A[c][6] / A[c][c]);
+    }
+    T.tz_n = N; T.tz_lo = d->z_min; T.tz_inv_h = 1.0 / h;
+  }
 
   std::vector<double> Amid_d(na);
   for (int i = 0; i < na; ++i) Amid_d[i] = 0.5 * (Ae[i] + Ae[i + 1]);
   T.A_edge_d = upload(Ae, st); T.A_mid_d = upload(Amid_d, st);
+  if (!tz.empty()) T.tz_coef = upload(tz, st);
   T.A_edge = upload(A_edge, st); T.A_mid = upload(A_mid, st); T.A_half = upload(A_half, st); T.e_edge = upload(e_edge, st);
   T.g_mid = upload(g_mid, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
   T.drude = upload(dr, st); T.l2r = upload(l2r, st); T.ssp = upload(ssp, st);
@@ -177,7 +210,7 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
 extern "C" sps_status sps_destroy_table(sps_table* t) {
   if (!t) return SPS_OK;
   TableDev& T = t->dev;
-  const void* ptrs[] = {T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
+  const void* ptrs[] = {T.tz_coef, T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp};
   for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
   sps_exact_teardown(t);
   sps_approx_tc_teardown(t);
