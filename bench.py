@@ -215,15 +215,15 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu --set full
 # captures (profiles/), taken at the launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("approx_contract", 40000): 85.2e6,   # profiles/r01_hmc_kernels_full.md: 79.82 MB read + 5.33 MB written (40,000 rows per launch)
+    ("approx_contract", 40000): 84.8e6,   # profiles/r01_hmc_kernels_full.md: 79.78 MB read + 5.00 MB written (40,000 rows per launch)
     ("exact_fwd", 8192): 74.2e6,          # profiles/r01_exact_gemm_full.md: 72.18 MB read + 2.02 MB written (8,192 rows per launch)
 }
 
 
 # warp instructions per row of the two row kernels, from the committed ncu --set full capture (smsp__inst_executed.sum over
 # 40,000 rows, profiles/r01_hmc_kernels_full.md): the prologue's work is transcendental-heavy quadrature, not a byte stream.
-NCU_WARP_INST_PER_ROW = {"prologue": 65137994 / 40000.0, "epilogue": 28996415 / 40000.0}
-NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 70.7e6, ("epilogue", 40000): 140.0e6}   # same capture: dram read + written per launch
+NCU_WARP_INST_PER_ROW = {"prologue": 62160578 / 40000.0, "epilogue": 28956415 / 40000.0}
+NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 71.1e6, ("epilogue", 40000): 139.9e6}   # same capture: dram read + written per launch
 
 
 def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, fused_leapfrog):
