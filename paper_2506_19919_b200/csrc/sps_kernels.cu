@@ -9,7 +9,7 @@
 #define PRO_MIN_BLOCKS 4                        // resident blocks per SM the prologue / epilogue are compiled for
 #endif
 #ifndef EPI_MIN_BLOCKS
-#define EPI_MIN_BLOCKS 3
+#define EPI_MIN_BLOCKS 4
 #endif
 
 // ---------------------------------------------------------------------------------------------
