@@ -525,17 +525,36 @@ __global__ void build_wconst_kernel(TableDev T, float4* __restrict__ wc) {
   wc[2 * k + 1] = make_float4(T.l2r[k], 0.f, 0.f, 0.f);
 }
 
-// forward A operand: W[r][ij] = Mn a_i m_j (a5: Eq. 2 and M_star), split
+// forward A operand: W[r][ij] = Mn a_i m_j (a5: Eq. 2 and M_star), split.  One block per row, two consecutive entries per
+// thread (packed stores); a_i and m_j of the row are staged in shared memory, ij -> (i, j) without an integer division.
 template <int PREC>
-__global__ void tc_weights_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, int Wld,
-                                  typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+__global__ void __launch_bounds__(128) tc_weights_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, int Wld,
+                                                         typename Op<PREC>::T* __restrict__ hi, typename Op<PREC>::T* __restrict__ lo) {
+  typedef typename Op<PREC>::T E;
   const int64_t r = blockIdx.x;
   const int64_t row = rows ? rows[r] : r;
-  const float Mn = B.sc[row].Mn;
-  for (int e = threadIdx.x; e < Wld; e += blockDim.x) {
-    float v = 0.f;
-    if (e < T.K) { const int i = e / T.n_Z, j = e - i * T.n_Z; v = Mn * B.a[row * ROW_A_STRIDE + i] * B.m[row * ROW_M_STRIDE + j]; }
-    Op<PREC>::split(v, hi[r * Wld + e], lo[r * Wld + e]);
+  __shared__ float a_s[ROW_A_STRIDE], m_s[ROW_M_STRIDE];
+  a_s[threadIdx.x] = B.a[row * ROW_A_STRIDE + threadIdx.x] * B.sc[row].Mn;
+  if (threadIdx.x < ROW_M_STRIDE) m_s[threadIdx.x] = B.m[row * ROW_M_STRIDE + threadIdx.x];
+  __syncthreads();
+  const float inv_nZ = 1.f / (float)T.n_Z;
+  for (int e = 2 * threadIdx.x; e < Wld; e += 2 * blockDim.x) {          // Wld is a multiple of the k block, hence even
+    E h2[2], l2[2];
+    int i = (int)(((float)e + 0.5f) * inv_nZ), j = e - i * T.n_Z;         // exact for e < 2^16 (n_age n_Z <= 2048)
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const float v = (e + u < T.K) ? a_s[min(i, ROW_A_STRIDE - 1)] * m_s[j] : 0.f;
+      Op<PREC>::split(v, h2[u], l2[u]);
+      if (++j == T.n_Z) { j = 0; ++i; }
+    }
+    const int64_t o = r * Wld + e;
+    if (sizeof(E) == 2) {
+      *reinterpret_cast<uint32_t*>(hi + o) = *reinterpret_cast<const uint32_t*>(h2);
+      *reinterpret_cast<uint32_t*>(lo + o) = *reinterpret_cast<const uint32_t*>(l2);
+    } else {
+      *reinterpret_cast<uint2*>(hi + o) = *reinterpret_cast<const uint2*>(h2);
+      *reinterpret_cast<uint2*>(lo + o) = *reinterpret_cast<const uint2*>(l2);
+    }
   }
 }
 
