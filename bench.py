@@ -222,7 +222,7 @@ NCU_TRAFFIC = {
 
 # warp instructions per row of the two row kernels, from the committed ncu --set full capture (smsp__inst_executed.sum over
 # 40,000 rows, profiles/r01_hmc_kernels_full.md): the prologue's work is transcendental-heavy quadrature, not a byte stream.
-NCU_WARP_INST_PER_ROW = {"prologue": 62160578 / 40000.0, "epilogue": 28956415 / 40000.0}
+NCU_WARP_INST_PER_ROW = {"prologue": 62160578 / 40000.0, "epilogue": 29196415 / 40000.0}
 NCU_TRAFFIC_ROW_KERNELS = {("prologue", 40000): 71.1e6, ("epilogue", 40000): 139.9e6}   # same capture: dram read + written per launch
 
 
@@ -252,7 +252,7 @@ def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, f
     peak = float(peaks["hbm_gbs"])
     return {**base, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
             "peak_note": f"HBM copy bandwidth ({peaks_src}); achieved = {bytes_row} algorithmic bytes per row; the kernel also issues "
-                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 64 % busy in the ncu capture)"}
+                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 72 % busy in the ncu capture)"}
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
