@@ -149,6 +149,21 @@ def test_weights_edge_cases(tiny):
     assert wa[1].max() > 0.999 and wm[2].max() > 0.999
 
 
+def test_weights_cosmic_time_table_and_closed_form(tiny):
+    # t_obs(z) is read from piecewise polynomials over the z grid's range and from the closed form of R11 outside it
+    # (DESIGN.md 5.1): redshifts at the range ends, on interval boundaries (3 k / 256) and beyond the range must all
+    # match the oracle, and the two evaluations must join continuously at the end of the range
+    cx = tiny
+    zs = np.array([0.0, 3.0 / 256, 3.0 * 17 / 256, 1.5, 3.0 * 255 / 256, 2.9999998, 3.0, 3.0000002, 3.001, 4.5], np.float32)
+    th = np.repeat(M.bound(W.draw_theta_unbounded(cx.prior, 1, 11), cx.P)[0], zs.size, axis=0)
+    th[:, M.I_Z] = zs
+    wa, wm, ms = (x.cpu().numpy().astype(np.float64) for x in cx.sps.sps_weights(cx.table, None, _dev(th), unbounded=False))
+    ow = M.weights(th.astype(np.float32).astype(np.float64), cx.grid)
+    assert (np.abs(wa - ow["a"]) / ow["a"].max(1, keepdims=True)).max() <= 1e-5
+    assert _rel(ms, ow["Mn"]).max() <= 1e-5
+    assert np.abs(wa[5] - wa[7]).max() <= 1e-5 * wa[5].max()          # z = 3 -/+ 2e-7: table vs closed form
+
+
 def test_empty_batch(tiny):
     cx = tiny
     e = torch.empty((0, 13), dtype=torch.float32, device="cuda")
