@@ -4,12 +4,18 @@
 #include <cstddef>
 #include "sps_rows.cuh"
 
-#define WARPS_PER_BLOCK 8
+#define WARPS_PER_BLOCK 8                       // rows per block of the small row kernels
+#ifndef PRO_WARPS
+#define PRO_WARPS 16                            // rows (warps) per prologue block
+#endif
+#ifndef EPI_WARPS_PER_BLOCK
+#define EPI_WARPS_PER_BLOCK 4                   // rows (warps) per epilogue block
+#endif
 #ifndef PRO_MIN_BLOCKS
-#define PRO_MIN_BLOCKS 4                        // resident blocks per SM the prologue / epilogue are compiled for
+#define PRO_MIN_BLOCKS 2                        // resident blocks per SM the prologue / epilogue are compiled for
 #endif
 #ifndef EPI_MIN_BLOCKS
-#define EPI_MIN_BLOCKS 4
+#define EPI_MIN_BLOCKS 8
 #endif
 
 // ---------------------------------------------------------------------------------------------
@@ -42,12 +48,12 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& 
 // a0-a5.  With WANT_GRAD the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
 // kept in B.part for the epilogue, which then has no quadrature to redo.
 template <bool WANT_GRAD>
-__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, PRO_MIN_BLOCKS)
+__global__ void __launch_bounds__(32 * PRO_WARPS, PRO_MIN_BLOCKS)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
-  const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
+  const int64_t r = (int64_t)blockIdx.x * PRO_WARPS + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
@@ -469,12 +475,12 @@ approx_contract_kernel(TableDev T, int64_t n, const int* __restrict__ order, con
 // with a_bar, m_bar, Mn_bar and the direct bars.  Only the cheap closed forms (C1, dt/dz, burst polynomial, MDF) are
 // re-evaluated; no quadrature is redone.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(32 * WARPS_PER_BLOCK, EPI_MIN_BLOCKS)
+__global__ void __launch_bounds__(32 * EPI_WARPS_PER_BLOCK, EPI_MIN_BLOCKS)
 epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbounded, bool with_prior,
                 const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad, LeapfrogFuse lf) {
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
-  const int64_t r = (int64_t)blockIdx.x * WARPS_PER_BLOCK + (threadIdx.x >> 5);
+  const int64_t r = (int64_t)blockIdx.x * EPI_WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
@@ -592,8 +598,9 @@ void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, i
   int* hist = nullptr;
   if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
   sps_prof_begin(SPS_K_PROLOGUE, s);
-  if (want_grad) prologue_kernel<true><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
-  else prologue_kernel<false><<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
+  const unsigned pro_blocks = (unsigned)((n + PRO_WARPS - 1) / PRO_WARPS);
+  if (want_grad) prologue_kernel<true><<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
+  else prologue_kernel<false><<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
@@ -653,7 +660,7 @@ void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, i
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s) {
   if (n <= 0) return;
   sps_prof_begin(SPS_K_EPILOGUE, s);
-  epilogue_kernel<<<blocks_for_rows(n), 32 * WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad, lf);
+  epilogue_kernel<<<(unsigned)((n + EPI_WARPS_PER_BLOCK - 1) / EPI_WARPS_PER_BLOCK), 32 * EPI_WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad, lf);
   sps_prof_end(SPS_K_EPILOGUE, s);
   sps_count_launch();
 }
