@@ -252,7 +252,7 @@ def row_kernel_roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, f
     peak = float(peaks["hbm_gbs"])
     return {**base, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
             "peak_note": f"HBM copy bandwidth ({peaks_src}); achieved = {bytes_row} algorithmic bytes per row; the kernel also issues "
-                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 72 % busy in the ncu capture)"}
+                         f"{NCU_WARP_INST_PER_ROW[kernel]:.0f} warp instructions per row (issue slots 76 % busy in the ncu capture)"}
 
 
 def roofline(prof, kernel, rows_per_launch, grid, peaks, peaks_src, pairs=0):
