@@ -297,6 +297,17 @@ def nuts_transition(theta, logp, grad, eps, inv_mass, max_depth, logp_grad1, see
     return prop[0], prop[1], prop[2], acc_sum / max(n_leaf, 1), n_leaf, diverged, depth
 
 
+def gaussian_target(mu, prec):
+    """SPS_MODEL_GAUSS_TEST: logP(theta) = -1/2 (theta-mu)^T P (theta-mu), grad = -P (theta-mu), the
+    correlated Gaussian on which north_star asks HMC and NUTS to recover the mean and the variance."""
+    mu = np.asarray(mu, float); prec = np.asarray(prec, float)
+
+    def f(th):
+        d = np.asarray(th, float) - mu
+        return -0.5 * np.einsum("bi,ij,bj->b", d, prec, d), -d @ prec.T
+    return f
+
+
 def init_chains(prior, seed, chain_ids, D):
     """R17: theta~_0 = xi + 0.1 omega N(0,1) from the chain's own stream (transition 0, purpose 5)."""
     xi, om = prior[4], prior[5]

@@ -39,8 +39,12 @@ _GL_X, _GL_W = leggauss(32)          # R6: 32-point Gauss-Legendre per age bin
 def bound(theta_unb, prior):
     """theta = y_lo + (y_hi-y_lo)/(1+exp(-k(theta~ - x0)));  returns theta and d theta/d theta~."""
     y_lo, y_hi, k, x0 = prior[0], prior[1], prior[2], prior[3]
-    s = 1.0 / (1.0 + np.exp(-k * (theta_unb - x0)))
-    return y_lo + (y_hi - y_lo) * s, (y_hi - y_lo) * k * s * (1.0 - s)
+    x = k * (theta_unb - x0)
+    # the same function, evaluated without overflow for saturated arguments (warmup reaches |x| ~ 20-90):
+    # e = exp(-|x|) <= 1;  s = 1/(1+e) for x >= 0, e/(1+e) for x < 0;  s (1-s) = e/(1+e)^2 either way
+    e = np.exp(-np.abs(x))
+    s = np.where(x >= 0.0, 1.0, e) / (1.0 + e)
+    return y_lo + (y_hi - y_lo) * s, (y_hi - y_lo) * k * e / ((1.0 + e) * (1.0 + e))
 
 
 def unbound(theta, prior):
@@ -313,6 +317,60 @@ def effective_wavelength(mu_A, sigma_A, n=20001):
     return out
 
 
+def tabulated_T(lam_obs_A, wave_A, trans):
+    """R4: a tabulated transmission curve (T(lambda) is a general curve; only App. B's test uses
+    Gaussians) is linearly interpolated between its knots and is zero outside its support [wave[0], wave[-1]].
+    Returns T and dT/dlambda_obs = the slope of the segment that holds lambda (R18: at a knot, the segment to its right)."""
+    w = np.asarray(wave_A, float); t = np.asarray(trans, float)
+    lam = np.asarray(lam_obs_A, float)
+    seg = np.clip(np.searchsorted(w, lam, side="right") - 1, 0, len(w) - 2)
+    slope = (t[1:] - t[:-1]) / (w[1:] - w[:-1])
+    inside = (lam >= w[0]) & (lam <= w[-1])
+    T = np.where(inside, t[seg] + (lam - w[seg]) * slope[seg], 0.0)
+    return T, np.where(inside, slope[seg], 0.0)
+
+
+def tabulated_effective_wavelength(wave_A, trans):
+    """Eq. (5) at z = 0 for a tabulated curve: int lam T / int T of the piecewise-linear interpolant, each segment
+    integrated exactly (T linear: trapezoid; lam T quadratic: Simpson)."""
+    w = np.asarray(wave_A, float); t = np.asarray(trans, float)
+    h = w[1:] - w[:-1]
+    wm = 0.5 * (w[1:] + w[:-1]); tm = 0.5 * (t[1:] + t[:-1])
+    den = (h * tm).sum()
+    num = (h / 6.0 * (w[:-1] * t[:-1] + 4.0 * wm * tm + w[1:] * t[1:])).sum()
+    return num / den
+
+
+def _filter_tab(grid):
+    return getattr(grid, "filt_tab", None)
+
+
+def n_bands(grid):
+    tab = _filter_tab(grid)
+    return len(tab[2]) - 1 if tab is not None else len(grid.filt_mu_A)
+
+
+def band_T(grid, lam_obs_A):
+    """T_b(lambda_obs) and dT_b/dlambda_obs of every band of the grid at the observed wavelengths lam_obs_A [N]
+    -> [n_band, N] each.  Gaussian filters (mu, sigma) or tabulated curves grid.filt_tab = (wave, trans, offsets):
+    band b owns the knots offsets[b] .. offsets[b+1]-1."""
+    lam = np.asarray(lam_obs_A, float)
+    tab = _filter_tab(grid)
+    if tab is None:
+        return filter_T(lam[None, :], np.asarray(grid.filt_mu_A, float)[:, None], np.asarray(grid.filt_sigma_A, float)[:, None])
+    wave, trans, off = tab
+    out = [tabulated_T(lam, wave[off[b]:off[b + 1]], trans[off[b]:off[b + 1]]) for b in range(len(off) - 1)]
+    return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
+
+
+def band_effective_wavelength(grid):
+    tab = _filter_tab(grid)
+    if tab is None:
+        return effective_wavelength(grid.filt_mu_A, grid.filt_sigma_A)
+    wave, trans, off = tab
+    return np.array([tabulated_effective_wavelength(wave[off[b]:off[b + 1]], trans[off[b]:off[b + 1]]) for b in range(len(off) - 1)])
+
+
 # ----------------------------------------------------------------------------------------------
 # a6  exact photometry, Eq. (4) with M_star restored (R1)   PAPER.md:60-69
 # ----------------------------------------------------------------------------------------------
@@ -325,7 +383,7 @@ def photometry_exact(theta, grid, want_jac=True):
     L = np.asarray(grid.ssp, float)                      # [K, N]
     lam = np.asarray(grid.wave_A, float)
     dlam = trapezoid_weights(lam)
-    n_band = len(grid.filt_mu_A)
+    n_band = n_bands(grid)
     flux = np.zeros((B, n_band)); J = np.zeros((B, n_band, NDIM))
     for r in range(B):
         a, m, Mn = W["a"][r], W["m"][r], W["Mn"][r]
@@ -333,7 +391,7 @@ def photometry_exact(theta, grid, want_jac=True):
         S = w @ L                                        # Eq. (1) without dust  [N]
         z = th[r, I_Z]
         F, F_av, F_del, F_fl, _ = attenuation(lam, th[r, I_AV], th[r, I_DEL], th[r, I_FFL])
-        T, dT = filter_T(lam[None, :] * (1.0 + z), grid.filt_mu_A[:, None], grid.filt_sigma_A[:, None])  # [b,N]
+        T, dT = band_T(grid, lam * (1.0 + z))                                                          # [b,N]
         flux[r] = (T * (S * F * dlam)[None, :]).sum(1)
         if not want_jac:
             continue
@@ -363,9 +421,9 @@ def cssp_table(grid, z_values=None):
     L = np.asarray(grid.ssp, float)
     lam = np.asarray(grid.wave_A, float)
     dlam = trapezoid_weights(lam)
-    out = np.empty((len(zs), L.shape[0], len(grid.filt_mu_A)))
+    out = np.empty((len(zs), L.shape[0], n_bands(grid)))
     for t, z in enumerate(zs):
-        T, _ = filter_T(lam[None, :] * (1.0 + z), grid.filt_mu_A[:, None], grid.filt_sigma_A[:, None])
+        T, _ = band_T(grid, lam * (1.0 + z))
         out[t] = L @ (T * dlam[None, :]).T
     return out
 
@@ -381,8 +439,8 @@ def photometry_approx(theta, grid, cssp, lam_eff_obs=None):
     W = weights(th, grid)
     B = th.shape[0]
     if lam_eff_obs is None:
-        lam_eff_obs = effective_wavelength(grid.filt_mu_A, grid.filt_sigma_A)
-    n_band = len(grid.filt_mu_A)
+        lam_eff_obs = band_effective_wavelength(grid)
+    n_band = n_bands(grid)
     n_age, n_Z = len(grid.log10_age_yr), len(grid.log10_Z)
     dz = (grid.z_max - grid.z_min) / (grid.n_z - 1)
     flux = np.zeros((B, n_band)); J = np.zeros((B, n_band, NDIM))

@@ -46,6 +46,16 @@ PRIOR_TABLE = {
     "z": (0.02, 2.98, 1.0, 0.6),
 }
 
+# SPS_MODEL_TINY5 (BASELINE.json configs[0]; R19): logM_star, log10 tau/Gyr, logZ, tau_V sampled; z = 0.5 is data
+TINY5_PARAM_NAMES = ("logM", "log_tau", "logZ", "tau_V")
+TINY5_PRIOR_TABLE = {
+    "logM": (8.0, 12.0, 10.0, 0.8),
+    "log_tau": (-0.5, 1.2, 0.5, 0.3),
+    "logZ": (-2.2, 0.4, -0.3, 0.4),
+    "tau_V": (0.0, 3.0, 0.5, 0.4),
+}
+TINY5_Z = 0.5
+
 
 @dataclasses.dataclass
 class Grid:
@@ -62,6 +72,9 @@ class Grid:
     H0: float = 67.74
     Om: float = 0.3089
     log10_mass_unit: float = 10.0
+    # tabulated filters (observed frame) instead of Gaussian ones: (wave_A [n_knot], trans [n_knot], offsets [n_band+1]);
+    # band b owns the knots offsets[b] .. offsets[b+1]-1 (strictly increasing wavelengths within a band)
+    filt_tab: tuple | None = None
 
     @property
     def n_age(self): return int(self.log10_age_yr.size)
@@ -70,7 +83,7 @@ class Grid:
     @property
     def n_wave(self): return int(self.wave_A.size)
     @property
-    def n_band(self): return int(self.filt_mu_A.size)
+    def n_band(self): return int(self.filt_mu_A.size) if self.filt_tab is None else int(len(self.filt_tab[2]) - 1)
 
 
 @dataclasses.dataclass
@@ -149,10 +162,28 @@ def make_grid(kind: str, seed: int | None = None) -> Grid:
         wave = np.geomspace(400.0, 4.0e4, 777)
         mu, sg = gaussian_filters(np.geomspace(3500.0, 10500.0, 12), np.geomspace(4.0, 12.0, 12))
         n_z = 9
+    elif kind == "tiny_tab":
+        # the tiny grid with TABULATED filters: three asymmetric curves on their own non-uniform wavelength grids
+        g = make_grid("tiny", seed)
+        return dataclasses.replace(g, filt_tab=tabulated_filters([4500.0, 6500.0, 9000.0], [900.0, 1300.0, 1700.0], SEED0 + 3))
     else:
         raise ValueError(kind)
     ssp = make_ssp_spectra(la, lz, wave, seed)
     return Grid(la, lz, wave, ssp, mu, sg, 0.0, 3.0, n_z)
+
+
+def tabulated_filters(centres_A, widths_A, seed, n_knot=(41, 57, 73)):
+    """Stand-ins for measured transmission curves: per band a smooth asymmetric bump (steep blue edge, slow red decline,
+    a ripple on top) sampled on a jittered, non-uniform grid of its own; zero at both ends.  Input data only."""
+    rng = _rng(seed)
+    waves, trans, off = [], [], [0]
+    for c, w, n in zip(centres_A, widths_A, n_knot):
+        u = np.sort(np.concatenate([[0.0, 1.0], rng.uniform(0.0, 1.0, n - 2)]))
+        lam = c - 0.5 * w + w * u
+        t = (1.0 - np.exp(-u / 0.08)) * np.clip(1.0 - u, 0.0, 1.0) ** 0.6 * (1.0 + 0.1 * np.sin(17.0 * u))
+        t[0] = 0.0; t[-1] = 0.0
+        waves.append(lam); trans.append(t / t.max()); off.append(off[-1] + n)
+    return np.concatenate(waves), np.concatenate(trans), np.array(off, np.int32)
 
 
 def _logit_inverse(theta, y_lo, y_hi, k, x0):
@@ -161,12 +192,13 @@ def _logit_inverse(theta, y_lo, y_hi, k, x0):
     return x0 + np.log(u / (1.0 - u)) / k
 
 
-def make_prior(seed: int = SEED0 + 100, n_fit: int = 20000) -> Prior:
-    """Bounds from PRIOR_TABLE, k = 4/(y_hi-y_lo), x0 = centre (unit slope at the centre,
-    PAPER.md:434); skew-normal (xi, omega, s) moment-fitted to Gaussian draws mapped to the
+def make_prior(seed: int = SEED0 + 100, n_fit: int = 20000, model: str = "dpl13") -> Prior:
+    """Bounds from PRIOR_TABLE (model = "dpl13") or TINY5_PRIOR_TABLE ("tiny5"), k = 4/(y_hi-y_lo), x0 = centre (unit
+    slope at the centre); skew-normal (xi, omega, s) moment-fitted to Gaussian draws mapped to the
     unbounded space (the fit itself is host-side setup, out of scope)."""
     rng = _rng(seed)
-    cols = [PRIOR_TABLE[n] for n in PARAM_NAMES]
+    cols = [PRIOR_TABLE[n] for n in PARAM_NAMES] if model == "dpl13" else [TINY5_PRIOR_TABLE[n] for n in TINY5_PARAM_NAMES]
+    NDIM = len(cols)
     y_lo = np.array([c[0] for c in cols]); y_hi = np.array([c[1] for c in cols])
     mean = np.array([c[2] for c in cols]); sd = np.array([c[3] for c in cols])
     k = 4.0 / (y_hi - y_lo); x0 = 0.5 * (y_lo + y_hi)
@@ -194,6 +226,7 @@ def draw_theta_unbounded(prior: Prior, n: int, seed: int, z_uniform: tuple[float
     """n draws of the unbounded parameters from the skew-normal prior [n, D] float64.
     z_uniform=(a,b) replaces the redshift column by U[a,b] in bounded space (configs[1], [2])."""
     rng = _rng(seed)
+    NDIM = prior.xi.size
     u0 = rng.standard_normal((n, NDIM)); u1 = rng.standard_normal((n, NDIM))
     dlt = prior.skew / np.sqrt(1.0 + prior.skew ** 2)
     x = dlt * np.abs(u0) + np.sqrt(1.0 - dlt ** 2) * u1
@@ -207,6 +240,17 @@ def draw_theta_unbounded(prior: Prior, n: int, seed: int, z_uniform: tuple[float
         zz = np.clip(zz, prior.y_lo[-1] + w, prior.y_hi[-1] - w)
         th[:, NDIM - 1] = _logit_inverse(zz, prior.y_lo[-1], prior.y_hi[-1], prior.k[-1], prior.x0[-1])
     return th
+
+
+def pad_prior(prior: Prior, fixed: dict[int, float] | None = None, ndim: int = NDIM) -> np.ndarray:
+    """[7, ndim] array for the C ABI from a prior over fewer sampled parameters (SPS_MODEL_TINY5: 4): unused slots get
+    the identity bounds (0, 1), k = 1, x0 = 0, omega = 1, skew = 0; `fixed` puts data values (the redshift) into xi."""
+    a = prior.as_array()
+    out = np.zeros((7, ndim)); out[1] = 1.0; out[2] = 1.0; out[5] = 1.0
+    out[:, :a.shape[1]] = a
+    for slot, v in (fixed or {}).items():
+        out[4, slot] = v
+    return out
 
 
 def noisy_observations(flux_true: np.ndarray, seed: int, frac_lo: float, frac_hi: float):

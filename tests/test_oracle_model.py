@@ -162,3 +162,21 @@ def test_met_weights(tiny):
     h = 1e-6
     assert np.allclose(dlz, (M.met_weights(lz + h, s, g)[0] - M.met_weights(lz - h, s, g)[0]) / (2 * h), atol=1e-8)
     assert np.allclose(ds, (M.met_weights(lz, s + h, g)[0] - M.met_weights(lz, s - h, g)[0]) / (2 * h), atol=1e-8)
+
+
+def test_bound_saturates_cleanly(prior):
+    # HMC warmup reaches |k (theta~ - x0)| ~ 20-90 (Eq. C1): no overflow, theta inside [y_lo, y_hi], the
+    # slope falls off as exp(-|x|), and the two branches agree with the textbook form where that one is finite
+    import warnings
+    x = np.array([-800.0, -90.0, -37.0, -20.0, -1.0, 0.0, 1.0, 20.0, 37.0, 90.0, 800.0])
+    thu = prior[3][None, :] + x[:, None] / prior[2][None, :]
+    with warnings.catch_warnings():
+        warnings.simplefilter("error")
+        th, d = M.bound(thu, prior)
+    w = prior[1] - prior[0]
+    assert np.all(np.isfinite(th)) and np.all(th >= prior[0]) and np.all(th <= prior[1] + 4e-16 * w) and np.all(d >= 0.0)
+    ref = prior[0] + w / (1.0 + np.exp(-x[3:8]))[:, None]                  # Eq. (C1) as printed, |x| <= 20
+    assert np.allclose(th[3:8], ref, rtol=1e-15)
+    assert np.allclose(d[[1, 9]], (w * prior[2] * np.exp(-90.0))[None, :], rtol=1e-12)
+    assert np.array_equal(th[0], prior[0]) and np.allclose(th[-1], prior[1], rtol=0, atol=4e-16 * w.max()) and np.all(d[[0, -1]] == 0.0)
+    assert np.allclose(th[1] - prior[0], w * np.exp(-90.0), rtol=1e-12)     # lower tail keeps relative accuracy

@@ -173,3 +173,73 @@ def test_gradient_matches_central_differences(tiny, prior, cssp, path):
     lp0, g0, _ = M.logp_and_grad(thu, tiny, prior, flux, s, path, cssp)
     pl, pg = M.log_skew_normal(thu, prior)
     assert np.allclose(lp0, pl.sum(1)) and np.allclose(g0, pg)
+
+
+# ---- tabulated filters (T(lambda) is a general transmission curve; R4: linear interpolation) ------------
+def test_tabulated_curve_interpolation_and_support():
+    w = np.array([4000.0, 4100.0, 4400.0, 5000.0]); t = np.array([0.0, 0.8, 1.0, 0.0])
+    lam = np.array([3999.9, 4000.0, 4050.0, 4100.0, 4250.0, 4700.0, 5000.0, 5000.1])
+    T, dT = M.tabulated_T(lam, w, t)
+    assert np.allclose(T, [0.0, 0.0, 0.4, 0.8, 0.9, 0.5, 0.0, 0.0], atol=1e-15)          # hand-computed
+    assert np.allclose(dT[[2, 4, 5]], [0.008, 0.2 / 300.0, -1.0 / 600.0]) and dT[0] == 0.0 and dT[-1] == 0.0
+    assert np.allclose(T[1:-1], np.interp(lam[1:-1], w, t))                               # library routine
+    # at an interior knot the slope is the one of the segment to its right (R18)
+    assert M.tabulated_T(np.array([4100.0]), w, t)[1][0] == pytest.approx(0.2 / 300.0)
+
+
+def test_tabulated_effective_wavelength_closed_forms():
+    # a linear ramp rising from a to b: centroid (a + 2 b) / 3 exactly, whatever the knots (Eq. 5)
+    a, b = 5000.0, 6200.0
+    w = np.array([a, 5100.0, 5350.0, 6000.0, b]); t = (w - a) / (b - a)
+    assert abs(M.tabulated_effective_wavelength(w, t) - (a + 2 * b) / 3) < 1e-9
+    # a symmetric triangle: its centre; a top-hat built from two steep edges: its centre
+    w = np.array([100.0, 150.0, 200.0]); t = np.array([0.0, 1.0, 0.0])
+    assert abs(M.tabulated_effective_wavelength(w, t) - 150.0) < 1e-12
+    # against adaptive quadrature of the interpolant for an asymmetric curve
+    from scipy import integrate
+    g = W.make_grid("tiny_tab")
+    wave, trans, off = g.filt_tab
+    for k in range(3):
+        ww, tt = wave[off[k]:off[k + 1]], trans[off[k]:off[k + 1]]
+        num = sum(integrate.quad(lambda x: x * np.interp(x, ww, tt), ww[i], ww[i + 1])[0] for i in range(len(ww) - 1))
+        den = sum(integrate.quad(lambda x: np.interp(x, ww, tt), ww[i], ww[i + 1])[0] for i in range(len(ww) - 1))
+        assert abs(M.band_effective_wavelength(g)[k] - num / den) < 1e-8
+
+
+def test_tabulated_filters_in_photometry(prior):
+    g = W.make_grid("tiny_tab")
+    assert M.n_bands(g) == 3
+    # (1) constant spectrum: flux_b = trapezoid sum of T_b over the SSP grid (R4), and close to the exact area
+    g1 = __import__("dataclasses").replace(g, ssp=np.ones_like(g.ssp))
+    th = _theta(prior, 2, 3, A_V=0.0, z=0.0)
+    w = M.weights(th, g1)
+    flux = M.photometry_exact(th, g1, want_jac=False)[0]
+    lam = g.wave_A; dlam = M.trapezoid_weights(lam)
+    wave, trans, off = g.filt_tab
+    for b in range(3):
+        Tb = np.interp(lam, wave[off[b]:off[b + 1]], trans[off[b]:off[b + 1]], left=0.0, right=0.0)
+        assert np.allclose(flux[:, b], w["Mn"] * (Tb * dlam).sum(), rtol=1e-12)
+    # (2) a curve tabulated from a Gaussian on a fine grid reproduces the Gaussian filter's photometry
+    gg = W.make_grid("tiny")
+    lam_f = [np.linspace(m - 5 * s, m + 5 * s, 4001) for m, s in zip(gg.filt_mu_A, gg.filt_sigma_A)]
+    tab = (np.concatenate(lam_f), np.concatenate([np.exp(-0.5 * ((l - m) / s) ** 2) for l, m, s in zip(lam_f, gg.filt_mu_A, gg.filt_sigma_A)]),
+           np.arange(4) * 4001)
+    gt = __import__("dataclasses").replace(gg, filt_tab=tab)
+    th = _theta(prior, 3, 4)
+    f_g, J_g = M.photometry_exact(th, gg)
+    f_t, J_t = M.photometry_exact(th, gt)
+    assert np.allclose(f_t, f_g, rtol=2e-6) and np.allclose(J_t[:, :, :12], J_g[:, :, :12], rtol=1e-4, atol=1e-6 * np.abs(J_g).max())
+    # d/dz sees the interpolant's piecewise-constant slope instead of the Gaussian's derivative: first order in the knot spacing
+    assert np.allclose(J_t[:, :, 12], J_g[:, :, 12], rtol=5e-3, atol=1e-4 * np.abs(J_g).max())
+    assert np.allclose(M.band_effective_wavelength(gt), M.band_effective_wavelength(gg), rtol=1e-6)
+    # (3) gradient of the log-posterior against central differences, both paths (kinks of the interpolant: R18)
+    cs = M.cssp_table(g)
+    P = W.make_prior()
+    thu = W.draw_theta_unbounded(P, 2, 8)
+    d, s = W.noisy_observations(M.photometry_approx(M.bound(thu, prior)[0], g, cs)[0], 9, 0.05, 0.05)
+    for path in ("exact", "approx"):
+        lp, gr, _ = M.logp_and_grad(thu, g, prior, d, s, path, cs)
+        for p in (0, 1, 9, 12):
+            e = np.zeros(13); e[p] = 1e-6
+            fd = (M.logp_and_grad(thu + e, g, prior, d, s, path, cs)[0] - M.logp_and_grad(thu - e, g, prior, d, s, path, cs)[0]) / 2e-6
+            assert np.allclose(gr[:, p], fd, rtol=2e-4, atol=2e-5 * np.abs(gr).max()), (path, p, gr[:, p], fd)

@@ -109,3 +109,41 @@ def test_hmc_and_nuts_agree():
     sd = np.sqrt(np.diag(cov))
     assert np.all(np.abs(a.mean(0) - b.mean(0)) < 0.1 * sd)
     assert np.all(np.abs(a.std(0) / b.std(0) - 1) < 0.1)
+
+
+def test_gaussian_target_definition():
+    # SPS_MODEL_GAUSS_TEST: log density of N(mu, P^-1) up to a constant (scipy), gradient by central differences
+    from scipy import stats
+    rng = np.random.default_rng(4)
+    A = rng.normal(size=(5, 5)); cov = A @ A.T + np.eye(5); mu = rng.normal(size=5)
+    f = S.gaussian_target(mu, np.linalg.inv(cov))
+    x = rng.normal(size=(7, 5))
+    lp, g = f(x)
+    ref = stats.multivariate_normal(mu, cov).logpdf(x)
+    assert np.allclose(lp - lp[0], ref - ref[0], atol=1e-12)
+    for p in range(5):
+        e = np.zeros(5); e[p] = 1e-6
+        assert np.allclose(g[:, p], (f(x + e)[0] - f(x - e)[0]) / 2e-6, atol=1e-7)
+
+
+def test_nuts_transition_leaves_a_gaussian_invariant():
+    # Detailed balance of the multinomial / biased-progressive sampling (R15): with a LARGE fixed step (energy errors of
+    # tens of per cent, so the leaf weights and the subtree acceptance matter) the chain started in the stationary
+    # distribution N(0, 1) must stay there: variance, quartile and tail mass to ~1 %.  A dropped weight, a uniform instead
+    # of the biased subtree choice, or a wrong U-turn sign all fail this.
+    f1 = lambda q: (-0.5 * float(q[0] * q[0]), -q)
+    n_chain, n_tr, eps = 64, 330, 1.3
+    x0 = np.concatenate([S.normals(99, c, 0, S.P_INIT, 1) for c in range(n_chain)])
+    xs = []
+    for c in range(n_chain):
+        q = np.array([x0[c]])
+        lp, g = f1(q)
+        for it in range(n_tr):
+            q, lp, g, acc, n_leaf, div, depth = S.nuts_transition(q, lp, g, eps, np.ones(1), 6, f1, 5, c, it)
+            xs.append(q[0])
+    xs = np.array(xs)
+    n_eff = xs.size / 1.5
+    assert abs(xs.mean()) < 3.0 / np.sqrt(n_eff)
+    assert abs(xs.var() - 1.0) < 3.0 * np.sqrt(2.0 / n_eff)
+    assert abs((np.abs(xs) < 0.6744897501960817).mean() - 0.5) < 3.0 * 0.5 / np.sqrt(n_eff)       # inter-quartile mass
+    assert abs((np.abs(xs) > 1.959963984540054).mean() - 0.05) < 3.0 * np.sqrt(0.05 * 0.95 / n_eff)  # tail mass
