@@ -8,13 +8,27 @@
  * Conventions (all entry points):
  *   - `*_dev` / "device" pointers are raw CUDA device pointers owned by the CALLER (e.g. torch
  *     data_ptr()); "host" pointers are ordinary host memory.  The library never frees caller memory.
- *   - Arrays are row-major, float32 unless stated.  n rows of D = 13 parameters in the order
- *       logM, tau, alpha, beta, F_burst, logT_peak, logT_max, logZ, sigma_logZ, A_V, delta, F_floor, z
- *     (z per BASELINE.json).
+ *   - Arrays are row-major, float32 unless stated.  A parameter row always has SPS_NDIM = 13 slots; the table's model
+ *     (sps_table_desc.model) fixes what they mean and how many of them are SAMPLED (sps_model_ndim):
+ *       SPS_MODEL_DPL13 (the paper's model; 13 sampled):
+ *         logM, tau, alpha, beta, F_burst, logT_peak, logT_max, logZ, sigma_logZ, A_V, delta, F_floor, z
+ *         (z per BASELINE.json configs[1])
+ *       SPS_MODEL_TINY5 (BASELINE.json configs[0]; R19; 4 sampled + the redshift as data):
+ *         logM_star, log10 tau [Gyr], logZ, tau_V, z (slot 4: read, never transformed, never moved by the samplers),
+ *         slots 5-12 ignored
+ *       SPS_MODEL_GAUSS_TEST (a correlated Gaussian target for the samplers; gauss_ndim sampled): theta_0 .. theta_{D-1}
+ *     Slots that are not sampled are ignored on input (except TINY5's z) and written as zero in gradients.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work and
  *     return without synchronising unless stated.
  *   - Every call returns an sps_status; no exception crosses the ABI; sps_last_error() gives a
  *     thread-local message for the last non-OK status.
+ *   - A table is immutable after sps_create_table.  Scratch memory is owned by the library PER (table, stream): calls on
+ *     different streams (from one or several host threads) use different scratch and may overlap; calls on the same
+ *     stream are ordered by the stream and must be issued from one host thread at a time.  Scratch grows on demand
+ *     (growing synchronises that stream) and is freed by sps_destroy_table.
+ *   - obs_sigma must be > 0 everywhere (it divides); with SPS_OPT_CHECK_FINITE set, non-finite parameters or
+ *     observations and non-positive sigmas are reported as SPS_ENONFINITE (a device reduction + one synchronisation per
+ *     call: a debugging aid, off by default so that the hot path never synchronises).
  *   - There is NO CPU fallback: without a compute-capability-10.x device every compute call returns
  *     SPS_EUNSUPPORTED.
  */
@@ -35,9 +49,11 @@ typedef enum {
   SPS_ESHAPE = 2,        /* a size is out of the supported range                      */
   SPS_ECUDA = 3,         /* a CUDA runtime call failed (message has the CUDA string)  */
   SPS_ENOMEM = 4,
-  SPS_EUNSUPPORTED = 5   /* no sm_100 device                                          */
+  SPS_EUNSUPPORTED = 5,  /* no sm_100 device                                          */
+  SPS_ENONFINITE = 6     /* SPS_OPT_CHECK_FINITE found a non-finite input             */
 } sps_status;
 
+enum { SPS_MODEL_TINY5 = 0, SPS_MODEL_DPL13 = 1, SPS_MODEL_GAUSS_TEST = 2 };
 enum { SPS_PATH_EXACT = 0, SPS_PATH_APPROX = 1 };
 enum { SPS_SAMPLER_HMC = 0, SPS_SAMPLER_NUTS = 1 };
 /* Operand format of the exact path's tensor-core contractions (three split products a_lo b_hi + a_hi b_lo + a_hi b_hi,
@@ -63,6 +79,22 @@ typedef struct {
   double H0, Om;               /* flat LCDM for t_obs(z) (R11)                       */
   double log10_mass_unit;      /* M_star is expressed in 10^this Msun so that fluxes are O(1)      */
   int32_t exact_precision;     /* SPS_EXACT_BF16X3 (0, default) or SPS_EXACT_TF32X3                */
+  int32_t model;               /* SPS_MODEL_TINY5 (0) | SPS_MODEL_DPL13 (1) | SPS_MODEL_GAUSS_TEST (2)            */
+  /* Tabulated filters (T(lambda) is a general transmission curve; R4): when filt_offsets != NULL the
+   * Gaussian arrays above are ignored and band b is the curve through the knots offsets[b] .. offsets[b+1]-1 of
+   * (filt_wave_A, filt_trans): observed-frame Angstrom, strictly increasing inside a band, at least 2 and at most 4096
+   * knots per band; linear interpolation between knots, zero outside [first knot, last knot]. */
+  const double*  filt_wave_A;  /* [filt_offsets[n_band]] or NULL                                    */
+  const double*  filt_trans;   /* [filt_offsets[n_band]] or NULL                                    */
+  const int32_t* filt_offsets; /* [n_band + 1] or NULL (Gaussian filters)                           */
+  /* Non-separable weights (R26; SPS_MODEL_DPL13 only): the median of the lognormal MDF of
+   * age bin i is logZ + dlogZ_dlogage (log10 age_i/yr - 9).  0 = the paper's separable model, Eq. (2). */
+  double dlogZ_dlogage;
+  /* SPS_MODEL_GAUSS_TEST: logP(theta) = -1/2 (theta - mu)^T P (theta - mu) over gauss_ndim <= 13 parameters; the grids,
+   * spectra and filters above may be NULL / 0 for this model, and observations are ignored by every call. */
+  int32_t gauss_ndim;
+  const double* gauss_mu;      /* [gauss_ndim]                                                      */
+  const double* gauss_prec;    /* [gauss_ndim][gauss_ndim] symmetric positive definite precision    */
 } sps_table_desc;
 
 /* Per-parameter hyper-parameters, HOST arrays of SPS_NDIM doubles each.
@@ -78,6 +110,21 @@ typedef struct {
  * Synchronises.  On success *out owns all device memory until sps_destroy_table. */
 sps_status sps_create_table(const sps_table_desc* desc, sps_table** out);
 sps_status sps_destroy_table(sps_table* t);
+
+/* Number of sampled parameters of the table's model: 13 (DPL13), 4 (TINY5), gauss_ndim (GAUSS_TEST); -1 for NULL. */
+int32_t sps_model_ndim(const sps_table* t);
+
+/* Library options (process-wide; testing and debugging aids, none is needed for normal use).  Returns SPS_EINVAL for an
+ * unknown option.
+ *   SPS_OPT_CHECK_FINITE   1: sps_weights / sps_photometry / sps_loglike_grad / sps_leapfrog / sps_hmc_run validate their
+ *                             device inputs (one reduction kernel + one synchronisation) and return SPS_ENONFINITE
+ *   SPS_OPT_EXACT_SIMT     1: the exact path runs its fp32 SIMT contraction kernels instead of the tcgen05 ones
+ *   SPS_OPT_APPROX_SIMT    1: the approximate path runs its fp32 SIMT contraction kernel instead of the tcgen05 one
+ *   SPS_OPT_NO_TC_SETUP    1: tables created from now on build no tensor-core operands (SIMT kernels only)
+ *   SPS_OPT_NO_GRAPH       1: sps_hmc_run launches every kernel directly instead of replaying a CUDA graph */
+enum { SPS_OPT_CHECK_FINITE = 0, SPS_OPT_EXACT_SIMT = 1, SPS_OPT_APPROX_SIMT = 2, SPS_OPT_NO_TC_SETUP = 3, SPS_OPT_NO_GRAPH = 4,
+       SPS_OPT_COUNT = 5 };
+sps_status sps_set_option(int option, int value);
 
 /* Copy the c_SSP table to a HOST buffer of n_z*n_age*n_Z*n_band floats (diagnostic; synchronises). */
 sps_status sps_table_cssp(const sps_table* t, float* cssp_host);
@@ -136,6 +183,10 @@ typedef struct {
   uint32_t first_transition;
   const float* eps_in_dev;       /* [n_gal*n_chain]    or NULL */
   const float* inv_mass_in_dev;  /* [n_gal*n_chain,13] or NULL */
+  /* RNG stream of each galaxy: chain k of galaxy g draws from Philox stream gal_id[g]*n_chain + k (NULL: gal_id[g] = g).
+   * Continuing only the unconverged galaxies of an earlier run with their original ids reproduces, bit for
+   * bit, what continuing every galaxy would have given them. */
+  const int32_t* gal_id_dev;     /* [n_gal] or NULL */
 } sps_hmc_config;
 
 /* Per-chain summaries, DEVICE pointers, any may be NULL.  Chain index c = gal*n_chain + chain. */
@@ -149,6 +200,8 @@ typedef struct {
   int32_t* divergences; /* [n_gal*n_chain]    divergent transitions in the sampling phase             */
   float* rhat;          /* [n_gal,13]         Gelman-Rubin statistic over the galaxy's chains */
   float* theta_last;    /* [n_gal*n_chain,13] state of every chain after its last transition (to continue from)     */
+  float* ess;           /* [n_gal,13]         effective sample size by batch means pooled over the galaxy's chains (R25)  */
+  int32_t* depth_hist;  /* [11]               NUTS: kept transitions per final tree depth 0..10       */
 } sps_hmc_summary;
 
 /* sps_hmc_run: n_gal galaxies x n_chain chains of (n_warmup + n_sample) transitions.
@@ -178,6 +231,13 @@ sps_status sps_profile_read(int kernel_id, double* total_ms, int64_t* timed_laun
  * under some filter's 5-sigma support at the row's redshift (everything else contributes exactly zero to Eq. 4 and is
  * skipped).  bench.py's tensor roofline counts 3 x 2 x n_age*n_Z flop per pair and pass.  Synchronises. */
 sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavelength_pairs);
+
+/* Throughput of one execution pipe, measured now on the current device (a microbenchmark of ~10 ms; synchronises):
+ * SPS_PEAK_MUFU: ex2.approx operations per second (the special-function units the SFH quadrature is bound by),
+ * SPS_PEAK_FFMA: fp32 fused multiply-adds per second.  bench.py's "alu" roofline uses them as denominators, so that
+ * they are taken at the clocks of the same run. */
+enum { SPS_PEAK_MUFU = 0, SPS_PEAK_FFMA = 1 };
+sps_status sps_measure_peak(int what, double* per_second, void* stream);
 
 /* Number of kernels this library launched since load (for bench.py's gpu_launches). */
 int64_t sps_launch_count(void);

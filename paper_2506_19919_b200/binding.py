@@ -16,10 +16,13 @@ NDIM = 13
 PATH_EXACT, PATH_APPROX = 0, 1
 SAMPLER_HMC, SAMPLER_NUTS = 0, 1
 EXACT_BF16X3, EXACT_TF32X3 = 0, 1
+MODEL_TINY5, MODEL_DPL13, MODEL_GAUSS_TEST = 0, 1, 2
+OPT_CHECK_FINITE, OPT_EXACT_SIMT, OPT_APPROX_SIMT, OPT_NO_TC_SETUP, OPT_NO_GRAPH = 0, 1, 2, 3, 4
+STATUS_ENONFINITE = 6
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
            "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
-           "sps_last_error", "sps_version", "sps_exact_last_work")
+           "sps_last_error", "sps_version", "sps_exact_last_work", "sps_model_ndim", "sps_set_option", "sps_measure_peak")
 
 
 class SpsError(RuntimeError):
@@ -31,7 +34,10 @@ class _TableDesc(C.Structure):
                 ("log10_age_yr", C.POINTER(C.c_double)), ("log10_Z", C.POINTER(C.c_double)), ("wave_A", C.POINTER(C.c_double)),
                 ("ssp", C.POINTER(C.c_float)), ("filt_mu_A", C.POINTER(C.c_double)), ("filt_sigma_A", C.POINTER(C.c_double)),
                 ("z_min", C.c_double), ("z_max", C.c_double), ("H0", C.c_double), ("Om", C.c_double),
-                ("log10_mass_unit", C.c_double), ("exact_precision", C.c_int32)]
+                ("log10_mass_unit", C.c_double), ("exact_precision", C.c_int32), ("model", C.c_int32),
+                ("filt_wave_A", C.POINTER(C.c_double)), ("filt_trans", C.POINTER(C.c_double)), ("filt_offsets", C.POINTER(C.c_int32)),
+                ("dlogZ_dlogage", C.c_double), ("gauss_ndim", C.c_int32), ("gauss_mu", C.POINTER(C.c_double)),
+                ("gauss_prec", C.POINTER(C.c_double))]
 
 
 class _Prior(C.Structure):
@@ -42,11 +48,12 @@ class _HmcConfig(C.Structure):
     _fields_ = [("sampler", C.c_int32), ("path", C.c_int32), ("n_chain", C.c_int32), ("n_warmup", C.c_int32),
                 ("n_sample", C.c_int32), ("n_leapfrog", C.c_int32), ("max_depth", C.c_int32), ("eps0", C.c_float),
                 ("target_accept", C.c_float), ("seed", C.c_uint64),
-                ("first_transition", C.c_uint32), ("eps_in", C.c_void_p), ("inv_mass_in", C.c_void_p)]
+                ("first_transition", C.c_uint32), ("eps_in", C.c_void_p), ("inv_mass_in", C.c_void_p), ("gal_id", C.c_void_p)]
 
 
 class _HmcSummary(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last")]
+    _fields_ = [(n, C.c_void_p) for n in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last",
+                                          "ess", "depth_hist")]
 
 
 _lib = None
@@ -63,13 +70,16 @@ def lib():
         L.sps_last_error.restype = C.c_char_p
         L.sps_version.restype = C.c_char_p
         L.sps_launch_count.restype = C.c_int64
+        L.sps_model_ndim.restype = C.c_int32
         _lib = L
     return _lib
 
 
 def _check(status: int, what: str):
     if status != 0:
-        raise SpsError(f"{what} failed with status {status}: {lib().sps_last_error().decode()}")
+        e = SpsError(f"{what} failed with status {status}: {lib().sps_last_error().decode()}")
+        e.status = status
+        raise e
 
 
 def _dptr(t):
@@ -103,21 +113,42 @@ class PriorHandle:
 
 
 class Table:
-    """Owner of an sps_table handle."""
+    """Owner of an sps_table handle.  model = MODEL_DPL13 (the paper's 13-parameter model), MODEL_TINY5 (BASELINE.json
+    configs[0]) or MODEL_GAUSS_TEST (grid = None, gauss = (mu [D], precision [D, D]))."""
 
-    def __init__(self, grid, exact_precision=0):
-        self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z = grid.n_age, grid.n_Z, grid.n_wave, grid.n_band, grid.n_z
-        keep = [_f64(grid.log10_age_yr), _f64(grid.log10_Z), _f64(grid.wave_A),
-                np.ascontiguousarray(grid.ssp, dtype=np.float32), _f64(grid.filt_mu_A), _f64(grid.filt_sigma_A)]
-        assert keep[3].shape == (self.n_age * self.n_Z, self.n_wave)
+    def __init__(self, grid, exact_precision=0, model=MODEL_DPL13, gauss=None, dlogZ_dlogage=0.0):
         dp = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
-        d = _TableDesc(self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z, dp(keep[0]), dp(keep[1]), dp(keep[2]),
-                       keep[3].ctypes.data_as(C.POINTER(C.c_float)), dp(keep[4]), dp(keep[5]),
-                       float(grid.z_min), float(grid.z_max), float(grid.H0), float(grid.Om), float(grid.log10_mass_unit),
-                       int(exact_precision))
+        d = _TableDesc()
+        d.model = int(model); d.exact_precision = int(exact_precision); d.dlogZ_dlogage = float(dlogZ_dlogage)
+        keep = []
+        if model == MODEL_GAUSS_TEST:
+            mu, prec = _f64(gauss[0]), _f64(gauss[1])
+            assert prec.shape == (mu.size, mu.size)
+            keep += [mu, prec]
+            d.gauss_ndim = mu.size; d.gauss_mu = dp(mu); d.gauss_prec = dp(prec)
+            self.n_age = self.n_Z = self.n_wave = self.n_band = self.n_z = 0
+        else:
+            self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z = grid.n_age, grid.n_Z, grid.n_wave, grid.n_band, grid.n_z
+            keep += [_f64(grid.log10_age_yr), _f64(grid.log10_Z), _f64(grid.wave_A), np.ascontiguousarray(grid.ssp, dtype=np.float32)]
+            assert keep[3].shape == (self.n_age * self.n_Z, self.n_wave)
+            d.n_age, d.n_Z, d.n_wave, d.n_band, d.n_z = self.n_age, self.n_Z, self.n_wave, self.n_band, self.n_z
+            d.log10_age_yr, d.log10_Z, d.wave_A = dp(keep[0]), dp(keep[1]), dp(keep[2])
+            d.ssp = keep[3].ctypes.data_as(C.POINTER(C.c_float))
+            tab = getattr(grid, "filt_tab", None)
+            if tab is None:
+                mu, sg = _f64(grid.filt_mu_A), _f64(grid.filt_sigma_A)
+                keep += [mu, sg]
+                d.filt_mu_A, d.filt_sigma_A = dp(mu), dp(sg)
+            else:
+                fw, ft, fo = _f64(tab[0]), _f64(tab[1]), np.ascontiguousarray(tab[2], dtype=np.int32)
+                keep += [fw, ft, fo]
+                d.filt_wave_A, d.filt_trans, d.filt_offsets = dp(fw), dp(ft), fo.ctypes.data_as(C.POINTER(C.c_int32))
+            d.z_min, d.z_max, d.H0, d.Om = float(grid.z_min), float(grid.z_max), float(grid.H0), float(grid.Om)
+            d.log10_mass_unit = float(grid.log10_mass_unit)
         h = C.c_void_p()
         _check(lib().sps_create_table(C.byref(d), C.byref(h)), "sps_create_table")
         self.handle = h
+        self.n_dim = int(lib().sps_model_ndim(h))
 
     def close(self):
         if getattr(self, "handle", None):
@@ -131,8 +162,12 @@ class Table:
             pass
 
 
-def sps_create_table(grid, exact_precision=EXACT_BF16X3) -> Table:
-    return Table(grid, exact_precision)
+def sps_create_table(grid, exact_precision=EXACT_BF16X3, model=MODEL_DPL13, gauss=None, dlogZ_dlogage=0.0) -> Table:
+    return Table(grid, exact_precision, model, gauss, dlogZ_dlogage)
+
+
+def sps_set_option(option: int, value: int):
+    _check(lib().sps_set_option(int(option), int(value)), "sps_set_option")
 
 
 def sps_table_cssp(table: Table) -> np.ndarray:
@@ -166,7 +201,7 @@ def sps_photometry(table, prior, path, theta, unbounded=True, flux_bar=None):
 def sps_loglike_grad(table, prior, path, theta_unb, obs_flux, obs_sigma, gal_of_row=None, want_grad=True, out=None):
     n = theta_unb.shape[0]
     logp, grad = out if out is not None else (_new((n,), like=theta_unb), _new((n, NDIM), like=theta_unb) if want_grad else None)
-    _check(lib().sps_loglike_grad(table.handle, prior.ref(), int(path), _dptr(theta_unb), C.c_int64(n), _dptr(gal_of_row),
+    _check(lib().sps_loglike_grad(table.handle, prior.ref() if prior is not None else None, int(path), _dptr(theta_unb), C.c_int64(n), _dptr(gal_of_row),
                                   _dptr(obs_flux), _dptr(obs_sigma), _dptr(logp), _dptr(grad), _stream()), "sps_loglike_grad")
     return logp, grad
 
@@ -175,7 +210,7 @@ def sps_leapfrog(table, prior, path, theta0, p0, eps, inv_mass, obs_flux, obs_si
     n = theta0.shape[0]
     traj = _new((n_steps, n, 2, NDIM), like=theta0)
     logp = _new((n_steps, n), like=theta0)
-    _check(lib().sps_leapfrog(table.handle, prior.ref(), int(path), _dptr(theta0), _dptr(p0), _dptr(eps), _dptr(inv_mass),
+    _check(lib().sps_leapfrog(table.handle, prior.ref() if prior is not None else None, int(path), _dptr(theta0), _dptr(p0), _dptr(eps), _dptr(inv_mass),
                               C.c_int64(n), _dptr(gal_of_row), _dptr(obs_flux), _dptr(obs_sigma), C.c_int32(n_steps),
                               _dptr(traj), _dptr(logp), _stream()), "sps_leapfrog")
     return traj, logp
@@ -183,21 +218,26 @@ def sps_leapfrog(table, prior, path, theta0, p0, eps, inv_mass, obs_flux, obs_si
 
 def sps_hmc_run(table, prior, obs_flux, obs_sigma, *, sampler=SAMPLER_HMC, path=PATH_APPROX, n_chain=4, n_warmup=500,
                 n_sample=500, n_leapfrog=16, max_depth=8, eps0=0.05, target_accept=0.8, seed=1, path_of_gal=None,
-                theta0=None, keep_samples=False, first_transition=0, eps_in=None, inv_mass_in=None):
+                theta0=None, keep_samples=False, first_transition=0, eps_in=None, inv_mass_in=None, gal_id=None, n_gal=None):
+    """obs_flux / obs_sigma [n_gal, n_band] (None for MODEL_GAUSS_TEST, which takes n_gal = number of independent groups of
+    n_chain chains)."""
     import torch
-    n_gal = obs_flux.shape[0]
+    n_gal = obs_flux.shape[0] if obs_flux is not None else int(n_gal)
     nc = n_gal * n_chain
-    dev = obs_flux.device
+    dev = obs_flux.device if obs_flux is not None else torch.device("cuda")
     f32 = lambda *s: torch.zeros(s, dtype=torch.float32, device=dev)
     i32 = lambda *s: torch.zeros(s, dtype=torch.int32, device=dev)
     out = dict(mean=f32(nc, NDIM), sd=f32(nc, NDIM), accept=f32(nc), eps=f32(nc), inv_mass=f32(nc, NDIM),
-               n_leapfrog=i32(nc), divergences=i32(nc), rhat=f32(n_gal, NDIM), theta_last=f32(nc, NDIM))
+               n_leapfrog=i32(nc), divergences=i32(nc), rhat=f32(n_gal, NDIM), theta_last=f32(nc, NDIM), ess=f32(n_gal, NDIM),
+               depth_hist=i32(11))
     samples = f32(nc, n_sample, NDIM) if keep_samples else None
     cfg = _HmcConfig(int(sampler), int(path), int(n_chain), int(n_warmup), int(n_sample), int(n_leapfrog), int(max_depth),
                      float(eps0), float(target_accept), int(seed), int(first_transition),
-                     eps_in.data_ptr() if eps_in is not None else None, inv_mass_in.data_ptr() if inv_mass_in is not None else None)
-    summ = _HmcSummary(*[out[k].data_ptr() for k in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last")])
-    _check(lib().sps_hmc_run(table.handle, prior.ref(), C.byref(cfg), _dptr(obs_flux), _dptr(obs_sigma), C.c_int64(n_gal),
+                     eps_in.data_ptr() if eps_in is not None else None, inv_mass_in.data_ptr() if inv_mass_in is not None else None,
+                     gal_id.data_ptr() if gal_id is not None else None)
+    summ = _HmcSummary(*[out[k].data_ptr() for k in ("mean", "sd", "accept", "eps", "inv_mass", "n_leapfrog", "divergences", "rhat", "theta_last",
+                                                     "ess", "depth_hist")])
+    _check(lib().sps_hmc_run(table.handle, prior.ref() if prior is not None else None, C.byref(cfg), _dptr(obs_flux), _dptr(obs_sigma), C.c_int64(n_gal),
                              _dptr(path_of_gal), _dptr(theta0), _dptr(samples), C.byref(summ), _stream()), "sps_hmc_run")
     if keep_samples:
         out["samples"] = samples
@@ -216,6 +256,13 @@ def sps_exact_last_work(table) -> int:
     v = C.c_int64()
     _check(lib().sps_exact_last_work(table.handle, C.byref(v)), "sps_exact_last_work")
     return int(v.value)
+
+
+def sps_measure_peak(what: str) -> float:
+    """'mufu' (ex2.approx / s) or 'ffma' (fp32 FMA / s), measured now on the current device."""
+    v = C.c_double()
+    _check(lib().sps_measure_peak({"mufu": 0, "ffma": 1}[what], C.byref(v), _stream()), "sps_measure_peak")
+    return float(v.value)
 
 
 def sps_launch_count() -> int:

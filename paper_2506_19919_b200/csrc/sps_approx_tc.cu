@@ -20,6 +20,15 @@
 #include <cmath>
 #include <cstring>
 #include "sps_internal.h"
+#include "sps_ptx.cuh"
+
+struct ApproxTc {
+  __half *C1_hi, *C1_lo;      // [n_cells * 256][128]  pass-1 B operand: row = (cell, entry), K = age contiguous
+  __half *C2_hi, *C2_lo;      // [n_cells * 128][256]  pass-2 B operand: row = (cell, age),   K = entry contiguous
+  CUtensorMap m1_hi, m1_lo, m2_hi, m2_lo;
+  float* Cm;                         // [n_cells][128] power of two >= max_e |c_t[i][e]| of each (cell, age): a_i Cm_i and c_t / Cm_i are what is split
+  float sD;                          // power of two: D_t sD / Cm_i <= 1 everywhere
+};
 
 namespace {
 
@@ -39,52 +48,13 @@ constexpr float H_TOP = 16384.f;                // operands are scaled so that t
 // band counts the kernel is instantiated for (other tables use the SIMT kernel of sps_kernels.cu)
 #define SPS_APPROX_TC_BANDS(X) X(3) X(10) X(12)
 
-struct ApproxTc {
-  __half *C1_hi, *C1_lo;      // [n_cells * 256][128]  pass-1 B operand: row = (cell, entry), K = age contiguous
-  __half *C2_hi, *C2_lo;      // [n_cells * 128][256]  pass-2 B operand: row = (cell, age),   K = entry contiguous
-  CUtensorMap m1_hi, m1_lo, m2_hi, m2_lo;
-  float* Cm;                         // [n_cells][128] power of two >= max_e |c_t[i][e]| of each (cell, age): a_i Cm_i and c_t / Cm_i are what is split
-  float sD;                          // power of two: D_t sD / Cm_i <= 1 everywhere
-  int sm_count;
-};
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory"); }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory"); }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t ok = 0;
-  while (!ok)
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-               ::"r"(dst), "l"(map), "r"(bar), "r"(c_inner), "r"(c_outer) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) { asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory"); }
-__device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-               ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-}
 // K-major operand tile, 128-byte rows, SWIZZLE_128B: 8-row atoms of 1024 B stacked along M/N
-__device__ __forceinline__ uint64_t desc_sw128(uint32_t saddr) {
-  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)1 << 16;
-  d |= (uint64_t)(1024 >> 4) << 32;
-  d |= (uint64_t)1 << 46;
-  d |= (uint64_t)2 << 61;
-  return d;
-}
+__device__ __forceinline__ uint64_t desc_sw128(uint32_t saddr) { return umma_desc_kmajor(saddr, 128); }
 // byte offset of the 16-byte chunk `c` (0..7) of row r in a 128-byte-swizzled tile (what TMA writes and tcgen05 reads)
 __device__ __forceinline__ uint32_t sw128_off(int r, int c) { return (uint32_t)((r >> 3) * 1024 + (r & 7) * 128 + ((c ^ (r & 7)) << 4)); }
-#define TLD16(taddr, v)                                                                                                \
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
-               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
-                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
-               : "r"(taddr))
-__device__ __forceinline__ void tld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+#define TLD16(taddr, v) TMEM_LD16(taddr, v)
+__device__ __forceinline__ void tld_wait() { tmem_ld_wait(); }
 
 __device__ __forceinline__ void split8(const float* v, uint4& hi, uint4& lo) {
   __half h[8], l[8];
@@ -132,12 +102,6 @@ __global__ void build_c_operands_kernel(TableDev T, const float* __restrict__ Cm
 constexpr uint32_t OFF_B = REG_AV, OFF_BAR = REG_AV + REG_B;
 enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M1, N_BARS };
 
-#ifdef SPS_ATC_TIMING
-__device__ long long g_atc_t[16];
-#define TSTAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { const long long t_now = clock64(); g_atc_t[i] += t_now - t_prev; t_prev = t_now; } } while (0)
-#else
-#define TSTAMP(i)
-#endif
 
 struct ApproxArgs {
   int64_t n;
@@ -179,7 +143,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
   if (threadIdx.x == 0) {
     mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), 2 * TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
     mbar_init(BAR(BAR_V0), 2 * TM); mbar_init(BAR(BAR_M1), 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_fence_init();
   }
   if (warp == 8) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bars + 128u), "n"(512) : "memory");
@@ -301,9 +265,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       const int rw = rw_next;
       const int64_t gal = gal_next;
       const int n_rows = r_end - r_begin;
-#ifdef SPS_ATC_TIMING
-      long long t_prev = clock64();
-#endif
       // the next tile's rows follow this tile's in `order`
       int r_end_next = r_end;
       if (w + 1 < w_end) {
@@ -326,9 +287,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       {
         const int kb = lane >> 4, c = (lane & 15) >> 1, half = lane & 1;
         const float4 cm4 = __ldg(reinterpret_cast<const float4*>(G.Cm + (int64_t)cell * NA) + lane);
-        TSTAMP(12);
         asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");        // every row thread is done with the previous tile's shared arrays
-        TSTAMP(13);
         if (h == 0) cm_s[r] = __ldg(G.Cm + (int64_t)cell * NA + r) * (1.f / H_TOP);
         float4 av[16];
 #pragma unroll
@@ -358,7 +317,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           *reinterpret_cast<uint2*>(gbase + 2 * TILE_A + off) = *reinterpret_cast<const uint2*>(ll);
         }
       }
-      TSTAMP(14);
       if (rw_next >= 0) {                                   // the next tile's weights start their way into L2
         if (h == 0) {
           const char* np_ = reinterpret_cast<const char*>(B.a + (int64_t)rw_next * ROW_A_STRIDE);
@@ -368,9 +326,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         if (!G.flux_bar) gal_next = G.gal_of_row ? __ldg(G.gal_of_row + rw_next) : rw_next;
       }
       tc_fence_before();                                    // the previous tile's TMEM reads are complete
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      fence_proxy_async_smem();
       mbar_arrive(BAR(BAR_A));
-      TSTAMP(0);
       asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");            // cm_s and rs_s of this tile are complete
       const float u0 = 1.f / (H_TOP * rs_s[r]), u1 = u0 * G.inv_sD;       // P^(s) back to table units
       const float f = sc.zfrac, Mn = sc.Mn, zp = 1.f + sc.z;
@@ -379,10 +336,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       float S0[NB], S1[NB];
 #pragma unroll
       for (int b = 0; b < NB; ++b) S0[b] = S1[b] = 0.f;
-      TSTAMP(1);
       mbar_wait(BAR(BAR_P), ph);
       tc_fence_after();
-      TSTAMP(2);
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         if ((c & 1) == h && 16 * c < E) {
@@ -400,7 +355,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           }
         }
       }
-      TSTAMP(3);
       // ---- band step (Eq. 6, dust at lambda_eff / (1+z) R14; Gaussian likelihood).  A rolled loop over this
       //      thread's bands keeps the kernel inside the instruction cache; per-band inputs and sbar_b sit in a scratch column
       //      of the A / V region (pass 1 has retired, V is written later).
@@ -420,7 +374,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       for (int b = h; b < NB; b += 2) {
         float F, F_av, F_del, F_fl, F_lam;
         const float lam_r = T.lam_eff[b] * izp;
-        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
+        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam, T.model == SPS_MODEL_TINY5);
         const float s1 = scr[(32 + b) * TM] + scr[(48 + b) * TM];
         const float Sint = (scr[b * TM] + scr[(16 + b) * TM]) + f * s1;
         const float flux = F * Mn * Sint;
@@ -447,7 +401,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           out->delta_bar = v_de + red_s[4 * TM + r]; out->Ffloor_bar = v_fl + red_s[5 * TM + r];
         }
       }
-      TSTAMP(4);
       if (!G.want_grad) { if (w + 1 < w_end) load_row(rw_next, gal_next); continue; }
       // ---- sweep 2 over P (this thread's chunks): m_bar_j = sum_b sbar_b (P^(0) + f P^(1))[j NB + b] ----
       float sbar[NB];
@@ -477,7 +430,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
           for (int j = 0; j < 16; ++j) mb_s[j * TM + r] = mb[j];
         }
       }
-      TSTAMP(5);
       tc_fence_before();
       asm volatile("bar.sync 1, %0;" ::"n"(2 * TM) : "memory");            // partial m_bar parked; every thread has read its scratch: V may overwrite it
       if (h == 0 && rw >= 0) {
@@ -534,15 +486,13 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
             *reinterpret_cast<uint4*>(gbase + 2 * TILE_A + off) = vl;
           }
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_proxy_async_smem();
         mbar_arrive(BAR(BAR_V0));
       }
-      TSTAMP(9);
       // ---- a_bar from TMEM (main + cross-term accumulators), this thread's 64 columns ----
       if (w + 1 < w_end) load_row(rw_next, gal_next);       // the next tile's row inputs travel while pass 2 runs
       mbar_wait(BAR(BAR_M1), ph);
       tc_fence_after();
-      TSTAMP(10);
       // thread = (row, half of the ages) reads its TMEM lane and parks the scaled values in the (free) A / V region, 16-byte
       // chunks XOR-swizzled by the row; then each warp writes 16 rows to global memory 512 contiguous bytes at a time
       const float ua = 1.f / sv, fa = f * G.inv_sD;      // a_bar_i = (acc^(0)_i + f / sD acc^(1)_i) Cm_i / (2^14 sv)
@@ -573,7 +523,6 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         const int rr = (warp & 3) * 32 + 16 * h + t;
         if (row_t >= 0) reinterpret_cast<float4*>(B.a_bar + (int64_t)row_t * ROW_A_STRIDE)[lane] = stage[rr * 32 + (lane ^ (rr & 7))];
       }
-      TSTAMP(11);
     }
   }
   tc_fence_before();
@@ -586,9 +535,7 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
 }
 
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+typedef SpsEncodeTiledFn EncodeTiledFn;
 
 // [rows][cols] fp16 row-major -> boxes of box_rows x 64 elements (128 bytes), 128-byte swizzle
 sps_status make_map_f16(EncodeTiledFn enc, CUtensorMap* m, const void* ptr, uint64_t rows, uint64_t cols, uint32_t box_rows) {
@@ -603,33 +550,24 @@ sps_status make_map_f16(EncodeTiledFn enc, CUtensorMap* m, const void* ptr, uint
 }
 
 template <int NB>
-sps_status launch_nb(const ApproxTc* S, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
+sps_status launch_nb(const ApproxTc* S, int sm_count, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
   if (configure_only)
     return sps_check_cuda(cudaFuncSetAttribute(approx_tc_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TC), "approximate tensor-core kernel shared memory opt-in");
-  approx_tc_kernel<NB><<<S->sm_count, THREADS_TC, SMEM_TC, s>>>(T, G, B, S->m1_hi, S->m1_lo, S->m2_hi, S->m2_lo);
+  approx_tc_kernel<NB><<<sm_count, THREADS_TC, SMEM_TC, s>>>(T, G, B, S->m1_hi, S->m1_lo, S->m2_hi, S->m2_lo);
   return SPS_OK;
 }
-sps_status dispatch(const ApproxTc* S, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
+sps_status dispatch(const ApproxTc* S, int sm_count, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
   switch (T.n_band) {
-#define CASE(NB) case NB: return launch_nb<NB>(S, T, G, B, s, configure_only);
+#define CASE(NB) case NB: return launch_nb<NB>(S, sm_count, T, G, B, s, configure_only);
     SPS_APPROX_TC_BANDS(CASE)
 #undef CASE
     default: return SPS_EUNSUPPORTED;
   }
 }
-int g_force_simt_approx = 0;
 
 }  // namespace
 
-extern "C" void sps_debug_approx_simt(int on) { g_force_simt_approx = on; }
-#ifdef SPS_ATC_TIMING
-extern "C" void sps_debug_atc_timing(long long* out16, int reset) {
-  cudaMemcpyFromSymbol(out16, g_atc_t, sizeof(long long) * 16);
-  if (reset) { long long z[16] = {0}; cudaMemcpyToSymbol(g_atc_t, z, sizeof(z)); }
-}
-#endif
-
-bool sps_approx_tc_active(const sps_table* t) { return t->approx_tc != nullptr && !g_force_simt_approx; }
+bool sps_approx_tc_active(const sps_table* t) { return t->approx_tc != nullptr && !sps_option(SPS_OPT_APPROX_SIMT); }
 
 // Table operands of the tensor-core contraction; leaves t->approx_tc null (SIMT kernel) for shapes outside its range.
 sps_status sps_approx_tc_setup(sps_table* t) {
@@ -640,16 +578,11 @@ sps_status sps_approx_tc_setup(sps_table* t) {
   SPS_APPROX_TC_BANDS(CASE)
 #undef CASE
   if (!band_ok || T.n_Z * T.n_band > 128 || T.n_age > NA || T.n_Z > 16 || 2 * T.n_z > BINS_S) return SPS_OK;
-  void* fn = nullptr;
-  cudaDriverEntryPointQueryResult qr;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
-    cudaGetLastError();
-    sps_set_error("cuTensorMapEncodeTiled is not available from this driver");
-    return SPS_EUNSUPPORTED;
-  }
+  if (sps_option(SPS_OPT_NO_TC_SETUP)) return SPS_OK;
+  EncodeTiledFn enc = sps_tensor_map_encoder();
+  if (!enc) return SPS_EUNSUPPORTED;
   ApproxTc* S = new ApproxTc();
   memset(S, 0, sizeof(*S));
-  int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&S->sm_count, cudaDevAttrMultiProcessorCount, dev);
   const int n_cells = T.n_z - 1;
   const size_t elems = (size_t)n_cells * NE * NA;
   sps_status st = SPS_OK;
@@ -675,19 +608,18 @@ sps_status sps_approx_tc_setup(sps_table* t) {
     sps_count_launch(2);
     st = sps_check_cuda(cudaDeviceSynchronize(), "approximate-path operand build");
   }
-  EncodeTiledFn enc = (EncodeTiledFn)fn;
   if (st == SPS_OK) st = make_map_f16(enc, &S->m1_hi, S->C1_hi, (uint64_t)n_cells * NE, NA, NE);
   if (st == SPS_OK) st = make_map_f16(enc, &S->m1_lo, S->C1_lo, (uint64_t)n_cells * NE, NA, NE);
   if (st == SPS_OK) st = make_map_f16(enc, &S->m2_hi, S->C2_hi, (uint64_t)n_cells * NA, NE, NA);
   if (st == SPS_OK) st = make_map_f16(enc, &S->m2_lo, S->C2_lo, (uint64_t)n_cells * NA, NE, NA);
-  if (st == SPS_OK) st = dispatch(S, T, ApproxArgs(), RowBuffers(), 0, true);
+  if (st == SPS_OK) st = dispatch(S, t->sm_count, T, ApproxArgs(), RowBuffers(), 0, true);
   t->approx_tc = S;
   if (st != SPS_OK) sps_approx_tc_teardown(t);
   return st;
 }
 
 void sps_approx_tc_teardown(sps_table* t) {
-  ApproxTc* S = reinterpret_cast<ApproxTc*>(t->approx_tc);
+  ApproxTc* S = t->approx_tc;
   if (!S) return;
   void* ptrs[] = {S->C1_hi, S->C1_lo, S->C2_hi, S->C2_lo, S->Cm};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -695,18 +627,18 @@ void sps_approx_tc_teardown(sps_table* t) {
   t->approx_tc = nullptr;
 }
 
-sps_status sps_approx_tc_contract(sps_table* t, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
+sps_status sps_approx_tc_contract(const sps_table* t, Workspace& ws, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
                                   const float* obs_sigma, const float* flux_bar, bool want_grad, cudaStream_t s) {
   if (n <= 0) return SPS_OK;
-  const ApproxTc* S = reinterpret_cast<const ApproxTc*>(t->approx_tc);
+  const ApproxTc* S = t->approx_tc;
   const TableDev& T = t->dev;
-  approx_group_rows(T, n, rows, t->rows, TM, s);
+  approx_group_rows(T, n, rows, ws.rows, TM, s);
   ApproxArgs G;
-  G.n = n; G.order = t->rows.order; G.bins = t->rows.bins; G.gal_of_row = gal_of_row; G.obs_flux = obs_flux; G.obs_sigma = obs_sigma;
+  G.n = n; G.order = ws.rows.order; G.bins = ws.rows.bins; G.gal_of_row = gal_of_row; G.obs_flux = obs_flux; G.obs_sigma = obs_sigma;
   G.flux_bar = flux_bar; G.want_grad = want_grad ? 1 : 0;
   G.Cm = S->Cm; G.inv_sD = 1.f / S->sD;
   sps_prof_begin(SPS_K_APPROX, s);
-  sps_status st = dispatch(S, T, G, t->rows, s, false);
+  sps_status st = dispatch(S, t->sm_count, T, G, ws.rows, s, false);
   sps_prof_end(SPS_K_APPROX, s);
   sps_count_launch();
   if (st != SPS_OK) return st;

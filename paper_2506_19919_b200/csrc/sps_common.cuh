@@ -11,11 +11,28 @@
 #define SPS_MAX_BAND 16
 #define SPS_AGE_PER_LANE 4          // ceil(SPS_MAX_AGE / 32)
 #define FULL_MASK 0xffffffffu
+#define SPS_FTAB_BINS 1024          // index bins per tabulated filter
+#define SPS_FTAB_MAX_KNOTS 4096     // knots per tabulated filter
+
+// Tabulated filter curves (R4: linear interpolation between knots, zero outside the support).  A lookup finds the
+// segment through a uniform index over the band's support (first[b][bin] = the segment holding the bin's left end) and
+// then walks right while lambda is past the segment's end.
+struct FilterTab {
+  const float4* knots;        // [n_knot] {w, t, slope to the next knot, w_next}; a band's last knot: slope 0, w_next = +huge
+  const int* first;           // [n_band][SPS_FTAB_BINS]
+  float lo[SPS_MAX_BAND], hi[SPS_MAX_BAND], inv_d[SPS_MAX_BAND];
+  int last[SPS_MAX_BAND];     // the band's last segment (index of the knot before its last knot)
+};
 
 // ---------------------------------------------------------------------------------------------
 // device-side view of a table (passed to kernels by value; arrays live in device memory)
 // ---------------------------------------------------------------------------------------------
 struct TableDev {
+  int model, n_dim;                            // SPS_MODEL_*; number of sampled parameters
+  int filt_tab;                                // 1: tabulated filters (ft), 0: Gaussian (filt_mu, filt_sigma)
+  float agez_gamma;                            // R26: d(median logZ) / d(log10 age); 0 = separable weights
+  const float* gauss;                          // SPS_MODEL_GAUSS_TEST: [13] mu then [13][13] precision (row stride 13)
+  FilterTab ft;
   int n_age, n_Z, n_wave, n_band, n_z, K;     // K = n_age * n_Z
   int n_wave_pad;                              // n_wave rounded up for the tensor-core tiles
   int cs_stride;                               // floats between consecutive ages in a c_SSP slice (n_Z*n_band padded)
@@ -50,6 +67,9 @@ struct TableDev {
   double tz_lo, tz_inv_h;
   int tz_n;
   float log10_mass_unit;
+  // exact path: bound of a band sum per unit M_star (largest bolometric integral of an SSP x largest transmission) and the
+  // headroom bits of the z partial (sps_exact.cuh: fixed-point band sums)
+  float part_bound; int part_shift_z;
 };
 
 struct PriorDev {
@@ -108,6 +128,17 @@ template <int N> __device__ __forceinline__ float warp_sum_multi(float (&v)[N]) 
 }
 template <int N> __device__ __forceinline__ constexpr int warp_multi_holder(int k) {
   return N == 8 ? 16 * ((k >> 2) & 1) + 8 * ((k >> 1) & 1) + 4 * (k & 1) : 16 * ((k >> 1) & 1) + 8 * (k & 1);
+}
+
+// T_b(lambda_obs) and dT_b/dlambda_obs of a tabulated filter
+__device__ __forceinline__ void filter_tab_eval(const FilterTab& F, int b, float lam, float& Tv, float& dT) {
+  Tv = 0.f; dT = 0.f;
+  if (!(lam >= F.lo[b]) || !(lam <= F.hi[b])) return;
+  const int bin = min((int)((lam - F.lo[b]) * F.inv_d[b]), SPS_FTAB_BINS - 1);
+  int seg = __ldg(F.first + b * SPS_FTAB_BINS + bin);
+  float4 k = __ldg(F.knots + seg);
+  while (lam >= k.w && seg < F.last[b]) { ++seg; k = __ldg(F.knots + seg); }
+  Tv = fmaf(lam - k.x, k.z, k.y); dT = k.z;
 }
 
 // launch counter (host side)

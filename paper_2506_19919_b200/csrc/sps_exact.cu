@@ -34,12 +34,20 @@ __device__ __forceinline__ void dust_tab(float k0, float dr, float l2r, float AV
   F = Ffl + (1.f - Ffl) * Tt; F_av = dF * A_av; F_del = dF * A_del; F_fl = 1.f - Tt;
 }
 
+// T_b(lam_obs) and dT_b/dlam_obs: Gaussian truncated at 5 sigma (R4) or tabulated curve
+__device__ __forceinline__ void filter_eval(const TableDev& T, int b, float lam_obs, float& Tb, float& dTb) {
+  if (T.filt_tab) { filter_tab_eval(T.ft, b, lam_obs, Tb, dTb); return; }
+  const float x = (lam_obs - T.filt_mu[b]) / T.filt_sigma[b];
+  Tb = 0.f; dTb = 0.f;
+  if (fabsf(x) <= 5.f) { Tb = expf(-0.5f * x * x); dTb = -Tb * x / T.filt_sigma[b]; }
+}
+
 // ---- forward SIMT: 64 rows x 64 wavelengths per CTA, 4x4 per thread ---------------------------------
 #define XB_M 64
 #define XB_N 64
 #define XB_K 16
 __global__ void __launch_bounds__(256) exact_fwd_simt_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B,
-                                                             const float* __restrict__ W, int ldw, float* __restrict__ part /*[n][5][16]*/) {
+                                                             const float* __restrict__ W, int ldw, long long* __restrict__ part /*[n][5][16]*/) {
   __shared__ float As[XB_K][XB_M + 4], Bs[XB_K][XB_N + 4];
   __shared__ float red[5][SPS_MAX_BAND][XB_M + 1];
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;          // tx: wavelength group, ty: row group
@@ -87,11 +95,12 @@ __global__ void __launch_bounds__(256) exact_fwd_simt_kernel(TableDev T, int64_t
       dust_tab(T.k0[k], T.drude[k], T.l2r[k], sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl);
       const float lam = T.wave[k], Sd = acc[i][j] * T.dlam[k];
       for (int b = 0; b < T.n_band; ++b) {
-        const float x = (lam * zp - T.filt_mu[b]) / T.filt_sigma[b];
-        if (fabsf(x) <= 5.f) {
-          const float Tb = expf(-0.5f * x * x) * Sd;
+        float Tv, dTv;
+        filter_eval(T, b, lam * zp, Tv, dTv);
+        if (Tv != 0.f || dTv != 0.f) {
+          const float Tb = Tv * Sd;
           s[0][b] += Tb * F; s[1][b] += Tb * F_av; s[2][b] += Tb * F_del; s[3][b] += Tb * F_fl;
-          s[4][b] += Tb * F * (-x / T.filt_sigma[b]) * lam;      // d/dz of T_b(lam (1+z))
+          s[4][b] += dTv * Sd * F * lam;                          // d/dz of T_b(lam (1+z))
         }
       }
     }
@@ -104,7 +113,10 @@ __global__ void __launch_bounds__(256) exact_fwd_simt_kernel(TableDev T, int64_t
     const int m = q % XB_M, cb = q / XB_M, c = cb / SPS_MAX_BAND, b = cb % SPS_MAX_BAND;
     const int64_t r = r0 + m;
     const float v = red[c][b][m];
-    if (r < n && b < T.n_band && v != 0.f) atomicAdd(&part[(r * 5 + c) * SPS_MAX_BAND + b], v);
+    if (r < n && b < T.n_band && v != 0.f) {
+      const int shift = c == 0 ? PART_SHIFT_FLUX : (c == 1 ? PART_SHIFT_AV : (c == 2 ? PART_SHIFT_DELTA : (c == 3 ? PART_SHIFT_FFLOOR : T.part_shift_z)));
+      part_add(&part[(r * 5 + c) * SPS_MAX_BAND + b], v, part_scale(B.sc[rows ? rows[r] : r].Mn, T.part_bound, shift));
+    }
   }
 }
 
@@ -112,16 +124,21 @@ __global__ void __launch_bounds__(256) exact_fwd_simt_kernel(TableDev T, int64_t
 __global__ void exact_mid_kernel(TableDev T, int64_t n, const int* __restrict__ rows, const int* __restrict__ gal_of_row,
                                  const float* __restrict__ obs_flux, const float* __restrict__ obs_sigma,
                                  const float* __restrict__ flux_bar, bool want_grad, RowBuffers B,
-                                 const float* __restrict__ part, float* __restrict__ gbuf) {
+                                 const long long* __restrict__ part, float* __restrict__ gbuf) {
   const int64_t r = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (r >= n) return;
   const int l = threadIdx.x & 31;
   const int64_t row = rows ? rows[r] : r;
   const bool isb = l < T.n_band;
-  const float* p = part + r * 5 * SPS_MAX_BAND;
-  float flux = 0.f, g = 0.f, chi2 = 0.f;
+  const long long* p = part + r * 5 * SPS_MAX_BAND;
+  const float Mn = B.sc[row].Mn;
+  float flux = 0.f, g = 0.f, chi2 = 0.f, p_av = 0.f, p_de = 0.f, p_fl = 0.f, p_z = 0.f;
   if (isb) {
-    flux = p[l];
+    flux = part_read(p + l, part_scale(Mn, T.part_bound, PART_SHIFT_FLUX));
+    p_av = part_read(p + 1 * SPS_MAX_BAND + l, part_scale(Mn, T.part_bound, PART_SHIFT_AV));
+    p_de = part_read(p + 2 * SPS_MAX_BAND + l, part_scale(Mn, T.part_bound, PART_SHIFT_DELTA));
+    p_fl = part_read(p + 3 * SPS_MAX_BAND + l, part_scale(Mn, T.part_bound, PART_SHIFT_FFLOOR));
+    p_z = part_read(p + 4 * SPS_MAX_BAND + l, part_scale(Mn, T.part_bound, T.part_shift_z));
     B.flux[row * SPS_MAX_BAND + l] = flux;
     if (flux_bar) g = flux_bar[row * T.n_band + l];
     else {
@@ -133,12 +150,11 @@ __global__ void exact_mid_kernel(TableDev T, int64_t n, const int* __restrict__ 
   }
   if (l < SPS_MAX_BAND) gbuf[r * SPS_MAX_BAND + l] = isb ? g : 0.f;
   chi2 = warp_sum(chi2);
-  const float Mn = B.sc[row].Mn;
   const float mn_bar = warp_sum(isb ? g * flux : 0.f) / Mn;
-  const float av = warp_sum(isb ? g * p[1 * SPS_MAX_BAND + l] : 0.f);
-  const float de = warp_sum(isb ? g * p[2 * SPS_MAX_BAND + l] : 0.f);
-  const float fl = warp_sum(isb ? g * p[3 * SPS_MAX_BAND + l] : 0.f);
-  const float zb = warp_sum(isb ? g * p[4 * SPS_MAX_BAND + l] : 0.f);
+  const float av = warp_sum(g * p_av);
+  const float de = warp_sum(g * p_de);
+  const float fl = warp_sum(g * p_fl);
+  const float zb = warp_sum(g * p_z);
   if (l == 0) {
     RowScalars* sc = &B.sc[row];
     sc->logp_like = -0.5f * chi2;
@@ -175,8 +191,9 @@ __global__ void __launch_bounds__(256) exact_bwd_simt_kernel(TableDev T, int64_t
         const float lam = T.wave[kg] * sc_s[m][0];
         float tsum = 0.f;
         for (int b = 0; b < T.n_band; ++b) {
-          const float x = (lam - T.filt_mu[b]) / T.filt_sigma[b];
-          if (fabsf(x) <= 5.f) tsum += g_s[m][b] * expf(-0.5f * x * x);
+          float Tv, dTv;
+          filter_eval(T, b, lam, Tv, dTv);
+          tsum += g_s[m][b] * Tv;
         }
         if (tsum != 0.f) {
           float F, a1, a2, a3;
@@ -266,9 +283,6 @@ __global__ void zsort_scatter_kernel(TableDev T, int64_t n, const int* __restric
 
 // ---- host side ----------------------------------------------------------------------------------------
 
-static int g_force_simt = 0;
-extern "C" void sps_debug_force_simt(int on) { g_force_simt = on; }
-
 sps_status sps_exact_setup(sps_table* t, int precision) {
   ExactState* X = new ExactState();
   memset(X, 0, sizeof(*X));
@@ -277,75 +291,76 @@ sps_status sps_exact_setup(sps_table* t, int precision) {
   return sps_exact_tc_setup(t, precision);
 }
 
-static void exact_free_buffers(ExactState* X) {
-  void* ptrs[] = {X->W, X->Wbar, X->part, X->gbuf, X->sorted, X->zhist};
+void sps_exact_free_scratch(ExactScratch& X) {
+  sps_exact_tc_free_scratch(X);
+  void* ptrs[] = {X.W, X.Wbar, X.part, X.gbuf, X.sorted, X.zhist};
   for (void* p : ptrs) if (p) cudaFree(p);
-  X->W = X->Wbar = X->part = X->gbuf = nullptr; X->sorted = X->zhist = nullptr; X->cap = 0;
+  X.W = X.Wbar = X.gbuf = nullptr; X.part = nullptr; X.sorted = X.zhist = nullptr; X.cap = 0;
 }
 
 void sps_exact_teardown(sps_table* t) {
   if (!t->exact) return;
   sps_exact_tc_teardown(t);
-  exact_free_buffers(t->exact);
   delete t->exact; t->exact = nullptr;
 }
 
-static sps_status exact_ensure(sps_table* t, int64_t n) {
-  ExactState* X = t->exact;
+static sps_status exact_ensure(const sps_table* t, ExactScratch& X, int64_t n, cudaStream_t s) {
+  const int ldw = t->exact->ldw;
   const int64_t need = (n + 127) / 128 * 128;                      // whole row tiles for the tensor-core kernels
-  if (X->cap >= need) return SPS_OK;
-  cudaDeviceSynchronize();
-  exact_free_buffers(X);
-  cudaError_t e = cudaMalloc(&X->W, need * X->ldw * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&X->Wbar, need * X->ldw * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&X->part, need * 5 * SPS_MAX_BAND * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&X->gbuf, need * SPS_MAX_BAND * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&X->sorted, need * sizeof(int));
-  if (e == cudaSuccess) e = cudaMalloc(&X->zhist, 2 * ZSORT_BINS * sizeof(int));
-  if (e != cudaSuccess) { exact_free_buffers(X); return sps_check_cuda(e, "exact-path scratch allocation"); }
-  cudaMemset(X->W, 0, need * X->ldw * sizeof(float));
-  cudaMemset(X->gbuf, 0, need * SPS_MAX_BAND * sizeof(float));
-  X->cap = need;
-  return sps_exact_tc_ensure(t, need);
+  if (X.cap >= need) return SPS_OK;
+  cudaStreamSynchronize(s);
+  sps_exact_free_scratch(X);
+  cudaError_t e = cudaMalloc(&X.W, need * ldw * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&X.Wbar, need * ldw * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&X.part, need * 5 * SPS_MAX_BAND * sizeof(long long));
+  if (e == cudaSuccess) e = cudaMalloc(&X.gbuf, need * SPS_MAX_BAND * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&X.sorted, need * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&X.zhist, 2 * ZSORT_BINS * sizeof(int));
+  if (e != cudaSuccess) { sps_exact_free_scratch(X); return sps_check_cuda(e, "exact-path scratch allocation"); }
+  cudaMemsetAsync(X.W, 0, need * ldw * sizeof(float), s);
+  cudaMemsetAsync(X.gbuf, 0, need * SPS_MAX_BAND * sizeof(float), s);
+  X.cap = need;
+  return sps_exact_tc_ensure(t, X, need);
 }
 
-sps_status sps_exact_contract(sps_table* t, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
+sps_status sps_exact_contract(const sps_table* t, Workspace& ws, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux,
                               const float* obs_sigma, const float* flux_bar, bool want_grad, cudaStream_t s) {
-  ExactState* X = t->exact;
+  ExactScratch& X = ws.x;
   const TableDev& T = t->dev;
-  sps_status st = exact_ensure(t, n); if (st != SPS_OK) return st;
-  const bool tc = X->use_tc && !g_force_simt;
+  const int ldw = t->exact->ldw;
+  sps_status st = exact_ensure(t, X, n, s); if (st != SPS_OK) return st;
+  const bool tc = t->exact->use_tc && !sps_option(SPS_OPT_EXACT_SIMT);
   if (tc) {                                                        // redshift-ordered row list for this call
-    cudaMemsetAsync(X->zhist, 0, 2 * ZSORT_BINS * sizeof(int), s);
+    cudaMemsetAsync(X.zhist, 0, 2 * ZSORT_BINS * sizeof(int), s);
     const unsigned nb = (unsigned)((n + 255) / 256);
-    zsort_hist_kernel<<<nb, 256, 0, s>>>(T, n, rows, t->rows, X->zhist);
-    zsort_scan_kernel<<<1, ZSORT_BINS, 0, s>>>(X->zhist);
-    zsort_scatter_kernel<<<nb, 256, 0, s>>>(T, n, rows, t->rows, X->zhist + ZSORT_BINS, X->sorted);
+    zsort_hist_kernel<<<nb, 256, 0, s>>>(T, n, rows, ws.rows, X.zhist);
+    zsort_scan_kernel<<<1, ZSORT_BINS, 0, s>>>(X.zhist);
+    zsort_scatter_kernel<<<nb, 256, 0, s>>>(T, n, rows, ws.rows, X.zhist + ZSORT_BINS, X.sorted);
     sps_count_launch(3);
-    rows = X->sorted;
+    rows = X.sorted;
   }
-  if (!tc) { exact_weights_kernel<<<(unsigned)n, 128, 0, s>>>(T, n, rows, t->rows, X->W, X->ldw); sps_count_launch(); }
-  cudaMemsetAsync(X->part, 0, n * 5 * SPS_MAX_BAND * sizeof(float), s);
-  if (tc) st = sps_exact_tc_forward(t, n, rows, s);             // (brackets its GEMM kernel for sps_profile itself)
+  if (!tc) { exact_weights_kernel<<<(unsigned)n, 128, 0, s>>>(T, n, rows, ws.rows, X.W, ldw); sps_count_launch(); }
+  cudaMemsetAsync(X.part, 0, n * 5 * SPS_MAX_BAND * sizeof(long long), s);
+  if (tc) st = sps_exact_tc_forward(t, ws, n, rows, s);          // (brackets its GEMM kernel for sps_profile itself)
   else {
     dim3 grid(T.n_wave_pad / XB_N, (unsigned)((n + XB_M - 1) / XB_M));
     sps_prof_begin(SPS_K_EXACT_FWD, s);
-    exact_fwd_simt_kernel<<<grid, 256, 0, s>>>(T, n, rows, t->rows, X->W, X->ldw, X->part); sps_count_launch();
+    exact_fwd_simt_kernel<<<grid, 256, 0, s>>>(T, n, rows, ws.rows, X.W, ldw, X.part); sps_count_launch();
     sps_prof_end(SPS_K_EXACT_FWD, s);
   }
   if (st != SPS_OK) return st;
   const unsigned wb = (unsigned)((n * 32 + 255) / 256);
-  exact_mid_kernel<<<wb, 256, 0, s>>>(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, t->rows, X->part, X->gbuf);
+  exact_mid_kernel<<<wb, 256, 0, s>>>(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, ws.rows, X.part, X.gbuf);
   sps_count_launch();
   if (!want_grad) return SPS_OK;
-  if (tc) st = sps_exact_tc_backward(t, n, rows, s);
+  if (tc) st = sps_exact_tc_backward(t, ws, n, rows, s);
   else {
-    dim3 grid((X->ldw + XB_N - 1) / XB_N, (unsigned)((n + XB_M - 1) / XB_M));
+    dim3 grid((ldw + XB_N - 1) / XB_N, (unsigned)((n + XB_M - 1) / XB_M));
     sps_prof_begin(SPS_K_EXACT_BWD, s);
-    exact_bwd_simt_kernel<<<grid, 256, 0, s>>>(T, n, rows, t->rows, X->gbuf, X->Wbar, X->ldw); sps_count_launch();
+    exact_bwd_simt_kernel<<<grid, 256, 0, s>>>(T, n, rows, ws.rows, X.gbuf, X.Wbar, ldw); sps_count_launch();
     sps_prof_end(SPS_K_EXACT_BWD, s);
   }
   if (st != SPS_OK) return st;
-  exact_final_kernel<<<wb, 256, 0, s>>>(T, n, rows, t->rows, X->Wbar, X->ldw); sps_count_launch();
+  exact_final_kernel<<<wb, 256, 0, s>>>(T, n, rows, ws.rows, X.Wbar, ldw); sps_count_launch();
   return SPS_OK;
 }

@@ -37,6 +37,7 @@
 #include <cstring>
 #include <vector>
 #include "sps_exact.cuh"
+#include "sps_ptx.cuh"
 
 namespace {
 
@@ -79,21 +80,14 @@ struct FilterConsts {                 // x = lam (1+z) isg + nmu ; T_b = exp2(-x
   float isg[SPS_MAX_BAND], nmu[SPS_MAX_BAND], dz[SPS_MAX_BAND], lo[SPS_MAX_BAND], hi[SPS_MAX_BAND];
 };
 
-struct TcState {
+struct TcState {                    // table constants of the tensor-core exact path
   int prec, es, BK;                 // operand format, element size, elements per k block
   void *LT_hi, *LT_lo;              // [n_wave_pad][Wld]    forward B operand (wavelength-major, K = ij contiguous)
   void *Lc_hi, *Lc_lo;              // [nb*BNb][n_wave_pad] reverse B operand (ij-major, K = wavelength contiguous)
-  void *W_hi, *W_lo;                // [cap][Wld]           forward A operand
-  void *SB_hi, *SB_lo;              // [cap][n_wave_pad]    reverse A operand (SEDbar)
   float4* wconst;                   // [n_wave_pad][2]      {lam, dlam, k0, drude}, {log2(lam/5500), -, -, -}
-  unsigned long long* work;         // [1] (row, wavelength) pairs of the last forward call
-  int* plan;                        // [4][plan_cap]: fwd item prefix, first wavelength tile, k-range begin / end (bytes/128)
-  int plan_cap;
-  CUtensorMap mLT_hi, mLT_lo, mLc_hi, mLc_lo, mW_hi, mW_lo, mSB_hi, mSB_lo;
+  CUtensorMap mLT_hi, mLT_lo, mLc_hi, mLc_lo;
   FilterConsts fc;
   int Kpad, Wld, nb, BNb;
-  int64_t cap;
-  int sm_count;
 };
 
 struct GemmArgs {
@@ -101,68 +95,16 @@ struct GemmArgs {
   int m_tiles, n_tiles, k_blocks, BN, BK;
   const int* rows;
   const int* plan; int plan_cap;
-  float* part;            // forward: [n][5][SPS_MAX_BAND] band sums (atomicAdd)
+  long long* part;        // forward: [n][5][SPS_MAX_BAND] fixed-point band sums (integer atomicAdd: order-independent)
   float* Wbar; int ldw;   // reverse
 };
 
-// ---- PTX wrappers ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t ok = 0;
-  while (!ok) {
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  }
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-               ::"r"(dst), "l"(map), "r"(bar), "r"(c_inner), "r"(c_outer) : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
 template <int PREC>
 __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
-  if (PREC == SPS_EXACT_BF16X3)
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
-  else
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+  if (PREC == SPS_EXACT_BF16X3) tc_mma_f16(d_tmem, a_desc, b_desc, idesc, accumulate);
+  else tc_mma_tf32(d_tmem, a_desc, b_desc, idesc, accumulate);
 }
-// K-major operand tile whose rows are one swizzle span (64 or 128 bytes): 8-row atoms stacked along M/N (SBO = 8 rows)
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
-  uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)1 << 16;
-  d |= (uint64_t)((8 * ROW_BYTES) >> 4) << 32;
-  d |= (uint64_t)1 << 46;            // descriptor version (sm_100)
-  d |= (uint64_t)(ROW_BYTES == 128 ? 2 : 4) << 61;   // SWIZZLE_128B / SWIZZLE_64B
-  return d;
-}
-#define TMEM_LD8(taddr, v)                                                                                             \
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"                               \
-               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])        \
-               : "r"(taddr))
-#define TMEM_LD4(taddr, v)                                                                                             \
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"                                           \
-               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(taddr))
-#define TMEM_LD16(taddr, v)                                                                                            \
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
-               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),       \
-                 "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])  \
-               : "r"(taddr))
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) { return umma_desc_kmajor(saddr, ROW_BYTES); }
 
 // 2^x for the moderate arguments of the epilogues (|x| < 64): the bare SFU instruction, without exp2f's denormal-range fix-up
 __device__ __forceinline__ float ex2_fast(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -170,23 +112,6 @@ __device__ __forceinline__ float ex2_fast(float x) { float y; asm("ex2.approx.ft
 // exp(-x^2/2) = exp2(-(x * FILT_SCALE)^2)
 #define FILT_SCALE 0.84932180028801907f
 #define FILT_CUT (5.f * FILT_SCALE)
-
-#define FLUSH_PART()                                                                                  \
-  do {                                                                                                \
-    if (cur_m >= 0 && valid) {                                                                        \
-      float* p = G.part + r * 5 * SPS_MAX_BAND;                                                       \
-      _Pragma("unroll") for (int b = 0; b < NB; ++b) {                                      \
-        if (b < T.n_band) {                                                                           \
-          if (s0[b] != 0.f) atomicAdd(p + b, s0[b]);                                                  \
-          if (s1[b] != 0.f) atomicAdd(p + SPS_MAX_BAND + b, s1[b]);                                   \
-          if (s2[b] != 0.f) atomicAdd(p + 2 * SPS_MAX_BAND + b, s2[b]);                               \
-          if (s3[b] != 0.f) atomicAdd(p + 3 * SPS_MAX_BAND + b, s3[b]);                               \
-          if (s4[b] != 0.f) atomicAdd(p + 4 * SPS_MAX_BAND + b, s4[b] * FC.dz[b]);                               \
-        }                                                                                             \
-      }                                                                                               \
-    }                                                                                                 \
-    _Pragma("unroll") for (int b = 0; b < NB; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f; \
-  } while (0)
 
 // Work items.  forward: item w -> (row tile m, wavelength tile nt) through the per-row-tile prefix plan[0][m] and
 // first tile plan[1][m]; reverse: w -> (m, w % n_tiles), k blocks plan[2][m] .. plan[3][m].
@@ -204,7 +129,7 @@ struct ItemCursor {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-template <int MODE, int PREC, int NB>   // MODE 0: forward with the fused photometry epilogue (NB = compiled band slots), 1: reverse, store epilogue
+template <int MODE, int PREC, int NB, int FILT>   // MODE 0: forward with the fused photometry epilogue (NB = compiled band slots; FILT 0 Gaussian / 1 tabulated filters), 1: reverse, store epilogue
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constant__ CUtensorMap tmAl,
                   const __grid_constant__ CUtensorMap tmBh, const __grid_constant__ CUtensorMap tmBl,
@@ -231,7 +156,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full(s), 1); mbar_init(bar_empty(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(bar_tfull(b), 1); mbar_init(bar_tempty(b), EPI_WARPS); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mbar_fence_init();
   }
   if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar_base + 96u), "r"(TMEM_COLS) : "memory");
@@ -302,31 +227,31 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
     int buf = 0; uint32_t bphase = 0;
     if (MODE == 0) {
       constexpr int COLS = BN_MAX / EPI_PARTS;
-      float s0[NB], s1[NB], s2[NB], s3[NB], s4[NB];
-#pragma unroll
-      for (int b = 0; b < NB; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f;
       int cur_m = -1; int64_t r = 0; bool valid = false;
       float zp = 1.f, AVs = 0.f, delta = 0.f, Ffl = 1.f, Eb = 0.85f, zp_min = 1.f, zp_max = 1.f;
+      float sc0 = 0.f, sc1 = 0.f, sc2 = 0.f, sc3 = 0.f, sc4 = 0.f;          // fixed-point scales of the row's five band sums
       for (int w = w_begin; w < w_end; ++w) {
         int m, nt, kb_lo, kb_hi;
         cur.seek<MODE>(w, m, nt, kb_lo, kb_hi, G.k_blocks);
         if (m != cur_m) {
-          FLUSH_PART();
           cur_m = m;
           r = (int64_t)m * BM + row_in_tile;
           valid = r < G.n;
           zp = 1.f; AVs = 0.f; delta = 0.f; Ffl = 1.f;
+          float Mn = 1.f;
           if (valid) {
             const RowScalars sc = B.sc[G.rows ? G.rows[r] : r];
-            zp = 1.f + sc.z; AVs = sc.AV * (1.f / 4.05f); delta = sc.delta; Ffl = sc.Ffloor;
+            zp = 1.f + sc.z; AVs = sc.AV * (1.f / 4.05f); delta = sc.delta; Ffl = sc.Ffloor; Mn = sc.Mn;
           }
+          sc0 = part_scale(Mn, T.part_bound, PART_SHIFT_FLUX); sc1 = part_scale(Mn, T.part_bound, PART_SHIFT_AV);
+          sc2 = part_scale(Mn, T.part_bound, PART_SHIFT_DELTA); sc3 = part_scale(Mn, T.part_bound, PART_SHIFT_FFLOOR);
+          sc4 = part_scale(Mn, T.part_bound, T.part_shift_z);
           Eb = 0.85f - 1.9f * delta;
           float lo = valid ? zp : 1e30f, hi = valid ? zp : 0.f;
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) { lo = fminf(lo, __shfl_xor_sync(FULL_MASK, lo, o)); hi = fmaxf(hi, __shfl_xor_sync(FULL_MASK, hi, o)); }
           zp_min = lo; zp_max = hi;
         }
-        const int n0 = nt * BN_MAX + half * COLS;
         // the tile's per-wavelength constants go to shared memory once (coalesced), then are read as broadcasts
         {
           const int et = (int)threadIdx.x - 64;               // 0..255 over the epilogue warps = column of the tile
@@ -341,7 +266,7 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
         // bands whose (truncated) support can meet this warp's columns for some of its rows
         unsigned mask = 0;
         {
-          const float lam_lo = cw[half * COLS] * zp_min * 0.999999f, lam_hi = cw[half * COLS + COLS - 1] * zp_max * 1.000001f;
+          const float lam_lo = cw[half * COLS] * zp_min * 0.99999f, lam_hi = cw[half * COLS + COLS - 1] * zp_max * 1.00001f;
 #pragma unroll
           for (int b = 0; b < NB; ++b)
             if (b < T.n_band && lam_hi >= FC.lo[b] && lam_lo <= FC.hi[b]) mask |= 1u << b;
@@ -349,6 +274,12 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
         mbar_wait(bar_tfull(buf), bphase);
         tc_fence_after();
         if (mask != 0) {
+          // Partial band sums of this warp's columns of this tile, from zero: what a (row, tile, column part) contributes is a
+          // fixed sequence of operations on that row's data alone, and the contributions are combined by integer atomics
+          // below, so a row's fluxes do not depend on the rows it shares a tile with nor on how tiles are spread over CTAs.
+          float s0[NB], s1[NB], s2[NB], s3[NB], s4[NB];
+#pragma unroll
+          for (int b = 0; b < NB; ++b) s0[b] = s1[b] = s2[b] = s3[b] = s4[b] = 0.f;
           const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * BN_MAX + half * COLS);
           constexpr int CH = EPI_WARPS > 8 ? 4 : 8;          // columns per step: fewer live registers with more warps
           for (int c = 0; c < COLS / CH; ++c) {
@@ -386,14 +317,34 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
               if (mask & (1u << b)) {
-                const float isg = FC.isg[b], nmu = FC.nmu[b];
+                if (FILT == 0) {
+                  const float isg = FC.isg[b], nmu = FC.nmu[b];
 #pragma unroll
-                for (int j = 0; j < CH; ++j) {
-                  const float x = fmaf(lamz[j], isg, nmu);
-                  const float Tb = (fabsf(x) <= FILT_CUT) ? ex2_fast(-x * x) : 0.f;
-                  s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
-                  s4[b] = fmaf(Tb * x, G4[j], s4[b]);   // d/dz of T_b(lam (1+z)) = -T x' lam / sigma: the band's factor FC.dz is applied at the flush
+                  for (int j = 0; j < CH; ++j) {
+                    const float x = fmaf(lamz[j], isg, nmu);
+                    const float Tb = (fabsf(x) <= FILT_CUT) ? ex2_fast(-x * x) : 0.f;
+                    s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
+                    s4[b] = fmaf(Tb * x, G4[j], s4[b]);   // d/dz of T_b(lam (1+z)) = -T x' lam / sigma: the band's factor FC.dz is applied at the flush
+                  }
+                } else {
+#pragma unroll
+                  for (int j = 0; j < CH; ++j) {
+                    float Tb, dTb;
+                    filter_tab_eval(T.ft, b, lamz[j], Tb, dTb);
+                    s0[b] = fmaf(Tb, G0[j], s0[b]); s1[b] = fmaf(Tb, G1[j], s1[b]); s2[b] = fmaf(Tb, G2[j], s2[b]); s3[b] = fmaf(Tb, G3[j], s3[b]);
+                    s4[b] = fmaf(dTb, G4[j], s4[b]);      // d/dz of T_b(lam (1+z)) = T_b' lam
+                  }
                 }
+              }
+            }
+          }
+          if (valid) {
+            long long* p = G.part + r * 5 * SPS_MAX_BAND;
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+              if (mask & (1u << b)) {
+                part_add(p + b, s0[b], sc0); part_add(p + SPS_MAX_BAND + b, s1[b], sc1); part_add(p + 2 * SPS_MAX_BAND + b, s2[b], sc2);
+                part_add(p + 3 * SPS_MAX_BAND + b, s3[b], sc3); part_add(p + 4 * SPS_MAX_BAND + b, s4[b] * (FILT == 0 ? FC.dz[b] : 1.f), sc4);
               }
             }
           }
@@ -403,7 +354,6 @@ exact_gemm_kernel(const __grid_constant__ CUtensorMap tmAh, const __grid_constan
         if (lane == 0) mbar_arrive(bar_tempty(buf));
         buf ^= 1; if (buf == 0) bphase ^= 1u;
       }
-      FLUSH_PART();
     } else {
       for (int w = w_begin; w < w_end; ++w) {
         int m, nt, kb_lo, kb_hi;
@@ -565,7 +515,7 @@ __global__ void __launch_bounds__(128) tc_weights_kernel(TableDev T, int64_t n, 
 // warp-uniformly (the filters overlap little, so two to four of them), and only those are evaluated.  The kernel is
 // instruction-issue bound (a per-element loop over all bands cost 148 instructions per element).
 constexpr int SB_G = 4, SB_THREADS = 128, SB_SPAN = 64 * SB_G;
-template <int PREC>
+template <int PREC, int FILT>
 __global__ void __launch_bounds__(SB_THREADS) tc_sedbar_kernel(TableDev T, int64_t n, const int* __restrict__ rows, RowBuffers B, FilterConsts FC,
                                                                const float* __restrict__ gbuf, const float4* __restrict__ wconst,
                                                                const int* __restrict__ plan, int plan_cap,
@@ -602,8 +552,14 @@ __global__ void __launch_bounds__(SB_THREADS) tc_sedbar_kernel(TableDev T, int64
         const float isg = FC.isg[b], nmu = FC.nmu[b], g = g_s[b];
 #pragma unroll
         for (int e = 0; e < 2 * SB_G; ++e) {
-          const float x = fmaf(lamz[e], isg, nmu);
-          if (fabsf(x) <= FILT_CUT) tsum[e] = fmaf(g, ex2_fast(-x * x), tsum[e]);
+          if (FILT == 0) {
+            const float x = fmaf(lamz[e], isg, nmu);
+            if (fabsf(x) <= FILT_CUT) tsum[e] = fmaf(g, ex2_fast(-x * x), tsum[e]);
+          } else {
+            float Tb, dTb;
+            filter_tab_eval(T.ft, b, lamz[e], Tb, dTb);
+            tsum[e] = fmaf(g, Tb, tsum[e]);
+          }
         }
       }
     }
@@ -640,42 +596,23 @@ __global__ void __launch_bounds__(SB_THREADS) tc_sedbar_kernel(TableDev T, int64
 }
 
 // ---- host side --------------------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-EncodeTiledFn g_encode = nullptr;
-
-sps_status get_encoder() {
-  if (g_encode) return SPS_OK;
-  void* fn = nullptr;
-  cudaDriverEntryPointQueryResult qr;
-  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
-    cudaGetLastError();
-    sps_set_error("cuTensorMapEncodeTiled is not available from this driver");
-    return SPS_EUNSUPPORTED;
-  }
-  g_encode = (EncodeTiledFn)fn;
-  return SPS_OK;
-}
-
-// [rows][cols] row-major with pitch `ld` elements -> tiles of box_rows x 128 bytes, 128-byte swizzle
+// [rows][cols] row-major with pitch `ld` elements -> tiles of box_rows x ROW_BYTES, swizzled
 sps_status make_map(const TcState* S, CUtensorMap* m, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
+  SpsEncodeTiledFn enc = sps_tensor_map_encoder();
+  if (!enc) return SPS_EUNSUPPORTED;
   const cuuint64_t dims[2] = {cols, rows};
   const cuuint64_t strides[1] = {ld * (uint64_t)S->es};
   const cuuint32_t box[2] = {(cuuint32_t)S->BK, box_rows};
   const cuuint32_t es[2] = {1, 1};
-  const CUresult r = g_encode(m, S->prec == SPS_EXACT_BF16X3 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
-                              const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, ROW_BYTES == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
-                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  const CUresult r = enc(m, S->prec == SPS_EXACT_BF16X3 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                         const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, ROW_BYTES == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { sps_set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return SPS_ECUDA; }
   return SPS_OK;
 }
 
-void free_row_operands(TcState* S) {
-  void* ptrs[] = {S->W_hi, S->W_lo, S->SB_hi, S->SB_lo, S->plan};
-  for (void* p : ptrs) if (p) cudaFree(p);
-  S->W_hi = S->W_lo = S->SB_hi = S->SB_lo = nullptr; S->plan = nullptr; S->cap = 0; S->plan_cap = 0;
-}
+template <int PREC, int NB, int FILT>
+sps_status optin_fwd() { return sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, NB, FILT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in"); }
 
 template <int PREC>
 sps_status build_tables(const TableDev& T, TcState* S, size_t lc_rows) {
@@ -686,45 +623,50 @@ sps_status build_tables(const TableDev& T, TcState* S, size_t lc_rows) {
   build_wconst_kernel<<<(T.n_wave_pad + 255) / 256, 256>>>(T, S->wconst);
   sps_count_launch(3);
   sps_status st = sps_check_cuda(cudaDeviceSynchronize(), "tensor-core operand build");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<0, PREC, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
-  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<1, PREC, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
+  if (st == SPS_OK) st = optin_fwd<PREC, 4, 0>();
+  if (st == SPS_OK) st = optin_fwd<PREC, 10, 0>();
+  if (st == SPS_OK) st = optin_fwd<PREC, 16, 0>();
+  if (st == SPS_OK) st = optin_fwd<PREC, 16, 1>();
+  if (st == SPS_OK) st = sps_check_cuda(cudaFuncSetAttribute(exact_gemm_kernel<1, PREC, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES), "smem opt-in");
   return st;
 }
 
 template <int PREC>
-sps_status launch_forward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
+sps_status launch_forward(const sps_table* t, const TcState* S, Workspace& ws, int64_t n, const int* rows, cudaStream_t s) {
   typedef typename Op<PREC>::T E;
-  ExactState* X = t->exact; const TableDev& T = t->dev;
-  tc_weights_kernel<PREC><<<(unsigned)n, 128, 0, s>>>(T, n, rows, t->rows, S->Wld, (E*)S->W_hi, (E*)S->W_lo);
+  ExactScratch& X = ws.x; const TableDev& T = t->dev;
+  tc_weights_kernel<PREC><<<(unsigned)n, 128, 0, s>>>(T, n, rows, ws.rows, S->Wld, (E*)X.W_hi, (E*)X.W_lo);
   GemmArgs G; memset(&G, 0, sizeof(G));
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = T.n_wave_pad / BN_MAX; G.k_blocks = S->Kpad / S->BK; G.BN = BN_MAX; G.BK = S->BK;
-  G.rows = rows; G.part = X->part; G.plan = S->plan; G.plan_cap = S->plan_cap;
-  cudaMemsetAsync(S->work, 0, sizeof(unsigned long long), s);
-  exact_plan_kernel<<<G.m_tiles, BM, 0, s>>>(T, n, rows, t->rows, S->fc, S->BK, S->plan, S->plan_cap, S->work);
-  exact_scan_kernel<<<1, 32, 0, s>>>(G.m_tiles, S->plan);
-  const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  G.rows = rows; G.part = X.part; G.plan = X.plan; G.plan_cap = X.plan_cap;
+  cudaMemsetAsync(X.work, 0, sizeof(unsigned long long), s);
+  exact_plan_kernel<<<G.m_tiles, BM, 0, s>>>(T, n, rows, ws.rows, S->fc, S->BK, X.plan, X.plan_cap, X.work);
+  exact_scan_kernel<<<1, 32, 0, s>>>(G.m_tiles, X.plan);
+  const int grid = std::min(t->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_FWD, s);
-  if (T.n_band <= 4) exact_gemm_kernel<0, PREC, 4><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
-  else if (T.n_band <= 10) exact_gemm_kernel<0, PREC, 10><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
-  else exact_gemm_kernel<0, PREC, 16><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mW_hi, S->mW_lo, S->mLT_hi, S->mLT_lo, T, t->rows, G, S->fc, S->wconst);
+#define FWD(NBV, FV) exact_gemm_kernel<0, PREC, NBV, FV><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(X.mW_hi, X.mW_lo, S->mLT_hi, S->mLT_lo, T, ws.rows, G, S->fc, S->wconst)
+  if (T.filt_tab) FWD(16, 1);
+  else if (T.n_band <= 4) FWD(4, 0);
+  else if (T.n_band <= 10) FWD(10, 0);
+  else FWD(16, 0);
+#undef FWD
   sps_prof_end(SPS_K_EXACT_FWD, s);
-  sps_count_launch(3);
+  sps_count_launch(4);
   return sps_check_cuda(cudaGetLastError(), "exact forward (tcgen05) launch");
 }
 
 template <int PREC>
-sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows, cudaStream_t s) {
+sps_status launch_backward(const sps_table* t, const TcState* S, Workspace& ws, int64_t n, const int* rows, cudaStream_t s) {
   typedef typename Op<PREC>::T E;
-  ExactState* X = t->exact; const TableDev& T = t->dev;
-  tc_sedbar_kernel<PREC><<<(unsigned)n, SB_THREADS, 0, s>>>(T, n, rows, t->rows, S->fc, X->gbuf, S->wconst, S->plan, S->plan_cap, (E*)S->SB_hi, (E*)S->SB_lo);
+  ExactScratch& X = ws.x; const TableDev& T = t->dev;
+  if (T.filt_tab) tc_sedbar_kernel<PREC, 1><<<(unsigned)n, SB_THREADS, 0, s>>>(T, n, rows, ws.rows, S->fc, X.gbuf, S->wconst, X.plan, X.plan_cap, (E*)X.SB_hi, (E*)X.SB_lo);
+  else tc_sedbar_kernel<PREC, 0><<<(unsigned)n, SB_THREADS, 0, s>>>(T, n, rows, ws.rows, S->fc, X.gbuf, S->wconst, X.plan, X.plan_cap, (E*)X.SB_hi, (E*)X.SB_lo);
   GemmArgs G; memset(&G, 0, sizeof(G));
   G.n = n; G.m_tiles = (int)((n + BM - 1) / BM); G.n_tiles = S->nb; G.k_blocks = T.n_wave_pad / S->BK; G.BN = S->BNb; G.BK = S->BK;
-  G.rows = rows; G.Wbar = X->Wbar; G.ldw = X->ldw; G.plan = S->plan; G.plan_cap = S->plan_cap;
-  const int grid = std::min(S->sm_count, G.m_tiles * G.n_tiles);
+  G.rows = rows; G.Wbar = X.Wbar; G.ldw = t->exact->ldw; G.plan = X.plan; G.plan_cap = X.plan_cap;
+  const int grid = std::min(t->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_BWD, s);
-  exact_gemm_kernel<1, PREC, 1><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(S->mSB_hi, S->mSB_lo, S->mLc_hi, S->mLc_lo, T, t->rows, G, S->fc, S->wconst);
+  exact_gemm_kernel<1, PREC, 1, 0><<<grid, NUM_THREADS, SMEM_BYTES, s>>>(X.mSB_hi, X.mSB_lo, S->mLc_hi, S->mLc_lo, T, ws.rows, G, S->fc, S->wconst);
   sps_prof_end(SPS_K_EXACT_BWD, s);
   sps_count_launch(2);
   return sps_check_cuda(cudaGetLastError(), "exact reverse (tcgen05) launch");
@@ -732,16 +674,12 @@ sps_status launch_backward(sps_table* t, TcState* S, int64_t n, const int* rows,
 
 }  // namespace
 
-static int g_disable_tc = 0;
-extern "C" void sps_debug_disable_tc(int on) { g_disable_tc = on; }
-
 sps_status sps_exact_tc_setup(sps_table* t, int precision) {
   ExactState* X = t->exact;
   X->use_tc = false; X->tc = nullptr;
-  if (g_disable_tc) return SPS_OK;
+  if (sps_option(SPS_OPT_NO_TC_SETUP)) return SPS_OK;
   if (precision != SPS_EXACT_TF32X3 && precision != SPS_EXACT_BF16X3) { sps_set_error("exact_precision must be SPS_EXACT_TF32X3 or SPS_EXACT_BF16X3"); return SPS_EINVAL; }
-  sps_status st = get_encoder();
-  if (st != SPS_OK) return st;
+  if (!sps_tensor_map_encoder()) return SPS_EUNSUPPORTED;
   const TableDev& T = t->dev;
   TcState* S = new TcState();
   memset(S, 0, sizeof(*S));
@@ -750,13 +688,12 @@ sps_status sps_exact_tc_setup(sps_table* t, int precision) {
   S->nb = (S->Kpad + BN_MAX - 1) / BN_MAX;
   S->BNb = ((S->Kpad + S->nb - 1) / S->nb + 15) / 16 * 16;
   S->Wld = (std::max(S->Kpad, S->nb * S->BNb) + 63) / 64 * 64;
-  int dev = 0; cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&S->sm_count, cudaDevAttrMultiProcessorCount, dev);
   for (int b = 0; b < SPS_MAX_BAND; ++b) {
     const float mu = b < T.n_band ? T.filt_mu[b] : 1.f, sg = b < T.n_band ? T.filt_sigma[b] : 1.f;
     S->fc.isg[b] = FILT_SCALE / sg; S->fc.nmu[b] = -mu * (FILT_SCALE / sg);
     S->fc.dz[b] = -1.f / (sg * FILT_SCALE);
     S->fc.lo[b] = mu - 5.f * sg; S->fc.hi[b] = mu + 5.f * sg;
+    if (T.filt_tab && b < T.n_band) { S->fc.lo[b] = T.ft.lo[b]; S->fc.hi[b] = T.ft.hi[b]; }     // the support of a tabulated curve
   }
   const size_t lt_n = (size_t)T.n_wave_pad * S->Wld, lc_rows = (size_t)S->nb * S->BNb, lc_n = lc_rows * T.n_wave_pad;
   cudaError_t e = cudaMalloc(&S->LT_hi, lt_n * S->es);
@@ -764,10 +701,9 @@ sps_status sps_exact_tc_setup(sps_table* t, int precision) {
   if (e == cudaSuccess) e = cudaMalloc(&S->Lc_hi, lc_n * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&S->Lc_lo, lc_n * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&S->wconst, (size_t)T.n_wave_pad * 2 * sizeof(float4));
-  if (e == cudaSuccess) e = cudaMalloc(&S->work, sizeof(unsigned long long));
   X->tc = S;
   if (e != cudaSuccess) { sps_exact_tc_teardown(t); return sps_check_cuda(e, "tensor-core operand allocation"); }
-  st = precision == SPS_EXACT_BF16X3 ? build_tables<SPS_EXACT_BF16X3>(T, S, lc_rows) : build_tables<SPS_EXACT_TF32X3>(T, S, lc_rows);
+  sps_status st = precision == SPS_EXACT_BF16X3 ? build_tables<SPS_EXACT_BF16X3>(T, S, lc_rows) : build_tables<SPS_EXACT_TF32X3>(T, S, lc_rows);
   if (st == SPS_OK) st = make_map(S, &S->mLT_hi, S->LT_hi, T.n_wave_pad, S->Wld, S->Wld, BN_MAX);
   if (st == SPS_OK) st = make_map(S, &S->mLT_lo, S->LT_lo, T.n_wave_pad, S->Wld, S->Wld, BN_MAX);
   if (st == SPS_OK) st = make_map(S, &S->mLc_hi, S->Lc_hi, lc_rows, T.n_wave_pad, T.n_wave_pad, S->BNb);
@@ -782,55 +718,63 @@ void sps_exact_tc_teardown(sps_table* t) {
   ExactState* X = t->exact;
   if (!X || !X->tc) return;
   TcState* S = (TcState*)X->tc;
-  free_row_operands(S);
-  void* ptrs[] = {S->LT_hi, S->LT_lo, S->Lc_hi, S->Lc_lo, S->wconst, S->work};
+  void* ptrs[] = {S->LT_hi, S->LT_lo, S->Lc_hi, S->Lc_lo, S->wconst};
   for (void* p : ptrs) if (p) cudaFree(p);
   delete S;
   X->tc = nullptr; X->use_tc = false;
 }
 
+void sps_exact_tc_free_scratch(ExactScratch& X) {
+  void* ptrs[] = {X.W_hi, X.W_lo, X.SB_hi, X.SB_lo, X.plan, X.work};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  X.W_hi = X.W_lo = X.SB_hi = X.SB_lo = nullptr; X.plan = nullptr; X.work = nullptr; X.tc_cap = 0; X.plan_cap = 0;
+}
+
 // row-side operand buffers for `cap` rows (cap is a multiple of 128); called when the exact scratch grows
-sps_status sps_exact_tc_ensure(sps_table* t, int64_t cap) {
-  ExactState* X = t->exact;
-  if (!X->use_tc) return SPS_OK;
-  TcState* S = (TcState*)X->tc;
-  if (S->cap >= cap) return SPS_OK;
-  free_row_operands(S);
+sps_status sps_exact_tc_ensure(const sps_table* t, ExactScratch& X, int64_t cap) {
+  if (!t->exact->use_tc) return SPS_OK;
+  const TcState* S = (const TcState*)t->exact->tc;
+  if (X.tc_cap >= cap) return SPS_OK;
+  sps_exact_tc_free_scratch(X);
   const TableDev& T = t->dev;
   const size_t wn = (size_t)cap * S->Wld, sn = (size_t)cap * T.n_wave_pad;
-  S->plan_cap = (int)(cap / BM) + 2;
-  cudaError_t e = cudaMalloc(&S->W_hi, wn * S->es);
-  if (e == cudaSuccess) e = cudaMalloc(&S->W_lo, wn * S->es);
-  if (e == cudaSuccess) e = cudaMalloc(&S->SB_hi, sn * S->es);
-  if (e == cudaSuccess) e = cudaMalloc(&S->SB_lo, sn * S->es);
-  if (e == cudaSuccess) e = cudaMalloc(&S->plan, (size_t)4 * S->plan_cap * sizeof(int));
-  if (e != cudaSuccess) { free_row_operands(S); return sps_check_cuda(e, "tensor-core row operand allocation"); }
-  cudaMemset(S->W_hi, 0, wn * S->es); cudaMemset(S->W_lo, 0, wn * S->es);
-  cudaMemset(S->SB_hi, 0, sn * S->es); cudaMemset(S->SB_lo, 0, sn * S->es);
-  S->cap = cap;
-  sps_status st = make_map(S, &S->mW_hi, S->W_hi, cap, S->Wld, S->Wld, BM);
-  if (st == SPS_OK) st = make_map(S, &S->mW_lo, S->W_lo, cap, S->Wld, S->Wld, BM);
-  if (st == SPS_OK) st = make_map(S, &S->mSB_hi, S->SB_hi, cap, T.n_wave_pad, T.n_wave_pad, BM);
-  if (st == SPS_OK) st = make_map(S, &S->mSB_lo, S->SB_lo, cap, T.n_wave_pad, T.n_wave_pad, BM);
+  X.plan_cap = (int)(cap / BM) + 2;
+  cudaError_t e = cudaMalloc(&X.W_hi, wn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&X.W_lo, wn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&X.SB_hi, sn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&X.SB_lo, sn * S->es);
+  if (e == cudaSuccess) e = cudaMalloc(&X.plan, (size_t)4 * X.plan_cap * sizeof(int));
+  if (e == cudaSuccess) e = cudaMalloc(&X.work, sizeof(unsigned long long));
+  if (e != cudaSuccess) { sps_exact_tc_free_scratch(X); return sps_check_cuda(e, "tensor-core row operand allocation"); }
+  cudaMemset(X.W_hi, 0, wn * S->es); cudaMemset(X.W_lo, 0, wn * S->es);
+  cudaMemset(X.SB_hi, 0, sn * S->es); cudaMemset(X.SB_lo, 0, sn * S->es);
+  cudaMemset(X.work, 0, sizeof(unsigned long long));
+  X.tc_cap = cap;
+  sps_status st = make_map(S, &X.mW_hi, X.W_hi, cap, S->Wld, S->Wld, BM);
+  if (st == SPS_OK) st = make_map(S, &X.mW_lo, X.W_lo, cap, S->Wld, S->Wld, BM);
+  if (st == SPS_OK) st = make_map(S, &X.mSB_hi, X.SB_hi, cap, T.n_wave_pad, T.n_wave_pad, BM);
+  if (st == SPS_OK) st = make_map(S, &X.mSB_lo, X.SB_lo, cap, T.n_wave_pad, T.n_wave_pad, BM);
   return st;
 }
 
-sps_status sps_exact_tc_forward(sps_table* t, int64_t n, const int* rows, cudaStream_t s) {
-  TcState* S = (TcState*)t->exact->tc;
-  return S->prec == SPS_EXACT_BF16X3 ? launch_forward<SPS_EXACT_BF16X3>(t, S, n, rows, s) : launch_forward<SPS_EXACT_TF32X3>(t, S, n, rows, s);
+sps_status sps_exact_tc_forward(const sps_table* t, Workspace& ws, int64_t n, const int* rows, cudaStream_t s) {
+  const TcState* S = (const TcState*)t->exact->tc;
+  return S->prec == SPS_EXACT_BF16X3 ? launch_forward<SPS_EXACT_BF16X3>(t, S, ws, n, rows, s) : launch_forward<SPS_EXACT_TF32X3>(t, S, ws, n, rows, s);
 }
 
-sps_status sps_exact_tc_backward(sps_table* t, int64_t n, const int* rows, cudaStream_t s) {
-  TcState* S = (TcState*)t->exact->tc;
-  return S->prec == SPS_EXACT_BF16X3 ? launch_backward<SPS_EXACT_BF16X3>(t, S, n, rows, s) : launch_backward<SPS_EXACT_TF32X3>(t, S, n, rows, s);
+sps_status sps_exact_tc_backward(const sps_table* t, Workspace& ws, int64_t n, const int* rows, cudaStream_t s) {
+  const TcState* S = (const TcState*)t->exact->tc;
+  return S->prec == SPS_EXACT_BF16X3 ? launch_backward<SPS_EXACT_BF16X3>(t, S, ws, n, rows, s) : launch_backward<SPS_EXACT_TF32X3>(t, S, ws, n, rows, s);
 }
 
 extern "C" sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavelength_pairs) {
   if (!t || !row_wavelength_pairs) { sps_set_error("sps_exact_last_work: null argument"); return SPS_EINVAL; }
   *row_wavelength_pairs = 0;
-  if (!t->exact || !t->exact->use_tc) return SPS_OK;
+  Workspace* ws = t->last_ws;
+  if (!t->exact || !t->exact->use_tc || !ws || !ws->x.work) return SPS_OK;
+  cudaDeviceSynchronize();
   unsigned long long v = 0;
-  sps_status st = sps_check_cuda(cudaMemcpy(&v, ((TcState*)t->exact->tc)->work, sizeof(v), cudaMemcpyDeviceToHost), "sps_exact_last_work");
+  sps_status st = sps_check_cuda(cudaMemcpy(&v, ws->x.work, sizeof(v), cudaMemcpyDeviceToHost), "sps_exact_last_work");
   *row_wavelength_pairs = (int64_t)v;
   return st;
 }

@@ -45,12 +45,13 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& 
   met_bin(T, R.th[7], R.th[8], R.m, R.dm_lz, R.dm_s);
 }
 
-// a0-a5.  With WANT_GRAD the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
-// kept in B.part for the epilogue, which then has no quadrature to redo.
-template <bool WANT_GRAD>
+// a0-a5.  With store_part the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
+// kept in B.part for the epilogue, which then has no quadrature to redo.  One instantiation serves forward-only and
+// gradient calls (the partials are computed either way), so that both give bit-identical weights and fluxes.
 __global__ void __launch_bounds__(32 * PRO_WARPS, PRO_MIN_BLOCKS)
-prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded,
+prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded, bool store_part,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
+  constexpr bool WANT_GRAD = true;
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
   const int64_t r = (int64_t)blockIdx.x * PRO_WARPS + (threadIdx.x >> 5);
@@ -64,7 +65,7 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     const int i = l + 32 * q;
     B.a[row * ROW_A_STRIDE + i] = (i < T.n_age) ? (1.f - Fb) * R.Q.dM[q] * inv_M + Fb * R.Bq.P[q] : 0.f;  // Eq. (A6)
-    if (WANT_GRAD) {
+    if (store_part) {
       float* p = B.part + row * (ROW_PARTS * ROW_A_STRIDE) + i;
       p[0] = R.Q.dM[q]; p[ROW_A_STRIDE] = R.Q.g_tau[q]; p[2 * ROW_A_STRIDE] = R.Q.g_al[q];
       p[3 * ROW_A_STRIDE] = R.Q.g_be[q]; p[4 * ROW_A_STRIDE] = R.Q.g_t[q];
@@ -321,7 +322,7 @@ __device__ __forceinline__ void ac_item(const TableDev& T, ACWarp& S, const floa
         for (int j = 0; j < T.n_Z; ++j) { S0 = fmaf(S.ms[r][j], S.Qs[r][0][j * T.n_band + b], S0); S1 = fmaf(S.ms[r][j], S.Qs[r][1][j * T.n_band + b], S1); }
         const float izp = __fdividef(1.f, zp);
         lam_r = T.lam_eff[b] * izp;
-        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam);
+        dust_at(lam_r, sc.AV, sc.delta, sc.Ffloor, F, F_av, F_del, F_fl, F_lam, T.model == SPS_MODEL_TINY5);
         const float flux = F * Mn * (S0 + f * S1);
         B.flux[(int64_t)rw * SPS_MAX_BAND + b] = flux;
         if (flux_bar) g = S.obs[r][0][b];
@@ -599,8 +600,7 @@ void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, i
   if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
   sps_prof_begin(SPS_K_PROLOGUE, s);
   const unsigned pro_blocks = (unsigned)((n + PRO_WARPS - 1) / PRO_WARPS);
-  if (want_grad) prologue_kernel<true><<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
-  else prologue_kernel<false><<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, rows, B, hist);
+  prologue_kernel<<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
@@ -641,14 +641,12 @@ void approx_group_rows(const TableDev& T, int64_t n, const int* rows, RowBuffers
   sps_count_launch(2);
 }
 
-void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
+void launch_approx_contract(const TableDev& T, int sm_count, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s) {
   if (n <= 0) return;
   const int nb = T.n_z - 1;
   approx_group_rows(T, n, rows, B, AC_ROWS_PER_CTA, s);
-  static int sm_count = 0;
-  if (!sm_count) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev); }
   const unsigned grid = (unsigned)std::min<int64_t>(sm_count, (n + AC_ROWS_PER_CTA - 1) / AC_ROWS_PER_CTA + nb);
   sps_prof_begin(SPS_K_APPROX, s);
   approx_contract_kernel<<<grid, 32 * AC_WARPS, approx_smem_bytes(T), s>>>(T, n, B.order, B.bins, gal_of_row, obs_flux, obs_sigma,

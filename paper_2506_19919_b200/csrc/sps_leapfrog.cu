@@ -3,18 +3,19 @@
 #include <vector>
 #include "sps_sampler.cuh"
 
-__global__ void gal_of_chain_kernel(int* out, int64_t n, int n_chain) {
+__global__ void gal_of_chain_kernel(int* out, int* rng_id, const int* __restrict__ gal_id, int64_t n, int n_chain) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) out[i] = (int)(i / n_chain);
+  if (i >= n) return;
+  const int g = (int)(i / n_chain), k = (int)(i - (int64_t)g * n_chain);
+  out[i] = g;
+  rng_id[i] = (gal_id ? gal_id[g] : g) * n_chain + k;        // Philox stream of the chain (sps_hmc_config.gal_id_dev)
 }
 
-sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
-                             const float* obs_flux, const float* obs_sigma) {
-  memset(&Q, 0, sizeof(Q));
-  Q.n = n_gal * cfg->n_chain; Q.obs_flux = obs_flux; Q.obs_sigma = obs_sigma;
+static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev) {
   sps_status st = sps_check_cuda(cudaMalloc(&Q.gal_of_chain, Q.n * sizeof(int)), "gal_of_chain allocation");
+  if (st == SPS_OK) st = sps_check_cuda(cudaMalloc(&Q.rng_id, Q.n * sizeof(int)), "rng_id allocation");
   if (st != SPS_OK) return st;
-  gal_of_chain_kernel<<<(unsigned)((Q.n + 255) / 256), 256>>>(Q.gal_of_chain, Q.n, cfg->n_chain); sps_count_launch();
+  gal_of_chain_kernel<<<(unsigned)((Q.n + 255) / 256), 256>>>(Q.gal_of_chain, Q.rng_id, cfg->gal_id_dev, Q.n, cfg->n_chain); sps_count_launch();
   st = sps_check_cuda(cudaMalloc(&Q.path_of_chain, Q.n), "path_of_chain allocation");
   if (st != SPS_OK) return st;
   if (!path_of_gal_dev) {
@@ -43,8 +44,19 @@ sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n
   return SPS_OK;
 }
 
+void hmc_problem_free(HmcProblem& Q);
+sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
+                             const float* obs_flux, const float* obs_sigma) {
+  memset(&Q, 0, sizeof(Q));
+  Q.n = n_gal * cfg->n_chain; Q.obs_flux = obs_flux; Q.obs_sigma = obs_sigma;
+  const sps_status st = hmc_problem_fill(Q, cfg, n_gal, path_of_gal_dev);
+  if (st != SPS_OK) hmc_problem_free(Q);                    // nothing allocated here outlives a rejected call
+  return st;
+}
+
 void hmc_problem_free(HmcProblem& Q) {
   if (Q.gal_of_chain) cudaFree(Q.gal_of_chain);
+  if (Q.rng_id) cudaFree(Q.rng_id);
   if (Q.path_of_chain) cudaFree(Q.path_of_chain);
   for (int p = 0; p < 2; ++p) if (Q.rows_path[p]) cudaFree(Q.rows_path[p]);
   memset(&Q, 0, sizeof(Q));
@@ -78,27 +90,30 @@ __global__ void lf_record_kernel(int64_t n, int step, const float* __restrict__ 
   theta_w[o] = th + e * inv_mass[o] * p;
 }
 
-extern "C" sps_status sps_leapfrog(const sps_table* tc, const sps_prior* prior, int path, const float* theta0, const float* p0,
+extern "C" sps_status sps_leapfrog(const sps_table* t, const sps_prior* prior, int path, const float* theta0, const float* p0,
                                    const float* eps, const float* inv_mass, int64_t n, const int32_t* gal_of_row,
                                    const float* obs_flux, const float* obs_sigma, int32_t n_steps, float* traj, float* logp_traj,
                                    void* stream) {
-  if (!tc || !prior || !theta0 || !p0 || !eps || !inv_mass || !obs_flux || !obs_sigma || !traj || !logp_traj) {
+  if (!t || !theta0 || !p0 || !eps || !inv_mass || !traj || !logp_traj ||
+      (t->dev.model != SPS_MODEL_GAUSS_TEST && (!prior || !obs_flux || !obs_sigma))) {
     sps_set_error("sps_leapfrog: null argument"); return SPS_EINVAL; }
   if (n < 0 || n_steps < 0 || (path != SPS_PATH_EXACT && path != SPS_PATH_APPROX)) { sps_set_error("sps_leapfrog: bad argument"); return SPS_EINVAL; }
   if (n == 0 || n_steps == 0) return SPS_OK;
-  sps_table* t = const_cast<sps_table*>(tc);
+  sps_status st = sps_require_device(); if (st != SPS_OK) return st;
   cudaStream_t s = (cudaStream_t)stream;
-  PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
-  st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
+  PriorDev P; st = sps_prior_to_dev(t, prior, P); if (st != SPS_OK) return st;
+  st = sps_check_finite(theta0, n * SPS_NDIM, p0, n * SPS_NDIM, eps, n, s); if (st != SPS_OK) return st;
+  Workspace& ws = *sps_workspace(t, s);
+  if (t->dev.model != SPS_MODEL_GAUSS_TEST) { st = sps_ensure_row_buffers(t, ws, n, s); if (st != SPS_OK) return st; }
   float* w = nullptr;
   const size_t nv = (size_t)n * SPS_NDIM;
   st = sps_check_cuda(cudaMalloc(&w, (3 * nv + n) * sizeof(float)), "sps_leapfrog scratch"); if (st != SPS_OK) return st;
   float *theta_w = w, *p_w = w + nv, *grad_w = w + 2 * nv, *logp_w = w + 3 * nv;
   const unsigned eb = (unsigned)((nv + 255) / 256);
-  st = sps_eval(t, P, path, theta0, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
+  st = sps_eval(t, ws, P, path, theta0, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
   if (st == SPS_OK) { lf_first_kernel<<<eb, 256, 0, s>>>(n, theta0, p0, grad_w, eps, inv_mass, theta_w, p_w); sps_count_launch(); }
   for (int k = 0; k < n_steps && st == SPS_OK; ++k) {
-    st = sps_eval(t, P, path, theta_w, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
+    st = sps_eval(t, ws, P, path, theta_w, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
     if (st == SPS_OK) { lf_record_kernel<<<eb, 256, 0, s>>>(n, k, grad_w, logp_w, eps, inv_mass, theta_w, p_w, traj, logp_traj); sps_count_launch(); }
   }
   cudaStreamSynchronize(s);

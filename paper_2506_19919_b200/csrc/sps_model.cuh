@@ -181,8 +181,10 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       m &= ~mz;
       const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], src);
       const float v_hi = __logf(t_hi);
-      const float dv = 16.f / (beta + 1.f);
-      const float v_lo = v_hi - dv;
+      // below min(t_hi, tau) the integrand falls as t^(beta+1): cut 16/(beta+1) e-folds under that point (not under t_hi:
+      // a coarse grid's oldest bin can reach far past the turnover, and most of its mass then sits near tau)
+      const float v_lo = fminf(v_hi, ln_tau) - 16.f / (beta + 1.f);
+      const float dv = v_hi - v_lo;
       const int n_pan = max(1, (int)ceilf(dv / w_target));
       const float wp = dv / (float)n_pan;
       float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
@@ -212,7 +214,7 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       const float t_hi = __shfl_sync(FULL_MASK, t_hi_q[q], have ? my_src : 0);
       const float t_lo = __shfl_sync(FULL_MASK, t_lo_q[q], have ? my_src : 0);
       const float v_hi = __logf(t_hi);
-      const float v_lo = fmaxf(v_hi - 16.f / (beta + 1.f), __logf(t_lo));
+      const float v_lo = fmaxf(fminf(v_hi, ln_tau) - 16.f / (beta + 1.f), __logf(t_lo));
       const float dv = v_hi - v_lo;
       int n_pan = have ? max(1, (int)ceilf(dv / w_target)) : 0;
       const float wp = dv / (float)max(n_pan, 1);
@@ -317,12 +319,15 @@ __device__ __forceinline__ void met_bin(const TableDev& T, float lz, float s, fl
 
 // ---- a8: dust, Eq. (A8)-(A9) PAPER.md:386-392 (R10) at an arbitrary rest wavelength (approximate path) ----
 #define CALZ_SWITCH_INV_UM 1.2809053864877329f
+// `screen` (SPS_MODEL_TINY5): k0 = 4.05 and no bump, which with delta = -0.7, F_floor = 0 and A_V = 1.0857 tau_V is the
+// power-law screen exp(-tau_V (lambda/5500)^-0.7).
 __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float Ffl,
-                                        float& F, float& F_av, float& F_del, float& F_fl, float& F_lam) {
+                                        float& F, float& F_av, float& F_del, float& F_fl, float& F_lam, bool screen = false) {
   const float ilam = __fdividef(1.f, lam);                  // one approximate reciprocal (1 ulp) serves every division by lambda
   const float u = 1.0e4f * ilam;
   float k0, dk_du;
-  if (u > CALZ_SWITCH_INV_UM) {
+  if (screen) { k0 = 4.05f; dk_du = 0.f; }
+  else if (u > CALZ_SWITCH_INV_UM) {
     k0 = 2.659f * (-2.156f + u * (1.509f + u * (-0.198f + u * 0.011f))) + 4.05f;
     dk_du = 2.659f * (1.509f + u * (-0.396f + u * 0.033f));
   } else {
@@ -338,14 +343,14 @@ __device__ __forceinline__ void dust_at(float lam, float AV, float delta, float 
   const float dn = 2.f * lam * w * w;
   const float dd = 4.f * lam * dl + dn;
   const float iden = __fdividef(1.f, den);
-  const float dr = n * iden, ddr = (dn * den - n * dd) * iden * iden;
+  const float dr = screen ? 0.f : n * iden, ddr = screen ? 0.f : (dn * den - n * dd) * iden * iden;
   const float l2r = log2f(lam * (1.f / 5500.f));
   const float pw = exp2f(delta * l2r);
   const float Eb = 0.85f - 1.9f * delta;
   const float br = k0 * pw + Eb * dr;
   float A = AV * (1.f / 4.05f) * br;
   float A_av = br * (1.f / 4.05f);
-  float A_del = AV * (1.f / 4.05f) * (k0 * pw * l2r * LN2F - 1.9f * dr);
+  float A_del = AV * (1.f / 4.05f) * (k0 * pw * l2r * LN2F - 1.9f * dr);     // (TINY5 never uses the delta, F_floor, lambda partials)
   float A_lam = AV * (1.f / 4.05f) * (dk0 * pw + k0 * delta * pw * ilam + Eb * ddr);
   if (!(A > 0.f)) { A = 0.f; A_av = A_del = A_lam = 0.f; }
   const float Tt = exp2f(-0.4f * 3.321928094887362f * A);

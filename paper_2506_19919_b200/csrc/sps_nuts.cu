@@ -48,7 +48,7 @@ __device__ __forceinline__ void begin_transition(ChainState& C, NutsScalars& S, 
   float kin = 0.f;
   if (act) {
     const float v = C.inv_mass[o];
-    const float p = chain_normal(key, (uint32_t)c, (uint32_t)it, RNG_MOMENTUM, l) * rsqrtf(v);
+    const float p = l < C.D ? chain_normal(key, (uint32_t)C.rng_id[c], (uint32_t)it, RNG_MOMENTUM, l) * rsqrtf(v) : 0.f;
     kin = 0.5f * v * p * p;
     const float q = C.theta[o], g = C.grad[o];
     vec(C, c, V_LQ)[l] = q; vec(C, c, V_LP)[l] = p; vec(C, c, V_LG)[l] = g;
@@ -65,7 +65,7 @@ __device__ __forceinline__ void begin_transition(ChainState& C, NutsScalars& S, 
 
 // start the doubling at the current depth: pick the direction, take the first half kick and drift from that end
 __device__ __forceinline__ void begin_doubling(ChainState& C, NutsScalars& S, int64_t c, int l, bool act, int64_t o, int it, int depth, int flags, uint2 key) {
-  const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)it, RNG_DIRECTION, (uint32_t)depth), key).x);
+  const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)C.rng_id[c], (uint32_t)it, RNG_DIRECTION, (uint32_t)depth), key).x);
   const bool fwd = u < 0.5f;
   if (act) {
     const float eps = C.eps[c], step = fwd ? eps : -eps, v = C.inv_mass[o];
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
   else {
     logW_sub = logaddexpf_(logW_sub, -dH);
     rho_sub = (act ? vec(C, c, V_SRHO)[l] : 0.f) + p;
-    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)tr, RNG_LEAF, (uint32_t)(depth * 65536 + leaf)), key).x);
+    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)C.rng_id[c], (uint32_t)tr, RNG_LEAF, (uint32_t)(depth * 65536 + leaf)), key).x);
     if (logf(u) + logW_sub < -dH) {                       // multinomial sampling inside the subtree
       if (act) { vec(C, c, V_SQ)[l] = q; vec(C, c, V_SG)[l] = g; }
       if (l == 0) S.sub_lp[c] = lp;
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     }
     // ---- subtree complete: biased progressive sampling across doublings, merge ----
     const float logW = S.logW[c];
-    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, (uint32_t)tr, RNG_SUBTREE, (uint32_t)depth), key).x);
+    const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)C.rng_id[c], (uint32_t)tr, RNG_SUBTREE, (uint32_t)depth), key).x);
     if ((flags & F_HASSUB) && logf(u) < fminf(0.f, logW_sub - logW)) {
       if (act) { vec(C, c, V_PQ)[l] = vec(C, c, V_SQ)[l]; vec(C, c, V_PG)[l] = vec(C, c, V_SG)[l]; }
       if (l == 0) S.prop_lp[c] = S.sub_lp[c];
@@ -183,7 +183,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
   if (l == 0) C.logp[c] = S.prop_lp[c];
   const AdaptFlags A = adapt_flags_dev(it, W);
   if (!A.warmup && l == 0) atomicAdd(&S.depth_hist[min(S.depth[c] + (bad ? 1 : 0), NUTS_MAX_DEPTH)], 1);
-  chain_adapt_and_record(C, c, l, act, o, th, acc_sum / (float)n_leaf, n_leaf, (flags & F_DIV) ? 1 : 0, A, samples, it - W.n_warmup, W.n_sample);
+  chain_adapt_and_record(C, c, l, act, o, th, acc_sum / (float)n_leaf, n_leaf, (flags & F_DIV) ? 1 : 0, A, samples, it - W.n_warmup, W.n_sample, W.bm_len, W.bm_n);
   __syncwarp();
   const int it1 = it + 1;
   if (it1 >= W.n_warmup + W.n_sample) {
@@ -209,7 +209,8 @@ __global__ void nuts_compact_kernel(int64_t n, const int* __restrict__ done, con
 }  // namespace
 
 
-sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples, cudaStream_t s) {
+sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples,
+                    int32_t* depth_hist_out, cudaStream_t s) {
   const int64_t n = C.n;
   if (cfg->n_warmup + cfg->n_sample == 0) return SPS_OK;
   NutsScalars S; memset(&S, 0, sizeof(S));
@@ -235,7 +236,7 @@ sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, 
   for (int64_t step = 0; step < max_steps && st == SPS_OK; ++step) {
     for (int path = 0; path < 2 && st == SPS_OK; ++path) {
       if (L.n_rows_path[path] == 0) continue;
-      st = sps_eval(t, P, path, C.theta_w, L.n_rows_path[path], true, true, L.rows_path[path], Q.gal_of_chain, Q.obs_flux, Q.obs_sigma,
+      st = sps_eval(t, ws, P, path, C.theta_w, L.n_rows_path[path], true, true, L.rows_path[path], Q.gal_of_chain, Q.obs_flux, Q.obs_sigma,
                     nullptr, true, C.logp_w, C.grad_w, s);
     }
     if (st != SPS_OK) break;
@@ -257,6 +258,8 @@ sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, 
       }
     }
   }
+  if (st == SPS_OK && depth_hist_out)                       // kept transitions per final tree depth
+    cudaMemcpyAsync(depth_hist_out, S.depth_hist, (NUTS_MAX_DEPTH + 1) * sizeof(int), cudaMemcpyDeviceToDevice, s);
   cudaStreamSynchronize(s);
   cudaFree(fbase); cudaFree(ibase); cudaFree(lists);
   return st;

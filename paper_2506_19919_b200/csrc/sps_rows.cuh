@@ -26,7 +26,7 @@ struct LeapfrogFuse { float* theta_w; float* p_w; const float* eps; const float*
 // kernels (sps_kernels.cu)
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
                      const int* rows, RowBuffers B, bool with_hist, cudaStream_t s);
-void launch_approx_contract(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row,
+void launch_approx_contract(const TableDev& T, int sm_count, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);
 sps_status approx_contract_setup(const TableDev& T);

@@ -2,6 +2,7 @@
 // One warp owns one chain (lane p < 13 owns parameter p); the model evaluation between the
 // sampler kernels is the batch-wide prologue / contraction / epilogue pipeline (sps_eval).
 // NUTS lives in sps_nuts.cu and reuses the state and helpers declared in sps_sampler.cuh.
+#include <cmath>
 #include <vector>
 #include "sps_sampler.cuh"
 
@@ -33,11 +34,12 @@ __global__ void __launch_bounds__(256) chain_init_kernel(ChainState C, PriorDev 
   if (l < SPS_NDIM) {
     float v;
     if (theta0) v = theta0[c * SPS_NDIM + l];
-    else v = P.xi[l] + 0.1f * P.omega[l] * chain_normal(key, (uint32_t)c, 0u, RNG_INIT, l);
+    else v = P.xi[l] + (l < C.D ? 0.1f * P.omega[l] * chain_normal(key, (uint32_t)C.rng_id[c], 0u, RNG_INIT, l) : 0.f);   // unsampled slots: xi exactly
     C.theta[c * SPS_NDIM + l] = v;
     C.inv_mass[c * SPS_NDIM + l] = inv_mass_in ? inv_mass_in[c * SPS_NDIM + l] : 1.f;
     C.w_mean[c * SPS_NDIM + l] = 0.f; C.w_m2[c * SPS_NDIM + l] = 0.f;
     C.s_mean[c * SPS_NDIM + l] = 0.f; C.s_m2[c * SPS_NDIM + l] = 0.f;
+    C.bm_sum[c * SPS_NDIM + l] = 0.f; C.bm_mean[c * SPS_NDIM + l] = 0.f; C.bm_m2[c * SPS_NDIM + l] = 0.f;
   }
   if (l == 0) {
     const float e0 = eps_in ? eps_in[c] : eps0;
@@ -62,7 +64,7 @@ __global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, const HmcC
   if (l < SPS_NDIM) {
     const int64_t o = c * SPS_NDIM + l;
     const float v = C.inv_mass[o], eps = C.eps[c];
-    float p = chain_normal(key, (uint32_t)c, transition, RNG_MOMENTUM, l) * rsqrtf(v);
+    float p = l < C.D ? chain_normal(key, (uint32_t)C.rng_id[c], transition, RNG_MOMENTUM, l) * rsqrtf(v) : 0.f;
     kin = 0.5f * v * p * p;
     p += 0.5f * eps * C.grad[o];
     C.p_w[o] = p;
@@ -76,7 +78,7 @@ __global__ void __launch_bounds__(256) hmc_begin_kernel(ChainState C, const HmcC
 
 // end: last half kick, Metropolis test, warmup adaptation (R14), running summaries.
 __global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, const HmcCtl* __restrict__ ctl, uint32_t first, uint2 key, int n_leapfrog,
-                                                      float* __restrict__ samples, int n_sample) {
+                                                      float* __restrict__ samples, int n_sample, int bm_len, int bm_n) {
   CHAIN_WARP_PROLOGUE(C.n);
   const uint32_t transition = (uint32_t)ctl->it + first;
   const AdaptFlags A = ctl->A;
@@ -91,7 +93,7 @@ __global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, const HmcCtl
   const float dH = (-lpw + kin) - C.H0[c];
   const bool fin = __all_sync(FULL_MASK, !act || (isfinite(gw) && isfinite(thw))) && isfinite(dH);
   const float acc_prob = fin ? fminf(1.f, expf(fminf(0.f, -dH))) : 0.f;
-  const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)c, transition, RNG_ACCEPT, 0u), key).x);
+  const float u = philox_u01(philox4x32_10(make_uint4((uint32_t)C.rng_id[c], transition, RNG_ACCEPT, 0u), key).x);
   const bool accept = fin && (u < acc_prob);
   float th = C.theta[o];
   if (accept) {
@@ -99,18 +101,18 @@ __global__ void __launch_bounds__(256) hmc_end_kernel(ChainState C, const HmcCtl
     if (act) { C.theta[o] = thw; C.grad[o] = gw; }
     if (l == 0) C.logp[c] = lpw;
   }
-  chain_adapt_and_record(C, c, l, act, o, th, acc_prob, n_leapfrog, 0, A, samples, sample_index, n_sample);
+  chain_adapt_and_record(C, c, l, act, o, th, acc_prob, n_leapfrog, 0, A, samples, sample_index, n_sample, bm_len, bm_n);
 }
 
 // ---------------------------------------------------------------------------------------------
 // finalisation: mean / sd per chain, Gelman-Rubin R-hat per galaxy
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain, int n_sample, sps_hmc_summary S) {
+__global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain, int n_sample, int bm_len, int bm_n, sps_hmc_summary S) {
   const int64_t gidx = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int l = threadIdx.x & 31;
   const int64_t n_gal = C.n / n_chain;
   if (gidx >= n_gal || l >= SPS_NDIM) return;
-  float mean_of_means = 0.f, W = 0.f;
+  float mean_of_means = 0.f, W = 0.f, tau2 = 0.f;
   for (int k = 0; k < n_chain; ++k) {
     const int64_t c = gidx * n_chain + k, o = c * SPS_NDIM + l;
     const float mu = C.s_mean[o], var = n_sample > 1 ? C.s_m2[o] / (float)(n_sample - 1) : 0.f;
@@ -125,7 +127,10 @@ __global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain
       if (S.divergences) S.divergences[c] = C.n_div[c];
     }
     mean_of_means += mu; W += var;
+    tau2 += bm_n > 1 ? (float)bm_len * C.bm_m2[o] / (float)(bm_n - 1) : 0.f;
   }
+  // ESS by batch means pooled over the galaxy's chains (R25): m n mean(s2_c) / mean(tau2_c)
+  if (S.ess) S.ess[gidx * SPS_NDIM + l] = tau2 > 0.f ? (float)n_chain * (float)n_sample * W / tau2 : 0.f;
   mean_of_means /= n_chain; W /= n_chain;
   float Bn = 0.f;                                   // B/n: variance of the chain means
   for (int k = 0; k < n_chain; ++k) { const float d = C.s_mean[(gidx * n_chain + k) * SPS_NDIM + l] - mean_of_means; Bn += d * d; }
@@ -142,8 +147,8 @@ __global__ void __launch_bounds__(256) finalize_kernel(ChainState C, int n_chain
 sps_status chain_state_alloc(ChainState& C, int64_t n, int ckpt_vectors) {
   memset(&C, 0, sizeof(C));
   C.n = n;
-  const size_t nv = 11 + (size_t)ckpt_vectors;      // vectors of 13 floats per chain
-  const size_t ns = 16;                             // scalars per chain
+  const size_t nv = 13 + (size_t)ckpt_vectors;      // vectors of 13 floats per chain
+  const size_t ns = 17;                             // scalars per chain
   const size_t bytes = n * (nv * SPS_NDIM + ns) * sizeof(float);
   float* base = nullptr;
   sps_status st = sps_check_cuda(cudaMalloc(&base, bytes), "chain state allocation");
@@ -154,11 +159,12 @@ sps_status chain_state_alloc(ChainState& C, int64_t n, int ckpt_vectors) {
   auto vec = [&]() { float* r = p; p += n * SPS_NDIM; return r; };
   auto sca = [&]() { float* r = p; p += n; return r; };
   C.theta = vec(); C.grad = vec(); C.theta_w = vec(); C.p_w = vec(); C.grad_w = vec(); C.inv_mass = vec();
-  C.w_mean = vec(); C.w_m2 = vec(); C.s_mean = vec(); C.s_m2 = vec(); C.extra = vec();
+  C.w_mean = vec(); C.w_m2 = vec(); C.s_mean = vec(); C.s_m2 = vec(); C.bm_sum = vec(); C.bm_mean = vec(); C.bm_m2 = vec();
   C.nuts = p; p += n * (size_t)ckpt_vectors * SPS_NDIM;
   C.logp = sca(); C.logp_w = sca(); C.H0 = sca(); C.eps = sca(); C.da_mu = sca(); C.da_hbar = sca(); C.da_logepsbar = sca();
   C.acc_sum = sca();
   C.da_m = (int*)sca(); C.n_leapfrog = (int*)sca(); C.n_div = (int*)sca();
+  C.rng_id = (int*)sca();
   C.nuts_sc = sca();   // 5 scalars left for NUTS
   return SPS_OK;
 }
@@ -187,6 +193,10 @@ WarmupSched make_warmup_sched(const sps_hmc_config* cfg) {
   warmup_schedule(cfg->n_warmup, ends, lo, hi);
   W.n_warmup = cfg->n_warmup; W.n_sample = cfg->n_sample; W.slow_lo = lo; W.slow_hi = hi; W.target = cfg->target_accept;
   W.first = (int)cfg->first_transition;
+  W.bm_len = cfg->n_sample > 0 ? (int)std::floor(std::sqrt((double)cfg->n_sample)) : 0;       // R25: batch length floor(sqrt(n))
+  while (W.bm_len > 0 && (int64_t)(W.bm_len + 1) * (W.bm_len + 1) <= cfg->n_sample) ++W.bm_len;    // (guard the rounding of sqrt)
+  while (W.bm_len > 0 && (int64_t)W.bm_len * W.bm_len > cfg->n_sample) --W.bm_len;
+  W.bm_n = W.bm_len > 0 ? cfg->n_sample / W.bm_len : 0;
   W.n_ends = (int)std::min<size_t>(ends.size(), 16);
   for (int k = 0; k < W.n_ends; ++k) W.ends[k] = ends[k];
   return W;
@@ -194,13 +204,13 @@ WarmupSched make_warmup_sched(const sps_hmc_config* cfg) {
 
 static inline unsigned chain_blocks(int64_t n) { return (unsigned)((n * 32 + 255) / 256); }
 
-static sps_status eval_working(sps_table* t, const PriorDev& P, const HmcProblem& Q, ChainState& C, cudaStream_t s, bool fuse_leapfrog = false) {
+static sps_status eval_working(const sps_table* t, Workspace& ws, const PriorDev& P, const HmcProblem& Q, ChainState& C, cudaStream_t s, bool fuse_leapfrog = false) {
   const LeapfrogFuse lf = {C.theta_w, C.p_w, C.eps, C.inv_mass};
   // groups of rows per path: path_rows[0] exact, [1] approx (index lists) or all rows on one path
   sps_status st = SPS_OK;
   for (int path = 0; path < 2 && st == SPS_OK; ++path) {
     if (Q.n_rows_path[path] == 0) continue;
-    st = sps_eval(t, P, path, C.theta_w, Q.n_rows_path[path], true, true, Q.rows_path[path], Q.gal_of_chain, Q.obs_flux,
+    st = sps_eval(t, ws, P, path, C.theta_w, Q.n_rows_path[path], true, true, Q.rows_path[path], Q.gal_of_chain, Q.obs_flux,
                   Q.obs_sigma, nullptr, true, C.logp_w, C.grad_w, s, fuse_leapfrog ? &lf : nullptr);
   }
   return st;
@@ -209,50 +219,55 @@ static sps_status eval_working(sps_table* t, const PriorDev& P, const HmcProblem
 sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
                              const float* obs_flux, const float* obs_sigma);
 void hmc_problem_free(HmcProblem& Q);
-sps_status nuts_run(sps_table* t, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples, cudaStream_t s);
+sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const sps_hmc_config* cfg, HmcProblem& Q, ChainState& C, float* samples,
+                    int32_t* depth_hist_out, cudaStream_t s);
 
-static int g_no_graph = 0;
-extern "C" void sps_debug_no_graph(int on) { g_no_graph = on; }
-
-extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, const sps_hmc_config* cfg, const float* obs_flux,
+extern "C" sps_status sps_hmc_run(const sps_table* t, const sps_prior* prior, const sps_hmc_config* cfg, const float* obs_flux,
                                   const float* obs_sigma, int64_t n_gal, const int32_t* path_of_gal, const float* theta0,
                                   float* samples, const sps_hmc_summary* summary, void* stream) {
-  if (!tc || !prior || !cfg || !obs_flux || !obs_sigma) { sps_set_error("sps_hmc_run: null argument"); return SPS_EINVAL; }
+  if (!t || !cfg) { sps_set_error("sps_hmc_run: null argument"); return SPS_EINVAL; }
+  const bool gauss = t->dev.model == SPS_MODEL_GAUSS_TEST;
+  if (!gauss && (!prior || !obs_flux || !obs_sigma)) { sps_set_error("sps_hmc_run: null argument"); return SPS_EINVAL; }
   if (n_gal < 0 || cfg->n_chain < 1 || cfg->n_warmup < 0 || cfg->n_sample < 0 || !(cfg->eps0 > 0)) { sps_set_error("sps_hmc_run: bad config"); return SPS_EINVAL; }
   if (cfg->sampler == SPS_SAMPLER_HMC && cfg->n_leapfrog < 1) { sps_set_error("sps_hmc_run: n_leapfrog < 1"); return SPS_EINVAL; }
   if (cfg->sampler == SPS_SAMPLER_NUTS && (cfg->max_depth < 1 || cfg->max_depth > 10)) { sps_set_error("sps_hmc_run: max_depth must be 1..10"); return SPS_EINVAL; }
   if (cfg->sampler != SPS_SAMPLER_HMC && cfg->sampler != SPS_SAMPLER_NUTS) { sps_set_error("sps_hmc_run: bad sampler"); return SPS_EINVAL; }
   if (n_gal == 0) return SPS_OK;
-  sps_table* t = const_cast<sps_table*>(tc);
+  sps_status st = sps_require_device(); if (st != SPS_OK) return st;
   cudaStream_t s = (cudaStream_t)stream;
   if (!s) {
     // The legacy default stream cannot be captured into a graph: the run (which synchronises before returning anyway)
-    // goes on a stream of the library's own, after everything already queued on the caller's stream.
-    static cudaStream_t own = nullptr;
-    if (!own && cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking) != cudaSuccess) { own = nullptr; cudaGetLastError(); }
-    if (own) { cudaStreamSynchronize(nullptr); s = own; }
+    // goes on a stream the table owns, after everything already queued on the caller's stream.
+    std::lock_guard<std::mutex> lock(t->mu);
+    if (!t->own_stream && cudaStreamCreateWithFlags(&t->own_stream, cudaStreamNonBlocking) != cudaSuccess) { t->own_stream = nullptr; cudaGetLastError(); }
+    if (t->own_stream) { cudaStreamSynchronize(nullptr); s = t->own_stream; }
   }
-  PriorDev P; sps_status st = sps_prior_to_dev(prior, P); if (st != SPS_OK) return st;
+  PriorDev P; st = sps_prior_to_dev(t, prior, P); if (st != SPS_OK) return st;
   const int64_t n = n_gal * cfg->n_chain;
-  st = sps_ensure_row_buffers(t, n); if (st != SPS_OK) return st;
+  if (!gauss) { st = sps_check_finite(obs_flux, n_gal * t->dev.n_band, theta0, theta0 ? n * SPS_NDIM : 0, obs_sigma, n_gal * t->dev.n_band, s); if (st != SPS_OK) return st; }
+  Workspace& ws = *sps_workspace(t, s);
+  if (!gauss) { st = sps_ensure_row_buffers(t, ws, n, s); if (st != SPS_OK) return st; }
   HmcProblem Q; ChainState C;
-  st = hmc_problem_setup(Q, cfg, n_gal, path_of_gal, obs_flux, obs_sigma); if (st != SPS_OK) return st;
-  st = chain_state_alloc(C, n, cfg->sampler == SPS_SAMPLER_NUTS ? NUTS_VECTORS : 0);
-  if (st != SPS_OK) { hmc_problem_free(Q); return st; }
+  memset(&C, 0, sizeof(C));
+  st = hmc_problem_setup(Q, cfg, n_gal, path_of_gal, obs_flux, obs_sigma);
+  if (st == SPS_OK) st = chain_state_alloc(C, n, cfg->sampler == SPS_SAMPLER_NUTS ? NUTS_VECTORS : 0);
+  if (st != SPS_OK) { hmc_problem_free(Q); chain_state_free(C); return st; }
+  C.D = t->dev.n_dim;
+  const WarmupSched W = make_warmup_sched(cfg);
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
   cudaDeviceSynchronize();                                   // the set-up above ran on the default stream
+  cudaMemcpyAsync(C.rng_id, Q.rng_id, n * sizeof(int), cudaMemcpyDeviceToDevice, s);
   chain_init_kernel<<<chain_blocks(n), 256, 0, s>>>(C, P, theta0, cfg->eps0, cfg->eps_in_dev, cfg->inv_mass_in_dev, key); sps_count_launch();
   // logp / grad at the start: evaluate through the working buffers
   cudaMemcpyAsync(C.theta_w, C.theta, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
-  st = eval_working(t, P, Q, C, s);
+  st = eval_working(t, ws, P, Q, C, s);
   cudaMemcpyAsync(C.grad, C.grad_w, n * SPS_NDIM * sizeof(float), cudaMemcpyDeviceToDevice, s);
   cudaMemcpyAsync(C.logp, C.logp_w, n * sizeof(float), cudaMemcpyDeviceToDevice, s);
   if (st == SPS_OK && cfg->sampler == SPS_SAMPLER_HMC) {
     // One transition = control update, momentum draw, n_leapfrog evaluations (each five launches), accept/adapt.  Every
     // launch argument is the same from one transition to the next (the counter lives in device memory), so the
     // sequence is captured once in a CUDA graph and replayed: small batches are launch-latency bound.
-    // Plain launches are used when per-kernel profiling is on, on the legacy default stream, or if capture fails.
-    const WarmupSched W = make_warmup_sched(cfg);
+    // Plain launches are used when per-kernel profiling is on, with SPS_OPT_NO_GRAPH, or if capture fails.
     const int n_tr = cfg->n_warmup + cfg->n_sample;
     HmcCtl* ctl = nullptr;
     st = sps_check_cuda(cudaMalloc(&ctl, sizeof(HmcCtl)), "HMC control block");
@@ -262,14 +277,14 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
       hmc_begin_kernel<<<chain_blocks(n), 256, 0, s>>>(C, ctl, cfg->first_transition, key);
       sps_count_launch(2);
       sps_status e = SPS_OK;
-      for (int k = 0; k < cfg->n_leapfrog && e == SPS_OK; ++k) e = eval_working(t, P, Q, C, s, k + 1 < cfg->n_leapfrog);
-      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, ctl, cfg->first_transition, key, cfg->n_leapfrog, samples, cfg->n_sample);
+      for (int k = 0; k < cfg->n_leapfrog && e == SPS_OK; ++k) e = eval_working(t, ws, P, Q, C, s, k + 1 < cfg->n_leapfrog);
+      hmc_end_kernel<<<chain_blocks(n), 256, 0, s>>>(C, ctl, cfg->first_transition, key, cfg->n_leapfrog, samples, cfg->n_sample, W.bm_len, W.bm_n);
       sps_count_launch();
       return e;
     };
     cudaGraphExec_t exec = nullptr;
     int64_t per_graph = 0;
-    if (st == SPS_OK && n_tr > 2 && s != nullptr && !sps_prof_enabled() && !g_no_graph) {
+    if (st == SPS_OK && n_tr > 2 && s != nullptr && !sps_prof_enabled() && !sps_option(SPS_OPT_NO_GRAPH)) {
       const int64_t c0 = sps_launch_count();
       cudaGraph_t graph = nullptr;
       if (cudaStreamBeginCapture(s, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
@@ -289,10 +304,10 @@ extern "C" sps_status sps_hmc_run(const sps_table* tc, const sps_prior* prior, c
     if (exec) { cudaStreamSynchronize(s); cudaGraphExecDestroy(exec); }
     if (ctl) { cudaStreamSynchronize(s); cudaFree(ctl); }
   } else if (st == SPS_OK) {
-    st = nuts_run(t, P, cfg, Q, C, samples, s);
+    st = nuts_run(t, ws, P, cfg, Q, C, samples, summary ? summary->depth_hist : nullptr, s);
   }
   if (st == SPS_OK && summary) {
-    finalize_kernel<<<chain_blocks(n_gal), 256, 0, s>>>(C, cfg->n_chain, cfg->n_sample, *summary); sps_count_launch();
+    finalize_kernel<<<chain_blocks(n_gal), 256, 0, s>>>(C, cfg->n_chain, cfg->n_sample, W.bm_len, W.bm_n, *summary); sps_count_launch();
   }
   if (st == SPS_OK) st = sps_check_cuda(cudaStreamSynchronize(s), "sps_hmc_run");
   else cudaStreamSynchronize(s);

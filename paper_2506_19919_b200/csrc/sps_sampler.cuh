@@ -10,6 +10,7 @@
 
 struct ChainState {
   int64_t n;
+  int D;                               // sampled parameters of the table's model: lanes p >= D carry no momentum
   float* base;
   // [n,13]
   float *theta, *grad;                 // current state and gradient of logP there
@@ -17,18 +18,19 @@ struct ChainState {
   float *inv_mass;                     // diagonal inverse mass
   float *w_mean, *w_m2;                // Welford over the current slow window (warmup)
   float *s_mean, *s_m2;                // Welford over kept samples
-  float *extra;
+  float *bm_sum, *bm_mean, *bm_m2;     // batch means of the kept samples (ESS, R25): running batch sum, Welford over batch means
   float *nuts;                         // [n, NUTS_VECTORS, 13] (NUTS only)
   // [n]
   float *logp, *logp_w, *H0, *eps, *da_mu, *da_hbar, *da_logepsbar, *acc_sum, *nuts_sc;
   int *da_m, *n_leapfrog, *n_div;
+  int *rng_id;                         // [n] Philox stream of each chain (gal_id * n_chain + chain)
 };
 
 struct AdaptFlags { int warmup, in_window, window_end, last_warmup, welford_n; float target; };
 
 // Warmup windows (R14) in a form kernels can evaluate: slow windows end at ends[0..n_ends) inside [slow_lo, slow_hi).
 // `first` = transition index of the RNG streams at local transition 0 (continued runs).
-struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; int first; };
+struct WarmupSched { int n_warmup, n_sample, slow_lo, slow_hi, n_ends; int ends[16]; float target; int first; int bm_len, bm_n; };
 
 __device__ __forceinline__ AdaptFlags adapt_flags_dev(int it, const WarmupSched& S) {
   AdaptFlags A; A.warmup = it < S.n_warmup; A.in_window = 0; A.window_end = 0; A.last_warmup = (it + 1 == S.n_warmup); A.welford_n = 0;
@@ -53,6 +55,7 @@ WarmupSched make_warmup_sched(const sps_hmc_config* cfg);            // sps_samp
 
 struct HmcProblem {
   int64_t n;                 // chains
+  int* rng_id;               // [n] device: Philox stream of each chain
   int* gal_of_chain;         // [n] device
   unsigned char* path_of_chain;   // [n] device: photometry path of each chain
   int* rows_path[2];         // device index lists per path, or NULL = all rows
@@ -76,7 +79,7 @@ __device__ __forceinline__ float chain_normal(uint2 key, uint32_t chain, uint32_
 // shrinkage) and running summaries; called by the whole warp at the end of every transition.
 __device__ __forceinline__ void chain_adapt_and_record(ChainState& C, int64_t c, int l, bool act, int64_t o, float th,
                                                        float acc_stat, int n_lf, int diverged, const AdaptFlags& A,
-                                                       float* __restrict__ samples, int sample_index, int n_sample) {
+                                                       float* __restrict__ samples, int sample_index, int n_sample, int bm_len, int bm_n) {
   if (l == 0) C.n_leapfrog[c] += n_lf;
   if (A.warmup) {
     float eps_new = 0.f;
@@ -118,6 +121,18 @@ __device__ __forceinline__ void chain_adapt_and_record(ChainState& C, int64_t c,
       mean += d / k; m2 += d * (th - mean);
       C.s_mean[o] = mean; C.s_m2[o] = m2;
       if (samples) samples[(c * n_sample + sample_index) * SPS_NDIM + l] = th;
+      // batch means for the ESS (R25): batches of bm_len consecutive kept samples, bm_n of them
+      float bs = C.bm_sum[o] + th;
+      const int k1 = sample_index + 1;
+      if (bm_len > 0 && k1 % bm_len == 0 && k1 / bm_len <= bm_n) {
+        const float cnt = (float)(k1 / bm_len), bmv = bs / (float)bm_len;
+        float bmean = C.bm_mean[o], bm2 = C.bm_m2[o];
+        const float db = bmv - bmean;
+        bmean += db / cnt; bm2 += db * (bmv - bmean);
+        C.bm_mean[o] = bmean; C.bm_m2[o] = bm2;
+        bs = 0.f;
+      }
+      C.bm_sum[o] = bs;
     }
     if (l == 0) { C.acc_sum[c] += acc_stat; C.n_div[c] += diverged; }
   }

@@ -37,25 +37,47 @@ def _grad_err(g, ref, floor=1e-3):
 
 
 TC_FLOOR = 1e-2          # tensor-core exact path: absolute term 1e-3 * 1e-2 |g|_inf
+# DESIGN.md reading R23: near the mode the log-likelihood gradient sum_b (d_b - f_b)/sigma_b^2 J_b is a difference of large
+# terms, so a relative flux error eps enters it as eps sum_b f_b/sigma_b^2 |J_b|.  eps per kernel family = its measured worst
+# flux error against the oracle (fp32 kernels 3.4e-6, tcgen05 approximate 3.2e-6, tcgen05 exact
+# 1.7e-5 from the truncating tensor-core accumulation), all far inside north_star's 1e-4 on fluxes.  Rows >= 1 sigma from
+# the mode are held to the unmodified rule (_far_rows_strict).
+FLUX_EPS_FP32, FLUX_EPS_TC_EXACT = 4e-6, 2e-5
+
+
+def _far_rows_strict(cx, path, name, truth_u, d, s, n_chain, floor=1e-3):
+    """Rows one prior-scale unit 1/k from the truth in every parameter (residuals of ~20 sigma): the gradient rule exactly as
+    SURVEY.md 8(c) states it, floor 1e-3 and no allowance, for every kernel family."""
+    n_gal = truth_u.shape[0]
+    sign = np.random.default_rng(17).choice([-1.0, 1.0], size=(n_gal * n_chain, 13))
+    thu = (np.repeat(truth_u, n_chain, 0) + 1.0 * sign / cx.P[2]).astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, path, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+    olp, og, of = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), name,
+                                  cx.cssp() if name == "approx" else None)
+    r = np.abs(of - d[gal]) / s[gal]
+    assert np.median(r.max(1)) > 3.0                                  # these rows are far from their data
+    assert _grad_err(g.cpu().numpy(), og, 1e-3).max() <= 1e-3, name
+    assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4, name
 
 
 @pytest.fixture(params=["tcgen05", "simt_fp32"])
 def exact_kernels(request):
     """Runs an exact-path test through the tcgen05 kernels and through the fp32 SIMT cross-check kernels."""
-    from paper_2506_19919_b200 import binding
+    sps = _sps()
     simt = request.param == "simt_fp32"
-    binding.lib().sps_debug_force_simt(int(simt))
+    sps.sps_set_option(sps.OPT_EXACT_SIMT, int(simt))
     yield 1e-3 if simt else TC_FLOOR
-    binding.lib().sps_debug_force_simt(0)
+    sps.sps_set_option(sps.OPT_EXACT_SIMT, 0)
 
 
 @pytest.fixture(params=["tcgen05", "simt_fp32"])
 def approx_kernels(request):
     """Runs an approximate-path test through the tcgen05 contraction (FP16 split) and through the fp32 SIMT contraction."""
-    from paper_2506_19919_b200 import binding
-    binding.lib().sps_debug_approx_simt(int(request.param == "simt_fp32"))
+    sps = _sps()
+    sps.sps_set_option(sps.OPT_APPROX_SIMT, int(request.param == "simt_fp32"))
     yield request.param
-    binding.lib().sps_debug_approx_simt(0)
+    sps.sps_set_option(sps.OPT_APPROX_SIMT, 0)
 
 
 class Ctx:
@@ -232,9 +254,10 @@ def test_loglike_grad_approx(kind, request, approx_kernels):
     # <= 3.6e-6 in all, against north_star's 1e-4 on fluxes)
     th, dth = M.bound(thu.astype(np.float64), cx.P)
     of, J = M.photometry_approx(th, cx.grid, cx.cssp())
-    allow = 4e-6 * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
+    allow = FLUX_EPS_FP32 * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
     err = np.maximum(np.abs(g.cpu().numpy() - og) - allow, 0.0)
     assert (err / np.maximum(np.abs(og), 1e-3 * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
+    _far_rows_strict(cx, cx.sps.PATH_APPROX, "approx", truth_u, d, s, n_chain)
 
 
 def test_leapfrog_trajectory_approx(tiny):
@@ -448,12 +471,13 @@ def test_loglike_grad_exact(kind, n_gal, request, exact_kernels):
     # The likelihood gradient is sum_b (d_b - f_b)/sigma_b^2 J_b: a flux error eps f_b enters as eps sum_b f_b/sigma_b^2 |J_b|,
     # which near the mode (d ~ f) is not small against g.  eps = 2e-5 covers the tensor-core accumulation bias
     # (measured <= 1.4e-5; north_star allows 1e-4 on fluxes); the fp32 kernels get no allowance.
-    eps_flux = 2e-5 if floor == TC_FLOOR else 0.0
+    eps_flux = FLUX_EPS_TC_EXACT if floor == TC_FLOOR else 0.0
     th, dth = M.bound(thu.astype(np.float64), cx.P)
     of, J = M.photometry_exact(th, cx.grid)
     allow = eps_flux * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
     err = np.abs(g.cpu().numpy() - og) - allow
     assert (err / np.maximum(np.abs(og), floor * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
+    _far_rows_strict(cx, cx.sps.PATH_EXACT, "exact", truth_u, d, s, n_chain, floor)
 
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled rows ---------------------------
@@ -514,7 +538,7 @@ def test_full_size_hmc_loglike_sampled(full):
     # band flux (measured <= 2.5e-6), thirty times below north_star's flux tolerance.
     th, dth = M.bound(thu[sel].astype(np.float64), cx.P)
     of, J = M.photometry_approx(th, cx.grid, cx.cssp())
-    allow = 3e-6 * np.einsum("rb,rbp->rp", of / s[gal[sel]].astype(np.float64) ** 2, np.abs(J)) * dth
+    allow = FLUX_EPS_FP32 * np.einsum("rb,rbp->rp", of / s[gal[sel]].astype(np.float64) ** 2, np.abs(J)) * dth
     err = np.maximum(np.abs(g.cpu().numpy()[sel] - og) - allow, 0.0)
     assert (err / np.maximum(np.abs(og), 1e-3 * np.abs(og).max(1, keepdims=True))).max() <= 1e-3
 
@@ -550,7 +574,7 @@ def test_odd_shape_both_paths(odd, exact_kernels):
         olp, og, _ = M.logp_and_grad(thu.astype(np.float64), cx.grid, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), name, cx.cssp())
         assert (np.abs(lp.cpu().numpy() - olp) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4, name
         J = (M.photometry_approx(th, cx.grid, cx.cssp())[1] if name == "approx" else M.photometry_exact(th, cx.grid)[1])
-        eps_flux = 2e-5 if fl == TC_FLOOR else 3e-6
+        eps_flux = FLUX_EPS_TC_EXACT if fl == TC_FLOOR else FLUX_EPS_FP32
         allow = eps_flux * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
         err = np.maximum(np.abs(g.cpu().numpy() - og) - allow, 0.0)
         assert (err / np.maximum(np.abs(og), fl * np.abs(og).max(1, keepdims=True))).max() <= 1e-3, name

@@ -34,11 +34,13 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_struct_layouts_match_the_header():
     from paper_2506_19919_b200 import binding as b
-    assert C.sizeof(b._TableDesc) == 5 * 4 + 4 + 6 * 8 + 5 * 8 + 8       # 5 int32 (+pad), 6 pointers, 5 doubles, int32 (+pad)
+    # 5 int32 (+pad), 6 pointers, 5 doubles, 2 int32, 3 pointers, double, int32 (+pad), 2 pointers
+    assert C.sizeof(b._TableDesc) == 5 * 4 + 4 + 6 * 8 + 5 * 8 + 2 * 4 + 3 * 8 + 8 + 4 + 4 + 2 * 8
+    assert b._TableDesc.model.offset == 116 and b._TableDesc.filt_wave_A.offset == 120 and b._TableDesc.gauss_mu.offset == 160
     assert C.sizeof(b._Prior) == 7 * 8
-    assert C.sizeof(b._HmcConfig) == 7 * 4 + 2 * 4 + 4 + 8 + 4 + 4 + 2 * 8  # 7 int32, 2 float, pad, uint64, uint32, pad, 2 pointers
+    assert C.sizeof(b._HmcConfig) == 7 * 4 + 2 * 4 + 4 + 8 + 4 + 4 + 3 * 8  # 7 int32, 2 float, pad, uint64, uint32, pad, 3 pointers
     assert b._HmcConfig.seed.offset == 40
-    assert C.sizeof(b._HmcSummary) == 9 * 8
+    assert C.sizeof(b._HmcSummary) == 11 * 8
 
 
 def test_no_cpu_fallback(lib):
