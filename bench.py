@@ -252,3 +252,241 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.workload, args.protocol, budget_s=args.cpu_budget)
     print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------
+# rooflines (DESIGN.md sections 5 and 6 derive every count used here)
+# ------------------------------------------------------------------------------------------------
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), at the
+# launch sizes named there; None where no capture of that launch size exists.
+NCU_TRAFFIC = {
+    ("prologue", 40000): 71.1e6, ("approx_contract", 40000): 84.8e6, ("epilogue", 40000): 139.9e6,   # profiles/r01_hmc_kernels_full.md
+    ("exact_fwd", 8192): 74.2e6,                                                                      # profiles/r01_exact_gemm_full.md
+}
+
+
+def algorithmic_counts(grid):
+    """Operations the METHOD needs per parameter row (13-parameter model), independent of this implementation
+    (DESIGN.md 5.1 derives them from the quadrature that the 1e-5 weights tolerance requires)."""
+    n_age, n_Z, n_band = grid.n_age, grid.n_Z, grid.n_band
+    nodes = 2 * n_age + 64                                   # two Gauss points per age bin + the panels of the bins that reach t ~ 0
+    c = {"quadrature_nodes": nodes}
+    c["prologue_mufu"] = 5 * nodes + 2 * 13 + 3 * (n_Z - 1) + 4          # lg2, 2 ex2, rcp, 1/t per node; C1; MDF edges; z -> t_obs
+    c["prologue_fma"] = 16 * nodes + 14 * n_age + 40
+    c["epilogue_mufu"] = 2 * 13 + 3 * (n_Z - 1) + 5 * 13                   # C1 slopes, MDF densities, skew-normal prior
+    c["epilogue_fma"] = (2 * 5 + 14) * n_age + 100
+    c["contract_mufu"] = 7 * n_band                                       # dust at lambda_eff / (1+z)
+    c["contract_fma"] = 6 * n_Z * n_band + 2 * 2 * n_Z * n_band + 200     # the sums over metallicity of P, m_bar, V
+    c["contract_flop_fp32"] = 2 * 2 * (2 * n_age * n_Z * n_band)          # Eq. (6) forward + reverse over the two c_SSP arrays of the z cell
+    c["hbm_bytes"] = 4 * (13 + n_band) * 2                                # theta + observations in, logP + gradient out (SURVEY 8(d): 184 B)
+    return c
+
+
+def kernel_roofline(kernel, avg_s, rows, grid, peaks, peaks_src, pipe, hmc, pairs=0):
+    base = {"kernel": kernel, "avg_launch_ms": 1e3 * avg_s, "traffic": NCU_TRAFFIC.get((kernel, rows))}
+    C = algorithmic_counts(grid)
+    tensor_peak = float(peaks["bf16_tflops_sustained" if hmc else "bf16_tflops"])
+    tensor_note = ("sustained bf16 peak: the kernel runs inside a seconds-long step" if hmc else "burst bf16 peak: the kernel is timed in a short step") + f" ({peaks_src})"
+    if kernel == "prologue":
+        ach = C["prologue_mufu"] * rows / avg_s / 1e9
+        peak = pipe["mufu_per_s"] / 1e9
+        return {**base, "bound": "alu", "achieved": ach, "peak": peak, "unit": "G MUFU/s", "frac": ach / peak,
+                "peak_note": f"special-function pipe, measured in this run (sps_measure_peak); achieved = {C['prologue_mufu']} algorithmic MUFU operations "
+                             f"per row ({C['quadrature_nodes']} quadrature nodes x 5 + C1 + MDF edges: DESIGN.md 5.1), not this implementation's instruction count"}
+    if kernel == "epilogue":
+        bytes_row = 4 * (6 * grid.n_age + grid.n_Z + 16 + 13 + 13 + 1 + ((3 * 13 + 1) + 2 * 13 if hmc else 0))
+        ach = bytes_row * rows / avg_s / 1e9
+        peak = float(peaks["hbm_gbs"])
+        return {**base, "bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "peak_note": f"HBM copy bandwidth ({peaks_src}); achieved = {bytes_row} bytes per row that this kernel must move as long as the per-bin "
+                             "partials travel through HBM (DESIGN.md 5.1); the method itself needs 184 B per row"}
+    if kernel == "approx_contract":
+        flop = 3.0 * C["contract_flop_fp32"] * rows
+        ach = flop / avg_s / 1e12
+        return {**base, "bound": "tensor", "achieved": ach, "peak": tensor_peak, "unit": "TFLOP/s", "frac": ach / tensor_peak,
+                "peak_note": f"{tensor_note}; achieved = 3 FP16 split products x {C['contract_flop_fp32']} fp32-equivalent flop per row (Eq. 6 forward + reverse)"}
+    K = grid.n_age * grid.n_Z
+    flop = 3.0 * 2.0 * K * float(pairs)
+    ach = flop / avg_s / 1e12
+    return {**base, "bound": "tensor", "achieved": ach, "peak": tensor_peak, "unit": "TFLOP/s", "frac": ach / tensor_peak,
+            "peak_note": f"{tensor_note}; achieved = 3 BF16 split products x 2 x {K} flop x {pairs} (row, wavelength) pairs under a filter's support "
+                         f"= {pairs / max(1, rows):.0f} of {grid.n_wave} wavelengths per row (skipped and padded columns never count)"}
+
+
+def evaluation_roofline(workload, kernel_ms, step_s, evals_per_step, rows, grid, peaks, peaks_src, pipe, pairs):
+    """One whole log-likelihood + gradient evaluation of `rows` rows: measured time against the bound
+    max(t_MUFU, t_FMA, t_tensor, t_HBM) of the METHOD's operation counts at this run's measured peaks."""
+    C = algorithmic_counts(grid)
+    launches_per_step = max(1.0, evals_per_step / rows)
+    measured_s = step_s / launches_per_step
+    kernels_s = sum(v["avg_ms"] for v in kernel_ms.values()) * 1e-3
+    mufu = (C["prologue_mufu"] + C["epilogue_mufu"] + (C["contract_mufu"] if workload != "c2_exact" else 0)) * rows / pipe["mufu_per_s"]
+    fma = (C["prologue_fma"] + C["epilogue_fma"] + (C["contract_fma"] if workload != "c2_exact" else 0)) * rows / pipe["ffma_per_s"]
+    if workload == "c2_exact":
+        tensor = 2 * 3.0 * 2.0 * grid.n_age * grid.n_Z * float(pairs) / (float(peaks["bf16_tflops"]) * 1e12)      # forward + reverse GEMM
+    else:
+        tensor = 3.0 * C["contract_flop_fp32"] * rows / (float(peaks["bf16_tflops_sustained"]) * 1e12)
+    hbm = C["hbm_bytes"] * rows / (float(peaks["hbm_gbs"]) * 1e9)
+    terms = {"mufu": mufu, "fma": fma, "tensor": tensor, "hbm": hbm}
+    binding = max(terms, key=terms.get)
+    tr = [NCU_TRAFFIC.get((k, rows)) for k in kernel_ms]
+    return {"rows": rows, "measured_us": 1e6 * measured_s, "sum_of_kernel_times_us": 1e6 * kernels_s, "bound_us": 1e6 * terms[binding], "binding": binding,
+            "frac": terms[binding] / measured_s, "terms_us": {k: 1e6 * v for k, v in terms.items()},
+            "algorithmic_hbm_bytes": C["hbm_bytes"] * rows, "dram_bytes_ncu": (sum(tr) if all(t is not None for t in tr) else None),
+            "note": "bound = max over pipes of (algorithmic operations per row x rows / peak measured in this run); the pipes overlap, so the terms are not added"}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------------
+_WK = {}
+
+
+def _worker_init(workload, seed):
+    from threadpoolctl import threadpool_limits
+    from oracle import sps_model as M
+    from paper_2506_19919_b200 import workloads as W
+    threadpool_limits(limits=1)
+    cfg = dict(W.CONFIGS[workload])
+    grid = W.make_grid(cfg["grid"]); prior = W.make_prior()
+    _WK.update(cfg=cfg, grid=grid, prior=prior, P=prior.as_array(), cssp=M.cssp_table(grid) if workload != "c2_exact" else None)
+
+
+def _worker_galaxy(task):
+    """One galaxy of the HMC workloads: n_chain chains x n_tr transitions of the oracle's sampler on the approximate path."""
+    from oracle import sampler as S
+    from oracle import sps_model as M
+    from paper_2506_19919_b200 import workloads as W
+    g, n_tr = task
+    cfg, grid, prior, P, cssp = (_WK[k] for k in ("cfg", "grid", "prior", "P", "cssp"))
+    n_chain, L = cfg["n_chain"], cfg.get("n_leapfrog", 16)
+    thu = W.draw_theta_unbounded(prior, 1, cfg["seed"] + 1000 + g)
+    f = M.photometry_approx(M.bound(thu, P)[0], grid, cssp)[0]
+    d, s = W.noisy_observations(f, cfg["seed"] + 7 + g, 0.05, 0.10)
+    gal = np.zeros(n_chain, int)
+    fn = lambda th: M.logp_and_grad(th, grid, P, d[gal], s[gal], "approx", cssp)[:2]
+    ids = np.arange(g * n_chain, (g + 1) * n_chain)
+    S.run_chains(S.init_chains(P, cfg["seed"], ids, 13), fn, cfg["seed"], 0, n_tr, 0.01, "hmc", n_leapfrog=L, chain_ids=ids)
+    return n_chain * n_tr * L
+
+
+def _worker_rows(task):
+    """A block of rows of the kernel-only workloads through the oracle (flux + full Jacobian)."""
+    from oracle import sps_model as M
+    from paper_2506_19919_b200 import workloads as W
+    block, n, workload = task
+    cfg, grid, prior, P, cssp = (_WK[k] for k in ("cfg", "grid", "prior", "P", "cssp"))
+    th = M.bound(W.draw_theta_unbounded(prior, n, cfg["seed"] + block, z_uniform=(0.1, 3.0)), P)[0]
+    (M.photometry_approx(th, grid, cssp) if workload == "c3_approx" else M.photometry_exact(th, grid))
+    return n
+
+
+def cpu_worker(workload, protocol, budget_s):
+    """Runs in a process of its own (no CUDA context): the float64 oracle, as it stands, over all host cores."""
+    import multiprocessing as mp
+    from paper_2506_19919_b200 import workloads as W
+    cores = os.cpu_count() or 1
+    cfg = dict(W.CONFIGS[workload])
+    if protocol == "paper":
+        cfg["n_warmup"], cfg["n_sample"] = 100, 3000
+    with mp.get_context("fork").Pool(cores, initializer=_worker_init, initargs=(workload, cfg["seed"])) as pool:
+        pool.map(abs, range(cores))                                    # workers up, tables built (setup, untimed as for the GPU)
+        if workload in ("c4_hmc", "c5_nuts"):
+            n_gal = max(64, 4 * cores)
+            t0 = time.perf_counter()
+            pool.map(_worker_galaxy, [(g, 1) for g in range(cores)])   # calibration: one transition per galaxy on every core
+            per_tr = (time.perf_counter() - t0)
+            n_tr = int(max(2, min(200, budget_s / max(per_tr, 1e-3) / (n_gal / cores))))
+            t0 = time.perf_counter()
+            evals = sum(pool.map(_worker_galaxy, [(g, n_tr) for g in range(n_gal)]))
+            sec = time.perf_counter() - t0
+            L = cfg.get("n_leapfrog", 16)
+            per_post = cfg["n_chain"] * (cfg["n_warmup"] + cfg["n_sample"]) * L
+            return {"value": 60.0 * (evals / sec) / per_post, "unit": "posteriors/min", "cores": cores, "kind": "oracle",
+                    "sample": f"{n_gal} galaxies x {cfg['n_chain']} chains x {n_tr} HMC transitions x {L} leapfrogs of the float64 numpy oracle over {cores} "
+                              f"processes ({evals} loglike+grad evals in {sec:.1f} s), scaled linearly in galaxies and transitions to {per_post} evals per posterior",
+                    "loglike_grad_evals_per_s": evals / sec}
+        n = 2 if workload == "c2_exact" else 64
+        t0 = time.perf_counter()
+        pool.map(_worker_rows, [(b, n, workload) for b in range(cores)])
+        per_block = time.perf_counter() - t0
+        blocks = int(max(cores, min(4096, cores * budget_s / max(per_block, 1e-3))))
+        t0 = time.perf_counter()
+        done = sum(pool.map(_worker_rows, [(1000 + b, n, workload) for b in range(blocks)]))
+        sec = time.perf_counter() - t0
+        return {"value": done / sec, "unit": "evals/s", "cores": cores, "kind": "oracle",
+                "sample": f"{done} rows of the workload's parameter draws through the float64 numpy oracle (flux + full Jacobian) over {cores} processes in {sec:.1f} s"}
+
+
+def cpu_baseline(workload, protocol, budget_s=20.0):
+    r = subprocess.run([sys.executable, os.path.abspath(__file__), "--cpu-worker", "--workload", workload, "--protocol", protocol,
+                        "--cpu-budget", str(budget_s)], capture_output=True, text=True, timeout=600)
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    if r.returncode != 0 or not lines:
+        return {"value": None, "unit": "", "cores": os.cpu_count(), "kind": "oracle", "sample": "failed: " + r.stderr[-300:]}
+    return json.loads(lines[-1])
+
+
+def run_reference(args):
+    """--impl reference: there is no reference implementation (the paper ships no code); for this tier the reference arm
+    is the oracle timed on the host cores.  Rank 0 alone runs it."""
+    if int(os.environ.get("RANK", 0)) != 0:
+        return
+    from paper_2506_19919_b200 import workloads as W
+    cfg = dict(W.CONFIGS[args.workload])
+    if args.protocol == "paper":
+        cfg["n_warmup"], cfg["n_sample"] = 100, 3000
+    per_step = max(4.0, min(25.0, 100.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        cpu_baseline(args.workload, args.protocol, budget_s=2.0)
+    t0 = time.perf_counter()
+    res = [cpu_baseline(args.workload, args.protocol, budget_s=per_step) for _ in range(args.steps)]
+    sec = time.perf_counter() - t0
+    v = float(np.mean([r["value"] for r in res]))
+    hmc = args.workload in ("c4_hmc", "c5_nuts")
+    out = {"impl": "reference", "metric": "galaxy posteriors/GPU-minute" if hmc else "flux+gradient evaluations/s", "value": v,
+           "unit": res[0]["unit"], "n_gpus": int(os.environ.get("WORLD_SIZE", 1)), "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": 1e3 * sec / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic (seeded stand-in SSP spectra, Gaussian filters, prior-drawn galaxies)",
+           "config": {"workload": args.workload, "protocol": args.protocol, **{k: v2 for k, v2 in cfg.items() if k != "seed"},
+                      "n_gal_per_gpu": args.n_gal or cfg.get("n_gal"), "l2": "flushed between timed steps (256 MB write)"},
+           "cpu_baseline": {**res[0], "value": v}, "e2e": {"value": v, "unit": res[0]["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4_hmc", choices=["c4_hmc", "c3_approx", "c2_exact", "c5_nuts"])
+    ap.add_argument("--protocol", default="config", choices=["config", "paper"],
+                    help="config: BASELINE.json's transition counts; paper: 100 adaptation + 3000 kept steps (PAPER.md:105)")
+    ap.add_argument("--n-gal", type=int, default=0)
+    ap.add_argument("--n-rows", type=int, default=0)
+    ap.add_argument("--n-warmup", type=int, default=0)
+    ap.add_argument("--n-sample", type=int, default=0)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end leg (side workloads only; the e2e value is then 0)")
+    ap.add_argument("--cpu-worker", action="store_true", help=argparse.SUPPRESS)
+    args = ap.parse_args()
+    if args.cpu_worker:
+        print(json.dumps(cpu_worker(args.workload, args.protocol, args.cpu_budget)))
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` on its own: one rank per GPU under torchrun (the driver launches torchrun itself)
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        sys.exit(subprocess.call(cmd))
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

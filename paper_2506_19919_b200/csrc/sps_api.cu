@@ -231,18 +231,20 @@ sps_status sps_prior_to_dev(const sps_table* t, const sps_prior* p, PriorDev& ou
 sps_status sps_eval(const sps_table* t, Workspace& ws, const PriorDev& P, int path, const float* theta, int64_t n, bool unbounded,
                     bool with_prior, const int* rows, const int* gal_of_row, const float* obs_flux,
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
-                    cudaStream_t s, const LeapfrogFuse* lf) {
+                    cudaStream_t s, const LeapfrogFuse* lf, bool overlap) {
   const TableDev& T = t->dev;
   const LeapfrogFuse fuse = (lf && want_grad) ? *lf : LeapfrogFuse{nullptr, nullptr, nullptr, nullptr};
   if (T.model == SPS_MODEL_GAUSS_TEST) {
     launch_gauss_eval(T, theta, n, rows, logp, want_grad ? grad : nullptr, fuse, s);
     return sps_check_cuda(cudaGetLastError(), "sps_eval launch");
   }
-  const bool tiny5 = T.model == SPS_MODEL_TINY5;
-  if (tiny5) launch_prologue_tiny5(T, P, theta, n, unbounded, rows, ws.rows, path == SPS_PATH_APPROX, s);
-  else launch_prologue(T, P, theta, n, unbounded, want_grad, rows, ws.rows, path == SPS_PATH_APPROX, s);
+  const bool tiny5 = T.model == SPS_MODEL_TINY5, nonsep = T.agez_gamma != 0.f;
+  const bool bucket = path == SPS_PATH_APPROX && !nonsep;   // the separable approximate kernels want rows grouped by z cell
+  if (tiny5) launch_prologue_tiny5(T, P, theta, n, unbounded, rows, ws.rows, bucket, s);
+  else launch_prologue(T, P, theta, n, unbounded, want_grad, rows, ws.rows, bucket, s, overlap);
   if (path == SPS_PATH_APPROX) {
-    if (sps_approx_tc_active(t)) {
+    if (nonsep) launch_nonsep_approx(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, ws.rows, s);
+    else if (sps_approx_tc_active(t)) {
       sps_status st = sps_approx_tc_contract(t, ws, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, s);
       if (st != SPS_OK) return st;
     } else launch_approx_contract(T, t->sm_count, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, ws.rows, s);

@@ -114,7 +114,10 @@ struct ApproxArgs {
 
 // NB = n_band (compile time: entry e -> (j, b) = (e / NB, e % NB) resolves to register names in the unrolled band step)
 template <int NB>
-__global__ void __launch_bounds__(THREADS_TC, 1)
+#ifndef ATC_MINB
+#define ATC_MINB 1
+#endif
+__global__ void __launch_bounds__(THREADS_TC, ATC_MINB)
 approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__ CUtensorMap m1h, const __grid_constant__ CUtensorMap m1l,
                  const __grid_constant__ CUtensorMap m2h, const __grid_constant__ CUtensorMap m2l) {
   extern __shared__ unsigned char smem_dyn[];

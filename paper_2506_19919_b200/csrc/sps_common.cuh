@@ -44,6 +44,7 @@ struct TableDev {
   const float* A_half;      // [n_age]   (A[i+1]-A[i])/2   (last: +huge)
   const float* e_edge;      // [n_age+1] log10(age/yr) of the edges (-huge, ..., +huge)
   const float* g_mid;       // [n_Z-1]   log10 Z bin edges (midpoints)
+  const float* la9;         // [n_age]   log10(age_i / yr) - 9 (R26: the MDF median of age bin i is logZ + agez_gamma la9[i])
   // wavelength grid and per-wavelength constants (exact path)
   const float* wave;        // [n_wave_pad] Angstrom (padding: copies of the last value)
   const float* dlam;        // [n_wave_pad] trapezoid weights (R4), 0 in the padding
@@ -92,7 +93,8 @@ struct RowScalars {           // 16 floats
   float z_bar;                // direct d logL / d z (table interpolation + dust at lambda_eff/(1+z) or filter shift)
   float AV_bar, delta_bar, Ffloor_bar;
   float Msum;                 // int_0^t_obs f dt for M_formed = 1 (Eq. A3), kept for the reverse pass
-  float pad1, pad2;
+  float pad1, pad2;           // non-separable weights (R26): logZ, sigma_logZ from the prologue; the contraction replaces them
+                              // by d logL / d logZ, d logL / d sigma_logZ (through every age bin's MDF) for the epilogue
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -12,9 +12,19 @@ __global__ void exact_weights_kernel(TableDev T, int64_t n, const int* __restric
   const int64_t r = blockIdx.x;
   const int64_t row = rows ? rows[r] : r;
   const float Mn = B.sc[row].Mn;
+  __shared__ float mt_s[SPS_MAX_AGE * SPS_MAX_Z];            // non-separable weights (R26): the MDF of every age bin
+  const bool nonsep = T.agez_gamma != 0.f;
+  if (nonsep && threadIdx.x < T.n_age) {
+    float d1[SPS_MAX_Z], d2[SPS_MAX_Z];
+    mdf_row(T, B.sc[row].pad1 + T.agez_gamma * T.la9[threadIdx.x], B.sc[row].pad2, mt_s + threadIdx.x * SPS_MAX_Z, d1, d2);
+  }
+  __syncthreads();
   for (int e = threadIdx.x; e < ldw; e += blockDim.x) {
     float v = 0.f;
-    if (e < T.K) { const int i = e / T.n_Z, j = e - i * T.n_Z; v = Mn * B.a[row * ROW_A_STRIDE + i] * B.m[row * ROW_M_STRIDE + j]; }
+    if (e < T.K) {
+      const int i = e / T.n_Z, j = e - i * T.n_Z;
+      v = Mn * B.a[row * ROW_A_STRIDE + i] * (nonsep ? mt_s[i * SPS_MAX_Z + j] : B.m[row * ROW_M_STRIDE + j]);
+    }
     W[r * ldw + e] = v;
   }
 }
@@ -237,6 +247,27 @@ __global__ void exact_final_kernel(TableDev T, int64_t n, const int* __restrict_
   const int64_t row = rows ? rows[r] : r;
   const float Mn = B.sc[row].Mn;
   const float* wb = Wbar + r * ldw;
+  if (T.agez_gamma != 0.f) {
+    // non-separable weights (R26): w_ij = Mn a_i m_ij with an MDF per age bin; the metallicity parameters collect their
+    // bars through every bin, handed to the epilogue in the row's scalars (m_bar is zero)
+    const float lz = B.sc[row].pad1, slz = B.sc[row].pad2;
+    float lz_bar = 0.f, slz_bar = 0.f;
+    for (int i0 = 0; i0 < ROW_A_STRIDE; i0 += 32) {
+      const int i = i0 + l;
+      float ab = 0.f;
+      if (i < T.n_age) {
+        float m[SPS_MAX_Z], d_mu[SPS_MAX_Z], d_s[SPS_MAX_Z];
+        mdf_row(T, lz + T.agez_gamma * T.la9[i], slz, m, d_mu, d_s);
+        const float ai = B.a[row * ROW_A_STRIDE + i];
+        for (int j = 0; j < T.n_Z; ++j) { const float w = wb[i * T.n_Z + j]; ab += w * m[j]; lz_bar += w * ai * d_mu[j]; slz_bar += w * ai * d_s[j]; }
+      }
+      B.a_bar[row * ROW_A_STRIDE + i] = Mn * ab;
+    }
+    lz_bar = warp_sum(lz_bar); slz_bar = warp_sum(slz_bar);
+    if (l < ROW_M_STRIDE) B.m_bar[row * ROW_M_STRIDE + l] = 0.f;
+    if (l == 0) { B.sc[row].pad1 = Mn * lz_bar; B.sc[row].pad2 = Mn * slz_bar; }
+    return;
+  }
   float mb[SPS_MAX_Z];
 #pragma unroll
   for (int j = 0; j < SPS_MAX_Z; ++j) mb[j] = 0.f;

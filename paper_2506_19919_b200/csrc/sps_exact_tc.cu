@@ -484,8 +484,14 @@ __global__ void __launch_bounds__(128) tc_weights_kernel(TableDev T, int64_t n, 
   const int64_t r = blockIdx.x;
   const int64_t row = rows ? rows[r] : r;
   __shared__ float a_s[ROW_A_STRIDE], m_s[ROW_M_STRIDE];
+  __shared__ float mt_s[SPS_MAX_AGE * SPS_MAX_Z];            // non-separable weights (R26): the MDF of every age bin
+  const bool nonsep = T.agez_gamma != 0.f;
   a_s[threadIdx.x] = B.a[row * ROW_A_STRIDE + threadIdx.x] * B.sc[row].Mn;
   if (threadIdx.x < ROW_M_STRIDE) m_s[threadIdx.x] = B.m[row * ROW_M_STRIDE + threadIdx.x];
+  if (nonsep && threadIdx.x < T.n_age) {
+    float d1[SPS_MAX_Z], d2[SPS_MAX_Z];
+    mdf_row(T, B.sc[row].pad1 + T.agez_gamma * T.la9[threadIdx.x], B.sc[row].pad2, mt_s + threadIdx.x * SPS_MAX_Z, d1, d2);
+  }
   __syncthreads();
   const float inv_nZ = 1.f / (float)T.n_Z;
   for (int e = 2 * threadIdx.x; e < Wld; e += 2 * blockDim.x) {          // Wld is a multiple of the k block, hence even
@@ -493,7 +499,7 @@ __global__ void __launch_bounds__(128) tc_weights_kernel(TableDev T, int64_t n, 
     int i = (int)(((float)e + 0.5f) * inv_nZ), j = e - i * T.n_Z;         // exact for e < 2^16 (n_age n_Z <= 2048)
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
-      const float v = (e + u < T.K) ? a_s[min(i, ROW_A_STRIDE - 1)] * m_s[j] : 0.f;
+      const float v = (e + u < T.K) ? a_s[min(i, ROW_A_STRIDE - 1)] * (nonsep ? mt_s[min(i, ROW_A_STRIDE - 1) * SPS_MAX_Z + j] : m_s[j]) : 0.f;
       Op<PREC>::split(v, h2[u], l2[u]);
       if (++j == T.n_Z) { j = 0; ++i; }
     }

@@ -42,7 +42,8 @@ struct sps_table {
   mutable std::map<cudaStream_t, Workspace*> ws;
   mutable Workspace* last_ws;          // for sps_exact_last_work
   mutable cudaStream_t own_stream;     // sps_hmc_run on the legacy default stream runs here (graph capture needs a real stream)
-  sps_table() : exact(nullptr), approx_tc(nullptr), sm_count(0), last_ws(nullptr), own_stream(nullptr) {}
+  mutable cudaStream_t aux_stream[3];  // streams of the sampler's additional row groups (sps_sampler.cu)
+  sps_table() : exact(nullptr), approx_tc(nullptr), sm_count(0), last_ws(nullptr), own_stream(nullptr) { aux_stream[0] = aux_stream[1] = aux_stream[2] = nullptr; }
 };
 
 // library options (sps_set_option)
@@ -77,7 +78,11 @@ sps_status sps_approx_tc_contract(const sps_table* t, Workspace& ws, int64_t n, 
 sps_status sps_eval(const sps_table* t, Workspace& ws, const PriorDev& P, int path, const float* theta, int64_t n, bool unbounded,
                     bool with_prior, const int* rows, const int* gal_of_row, const float* obs_flux,
                     const float* obs_sigma, const float* flux_bar, bool want_grad, float* logp, float* grad,
-                    cudaStream_t s, const LeapfrogFuse* lf = nullptr);
+                    cudaStream_t s, const LeapfrogFuse* lf = nullptr, bool overlap = false);
+
+// approximate path with non-separable weights (sps_nonsep.cu; R26)
+void launch_nonsep_approx(const TableDev& T, int64_t n, const int* rows, const int* gal_of_row, const float* obs_flux, const float* obs_sigma,
+                          const float* flux_bar, bool want_grad, RowBuffers B, cudaStream_t s);
 
 // other models (sps_models.cu): SPS_MODEL_TINY5 row kernels and the SPS_MODEL_GAUSS_TEST target
 void launch_prologue_tiny5(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, const int* rows,

@@ -48,13 +48,16 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& 
 // a0-a5.  With store_part the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
 // kept in B.part for the epilogue, which then has no quadrature to redo.  One instantiation serves forward-only and
 // gradient calls (the partials are computed either way), so that both give bit-identical weights and fluxes.
-__global__ void __launch_bounds__(32 * PRO_WARPS, PRO_MIN_BLOCKS)
+// PW = rows (warps) per block: 16 when the kernel has the SMs to itself; 8 when the sampler overlaps two row groups, so
+// that a block fits in the registers the persistent contraction CTA of the other group leaves free on an SM.
+template <int PW>
+__global__ void __launch_bounds__(32 * PW, 32 / PW)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded, bool store_part,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
   constexpr bool WANT_GRAD = true;
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
-  const int64_t r = (int64_t)blockIdx.x * PRO_WARPS + (threadIdx.x >> 5);
+  const int64_t r = (int64_t)blockIdx.x * PW + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
   const int l = lane_id();
@@ -81,7 +84,7 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     sc.z = z; sc.zbin = (int)zi; sc.zfrac = (z - (T.z_min + zi * T.dz)) * T.inv_dz;
     sc.AV = R.th[9]; sc.delta = R.th[10]; sc.Ffloor = R.th[11];
     sc.logp_like = 0.f; sc.Mn_bar = sc.z_bar = sc.AV_bar = sc.delta_bar = sc.Ffloor_bar = 0.f;
-    sc.Msum = R.Msum; sc.pad1 = sc.pad2 = 0.f;
+    sc.Msum = R.Msum; sc.pad1 = R.th[7]; sc.pad2 = R.th[8];       // logZ, sigma_logZ for the non-separable contraction (R26)
     B.sc[row] = sc;
     if (hist) atomicAdd(&hist[sc.zbin], 1);                 // z-cell histogram for the approximate path's row grouping
   }
@@ -543,6 +546,7 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
   // dL/d(dM_i) = (1-Fb)/Msum (a_bar_i - sum_k a_bar_k Ps_k) + Mn_bar * Mf
   // round 2: {tau, alpha, beta, t_obs sums; MDF sums; prior}
   float r2[8] = {0.f, 0.f, 0.f, 0.f, mb * dm_lz, mb * dm_s, lp, 0.f};
+  if (T.agez_gamma != 0.f && l == 0) { r2[4] += sc.pad1; r2[5] += sc.pad2; }   // R26: the bars through every age bin's MDF
   const float c1 = (1.f - Fb) * inv_M, c2 = sc.Mn_bar * Mf;
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
@@ -594,13 +598,13 @@ __global__ void copy_flux_kernel(TableDev T, int64_t n, RowBuffers B, float* flu
 static inline unsigned blocks_for_rows(int64_t n) { return (unsigned)((n + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK); }
 
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s) {
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks) {
   if (n <= 0) return;
   int* hist = nullptr;
   if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
   sps_prof_begin(SPS_K_PROLOGUE, s);
-  const unsigned pro_blocks = (unsigned)((n + PRO_WARPS - 1) / PRO_WARPS);
-  prologue_kernel<<<pro_blocks, 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
+  if (small_blocks) prologue_kernel<8><<<(unsigned)((n + 7) / 8), 256, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
+  else prologue_kernel<PRO_WARPS><<<(unsigned)((n + PRO_WARPS - 1) / PRO_WARPS), 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }

@@ -22,6 +22,13 @@ static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int
     if (cfg->path != SPS_PATH_EXACT && cfg->path != SPS_PATH_APPROX) { sps_set_error("bad path"); return SPS_EINVAL; }
     Q.n_rows_path[cfg->path] = Q.n;
     cudaMemset(Q.path_of_chain, cfg->path, Q.n);
+    if (Q.n_groups > 1) {                                     // row groups need an explicit (identity) list to offset into
+      std::vector<int> ident(Q.n);
+      for (int64_t i = 0; i < Q.n; ++i) ident[i] = (int)i;
+      st = sps_check_cuda(cudaMalloc(&Q.rows_path[cfg->path], Q.n * sizeof(int)), "row list allocation");
+      if (st != SPS_OK) return st;
+      cudaMemcpy(Q.rows_path[cfg->path], ident.data(), Q.n * sizeof(int), cudaMemcpyHostToDevice);
+    }
     return SPS_OK;
   }
   std::vector<int32_t> pg(n_gal);
@@ -46,12 +53,17 @@ static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int
 
 void hmc_problem_free(HmcProblem& Q);
 sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev,
-                             const float* obs_flux, const float* obs_sigma) {
+                             const float* obs_flux, const float* obs_sigma, int n_groups) {
   memset(&Q, 0, sizeof(Q));
-  Q.n = n_gal * cfg->n_chain; Q.obs_flux = obs_flux; Q.obs_sigma = obs_sigma;
+  Q.n = n_gal * cfg->n_chain; Q.obs_flux = obs_flux; Q.obs_sigma = obs_sigma; Q.n_groups = n_groups;
   const sps_status st = hmc_problem_fill(Q, cfg, n_gal, path_of_gal_dev);
-  if (st != SPS_OK) hmc_problem_free(Q);                    // nothing allocated here outlives a rejected call
-  return st;
+  if (st != SPS_OK) { hmc_problem_free(Q); return st; }     // nothing allocated here outlives a rejected call
+  for (int p = 0; p < 2; ++p)                               // contiguous, balanced shares of each path's rows
+    for (int g = 0; g < n_groups; ++g) {
+      const int64_t a = Q.n_rows_path[p] * g / n_groups, b = Q.n_rows_path[p] * (g + 1) / n_groups;
+      Q.g_off[g][p] = a; Q.g_n[g][p] = b - a;
+    }
+  return SPS_OK;
 }
 
 void hmc_problem_free(HmcProblem& Q) {

@@ -317,6 +317,27 @@ __device__ __forceinline__ void met_bin(const TableDev& T, float lz, float s, fl
   }
 }
 
+// The same MDF for one median, serially in one thread (non-separable weights, R26: every age bin has its own median):
+// m[j], dm/dmedian, dm/dsigma for j < n_Z.
+__device__ __forceinline__ void mdf_row(const TableDev& T, float mu, float s, float* __restrict__ m, float* __restrict__ d_mu, float* __restrict__ d_s) {
+  const float inv_s = 1.f / s, r2 = 0.7071067811865476f, c = 0.3989422804014327f;
+  float ua = -1e30f, ea = 0.f, pa = 0.f;                    // lower edge of bin 0: -infinity
+  for (int j = 0; j < T.n_Z; ++j) {
+    const bool has_hi = j < T.n_Z - 1;
+    const float ub = has_hi ? (T.g_mid[j] - mu) * inv_s : 1e30f;
+    const float eb = has_hi ? erfcf(fabsf(ub) * r2) : 0.f;
+    const float pb = has_hi ? c * expf(-0.5f * ub * ub) : 0.f;
+    float mj;
+    if (ua > 0.f) mj = 0.5f * (ea - eb);
+    else if (ub < 0.f) mj = 0.5f * (eb - ea);
+    else mj = 1.f - 0.5f * (eb + ea);
+    m[j] = mj;
+    d_mu[j] = -(pb - pa) * inv_s;
+    d_s[j] = -(pb * (has_hi ? ub : 0.f) - pa * (j > 0 ? ua : 0.f)) * inv_s;
+    ua = ub; ea = eb; pa = pb;
+  }
+}
+
 // ---- a8: dust, Eq. (A8)-(A9) PAPER.md:386-392 (R10) at an arbitrary rest wavelength (approximate path) ----
 #define CALZ_SWITCH_INV_UM 1.2809053864877329f
 // `screen` (SPS_MODEL_TINY5): k0 = 4.05 and no bump, which with delta = -0.7, F_floor = 0 and A_V = 1.0857 tau_V is the

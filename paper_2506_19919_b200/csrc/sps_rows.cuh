@@ -22,10 +22,11 @@ struct RowBuffers {
 // Optional leapfrog update fused into the epilogue (HMC inner steps): after the gradient of a row is known,
 //   p += eps grad;  theta~ += eps invM p     (the two half kicks between consecutive evaluations merged)
 struct LeapfrogFuse { float* theta_w; float* p_w; const float* eps; const float* inv_mass; };
+// (sps_eval's `overlap` flag: the call is one of several row groups running on different streams, see sps_sampler.cu)
 
 // kernels (sps_kernels.cu)
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s);
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks = false);
 void launch_approx_contract(const TableDev& T, int sm_count, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);

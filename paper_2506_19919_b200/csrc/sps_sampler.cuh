@@ -60,6 +60,9 @@ struct HmcProblem {
   unsigned char* path_of_chain;   // [n] device: photometry path of each chain
   int* rows_path[2];         // device index lists per path, or NULL = all rows
   int64_t n_rows_path[2];
+  // row groups of fixed-length HMC (SPS_OPT_ROW_GROUPS): group g evaluates rows_path[p][g_off[g][p] .. + g_n[g][p]) of each path
+  int n_groups;
+  int64_t g_off[4][2], g_n[4][2];
   const float *obs_flux, *obs_sigma;
 };
 

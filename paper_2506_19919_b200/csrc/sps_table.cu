@@ -158,6 +158,8 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   const int na = d->n_age;
   std::vector<float> A_edge(na + 1), A_mid(na), A_half(na), e_edge(na + 1), g_mid(d->n_Z - 1 > 0 ? d->n_Z - 1 : 1);
   std::vector<double> Ae(na + 1);
+  std::vector<float> la9(na);
+  for (int i = 0; i < na; ++i) la9[i] = (float)(d->log10_age_yr[i] - 9.0);
   Ae[0] = 0.0; e_edge[0] = -1e30f;
   for (int i = 1; i < na; ++i) { const double mid = 0.5 * (d->log10_age_yr[i] + d->log10_age_yr[i - 1]); Ae[i] = pow(10.0, mid - 9.0); e_edge[i] = (float)mid; }
   Ae[na] = 1e30; e_edge[na] = 1e30f;
@@ -290,7 +292,7 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   T.A_edge_d = upload(Ae, st); T.A_mid_d = upload(Amid_d, st);
   if (!tz.empty()) T.tz_coef = upload(tz, st);
   T.A_edge = upload(A_edge, st); T.A_mid = upload(A_mid, st); T.A_half = upload(A_half, st); T.e_edge = upload(e_edge, st);
-  T.g_mid = upload(g_mid, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
+  T.g_mid = upload(g_mid, st); T.la9 = upload(la9, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
   T.drude = upload(dr, st); T.l2r = upload(l2r, st); T.ssp = upload(ssp, st);
   float* cssp = nullptr;
   const size_t cs_n = (size_t)T.n_z * 2 * T.n_age * T.cs_stride;
@@ -329,13 +331,14 @@ extern "C" sps_status sps_destroy_table(sps_table* t) {
   TableDev& T = t->dev;
   cudaDeviceSynchronize();
   const void* ptrs[] = {T.tz_coef, T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp,
-                        T.gauss, T.ft.knots, T.ft.first};
+                        T.gauss, T.ft.knots, T.ft.first, T.la9};
   for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
   sps_exact_teardown(t);
   sps_approx_tc_teardown(t);
   for (auto& kv : t->ws) sps_free_workspace(kv.second);
   t->ws.clear();
   if (t->own_stream) cudaStreamDestroy(t->own_stream);
+  for (cudaStream_t a : t->aux_stream) if (a) cudaStreamDestroy(a);
   delete t;
   return SPS_OK;
 }

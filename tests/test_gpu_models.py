@@ -518,3 +518,62 @@ def test_posterior_overlay_exact_vs_approximate(tiny):
     mc = np.sqrt(se ** 2 / np.maximum(ee, 1.0) + sa ** 2 / np.maximum(ea, 1.0))
     assert np.all(np.abs(me - ma)[okm] <= 0.15 * np.maximum(se, sa)[okm] + 4.0 * mc[okm])
     assert np.all(np.abs(np.log(se / sa))[okm] < 0.25)
+
+
+# ---- NEXT-4: non-separable weights, an MDF whose median drifts with log age (R26) ------------------
+@pytest.mark.parametrize("kind,n_gal", [("tiny", 30), ("full", 6)])
+def test_nonseparable_weights(kind, n_gal, kernels):
+    from oracle import nonsep as N
+    gamma = -0.3
+    cx = Ctx(kind, dlogZ_dlogage=gamma)
+    n_chain = 3
+    truth_u = W.draw_theta_unbounded(cx.prior, n_gal, 33).astype(np.float32).astype(np.float64)
+    f = N.photometry_approx(M.bound(truth_u, cx.P)[0], cx.grid, gamma, cx.cssp())[0]
+    d, s = W.noisy_observations(f, 34, 0.05, 0.10)
+    d = d.astype(np.float32); s = s.astype(np.float32)
+    thu = (np.repeat(truth_u, n_chain, 0) + 0.3 * np.random.default_rng(2).normal(size=(n_gal * n_chain, 13)) / cx.P[2]).astype(np.float32)
+    gal = np.repeat(np.arange(n_gal), n_chain).astype(np.int32)
+    th, dth = M.bound(thu.astype(np.float64), cx.P)
+    for path, name in ((cx.sps.PATH_APPROX, "approx"), (cx.sps.PATH_EXACT, "exact")):
+        of, J = (N.photometry_approx(th, cx.grid, gamma, cx.cssp()) if name == "approx" else N.photometry_exact(th, cx.grid, gamma))
+        flux = cx.sps.sps_photometry(cx.table, cx.ph, path, _dev(thu)).cpu().numpy()
+        assert _rel(flux, of).max() <= 1e-4, name
+        # the model is really different from the separable one (so the test would see a kernel that ignored gamma)
+        assert _rel(flux, (M.photometry_approx(th, cx.grid, cx.cssp()) if name == "approx" else M.photometry_exact(th, cx.grid, False))[0]).max() > 1e-2
+        floor = 1e-2 if (name == "exact" and kernels == "tcgen05") else 1e-3            # the tcgen05 exact path's floor (test_gpu_parity.TC_FLOOR)
+        for b in range(cx.grid.n_band):
+            fb = np.zeros((thu.shape[0], cx.grid.n_band), np.float32); fb[:, b] = 1.0
+            _, tb = cx.sps.sps_photometry(cx.table, cx.ph, path, _dev(thu), True, _dev(fb))
+            assert _grad_err(tb.cpu().numpy(), J[:, b, :] * dth, floor).max() <= 1e-3, (name, b)
+        lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, path, _dev(thu), _dev(d), _dev(s), _dev(gal, torch.int32))
+        olp, og, _ = N.logp_and_grad(thu.astype(np.float64), cx.grid, gamma, cx.P, d[gal].astype(np.float64), s[gal].astype(np.float64), name, cx.cssp())
+        lp_allow = FLUX_EPS[name] * (np.abs(of - d[gal]) * of / s[gal].astype(np.float64) ** 2).sum(1)
+        assert (np.maximum(np.abs(lp.cpu().numpy() - olp) - lp_allow, 0.0) / np.maximum(1.0, np.abs(olp))).max() <= 1e-4, name
+        allow = FLUX_EPS[name] * np.einsum("rb,rbp->rp", of / s[gal].astype(np.float64) ** 2, np.abs(J)) * dth
+        err = np.maximum(np.abs(g.cpu().numpy() - og) - allow, 0.0)
+        assert (err / np.maximum(np.abs(og), floor * np.abs(og).max(1, keepdims=True))).max() <= 1e-3, name
+    # and inside the sampler: a short NUTS run on the approximate path stays coupled to the oracle's
+    if kind == "tiny":
+        n_g, n_c, n_s, seed = 2, 2, 10, 29
+        gl = np.repeat(np.arange(n_g), n_c)
+        out = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d[:n_g]), _dev(s[:n_g]), sampler=cx.sps.SAMPLER_HMC, path=cx.sps.PATH_APPROX, n_chain=n_c, n_warmup=0,
+                                 n_sample=n_s, n_leapfrog=5, eps0=0.004, seed=seed, keep_samples=True)
+        fh = lambda x: N.logp_and_grad(x, cx.grid, gamma, cx.P, d[gl].astype(np.float64), s[gl].astype(np.float64), "approx", cx.cssp())[:2]
+        ref = S.run_chains(S.init_chains(cx.P, seed, np.arange(n_g * n_c), 13), fh, seed, 0, n_s, 0.004, "hmc", n_leapfrog=5)
+        assert (np.abs(out["samples"].cpu().numpy() - ref["samples"]) / np.maximum(1.0, np.abs(ref["samples"]))).max() <= 1e-3
+
+
+def test_row_groups_do_not_change_results(full):
+    # SPS_OPT_ROW_GROUPS splits the chains of a fixed-length HMC run over several streams: same chains, bit for bit
+    cx = full
+    n_gal = 300
+    _, d, s = cx.observations(n_gal, 97, frac=(0.05, 0.10))
+    kw = dict(sampler=cx.sps.SAMPLER_HMC, path=cx.sps.PATH_APPROX, n_chain=4, n_warmup=6, n_sample=6, n_leapfrog=4, eps0=0.01, seed=3)
+    ref = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), **kw)
+    try:
+        for G in (2, 3):
+            cx.sps.sps_set_option(cx.sps.OPT_ROW_GROUPS, G)
+            out = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), **kw)
+            assert torch.equal(out["theta_last"], ref["theta_last"]) and torch.equal(out["mean"], ref["mean"]) and torch.equal(out["eps"], ref["eps"])
+    finally:
+        cx.sps.sps_set_option(cx.sps.OPT_ROW_GROUPS, 0)
