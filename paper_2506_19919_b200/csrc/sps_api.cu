@@ -169,7 +169,7 @@ sps_status sps_check_finite(const float* a, int64_t na, const float* b, int64_t 
 
 // ---- scratch per (table, stream) ----------------------------------------------------------------------------
 static void free_row_buffers(RowBuffers& B) {
-  void* ptrs[] = {B.a, B.m, B.a_bar, B.m_bar, B.sc, B.flux, B.part, B.order, B.bins};
+  void* ptrs[] = {B.a, B.m, B.a_bar, B.m_bar, B.sc, B.flux, B.part, B.order, B.bins, B.cell_list};
   for (void* p : ptrs) if (p) cudaFree(p);
   B = RowBuffers();
 }
@@ -204,6 +204,10 @@ sps_status sps_ensure_row_buffers(const sps_table* t, Workspace& ws, int64_t n, 
   al((void**)&B.part, cap * ROW_PARTS * ROW_A_STRIDE * sizeof(float));
   al((void**)&B.order, cap * sizeof(int));
   al((void**)&B.bins, 4 * (size_t)(t->dev.n_z + 1) * sizeof(int));
+  // per-cell row lists for the approximate path (the prologue appends, the contraction walks them): [n_cells][cap] ints,
+  // kept under 1 GiB (beyond that the rows are grouped by a scan / scatter pass instead)
+  const size_t list_bytes = (size_t)std::max(t->dev.n_z - 1, 1) * cap * sizeof(int);
+  if (t->dev.n_z >= 2 && list_bytes <= ((size_t)1 << 30) && t->approx_tc) { al((void**)&B.cell_list, list_bytes); B.cell_cap = cap; }
   if (e != cudaSuccess) { free_row_buffers(B); return sps_check_cuda(e, "row scratch allocation"); }
   B.capacity = cap;
   return SPS_OK;

@@ -106,6 +106,7 @@ enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M1, N_BARS };
 struct ApproxArgs {
   int64_t n;
   const int* order; const int* bins;
+  int64_t cap;             // > 0: `order` is the prologue's per-cell row lists [cell][cap] and bins[0..nb) their lengths (no scan / scatter pass)
   const int* gal_of_row; const float* obs_flux; const float* obs_sigma; const float* flux_bar;
   int want_grad;
   const float* Cm;         // [n_cells][128]
@@ -122,12 +123,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
                  const __grid_constant__ CUtensorMap m2h, const __grid_constant__ CUtensorMap m2l) {
   extern __shared__ unsigned char smem_dyn[];
   const int nb = T.n_z - 1, stride = nb + 2;
+  const bool direct = G.cap > 0;
   const int* row_start_g = G.bins + stride; const int* cta_start_g = G.bins + 2 * stride;
-  const int total = cta_start_g[nb];
-  const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
-  const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
-  const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
-  if (w_begin >= w_end) return;
   const uint32_t base = (smem_u32(smem_dyn) + 1023u) & ~1023u;
   unsigned char* gbase = smem_dyn + (base - smem_u32(smem_dyn));
   const uint32_t bars = base + OFF_BAR;
@@ -140,9 +137,34 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
 #define BAR(i) (bars + 8u * (i))
   // cell offsets of the call in shared memory when they fit (they are walked once per tile by every thread)
   int* bins_s = reinterpret_cast<int*>(gbase + OFF_EXTRA + (2 + 6 + 16) * 128 * 4);
-  for (int i = threadIdx.x; i <= nb; i += blockDim.x) { bins_s[i] = row_start_g[i]; bins_s[nb + 1 + i] = cta_start_g[i]; }
-  const int* row_start = bins_s;
+  if (!direct) {
+    for (int i = threadIdx.x; i <= nb; i += blockDim.x) { bins_s[i] = row_start_g[i]; bins_s[nb + 1 + i] = cta_start_g[i]; }
+  } else {
+    // the prologue left a row list and a count per z cell: every CTA turns the counts into tile offsets itself
+    for (int i = threadIdx.x; i <= nb; i += blockDim.x) { const int c = i < nb ? G.bins[i] : 0; bins_s[i] = c; bins_s[nb + 1 + i] = (c + TM - 1) / TM; }
+    __syncthreads();
+    if (warp == 0) {
+      int carry = 0;
+      for (int b0 = 0; b0 <= nb; b0 += 32) {
+        const int idx = b0 + lane, v = idx <= nb ? bins_s[nb + 1 + idx] : 0;
+        int inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(FULL_MASK, inc, o); if (lane >= o) inc += u; }
+        if (idx <= nb) bins_s[nb + 1 + idx] = carry + inc - v;
+        carry += __shfl_sync(FULL_MASK, inc, 31);
+      }
+    }
+  }
+  __syncthreads();
+  const int* row_start = bins_s;                            // legacy: first position of each cell in `order`; direct: the cell's row count
   const int* cta_start = bins_s + nb + 1;
+  auto cell_begin = [&](int c) { return direct ? (int64_t)c * G.cap : (int64_t)row_start[c]; };
+  auto cell_end = [&](int c) { return direct ? (int64_t)c * G.cap + row_start[c] : (int64_t)row_start[c + 1]; };
+  const int total = cta_start[nb];
+  const int per = total / (int)gridDim.x, rem = total % (int)gridDim.x;
+  const int w_begin = (int)blockIdx.x * per + min((int)blockIdx.x, rem);
+  const int w_end = w_begin + per + ((int)blockIdx.x < rem ? 1 : 0);
+  if (w_begin >= w_end) return;
   if (threadIdx.x == 0) {
     mbar_init(BAR(BAR_B1), 1); mbar_init(BAR(BAR_A), 2 * TM); mbar_init(BAR(BAR_P), 1); mbar_init(BAR(BAR_B2), 1);
     mbar_init(BAR(BAR_V0), 2 * TM); mbar_init(BAR(BAR_M1), 1);
@@ -234,8 +256,8 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
     int rw_next, gal_next = 0;
     {
       while (cta_start[cell + 1] <= w_begin) ++cell;
-      const int rb = row_start[cell] + (w_begin - cta_start[cell]) * TM;
-      rw_next = (rb + r < min(row_start[cell + 1], rb + TM)) ? __ldg(G.order + rb + r) : -1;
+      const int64_t rb = cell_begin(cell) + (int64_t)(w_begin - cta_start[cell]) * TM;
+      rw_next = (rb + r < min(cell_end(cell), rb + TM)) ? __ldg(G.order + rb + r) : -1;
       if (rw_next >= 0 && !G.flux_bar) gal_next = G.gal_of_row ? __ldg(G.gal_of_row + rw_next) : rw_next;
     }
     RowScalars sc_n;
@@ -263,19 +285,19 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
     load_row(rw_next, gal_next);
     for (int w = w_begin; w < w_end; ++w, ph ^= 1u) {
       while (cta_start[cell + 1] <= w) ++cell;
-      const int r_begin = row_start[cell] + (w - cta_start[cell]) * TM;
-      const int r_end = min(row_start[cell + 1], r_begin + TM);
+      const int64_t r_begin = cell_begin(cell) + (int64_t)(w - cta_start[cell]) * TM;
+      const int64_t r_end = min(cell_end(cell), r_begin + TM);
       const int rw = rw_next;
       const int64_t gal = gal_next;
-      const int n_rows = r_end - r_begin;
-      // the next tile's rows follow this tile's in `order`
-      int r_end_next = r_end;
+      const int n_rows = (int)(r_end - r_begin);
+      // the next tile's rows
+      rw_next = -1;
       if (w + 1 < w_end) {
         int cn = cell;
         while (cta_start[cn + 1] <= w + 1) ++cn;
-        r_end_next = min(row_start[cn + 1], r_end + TM);
+        const int64_t rbn = cell_begin(cn) + (int64_t)(w + 1 - cta_start[cn]) * TM;
+        if (rbn + r < min(cell_end(cn), rbn + TM)) rw_next = __ldg(G.order + rbn + r);
       }
-      rw_next = (r_end + r < r_end_next) ? __ldg(G.order + r_end + r) : -1;
       gal_next = 0;
       // ---- the row's scalars, metallicity weights and this thread's bands of the observations: requested during the
       //      previous tile (before its wait for pass 2) ----
@@ -635,9 +657,10 @@ sps_status sps_approx_tc_contract(const sps_table* t, Workspace& ws, int64_t n, 
   if (n <= 0) return SPS_OK;
   const ApproxTc* S = t->approx_tc;
   const TableDev& T = t->dev;
-  approx_group_rows(T, n, rows, ws.rows, TM, s);
   ApproxArgs G;
-  G.n = n; G.order = ws.rows.order; G.bins = ws.rows.bins; G.gal_of_row = gal_of_row; G.obs_flux = obs_flux; G.obs_sigma = obs_sigma;
+  if (ws.rows.cell_list) { G.order = ws.rows.cell_list; G.cap = ws.rows.cell_cap; }      // the prologue filled the per-cell lists
+  else { approx_group_rows(T, n, rows, ws.rows, TM, s); G.order = ws.rows.order; G.cap = 0; }
+  G.n = n; G.bins = ws.rows.bins; G.gal_of_row = gal_of_row; G.obs_flux = obs_flux; G.obs_sigma = obs_sigma;
   G.flux_bar = flux_bar; G.want_grad = want_grad ? 1 : 0;
   G.Cm = S->Cm; G.inv_sD = 1.f / S->sD;
   sps_prof_begin(SPS_K_APPROX, s);

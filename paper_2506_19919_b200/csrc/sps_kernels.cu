@@ -86,7 +86,10 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
     sc.logp_like = 0.f; sc.Mn_bar = sc.z_bar = sc.AV_bar = sc.delta_bar = sc.Ffloor_bar = 0.f;
     sc.Msum = R.Msum; sc.pad1 = R.th[7]; sc.pad2 = R.th[8];       // logZ, sigma_logZ for the non-separable contraction (R26)
     B.sc[row] = sc;
-    if (hist) atomicAdd(&hist[sc.zbin], 1);                 // z-cell histogram for the approximate path's row grouping
+    if (hist) {                                             // z-cell histogram (and row list) for the approximate path's row grouping
+      const int pos = atomicAdd(&hist[sc.zbin], 1);
+      if (B.cell_list) B.cell_list[(int64_t)sc.zbin * B.cell_cap + pos] = (int)row;
+    }
   }
 }
 

@@ -78,7 +78,10 @@ __global__ void __launch_bounds__(256) tiny5_prologue_kernel(TableDev T, PriorDe
     sc.logp_like = 0.f; sc.Mn_bar = sc.z_bar = sc.AV_bar = sc.delta_bar = sc.Ffloor_bar = 0.f;
     sc.Msum = (float)R.G_obs; sc.pad1 = sc.pad2 = 0.f;
     B.sc[row] = sc;
-    if (hist) atomicAdd(&hist[sc.zbin], 1);
+    if (hist) {
+      const int pos = atomicAdd(&hist[sc.zbin], 1);
+      if (B.cell_list) B.cell_list[(int64_t)sc.zbin * B.cell_cap + pos] = (int)row;
+    }
   }
 }
 

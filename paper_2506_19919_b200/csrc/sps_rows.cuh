@@ -16,6 +16,8 @@ struct RowBuffers {
                    //                              gradient prologue and contracted with a_bar by the epilogue
   int* order;      // [n]  rows of the current approximate-path call grouped by z cell
   int* bins;       // [4][n_z + 1] histogram, row offsets, CTA offsets, cursors of that grouping
+  int* cell_list;  // [n_z - 1][cell_cap] rows of every z cell, appended by the prologue (or null: scan / scatter pass instead)
+  int64_t cell_cap;
   int64_t capacity;
 };
 
