@@ -387,20 +387,10 @@ def test_nuts_mixed_paths_config5_shape(tiny):
         single = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path=path, **kw)["samples"].cpu().numpy().reshape(n_gal, n_chain, 20, 13)
         sel = mask == path
         err = np.abs(ms[sel] - single[sel]) / np.maximum(1.0, np.abs(single[sel]))
-        if path == 1:                                                   # approximate path: deterministic, so bit-identical
-            assert err.max() == 0.0
-        else:                                                           # exact path: a row's band sums depend in the last bit on the rows it
-            # shares a tile with (wavelength ranges of the tile's plan, atomics), and NUTS amplifies that from one transition
-            # to the next, so after the 20 warmup transitions only the bulk agrees; what is unique is the start (below)
-            assert np.median(err.reshape(sel.sum() * n_chain, -1).max(1)) <= 5e-2
-    # the first transitions, before the dynamics has amplified the last-bit differences: every exact-path chain of the
-    # mixed run must reproduce the exact-only run
-    kw0 = dict(kw, n_warmup=0, n_sample=3)
-    m0 = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path_of_gal=_dev(mask, torch.int32), **kw0)["samples"].cpu().numpy().reshape(n_gal, n_chain, 3, 13)
-    s0 = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), path=0, **kw0)["samples"].cpu().numpy().reshape(n_gal, n_chain, 3, 13)
-    sel = mask == 0
-    assert (np.abs(m0[sel] - s0[sel]) / np.maximum(1.0, np.abs(s0[sel]))).max() <= 1e-4
-    assert np.abs(m0[sel][:, :, 1:] - m0[sel][:, :, :1]).max() > 0.0      # and the chains do move
+        # both paths are deterministic (the exact path's band sums are integer atomics: a row's result does not depend on
+        # the rows it shares a launch with), so after 20 warmup + 20 kept NUTS transitions the chains are bit-identical
+        assert err.max() == 0.0, path
+    assert np.abs(ms[:, :, 1:] - ms[:, :, :1]).max() > 0.0                # and the chains do move
     assert (mixed["n_leapfrog"].cpu().numpy() >= 40).all()
 
 
