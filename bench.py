@@ -219,7 +219,7 @@ def run_ours(args):
             hist = o["depth_hist"].cpu().numpy().tolist()
             extra.update({"mean_leapfrogs_per_transition": evals_per_step / (n_gal * cfg["n_chain"] * (n_warmup + n_sample)),
                           "divergences": int(o["divergences"].sum().item()), "tree_depth_hist": hist})
-    pairs = sps.sps_exact_last_work(table) if args.workload == "c2_exact" else 0
+    pairs = sps.sps_exact_last_work(table) if args.workload in ("c2_exact", "c5_nuts") else 0    # c5: the last exact launch of the run
     if rank != 0:
         return
     value = to_value(aggregate_throughput(units_per_step * args.steps, world, dev_s), 1.0)
@@ -260,8 +260,8 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), at the
 # launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("prologue", 40000): 71.1e6, ("approx_contract", 40000): 84.8e6, ("epilogue", 40000): 139.9e6,   # profiles/r01_hmc_kernels_full.md
-    ("exact_fwd", 8192): 74.2e6,                                                                      # profiles/r01_exact_gemm_full.md
+    ("prologue", 40000): 71.7e6, ("approx_contract", 40000): 58.4e6, ("epilogue", 40000): 142.8e6,   # profiles/r02_hmc_kernels_full.md
+    ("exact_fwd", 8192): 96.4e6, ("exact_bwd", 8192): 252.1e6,                                        # profiles/r02_exact_gemm_full.md
 }
 
 
