@@ -39,6 +39,7 @@ struct TableDev {
   // age grid (R5): A[i] lower age edge of bin i in Gyr (A[0] = 0, A[n_age] = +huge)
   const double* A_edge_d;   // [n_age+1] the same in double: t_obs - A is formed in double (old bins cancel)
   const double* A_mid_d;    // [n_age]
+  const float2* A_edge_hl;  // [128] the edges as float pairs (hi, lo = double - hi; entries past n_age: +huge): t_obs - A in two-float arithmetic
   const float* A_edge;      // [n_age+1]
   const float* A_mid;       // [n_age]   (A[i]+A[i+1])/2   (last: unused)
   const float* A_half;      // [n_age]   (A[i+1]-A[i])/2   (last: +huge)

@@ -22,6 +22,23 @@ __device__ __forceinline__ PriorView stage_prior(const PriorDev& P, float* s_pri
                    s_prior + 5 * SPS_NDIM, s_prior + 6 * SPS_NDIM};
 }
 
+// 1 / (1 + exp(-x)) in double at ~30 instructions (libdevice's exp and the division cost ~80): exp(-|x|) = 2^-n exp(-r) with
+// |r| <= ln2 / 2 by a degree-10 Taylor polynomial (2e-13), the reciprocal by one Newton step from the fp32 one (4e-15).
+__device__ __forceinline__ double sigmoid_d(double x) {
+  const double a = fmin(fabs(x), 44.0);
+  const double nd = rint(a * 1.4426950408889634);
+  const double r = fma(nd, -1.9082149292705877e-10, fma(nd, -0.693147180369123816490, a));      // a - n ln2 (ln2 = hi + lo)
+  double p = 2.755731922398589e-7;                                                                  // exp(-r): 1/10!, -1/9!, ...
+  p = fma(p, r, -2.755731922398589e-6); p = fma(p, r, 2.48015873015873e-5); p = fma(p, r, -1.984126984126984e-4);
+  p = fma(p, r, 1.388888888888889e-3); p = fma(p, r, -8.333333333333333e-3); p = fma(p, r, 4.166666666666666e-2);
+  p = fma(p, r, -1.6666666666666666e-1); p = fma(p, r, 0.5); p = fma(p, r, -1.0); p = fma(p, r, 1.0);
+  const double e = p * __hiloint2double((1023 - (int)nd) << 20, 0);
+  const double d = 1.0 + e;
+  const double y0 = (double)__frcp_rn((float)d);
+  const double y = fma(y0, fma(-d, y0, 1.0), y0);                                                   // 1 / (1 + e^-|x|)
+  return x >= 0.0 ? y : e * y;
+}
+
 template <bool NEED_ZD = true, class PR = PriorDev>
 __device__ __forceinline__ void load_params(const float* __restrict__ row, bool unbounded, const PR& pr,
                                             float th[SPS_NDIM], double& z_d) {
@@ -35,7 +52,7 @@ __device__ __forceinline__ void load_params(const float* __restrict__ row, bool 
       float s = 1.f / (1.f + expf(-pr.k[l] * (v - pr.x0[l])));
       float w = pr.y_hi[l] - pr.y_lo[l];
       if (NEED_ZD && l == SPS_NDIM - 1) {
-        const double sd = 1.0 / (1.0 + exp(-(double)pr.k[l] * ((double)v - (double)pr.x0[l])));
+        const double sd = sigmoid_d((double)pr.k[l] * ((double)v - (double)pr.x0[l]));
         vd = (double)pr.y_lo[l] + ((double)pr.y_hi[l] - (double)pr.y_lo[l]) * sd;
       }
       v = pr.y_lo[l] + w * s;
@@ -79,17 +96,34 @@ __device__ __forceinline__ void cosmic_time(const TableDev& T, double z_d, doubl
 }
 
 // ---- a2: double power law, Eq. (A4) PAPER.md:346 ---------------------------------------------------
-// f = 1/(x^alpha + x^-beta) at x = 2^lx2, plus q = f^2 (alpha x^alpha - beta x^-beta)  (df/dtau = q/tau,
-// df/dt = -q/t), fa = df/dalpha, fb = df/dbeta.
-__device__ __forceinline__ void sfr_node(float lx2, float alpha, float beta, float& f, float& q, float& fa, float& fb) {
-  float xa = exp2f(fminf(alpha * lx2, 60.f));
-  float xb = exp2f(fminf(-beta * lx2, 60.f));
-  f = __fdividef(1.f, xa + xb);
-  float f2 = f * f, lx = lx2 * LN2F;
-  q = f2 * (alpha * xa - beta * xb);
-  fa = -f2 * xa * lx;
-  fb = f2 * xb * lx;
+// f = 1/(x^alpha + x^-beta) at x = 2^lx2.  With A = f^2 x^alpha and B = f^2 x^-beta the partials are
+//   t df/dt = -(alpha A - beta B) = -q,  df/dtau = q / tau,  df/dalpha = -A ln x,  df/dbeta = B ln x,
+// so a quadrature accumulates sum w f, sum w A, sum w B, sum w A lx2, sum w B lx2 (and sum w A / t, sum w B / t for the
+// t_obs partial) and combines them once per bin (SfrSums::finish) instead of forming q, fa, fb at every node.
+struct SfrNode { float f, A, B, lx2; };
+__device__ __forceinline__ SfrNode sfr_node(float lx2, float alpha, float beta) {
+  const float xa = exp2f(fminf(alpha * lx2, 60.f));
+  const float xb = exp2f(fminf(-beta * lx2, 60.f));
+  SfrNode n;
+  n.f = __fdividef(1.f, xa + xb);
+  const float f2 = n.f * n.f;
+  n.A = f2 * xa; n.B = f2 * xb; n.lx2 = lx2;
+  return n;
 }
+struct SfrSums {
+  float f = 0.f, A = 0.f, B = 0.f, Al = 0.f, Bl = 0.f, At = 0.f, Bt = 0.f;
+  __device__ __forceinline__ void add(const SfrNode& n, float w) {
+    f = fmaf(w, n.f, f);
+    const float wA = w * n.A, wB = w * n.B;
+    A += wA; B += wB; Al = fmaf(wA, n.lx2, Al); Bl = fmaf(wB, n.lx2, Bl);
+  }
+  __device__ __forceinline__ void add_t(const SfrNode& n, float w, float inv_t) {      // also the d/dt_obs sums (linear-t rules)
+    f = fmaf(w, n.f, f);
+    const float wA = w * n.A, wB = w * n.B;
+    A += wA; B += wB; Al = fmaf(wA, n.lx2, Al); Bl = fmaf(wB, n.lx2, Bl);
+    At = fmaf(wA, inv_t, At); Bt = fmaf(wB, inv_t, Bt);
+  }
+};
 __device__ __forceinline__ float sfr_value(float t, float tau, float alpha, float beta) {
   if (!(t > 0.f)) return 0.f;
   float lx2 = __log2f(t / tau);
@@ -110,61 +144,87 @@ __device__ __constant__ float GL8_X[8] = {-0.9602898564975363f, -0.7966664774136
 __device__ __constant__ float GL8_W[8] = {0.1012285362903763f, 0.2223810344533745f, 0.3137066458778873f, 0.3626837833783620f,
                                           0.3626837833783620f, 0.3137066458778873f, 0.2223810344533745f, 0.1012285362903763f};
 
+// Four values summed over the warp in 6 shuffles (instead of 4 x 5): the halves of the warp swap two of the four, then the
+// quarters one of the two, then three plain steps.  Afterwards lane l holds the total of value (l >> 3) & 3.
+__device__ __forceinline__ float warp_sum4(float v0, float v1, float v2, float v3) {
+  const int l = lane_id();
+  const bool h16 = l & 16, h8 = l & 8;
+  float k0 = h16 ? v2 : v0, k1 = h16 ? v3 : v1;
+  k0 += __shfl_xor_sync(FULL_MASK, h16 ? v0 : v2, 16);
+  k1 += __shfl_xor_sync(FULL_MASK, h16 ? v1 : v3, 16);
+  float k = h8 ? k1 : k0;
+  k += __shfl_xor_sync(FULL_MASK, h8 ? k0 : k1, 8);
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) k += __shfl_xor_sync(FULL_MASK, k, o);
+  return k;
+}
+
 // Mass formed per age bin (Eq. A5; R5, R6 restated for fp32):
 //  * bins whose span in ln t is small against the width 1/(alpha+beta) of the SFR turnover are
 //    integrated by 2- or 4-point Gauss-Legendre in linear t with the tabulated bin width (no
 //    t_obs - age cancellation in the width);
 //  * the few old bins near age ~ t_obs (and the one that reaches t = 0) are integrated by the whole
 //    warp: 8-point Gauss-Legendre panels in v = ln t, cut at ln t_hi - 16/(beta+1).
+// t = t_obs - age in two-float arithmetic: t_obs = th + tl, edge = ah + al; (th - ah) is exact where the two are within a
+// factor of two (the old bins, where the difference cancels), so t is within an ulp of the double difference everywhere.
 template <bool WANT_GRAD>
 __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, float tau, float alpha, float beta, AgeQuad& Q) {
   const int l = lane_id();
   const float l2tau = __log2f(tau);
   const float ab = alpha + beta;
+  const float th = (float)t_obs_d, tl = (float)(t_obs_d - (double)th);
+  float t_edge[SPS_AGE_PER_LANE + 1];       // t at the lower age edge of the lane's bins (= t_hi of the bin), clipped at 0
+#pragma unroll
+  for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
+    const float2 e = T.A_edge_hl[l + 32 * q];
+    t_edge[q] = fmaxf((th - e.x) + (tl - e.y), 0.f);
+  }
+  t_edge[SPS_AGE_PER_LANE] = 0.f;
   unsigned problem_mask[SPS_AGE_PER_LANE];
   float t_lo_q[SPS_AGE_PER_LANE], t_hi_q[SPS_AGE_PER_LANE];
 #pragma unroll
   for (int q = 0; q < SPS_AGE_PER_LANE; ++q) {
     const int i = l + 32 * q;
     Q.dM[q] = Q.g_tau[q] = Q.g_al[q] = Q.g_be[q] = Q.g_t[q] = 0.f;
-    float t_hi = 0.f, t_lo = 0.f, half = 0.f, t_mid = 1.f;
+    // the bin's upper age edge is the lower edge of the next bin: lane + 1, or lane 0's next slot
+    float t_lo = __shfl_down_sync(FULL_MASK, t_edge[q], 1);
+    const float t_lo0 = __shfl_sync(FULL_MASK, t_edge[q + 1], 0);
+    if (l == 31) t_lo = t_lo0;
+    float t_hi = 0.f, half = 0.f, t_mid = 1.f;
     int kind = 0;                       // 0 empty, 1 GL2, 2 GL4, 3 warp-cooperative
-    if (i < T.n_age) {
-      t_hi = (float)(t_obs_d - T.A_edge_d[i]);
-      t_lo = fmaxf((float)(t_obs_d - T.A_edge_d[i + 1]), 0.f);
+    if (i < T.n_age && t_edge[q] > 0.f) {
+      t_hi = t_edge[q];
       half = T.A_half[i];
-      t_mid = (float)(t_obs_d - T.A_mid_d[i]);
-      if (t_hi > 0.f) {
-        // half-width over the distance to the nearest singularity: the turnover poles at Im ln t = pi/(alpha+beta)
-        // and the branch point of t^beta at t = 0
-        float s = (t_lo > 0.f) ? (half / t_mid) * fmaxf(ab * 0.3183098861837907f, 1.f) : 1e9f;
-        kind = (s < 0.06f) ? 1 : (s < 0.36f ? 2 : 3);
-      } else t_hi = 0.f;
-    }
+      t_mid = t_hi - half;
+      // half-width over the distance to the nearest singularity: the turnover poles at Im ln t = pi/(alpha+beta)
+      // and the branch point of t^beta at t = 0
+      const float s = (t_lo > 0.f) ? __fdividef(half, t_mid) * fmaxf(ab * 0.3183098861837907f, 1.f) : 1e9f;
+      kind = (s < 0.06f) ? 1 : (s < 0.36f ? 2 : 3);
+    } else t_lo = 0.f;
     t_lo_q[q] = t_lo; t_hi_q[q] = t_hi;
     problem_mask[q] = __ballot_sync(FULL_MASK, kind == 3);
     const bool any4 = __any_sync(FULL_MASK, kind == 2);
     if (kind == 1 || kind == 2) {
-      float s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+      SfrSums S;
       if (!any4) {
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
-          float t = t_mid + half * GL2_X[k], f, qq, fa, fb;
-          sfr_node(__log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
-          s0 += f;
-          if (WANT_GRAD) { s1 += qq; s2 += fa; s3 += fb; s4 -= __fdividef(qq, t); }
+          const float t = t_mid + half * GL2_X[k];
+          S.add_t(sfr_node(__log2f(t) - l2tau, alpha, beta), 1.f, __fdividef(1.f, t));
         }
       } else {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          float t = t_mid + half * GL4_X[k], f, qq, fa, fb, w = GL4_W[k];
-          sfr_node(__log2f(t) - l2tau, alpha, beta, f, qq, fa, fb);
-          s0 += w * f;
-          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; s4 -= w * __fdividef(qq, t); }
+          const float t = t_mid + half * GL4_X[k];
+          S.add_t(sfr_node(__log2f(t) - l2tau, alpha, beta), GL4_W[k], __fdividef(1.f, t));
         }
       }
-      Q.dM[q] = half * s0;
-      if (WANT_GRAD) { Q.g_tau[q] = half * s1 / tau; Q.g_al[q] = half * s2; Q.g_be[q] = half * s3; Q.g_t[q] = half * s4; }
+      Q.dM[q] = half * S.f;
+      if (WANT_GRAD) {
+        Q.g_tau[q] = half * (alpha * S.A - beta * S.B) / tau;
+        Q.g_al[q] = -half * LN2F * S.Al; Q.g_be[q] = half * LN2F * S.Bl;
+        Q.g_t[q] = -half * (alpha * S.At - beta * S.Bt);
+      }
     }
   }
   // warp-cooperative bins: 8-point Gauss-Legendre panels in v = ln t.
@@ -187,21 +247,19 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       const float dv = v_hi - v_lo;
       const int n_pan = max(1, (int)ceilf(dv / w_target));
       const float wp = dv / (float)n_pan;
-      float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+      SfrSums S;
+      const float xk = 0.5f + 0.5f * GL8_X[l & 7], wk = 0.5f * wp * GL8_W[l & 7];
       for (int n = l; n < n_pan * 8; n += 32) {
-        const int pan = n >> 3, k = n & 7;
-        const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
-        const float w = 0.5f * wp * GL8_W[k] * __expf(v);        // dt = t dv
-        float f, qq, fa, fb;
-        sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
-        s0 += w * f;
-        if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; }
+        const float v = v_lo + ((float)(n >> 3) + xk) * wp;
+        S.add(sfr_node((v - ln_tau) * LOG2EF, alpha, beta), wk * __expf(v));        // dt = t dv
       }
-      s0 = warp_sum(s0);
-      if (WANT_GRAD) { s1 = warp_sum(s1); s2 = warp_sum(s2); s3 = warp_sum(s3); }
+      const float s0 = warp_sum(S.f);
+      // the four gradient sums in one pass: lane l ends up with the total of sum (l >> 3) & 3
+      const float g = warp_sum4(alpha * S.A - beta * S.B, S.Al, S.Bl, 0.f);
+      const float r1 = __shfl_sync(FULL_MASK, g, 0), r2 = __shfl_sync(FULL_MASK, g, 8), r3 = __shfl_sync(FULL_MASK, g, 16);
       if (l == src) {
         Q.dM[q] = s0;
-        if (WANT_GRAD) { Q.g_tau[q] = s1 / tau; Q.g_al[q] = s2; Q.g_be[q] = s3; Q.g_t[q] = sfr_value(t_hi, tau, alpha, beta); }   // Leibniz, f(0) = 0
+        if (WANT_GRAD) { Q.g_tau[q] = r1 / tau; Q.g_al[q] = -LN2F * r2; Q.g_be[q] = LN2F * r3; Q.g_t[q] = sfr_value(t_hi, tau, alpha, beta); }   // Leibniz, f(0) = 0
       }
     }
     while (m) {
@@ -220,17 +278,15 @@ __device__ __forceinline__ void smooth_bins(const TableDev& T, double t_obs_d, f
       const float wp = dv / (float)max(n_pan, 1);
       int n_max = max(n_pan, __shfl_xor_sync(FULL_MASK, n_pan, 8));
       n_max = max(n_max, __shfl_xor_sync(FULL_MASK, n_max, 16));
-      float s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+      SfrSums S;
+      const float xk = 0.5f + 0.5f * GL8_X[k], wk = 0.5f * wp * GL8_W[k];
       for (int pan = 0; pan < n_max; ++pan) {
         if (pan < n_pan) {
-          const float v = v_lo + ((float)pan + 0.5f + 0.5f * GL8_X[k]) * wp;
-          const float w = 0.5f * wp * GL8_W[k] * __expf(v);
-          float f, qq, fa, fb;
-          sfr_node((v - ln_tau) * LOG2EF, alpha, beta, f, qq, fa, fb);
-          s0 += w * f;
-          if (WANT_GRAD) { s1 += w * qq; s2 += w * fa; s3 += w * fb; }
+          const float v = v_lo + ((float)pan + xk) * wp;
+          S.add(sfr_node((v - ln_tau) * LOG2EF, alpha, beta), wk * __expf(v));
         }
       }
+      float s0 = S.f, s1 = alpha * S.A - beta * S.B, s2 = -LN2F * S.Al, s3 = LN2F * S.Bl;
 #pragma unroll
       for (int o = 4; o > 0; o >>= 1) {
         s0 += __shfl_xor_sync(FULL_MASK, s0, o);

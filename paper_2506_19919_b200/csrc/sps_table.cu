@@ -290,6 +290,9 @@ extern "C" sps_status sps_create_table(const sps_table_desc* d, sps_table** out)
   std::vector<double> Amid_d(na);
   for (int i = 0; i < na; ++i) Amid_d[i] = 0.5 * (Ae[i] + Ae[i + 1]);
   T.A_edge_d = upload(Ae, st); T.A_mid_d = upload(Amid_d, st);
+  std::vector<float2> Ahl(SPS_AGE_PER_LANE * 32, make_float2(1e30f, 0.f));
+  for (int i = 0; i <= na && i < (int)Ahl.size(); ++i) { const float hi = (float)Ae[i]; Ahl[i] = make_float2(hi, (float)(Ae[i] - (double)hi)); }
+  T.A_edge_hl = upload(Ahl, st);
   if (!tz.empty()) T.tz_coef = upload(tz, st);
   T.A_edge = upload(A_edge, st); T.A_mid = upload(A_mid, st); T.A_half = upload(A_half, st); T.e_edge = upload(e_edge, st);
   T.g_mid = upload(g_mid, st); T.la9 = upload(la9, st); T.wave = upload(wave, st); T.dlam = upload(dlam, st); T.k0 = upload(k0, st);
@@ -330,7 +333,7 @@ extern "C" sps_status sps_destroy_table(sps_table* t) {
   if (!t) return SPS_OK;
   TableDev& T = t->dev;
   cudaDeviceSynchronize();
-  const void* ptrs[] = {T.tz_coef, T.A_edge_d, T.A_mid_d, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp,
+  const void* ptrs[] = {T.tz_coef, T.A_edge_d, T.A_mid_d, T.A_edge_hl, T.A_edge, T.A_mid, T.A_half, T.e_edge, T.g_mid, T.wave, T.dlam, T.k0, T.drude, T.l2r, T.ssp, T.cssp,
                         T.gauss, T.ft.knots, T.ft.first, T.la9};
   for (const void* p : ptrs) if (p) cudaFree(const_cast<void*>(p));
   sps_exact_teardown(t);
