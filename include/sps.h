@@ -124,9 +124,12 @@ int32_t sps_model_ndim(const sps_table* t);
  *   SPS_OPT_NO_GRAPH       1: sps_hmc_run launches every kernel directly instead of replaying a CUDA graph
  *   SPS_OPT_ROW_GROUPS     n: fixed-length HMC splits its chains into n (1..4) groups whose evaluations run on different
  *                             streams (an experiment in overlapping one group's contraction with another's row
- *                             kernels; measured slower); 0 or 1 = one group.  Results do not depend on it. */
+ *                             kernels; measured slower); 0 or 1 = one group.  Results do not depend on it.
+ *   SPS_OPT_NO_PDL         1: the prologue / contraction / epilogue kernels are launched with plain stream order instead of
+ *                             programmatic dependent launch (each kernel's launch and set-up then no longer overlap the
+ *                             tail of the one before it).  Results do not depend on it. */
 enum { SPS_OPT_CHECK_FINITE = 0, SPS_OPT_EXACT_SIMT = 1, SPS_OPT_APPROX_SIMT = 2, SPS_OPT_NO_TC_SETUP = 3, SPS_OPT_NO_GRAPH = 4,
-       SPS_OPT_ROW_GROUPS = 5, SPS_OPT_COUNT = 6 };
+       SPS_OPT_ROW_GROUPS = 5, SPS_OPT_NO_PDL = 6, SPS_OPT_COUNT = 7 };
 sps_status sps_set_option(int option, int value);
 
 /* Copy the c_SSP table to a HOST buffer of n_z*n_age*n_Z*n_band floats (diagnostic; synchronises). */

@@ -17,7 +17,7 @@ PATH_EXACT, PATH_APPROX = 0, 1
 SAMPLER_HMC, SAMPLER_NUTS = 0, 1
 EXACT_BF16X3, EXACT_TF32X3 = 0, 1
 MODEL_TINY5, MODEL_DPL13, MODEL_GAUSS_TEST = 0, 1, 2
-OPT_CHECK_FINITE, OPT_EXACT_SIMT, OPT_APPROX_SIMT, OPT_NO_TC_SETUP, OPT_NO_GRAPH, OPT_ROW_GROUPS = 0, 1, 2, 3, 4, 5
+OPT_CHECK_FINITE, OPT_EXACT_SIMT, OPT_APPROX_SIMT, OPT_NO_TC_SETUP, OPT_NO_GRAPH, OPT_ROW_GROUPS, OPT_NO_PDL = 0, 1, 2, 3, 4, 5, 6
 STATUS_ENONFINITE = 6
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",

@@ -192,6 +192,7 @@ sps_status sps_ensure_row_buffers(const sps_table* t, Workspace& ws, int64_t n, 
   if (B.capacity >= n) return SPS_OK;
   cudaStreamSynchronize(s);                                  // earlier calls on this stream may still use the old scratch
   free_row_buffers(B);
+  ws.bins_clean = false;
   const int64_t cap = n;
   cudaError_t e = cudaSuccess;
   auto al = [&](void** p, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(p, bytes); };
@@ -244,8 +245,11 @@ sps_status sps_eval(const sps_table* t, Workspace& ws, const PriorDev& P, int pa
   }
   const bool tiny5 = T.model == SPS_MODEL_TINY5, nonsep = T.agez_gamma != 0.f;
   const bool bucket = path == SPS_PATH_APPROX && !nonsep;   // the separable approximate kernels want rows grouped by z cell
+  // tensor-core contraction on the prologue's cell lists: it leaves the cell counts cleared (Workspace::bins_clean)
+  const bool direct_tc = bucket && sps_approx_tc_active(t) && ws.rows.cell_list != nullptr;
   if (tiny5) launch_prologue_tiny5(T, P, theta, n, unbounded, rows, ws.rows, bucket, s);
-  else launch_prologue(T, P, theta, n, unbounded, want_grad, rows, ws.rows, bucket, s, overlap);
+  else launch_prologue(T, P, theta, n, unbounded, want_grad, rows, ws.rows, bucket, s, overlap, !(direct_tc && ws.bins_clean));
+  if (bucket) ws.bins_clean = direct_tc;
   if (path == SPS_PATH_APPROX) {
     if (nonsep) launch_nonsep_approx(T, n, rows, gal_of_row, obs_flux, obs_sigma, flux_bar, want_grad, ws.rows, s);
     else if (sps_approx_tc_active(t)) {

@@ -105,7 +105,7 @@ enum { BAR_B1 = 0, BAR_A, BAR_P, BAR_B2, BAR_V0, BAR_M1, N_BARS };
 
 struct ApproxArgs {
   int64_t n;
-  const int* order; const int* bins;
+  const int* order; int* bins;   // (direct mode: the last CTA to read the counts clears them for the next prologue)
   int64_t cap;             // > 0: `order` is the prologue's per-cell row lists [cell][cap] and bins[0..nb) their lengths (no scan / scatter pass)
   const int* gal_of_row; const float* obs_flux; const float* obs_sigma; const float* flux_bar;
   int want_grad;
@@ -122,6 +122,7 @@ __global__ void __launch_bounds__(THREADS_TC, ATC_MINB)
 approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__ CUtensorMap m1h, const __grid_constant__ CUtensorMap m1l,
                  const __grid_constant__ CUtensorMap m2h, const __grid_constant__ CUtensorMap m2l) {
   extern __shared__ unsigned char smem_dyn[];
+  __shared__ int s_last;
   const int nb = T.n_z - 1, stride = nb + 2;
   const bool direct = G.cap > 0;
   const int* row_start_g = G.bins + stride; const int* cta_start_g = G.bins + 2 * stride;
@@ -137,12 +138,16 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
 #define BAR(i) (bars + 8u * (i))
   // cell offsets of the call in shared memory when they fit (they are walked once per tile by every thread)
   int* bins_s = reinterpret_cast<int*>(gbase + OFF_EXTRA + (2 + 6 + 16) * 128 * 4);
+  pdl_wait();                                               // the prologue's counts, lists and row buffers
   if (!direct) {
     for (int i = threadIdx.x; i <= nb; i += blockDim.x) { bins_s[i] = row_start_g[i]; bins_s[nb + 1 + i] = cta_start_g[i]; }
   } else {
     // the prologue left a row list and a count per z cell: every CTA turns the counts into tile offsets itself
     for (int i = threadIdx.x; i <= nb; i += blockDim.x) { const int c = i < nb ? G.bins[i] : 0; bins_s[i] = c; bins_s[nb + 1 + i] = (c + TM - 1) / TM; }
     __syncthreads();
+    // arrival count (bins[3 stride]): the last CTA to have read the counts clears them, so the next prologue of this
+    // workspace can append to its cells without a memset in between
+    if (threadIdx.x == 0) { __threadfence(); s_last = atomicAdd(G.bins + 3 * stride, 1) == (int)gridDim.x - 1; }
     if (warp == 0) {
       int carry = 0;
       for (int b0 = 0; b0 <= nb; b0 += 32) {
@@ -156,6 +161,10 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
     }
   }
   __syncthreads();
+  if (direct && s_last) {
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) G.bins[i] = 0;
+    if (threadIdx.x == 0) G.bins[3 * stride] = 0;
+  }
   const int* row_start = bins_s;                            // legacy: first position of each cell in `order`; direct: the cell's row count
   const int* cta_start = bins_s + nb + 1;
   auto cell_begin = [&](int c) { return direct ? (int64_t)c * G.cap : (int64_t)row_start[c]; };
@@ -578,8 +587,7 @@ template <int NB>
 sps_status launch_nb(const ApproxTc* S, int sm_count, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
   if (configure_only)
     return sps_check_cuda(cudaFuncSetAttribute(approx_tc_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TC), "approximate tensor-core kernel shared memory opt-in");
-  approx_tc_kernel<NB><<<sm_count, THREADS_TC, SMEM_TC, s>>>(T, G, B, S->m1_hi, S->m1_lo, S->m2_hi, S->m2_lo);
-  return SPS_OK;
+  return sps_check_cuda(sps_launch(approx_tc_kernel<NB>, dim3(sm_count), dim3(THREADS_TC), SMEM_TC, s, T, G, B, S->m1_hi, S->m1_lo, S->m2_hi, S->m2_lo), "approximate contraction (tcgen05) launch");
 }
 sps_status dispatch(const ApproxTc* S, int sm_count, const TableDev& T, const ApproxArgs& G, const RowBuffers& B, cudaStream_t s, bool configure_only) {
   switch (T.n_band) {

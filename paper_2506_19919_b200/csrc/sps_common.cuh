@@ -148,6 +148,18 @@ __device__ __forceinline__ void filter_tab_eval(const FilterTab& F, int b, float
 extern "C" int64_t sps_launch_count(void);
 void sps_count_launch(int n = 1);
 bool sps_prof_enabled();
+
+// Programmatic dependent launch (griddepcontrol): a kernel launched with sps_launch() may start while the kernel before it
+// in the stream is still draining; it must not touch that kernel's results before pdl_wait() (which returns once the
+// preceding grid has completed and its writes are visible).  pdl_launch_dependents() would let the NEXT kernel's blocks be
+// scheduled as soon as every block of this grid has issued it; no kernel here calls it (measured at 40,000 rows: early-
+// resident blocks of the next kernel cost more than they save: contraction +7 us, prologue 0, epilogue -1), so a
+// dependent kernel's launch overlaps the tail of the one before and its blocks start as the last ones exit.
+// Both are no-ops under a plain launch.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#endif
 void sps_prof_begin(int id, cudaStream_t s);
 void sps_prof_end(int id, cudaStream_t s);
 void sps_set_error(const char* fmt, ...);

@@ -29,7 +29,10 @@ struct ExactScratch {
 struct Workspace {
   RowBuffers rows;
   ExactScratch x;
-  Workspace() { rows = RowBuffers(); x = ExactScratch(); }
+  // the z-cell counts in rows.bins are all zero (stream order): true after the tensor-core contraction, whose last CTA to
+  // read them clears them, so the next prologue of this workspace needs no memset node in front of it
+  bool bins_clean;
+  Workspace() : bins_clean(false) { rows = RowBuffers(); x = ExactScratch(); }
 };
 
 struct sps_table {

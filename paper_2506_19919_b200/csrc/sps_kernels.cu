@@ -57,6 +57,7 @@ prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t
   constexpr bool WANT_GRAD = true;
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
+  pdl_wait();                                                // theta, the z-cell counts and the row buffers belong to the kernels before
   const int64_t r = (int64_t)blockIdx.x * PW + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
@@ -487,6 +488,7 @@ epilogue_kernel(TableDev T, PriorDev P, const float* theta, int64_t n, bool unbo
                 const int* __restrict__ rows, RowBuffers B, float* __restrict__ logp, float* __restrict__ grad, LeapfrogFuse lf) {
   __shared__ float s_prior[7 * SPS_NDIM];
   const PriorView PV = stage_prior(P, s_prior);
+  pdl_wait();
   const int64_t r = (int64_t)blockIdx.x * EPI_WARPS_PER_BLOCK + (threadIdx.x >> 5);
   if (r >= n) return;
   const int64_t row = rows ? rows[r] : r;
@@ -601,13 +603,13 @@ __global__ void copy_flux_kernel(TableDev T, int64_t n, RowBuffers B, float* flu
 static inline unsigned blocks_for_rows(int64_t n) { return (unsigned)((n + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK); }
 
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks) {
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks, bool zero_bins) {
   if (n <= 0) return;
   int* hist = nullptr;
-  if (with_hist) { hist = B.bins; cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
+  if (with_hist) { hist = B.bins; if (zero_bins) cudaMemsetAsync(B.bins, 0, 4 * (size_t)(T.n_z + 1) * sizeof(int), s); }   // histogram and scatter cursors
   sps_prof_begin(SPS_K_PROLOGUE, s);
-  if (small_blocks) prologue_kernel<8><<<(unsigned)((n + 7) / 8), 256, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
-  else prologue_kernel<PRO_WARPS><<<(unsigned)((n + PRO_WARPS - 1) / PRO_WARPS), 32 * PRO_WARPS, 0, s>>>(T, P, theta, n, unbounded, want_grad, rows, B, hist);
+  if (small_blocks) sps_launch(prologue_kernel<8>, dim3((unsigned)((n + 7) / 8)), dim3(256), 0, s, T, P, theta, n, unbounded, want_grad, rows, B, hist);
+  else sps_launch(prologue_kernel<PRO_WARPS>, dim3((unsigned)((n + PRO_WARPS - 1) / PRO_WARPS)), dim3(32 * PRO_WARPS), 0, s, T, P, theta, n, unbounded, want_grad, rows, B, hist);
   sps_prof_end(SPS_K_PROLOGUE, s);
   sps_count_launch();
 }
@@ -665,7 +667,7 @@ void launch_epilogue(const TableDev& T, const PriorDev& P, const float* theta, i
                      bool with_prior, const int* rows, RowBuffers B, float* logp, float* grad, LeapfrogFuse lf, cudaStream_t s) {
   if (n <= 0) return;
   sps_prof_begin(SPS_K_EPILOGUE, s);
-  epilogue_kernel<<<(unsigned)((n + EPI_WARPS_PER_BLOCK - 1) / EPI_WARPS_PER_BLOCK), 32 * EPI_WARPS_PER_BLOCK, 0, s>>>(T, P, theta, n, unbounded, with_prior, rows, B, logp, grad, lf);
+  sps_launch(epilogue_kernel, dim3((unsigned)((n + EPI_WARPS_PER_BLOCK - 1) / EPI_WARPS_PER_BLOCK)), dim3(32 * EPI_WARPS_PER_BLOCK), 0, s, T, P, theta, n, unbounded, with_prior, rows, B, logp, grad, lf);
   sps_prof_end(SPS_K_EPILOGUE, s);
   sps_count_launch();
 }

@@ -1,6 +1,7 @@
 // sps_rows.cuh -- buffers exchanged between the per-row prologue / epilogue kernels (one warp per
 // parameter row; shared by the exact and the approximate photometry paths) and the contraction kernels.
 #pragma once
+#include <utility>
 #include "sps_model.cuh"
 
 // Work buffers for n rows (device memory owned by the library, grown on demand).
@@ -26,9 +27,24 @@ struct RowBuffers {
 struct LeapfrogFuse { float* theta_w; float* p_w; const float* eps; const float* inv_mass; };
 // (sps_eval's `overlap` flag: the call is one of several row groups running on different streams, see sps_sampler.cu)
 
+// Launch with the programmatic-stream-serialisation attribute (see pdl_wait in sps_common.cuh) unless SPS_OPT_NO_PDL is set
+// or the per-kernel profiling hooks are on (their events sit between the kernels anyway).
+int sps_option(int option);
+template <class... KA, class... A>
+inline cudaError_t sps_launch(void (*kernel)(KA...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, A&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at = {};
+  at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at.val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = &at;
+  cfg.numAttrs = (sps_option(6 /* SPS_OPT_NO_PDL */) || sps_prof_enabled()) ? 0 : 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<A>(args)...);
+}
+
 // kernels (sps_kernels.cu)
 void launch_prologue(const TableDev& T, const PriorDev& P, const float* theta, int64_t n, bool unbounded, bool want_grad,
-                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks = false);
+                     const int* rows, RowBuffers B, bool with_hist, cudaStream_t s, bool small_blocks = false, bool zero_bins = true);
 void launch_approx_contract(const TableDev& T, int sm_count, int64_t n, const int* rows, const int* gal_of_row,
                             const float* obs_flux, const float* obs_sigma, const float* flux_bar,
                             bool want_grad, RowBuffers B, cudaStream_t s);

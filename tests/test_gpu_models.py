@@ -577,3 +577,33 @@ def test_row_groups_do_not_change_results(full):
             assert torch.equal(out["theta_last"], ref["theta_last"]) and torch.equal(out["mean"], ref["mean"]) and torch.equal(out["eps"], ref["eps"])
     finally:
         cx.sps.sps_set_option(cx.sps.OPT_ROW_GROUPS, 0)
+
+
+def test_dependent_launch_and_cell_counts(full):
+    # The prologue / contraction / epilogue kernels are launched programmatically dependent on one another, and the
+    # tensor-core contraction clears the z-cell counts for the next prologue (no memset in between).  Neither may change a
+    # result: the same HMC run with SPS_OPT_NO_PDL, and log-posterior calls that alternate between the tensor-core kernel
+    # (clears the counts) and the SIMT kernel (needs them zeroed by the prologue's memset), bit for bit.
+    cx = full
+    n_gal = 300
+    thu, d, s = cx.observations(n_gal, 98, frac=(0.05, 0.10))
+    kw = dict(sampler=cx.sps.SAMPLER_HMC, path=cx.sps.PATH_APPROX, n_chain=4, n_warmup=6, n_sample=6, n_leapfrog=4, eps0=0.01, seed=3)
+    ref = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), **kw)
+    try:
+        cx.sps.sps_set_option(cx.sps.OPT_NO_PDL, 1)
+        out = cx.sps.sps_hmc_run(cx.table, cx.ph, _dev(d), _dev(s), **kw)
+        assert torch.equal(out["theta_last"], ref["theta_last"]) and torch.equal(out["mean"], ref["mean"]) and torch.equal(out["eps"], ref["eps"])
+    finally:
+        cx.sps.sps_set_option(cx.sps.OPT_NO_PDL, 0)
+    th = _dev(thu.astype(np.float32))
+    runs = []
+    try:
+        for simt in (0, 0, 1, 0, 1, 1, 0):
+            cx.sps.sps_set_option(cx.sps.OPT_APPROX_SIMT, simt)
+            lp, g = cx.sps.sps_loglike_grad(cx.table, cx.ph, cx.sps.PATH_APPROX, th, _dev(d), _dev(s))
+            runs.append((simt, lp.clone(), g.clone()))
+    finally:
+        cx.sps.sps_set_option(cx.sps.OPT_APPROX_SIMT, 0)
+    for simt, lp, g in runs:
+        first = next(r for r in runs if r[0] == simt)
+        assert torch.equal(lp, first[1]) and torch.equal(g, first[2])
