@@ -144,7 +144,7 @@ def run_ours(args):
             return out["mean"].cpu(), out["sd"].cpu(), out["rhat"].cpu()
 
         def profile_step():                                                      # a short run of the same launch shape, for kernel times
-            sps.sps_hmc_run(table, ph, d_dev, s_dev, **{**kw, "n_warmup": min(n_warmup, 12), "n_sample": min(n_sample, 12)})
+            last["prof"] = sps.sps_hmc_run(table, ph, d_dev, s_dev, **{**kw, "n_warmup": min(n_warmup, 12), "n_sample": min(n_sample, 12)})
         h2d = d_host.numel() * 4 * 2
         d2h = n_gal * cfg["n_chain"] * 13 * 4 * 2 + n_gal * 13 * 4
         metric, unit, to_value = "galaxy posteriors/GPU-minute", "posteriors/min", lambda units, sec: 60.0 * units / sec
@@ -204,8 +204,10 @@ def run_ours(args):
     dev_s, e2e_s = max_over_ranks([dev_s, e2e_s], dist, device="cuda")
     # ---- untimed: per-kernel event timing of the same launch shape, and the pipe peaks of this run -----------------------
     sps.sps_profile(True, 4)
+    sps.sps_exact_work_since(table)                                              # (reset)
     profile_step()
     torch.cuda.synchronize()
+    pair_sum, pair_calls = sps.sps_exact_work_since(table)
     prof = {k: sps.sps_profile_read(k) for k in ("prologue", "approx_contract", "epilogue", "exact_fwd", "exact_bwd")}
     sps.sps_profile(False, 1)
     pipe = {"mufu_per_s": sps.sps_measure_peak("mufu"), "ffma_per_s": sps.sps_measure_peak("ffma")}
@@ -219,7 +221,7 @@ def run_ours(args):
             hist = o["depth_hist"].cpu().numpy().tolist()
             extra.update({"mean_leapfrogs_per_transition": evals_per_step / (n_gal * cfg["n_chain"] * (n_warmup + n_sample)),
                           "divergences": int(o["divergences"].sum().item()), "tree_depth_hist": hist})
-    pairs = sps.sps_exact_last_work(table) if args.workload in ("c2_exact", "c5_nuts") else 0    # c5: the last exact launch of the run
+    pairs = pair_sum // max(1, pair_calls)                                       # average exact-path work per launch of the profiled pass
     if rank != 0:
         return
     value = to_value(aggregate_throughput(units_per_step * args.steps, world, dev_s), 1.0)
@@ -244,7 +246,17 @@ def run_ours(args):
         kernel_ms[k]["share_of_profiled_kernels"] = share[k] / tot
     dom = max(share, key=share.get)                                              # the dominant kernel of THIS run
     out["kernel_ms"] = kernel_ms
-    roofs = {k: kernel_roofline(k, kernel_ms[k]["avg_ms"] * 1e-3, rows_per_launch, grid, peaks, peaks_src, pipe, hmc, pairs) for k in kernel_ms}
+    # rows per launch: the batch, except under NUTS, whose launches shrink as trees finish and are split by path: there the
+    # average over the profiled pass = its row evaluations (sum of the chains' leapfrog counts) x the path's share / launches
+    rows_k = {k: rows_per_launch for k in kernel_ms}
+    if args.workload == "c5_nuts":
+        prof_evals = float(last["prof"]["n_leapfrog"].sum().item())
+        fx = cfg["exact_fraction"]
+        share_k = {"prologue": 1.0, "epilogue": 1.0, "approx_contract": 1.0 - fx, "exact_fwd": fx, "exact_bwd": fx}
+        rows_k = {k: max(1, int(round(prof_evals * share_k[k] / max(1, prof[k][2])))) for k in kernel_ms}
+    roofs = {k: kernel_roofline(k, kernel_ms[k]["avg_ms"] * 1e-3, rows_k[k], grid, peaks, peaks_src, pipe, hmc, pairs) for k in kernel_ms}
+    for k in kernel_ms:
+        roofs[k]["rows_per_launch"] = rows_k[k]
     out["roofline"] = roofs[dom]
     out["roofline_step"] = [roofs[k] for k in kernel_ms if k != dom]
     out["evaluation"] = evaluation_roofline(args.workload, kernel_ms, dev_s / args.steps, evals_per_step, rows_per_launch, grid, peaks, peaks_src, pipe, pairs)

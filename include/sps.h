@@ -237,6 +237,9 @@ sps_status sps_profile_read(int kernel_id, double* total_ms, int64_t* timed_laun
  * under some filter's 5-sigma support at the row's redshift (everything else contributes exactly zero to Eq. 4 and is
  * skipped).  bench.py's tensor roofline counts 3 x 2 x n_age*n_Z flop per pair and pass.  Synchronises. */
 sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavelength_pairs);
+/* The same summed over the exact-path forward calls (on the stream used last) since the previous call of this function,
+ * and their number: the average work per launch of a sampler run, whose launches shrink as trees finish.  Synchronises. */
+sps_status sps_exact_work_since(const sps_table* t, int64_t* row_wavelength_pairs, int64_t* calls);
 
 /* Throughput of one execution pipe, measured now on the current device (a microbenchmark of ~10 ms; synchronises):
  * SPS_PEAK_MUFU: ex2.approx operations per second (the special-function units the SFH quadrature is bound by),

@@ -22,7 +22,7 @@ STATUS_ENONFINITE = 6
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
            "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
-           "sps_last_error", "sps_version", "sps_exact_last_work", "sps_model_ndim", "sps_set_option", "sps_measure_peak")
+           "sps_last_error", "sps_version", "sps_exact_last_work", "sps_exact_work_since", "sps_model_ndim", "sps_set_option", "sps_measure_peak")
 
 
 class SpsError(RuntimeError):
@@ -256,6 +256,13 @@ def sps_exact_last_work(table) -> int:
     v = C.c_int64()
     _check(lib().sps_exact_last_work(table.handle, C.byref(v)), "sps_exact_last_work")
     return int(v.value)
+
+
+def sps_exact_work_since(table):
+    """-> ((row, wavelength) pairs, exact forward calls) since the previous call."""
+    v, c = C.c_int64(), C.c_int64()
+    _check(lib().sps_exact_work_since(table.handle, C.byref(v), C.byref(c)), "sps_exact_work_since")
+    return int(v.value), int(c.value)
 
 
 def sps_measure_peak(what: str) -> float:

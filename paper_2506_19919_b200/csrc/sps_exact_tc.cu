@@ -421,7 +421,8 @@ __global__ void __launch_bounds__(BM) exact_plan_kernel(TableDev T, int64_t n, c
   if (threadIdx.x == 0) {
     unsigned long long tot = 0;
     for (int w = 0; w < BM / 32; ++w) { zmin = fminf(zmin, s_min[w]); zmax = fmaxf(zmax, s_max[w]); tot += s_pairs[w]; }
-    atomicAdd(work, tot);
+    atomicAdd(work, tot);                                   // this call
+    atomicAdd(work + 1, tot);                               // running total (sps_exact_work_since)
     const float lo = obs_lo / (1.f + zmax) * 0.99999f, hi = obs_hi / (1.f + zmin) * 1.00001f;
     int a = 0, c = T.n_wave;
     while (a < c) { const int mid = (a + c) >> 1; if (T.wave[mid] < lo) a = mid + 1; else c = mid; }
@@ -647,6 +648,7 @@ sps_status launch_forward(const sps_table* t, const TcState* S, Workspace& ws, i
   G.rows = rows; G.part = X.part; G.plan = X.plan; G.plan_cap = X.plan_cap;
   cudaMemsetAsync(X.work, 0, sizeof(unsigned long long), s);
   exact_plan_kernel<<<G.m_tiles, BM, 0, s>>>(T, n, rows, ws.rows, S->fc, S->BK, X.plan, X.plan_cap, X.work);
+  ++X.work_calls;
   exact_scan_kernel<<<1, 32, 0, s>>>(G.m_tiles, X.plan);
   const int grid = std::min(t->sm_count, G.m_tiles * G.n_tiles);
   sps_prof_begin(SPS_K_EXACT_FWD, s);
@@ -750,11 +752,12 @@ sps_status sps_exact_tc_ensure(const sps_table* t, ExactScratch& X, int64_t cap)
   if (e == cudaSuccess) e = cudaMalloc(&X.SB_hi, sn * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&X.SB_lo, sn * S->es);
   if (e == cudaSuccess) e = cudaMalloc(&X.plan, (size_t)4 * X.plan_cap * sizeof(int));
-  if (e == cudaSuccess) e = cudaMalloc(&X.work, sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&X.work, 2 * sizeof(unsigned long long));
   if (e != cudaSuccess) { sps_exact_tc_free_scratch(X); return sps_check_cuda(e, "tensor-core row operand allocation"); }
   cudaMemset(X.W_hi, 0, wn * S->es); cudaMemset(X.W_lo, 0, wn * S->es);
   cudaMemset(X.SB_hi, 0, sn * S->es); cudaMemset(X.SB_lo, 0, sn * S->es);
-  cudaMemset(X.work, 0, sizeof(unsigned long long));
+  cudaMemset(X.work, 0, 2 * sizeof(unsigned long long));
+  X.work_calls = 0;
   X.tc_cap = cap;
   sps_status st = make_map(S, &X.mW_hi, X.W_hi, cap, S->Wld, S->Wld, BM);
   if (st == SPS_OK) st = make_map(S, &X.mW_lo, X.W_lo, cap, S->Wld, S->Wld, BM);
@@ -782,5 +785,19 @@ extern "C" sps_status sps_exact_last_work(const sps_table* t, int64_t* row_wavel
   unsigned long long v = 0;
   sps_status st = sps_check_cuda(cudaMemcpy(&v, ws->x.work, sizeof(v), cudaMemcpyDeviceToHost), "sps_exact_last_work");
   *row_wavelength_pairs = (int64_t)v;
+  return st;
+}
+
+extern "C" sps_status sps_exact_work_since(const sps_table* t, int64_t* row_wavelength_pairs, int64_t* calls) {
+  if (!t || !row_wavelength_pairs || !calls) { sps_set_error("sps_exact_work_since: null argument"); return SPS_EINVAL; }
+  *row_wavelength_pairs = 0; *calls = 0;
+  Workspace* ws = t->last_ws;
+  if (!t->exact || !t->exact->use_tc || !ws || !ws->x.work) return SPS_OK;
+  cudaDeviceSynchronize();
+  unsigned long long v = 0;
+  sps_status st = sps_check_cuda(cudaMemcpy(&v, ws->x.work + 1, sizeof(v), cudaMemcpyDeviceToHost), "sps_exact_work_since");
+  if (st == SPS_OK) st = sps_check_cuda(cudaMemset(ws->x.work + 1, 0, sizeof(v)), "sps_exact_work_since");
+  *row_wavelength_pairs = (int64_t)v; *calls = ws->x.work_calls;
+  ws->x.work_calls = 0;
   return st;
 }

@@ -21,7 +21,8 @@ struct ExactScratch {
   // tensor-core row operands (split W and SEDbar), their TMA maps and the per-row-tile plan
   void *W_hi, *W_lo, *SB_hi, *SB_lo;
   int* plan; int plan_cap;
-  unsigned long long* work; // [1] (row, wavelength) pairs of the last forward call
+  unsigned long long* work; // [2] (row, wavelength) pairs of the last forward call; running total since the last sps_exact_work_since
+  int64_t work_calls;       // forward calls since then
   CUtensorMap mW_hi, mW_lo, mSB_hi, mSB_lo;
   int64_t tc_cap;
 };
