@@ -203,7 +203,9 @@ def run_ours(args):
     e2e_s = (time.perf_counter() - t0) if not args.no_e2e else float("inf")
     dev_s, e2e_s = max_over_ranks([dev_s, e2e_s], dist, device="cuda")
     # ---- untimed: per-kernel event timing of the same launch shape, and the pipe peaks of this run -----------------------
-    sps.sps_profile(True, 4)
+    # every 4th launch of a kernel is timed (NUTS alternates the approximate and the exact rows' launches of the row kernels:
+    # an odd stride samples both)
+    sps.sps_profile(True, 3 if args.workload == "c5_nuts" else 4)
     sps.sps_exact_work_since(table)                                              # (reset)
     profile_step()
     torch.cuda.synchronize()

@@ -138,7 +138,8 @@ sps_status sps_table_cssp(const sps_table* t, float* cssp_host);
 /* sps_weights (diagnostic observable for the 1e-5 weights tolerance): Eq. (A3)-(A7), (2).
  * theta_dev [n,13]; unbounded != 0 means theta_dev holds theta~ and needs `prior` for Eq. (C1)
  * (prior may be NULL when unbounded == 0).  Outputs (device): w_age [n,n_age] = P_SFH (Eq. A6),
- * w_met [n,n_Z] = P_met, mstar [n] = M_star / mass_unit (Eq. A3). */
+ * w_met [n,n_Z] = P_met, mstar [n] = M_star / mass_unit (Eq. A3).  For a table with dlogZ_dlogage != 0 (non-separable
+ * weights: every age bin has its own MDF) w_met is the MDF at age 1 Gyr, i.e. with median logZ itself. */
 sps_status sps_weights(const sps_table* t, const sps_prior* prior, const float* theta_dev, int64_t n,
                        int unbounded, float* w_age_dev, float* w_met_dev, float* mstar_dev, void* stream);
 
