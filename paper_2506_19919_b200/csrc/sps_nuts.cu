@@ -1,7 +1,7 @@
 // sps_nuts.cu -- NUTS engine (a13; reading R15).
 //
-// Multinomial NUTS with iterative doubling and O(depth) U-turn checkpoints, one warp per chain (lane p < 13 owns
-// parameter p).  The paper's finding is that lock-step batches of NUTS transitions run at the speed of the slowest
+// Multinomial NUTS with iterative doubling and O(depth) U-turn checkpoints, half a warp per chain (lane p < 13 of the half
+// owns parameter p; a warp advances two chains).  The paper's finding is that lock-step batches of NUTS transitions run at the speed of the slowest
 // chain.  Here the batch dimension is the LEAPFROG STEP, not the transition: every batch-wide step is
 //   (1) one model evaluation (log-posterior + gradient) at each live chain's working point (sps_eval), then
 //   (2) nuts_step_kernel: each chain advances its own state machine by one leaf -- finish the leapfrog, weigh the
@@ -37,14 +37,22 @@ __device__ __forceinline__ float logaddexpf_(float a, float b) {
 
 __device__ __forceinline__ float* vec(const ChainState& C, int64_t c, int v) { return C.nuts + (c * NUTS_VECTORS + v) * SPS_NDIM; }
 
+// A chain occupies HALF a warp (16 lanes, 13 of them parameters), so a warp advances two chains: `hm` is the lane mask of the
+// chain's half, and every collective of a chain names it (the two halves take different branches of the state machine).
+__device__ __forceinline__ float sum16(float x, unsigned hm) {
+#pragma unroll
+  for (int o = 8; o > 0; o >>= 1) x += __shfl_xor_sync(hm, x, o);
+  return x;
+}
+
 // generalised U-turn criterion: stop unless rho.(invM p_a) > 0 and rho.(invM p_b) > 0
-__device__ __forceinline__ bool uturn(float rho, float pa, float pb, float v, bool act) {
-  const float da = warp_sum(act ? rho * v * pa : 0.f), db = warp_sum(act ? rho * v * pb : 0.f);
+__device__ __forceinline__ bool uturn(float rho, float pa, float pb, float v, bool act, unsigned hm) {
+  const float da = sum16(act ? rho * v * pa : 0.f, hm), db = sum16(act ? rho * v * pb : 0.f, hm);
   return !(da > 0.f) || !(db > 0.f);
 }
 
 // start transition `it`: momentum draw, H0, single-node tree
-__device__ __forceinline__ void begin_transition(ChainState& C, NutsScalars& S, int64_t c, int l, bool act, int64_t o, int it, uint2 key) {
+__device__ __forceinline__ void begin_transition(ChainState& C, NutsScalars& S, int64_t c, int l, bool act, int64_t o, int it, uint2 key, unsigned hm) {
   float kin = 0.f;
   if (act) {
     const float v = C.inv_mass[o];
@@ -55,7 +63,7 @@ __device__ __forceinline__ void begin_transition(ChainState& C, NutsScalars& S, 
     vec(C, c, V_RQ)[l] = q; vec(C, c, V_RP)[l] = p; vec(C, c, V_RG)[l] = g;
     vec(C, c, V_RHO)[l] = p; vec(C, c, V_PQ)[l] = q; vec(C, c, V_PG)[l] = g;
   }
-  kin = warp_sum(kin);
+  kin = sum16(kin, hm);
   if (l == 0) {
     C.H0[c] = -C.logp[c] + kin;
     S.logW[c] = 0.f; S.acc_sum[c] = 0.f; S.prop_lp[c] = C.logp[c];
@@ -81,23 +89,29 @@ __device__ __forceinline__ void begin_doubling(ChainState& C, NutsScalars& S, in
   }
 }
 
+// two chains per warp: lanes 0-15 / 16-31
+#define NUTS_HALF_PROLOGUE(SLOT_COUNT)                                                         \
+  const int64_t slot = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 2 + ((threadIdx.x >> 4) & 1); \
+  const int l = threadIdx.x & 15;                                                              \
+  const unsigned hm = 0xFFFFu << (threadIdx.x & 16);                                           \
+  if (slot >= (SLOT_COUNT)) return;
+
 __global__ void __launch_bounds__(256) nuts_begin_kernel(ChainState C, NutsScalars S, int first, uint2 key) {
-  CHAIN_WARP_PROLOGUE(C.n);
+  NUTS_HALF_PROLOGUE(C.n);
+  const int64_t c = slot;
   const bool act = l < SPS_NDIM;
   const int64_t o = c * SPS_NDIM + (act ? l : 0);
   if (l == 0) { S.it[c] = 0; S.done[c] = 0; }
-  begin_transition(C, S, c, l, act, o, first, key);
-  __syncwarp();
+  begin_transition(C, S, c, l, act, o, first, key, hm);
+  __syncwarp(hm);
   begin_doubling(C, S, c, l, act, o, first, 0, 0, key);
 }
 
 // One leaf per call for every live chain (see the header).  `live` lists the chains to advance (NULL: all).
 __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalars S, WarmupSched W, int max_depth, uint2 key,
                                                         const int* __restrict__ live, int64_t n_live, float* __restrict__ samples) {
-  const int64_t wi = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int l = threadIdx.x & 31;
-  if (wi >= n_live) return;
-  const int64_t c = live ? live[wi] : wi;
+  NUTS_HALF_PROLOGUE(n_live);
+  const int64_t c = live ? live[slot] : slot;
   if (S.done[c]) return;
   const bool act = l < SPS_NDIM;
   const int64_t o = c * SPS_NDIM + (act ? l : 0);
@@ -109,9 +123,9 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
   // ---- finish the leapfrog: second half kick with the gradient just evaluated at theta_w ----
   const float g = C.grad_w[o], q = C.theta_w[o], lp = C.logp_w[c];
   const float p = C.p_w[o] + 0.5f * step * g;
-  const float kin = warp_sum(act ? 0.5f * v * p * p : 0.f);
+  const float kin = sum16(act ? 0.5f * v * p * p : 0.f, hm);
   float dH = -lp + kin - C.H0[c];
-  const bool fin = __all_sync(FULL_MASK, !act || (isfinite(g) && isfinite(q))) && isfinite(dH);
+  const bool fin = __all_sync(hm, !act || (isfinite(g) && isfinite(q))) && isfinite(dH);
   if (!fin) dH = INFINITY;
   const float acc_sum = S.acc_sum[c] + expf(fminf(0.f, -dH));
   const int n_leaf = S.n_leaf[c] + 1;
@@ -137,7 +151,7 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     } else {
       for (int i = i_max; i >= i_min && !bad; --i) {
         const float pc = act ? vec(C, c, V_PCK + i)[l] : 0.f, rc = act ? vec(C, c, V_RCK + i)[l] : 0.f;
-        if (uturn(rho_sub - rc + pc, pc, p, v, act)) bad = true;
+        if (uturn(rho_sub - rc + pc, pc, p, v, act, hm)) bad = true;
       }
     }
   }
@@ -169,30 +183,30 @@ __global__ void __launch_bounds__(256) nuts_step_kernel(ChainState C, NutsScalar
     }
     const int new_depth = depth + 1;
     if (l == 0) { S.logW[c] = logaddexpf_(logW, logW_sub); S.depth[c] = new_depth; S.acc_sum[c] = acc_sum; S.n_leaf[c] = n_leaf; }
-    finish = uturn(rho, pl, pr, v, act) || new_depth >= max_depth;
+    finish = uturn(rho, pl, pr, v, act, hm) || new_depth >= max_depth;
     if (!finish) {
-      __syncwarp();
+      __syncwarp(hm);
       begin_doubling(C, S, c, l, act, o, tr, new_depth, flags, key);
       return;
     }
   }
   // ---- transition complete: the proposal becomes the state; adaptation and summaries; next transition ----
-  __syncwarp();
+  __syncwarp(hm);
   float th = 0.f;
   if (act) { th = vec(C, c, V_PQ)[l]; C.theta[o] = th; C.grad[o] = vec(C, c, V_PG)[l]; }
   if (l == 0) C.logp[c] = S.prop_lp[c];
   const AdaptFlags A = adapt_flags_dev(it, W);
   if (!A.warmup && l == 0) atomicAdd(&S.depth_hist[min(S.depth[c] + (bad ? 1 : 0), NUTS_MAX_DEPTH)], 1);
   chain_adapt_and_record(C, c, l, act, o, th, acc_sum / (float)n_leaf, n_leaf, (flags & F_DIV) ? 1 : 0, A, samples, it - W.n_warmup, W.n_sample, W.bm_len, W.bm_n);
-  __syncwarp();
+  __syncwarp(hm);
   const int it1 = it + 1;
   if (it1 >= W.n_warmup + W.n_sample) {
     if (l == 0) { S.it[c] = it1; S.done[c] = 1; atomicAdd(S.n_done, 1); }
     return;
   }
   if (l == 0) S.it[c] = it1;
-  begin_transition(C, S, c, l, act, o, it1 + W.first, key);
-  __syncwarp();
+  begin_transition(C, S, c, l, act, o, it1 + W.first, key, hm);
+  __syncwarp(hm);
   begin_doubling(C, S, c, l, act, o, it1 + W.first, 0, 0, key);
 }
 
@@ -226,7 +240,7 @@ sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const 
   cudaMemsetAsync(ibase, 0, (6 * n + 4 + NUTS_MAX_DEPTH + 1 + 4) * sizeof(int), s);
   const WarmupSched W = make_warmup_sched(cfg);
   const uint2 key = make_uint2((uint32_t)cfg->seed, (uint32_t)(cfg->seed >> 32));
-  const unsigned cb = (unsigned)((n * 32 + 255) / 256);
+  const unsigned cb = (unsigned)((n * 16 + 255) / 256);          // two chains per warp
   nuts_begin_kernel<<<cb, 256, 0, s>>>(C, S, (int)cfg->first_transition, key); sps_count_launch();
   // live lists: start from the problem's own per-path lists (NULL = all rows on one path)
   HmcProblem L = Q;
@@ -240,7 +254,7 @@ sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const 
                     nullptr, true, C.logp_w, C.grad_w, s);
     }
     if (st != SPS_OK) break;
-    nuts_step_kernel<<<(unsigned)((n_live * 32 + 255) / 256), 256, 0, s>>>(C, S, W, cfg->max_depth, key, live, n_live, samples); sps_count_launch();
+    nuts_step_kernel<<<(unsigned)((n_live * 16 + 255) / 256), 256, 0, s>>>(C, S, W, cfg->max_depth, key, live, n_live, samples); sps_count_launch();
     if ((step & 15) == 15) {
       st = sps_check_cuda(cudaMemcpyAsync(&done_host, S.n_done, sizeof(int), cudaMemcpyDeviceToHost, s), "NUTS poll");
       if (st == SPS_OK) st = sps_check_cuda(cudaStreamSynchronize(s), "NUTS poll");
