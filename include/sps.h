@@ -162,6 +162,20 @@ sps_status sps_loglike_grad(const sps_table* t, const sps_prior* prior, int path
                             const float* obs_flux_dev, const float* obs_sigma_dev, float* logp_dev,
                             float* grad_dev, void* stream);
 
+/* sps_loglike_grad_noalloc: sps_loglike_grad on the approximate path (Eq. 6) for callers that may not
+ * allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, results
+ * and kernels; the per-row scratch lives in one fixed 15.8 MB device array inside the library (held by every GPU that loads
+ * it until the process exits) instead of the per-stream workspace, and the call makes no cudaMalloc / cudaFree.
+ * Limits: n <= SPS_NOALLOC_MAX_ROWS and the table's n_z <= SPS_NOALLOC_MAX_NZ, else SPS_ESHAPE; not for
+ * SPS_MODEL_GAUSS_TEST (no scratch there) and not while sps_profile is on (SPS_EINVAL); SPS_OPT_CHECK_FINITE is not applied.
+ * All calls on a device share the array: calls that overlap on the GPU (different streams) race, so order them.  The first
+ * call on each device resolves the array's device address and should be made outside graph capture.  Does not synchronise. */
+#define SPS_NOALLOC_MAX_ROWS 4096
+#define SPS_NOALLOC_MAX_NZ 1024
+sps_status sps_loglike_grad_noalloc(const sps_table* t, const sps_prior* prior, const float* theta_unb_dev, int64_t n,
+                                    const int32_t* gal_of_row_dev, const float* obs_flux_dev, const float* obs_sigma_dev,
+                                    float* logp_dev, float* grad_dev, void* stream);
+
 /* sps_leapfrog (diagnostic for the trajectory tolerance): n_steps leapfrog steps
  * p += eps/2 grad; theta~ += eps invM*p; p += eps/2 grad from (theta0, p0); per-row eps
  * [n] and diagonal inverse mass [n,13].  traj_dev [n_steps,n,2,13] receives (theta~, p) after each

@@ -22,7 +22,7 @@ STATUS_ENONFINITE = 6
 
 EXPORTS = ("sps_create_table", "sps_destroy_table", "sps_table_cssp", "sps_weights", "sps_photometry",
            "sps_loglike_grad", "sps_leapfrog", "sps_hmc_run", "sps_philox_words", "sps_profile", "sps_profile_read", "sps_launch_count",
-           "sps_last_error", "sps_version", "sps_exact_last_work", "sps_exact_work_since", "sps_model_ndim", "sps_set_option", "sps_measure_peak")
+           "sps_last_error", "sps_version", "sps_exact_last_work", "sps_exact_work_since", "sps_loglike_grad_noalloc", "sps_model_ndim", "sps_set_option", "sps_measure_peak")
 
 
 class SpsError(RuntimeError):
@@ -203,6 +203,18 @@ def sps_loglike_grad(table, prior, path, theta_unb, obs_flux, obs_sigma, gal_of_
     logp, grad = out if out is not None else (_new((n,), like=theta_unb), _new((n, NDIM), like=theta_unb) if want_grad else None)
     _check(lib().sps_loglike_grad(table.handle, prior.ref() if prior is not None else None, int(path), _dptr(theta_unb), C.c_int64(n), _dptr(gal_of_row),
                                   _dptr(obs_flux), _dptr(obs_sigma), _dptr(logp), _dptr(grad), _stream()), "sps_loglike_grad")
+    return logp, grad
+
+
+NOALLOC_MAX_ROWS, NOALLOC_MAX_NZ = 4096, 1024
+
+
+def sps_loglike_grad_noalloc(table, prior, theta_unb, obs_flux, obs_sigma, logp, grad, gal_of_row=None):
+    """sps_loglike_grad on the approximate path with the library's fixed scratch array: no allocation here or in the
+    library (the caller passes the outputs: logp [n], grad [n, 13] or None).  n <= NOALLOC_MAX_ROWS."""
+    n = theta_unb.shape[0]
+    _check(lib().sps_loglike_grad_noalloc(table.handle, prior.ref(), _dptr(theta_unb), C.c_int64(n), _dptr(gal_of_row), _dptr(obs_flux),
+                                          _dptr(obs_sigma), _dptr(logp), _dptr(grad), _stream()), "sps_loglike_grad_noalloc")
     return logp, grad
 
 

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsps_b200.so")
-SOURCES = ["sps_api.cu", "sps_table.cu", "sps_kernels.cu", "sps_models.cu", "sps_nonsep.cu", "sps_approx_tc.cu", "sps_exact.cu", "sps_exact_tc.cu", "sps_sampler.cu", "sps_leapfrog.cu", "sps_nuts.cu"]
+SOURCES = ["sps_api.cu", "sps_table.cu", "sps_kernels.cu", "sps_models.cu", "sps_nonsep.cu", "sps_noalloc.cu", "sps_approx_tc.cu", "sps_exact.cu", "sps_exact_tc.cu", "sps_sampler.cu", "sps_leapfrog.cu", "sps_nuts.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr", "-use_fast_math", "-Xptxas", "-v"]
 
