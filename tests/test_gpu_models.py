@@ -607,3 +607,50 @@ def test_dependent_launch_and_cell_counts(full):
     for simt, lp, g in runs:
         first = next(r for r in runs if r[0] == simt)
         assert torch.equal(lp, first[1]) and torch.equal(g, first[2])
+
+
+# ---- degenerate launch shapes ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 129, 257])
+def test_exact_path_ragged_sizes(full, n):
+    # one row, one row past a 128-row tile, one past two: fluxes and the VJP against the oracle on sampled rows, and every
+    # row bit-identical to the same row evaluated alone (the exact path's band sums are order-independent)
+    cx = full
+    thu = W.draw_theta_unbounded(cx.prior, n, 900 + n, z_uniform=(0.05, 2.95)).astype(np.float32)
+    fb = np.random.default_rng(n).normal(size=(n, cx.grid.n_band)).astype(np.float32)
+    flux, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_EXACT, _dev(thu), True, _dev(fb))
+    pick = np.unique(np.r_[0, n - 1, np.random.default_rng(3).integers(0, n, 4)])
+    th, dth = M.bound(thu[pick].astype(np.float64), cx.P)
+    of, J = M.photometry_exact(th, cx.grid, True)
+    assert (np.abs(flux.cpu().numpy()[pick] - of) / np.abs(of)).max() <= 1e-4
+    ref = np.einsum("rb,rbp->rp", fb[pick].astype(np.float64), J * dth[:, None, :])
+    scale = np.einsum("rb,rbp->rp", np.abs(fb[pick]).astype(np.float64), np.abs(J * dth[:, None, :]))
+    assert (np.abs(tb.cpu().numpy()[pick] - ref) / np.maximum(scale, TAB_FLOOR["exact"] * scale.max(1, keepdims=True))).max() <= 1e-3
+    for r in pick[:3]:
+        f1, t1 = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_EXACT, _dev(thu[r:r + 1]), True, _dev(fb[r:r + 1]))
+        assert torch.equal(f1[0], flux[r]) and torch.equal(t1[0], tb[r])
+
+
+def test_all_rows_in_one_z_cell_and_at_the_grid_ends(full, kernels):
+    # the approximate path groups rows by z cell: 700 rows of ONE cell (six tiles of the same cell, the others empty), and
+    # rows whose redshift saturates at the bounds of the prior (first / last cell of the table)
+    cx = full
+    n = 700
+    thu = W.draw_theta_unbounded(cx.prior, n, 31).astype(np.float64)
+    k, x0 = cx.P[2][12], cx.P[3][12]
+    y_lo, y_hi = cx.P[0][12], cx.P[1][12]
+    z_target = 1.2345
+    thu[:, 12] = x0 + np.log((z_target - y_lo) / (y_hi - z_target)) / k          # Eq. (C1) inverted: every row at z = 1.2345
+    thu[-8:-4, 12] = x0 - 60.0 / k                                               # z -> lower bound
+    thu[-4:, 12] = x0 + 60.0 / k                                                 # z -> upper bound
+    thu = thu.astype(np.float32)
+    th, dth = M.bound(thu.astype(np.float64), cx.P)
+    assert np.abs(th[:-8, 12] - z_target).max() < 1e-5
+    of, J = M.photometry_approx(th, cx.grid, cx.cssp())
+    fb = np.random.default_rng(8).normal(size=(n, cx.grid.n_band)).astype(np.float32)
+    flux, tb = cx.sps.sps_photometry(cx.table, cx.ph, cx.sps.PATH_APPROX, _dev(thu), True, _dev(fb))
+    assert (np.abs(flux.cpu().numpy() - of) / np.abs(of)).max() <= 1e-4
+    ref = np.einsum("rb,rbp->rp", fb.astype(np.float64), J * dth[:, None, :])
+    scale = np.einsum("rb,rbp->rp", np.abs(fb).astype(np.float64), np.abs(J * dth[:, None, :]))
+    err = np.abs(tb.cpu().numpy() - ref) / np.maximum(scale, 1e-3 * scale.max(1, keepdims=True))
+    err[-8:, 12] = 0.0             # saturated sigmoid: d z / d theta~ ~ 1e-26, nothing to compare
+    assert err.max() <= 1e-3
