@@ -209,18 +209,23 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         mbar_wait(BAR(BAR_B1), ph);
         mbar_wait(BAR(BAR_A), ph);
         tc_fence_after();
+        // Split products in ONE accumulator, the cross terms a_lo c_hi + a_hi c_lo (2^-11 of the main one) first: tensor-core
+        // accumulation truncates every update to fp32, an error relative to the accumulator's size at that
+        // moment, so the 16 cross updates cost nothing and the sum sees the 8 full-size updates of the main products only.
 #pragma unroll
         for (int kb = 0; kb < 2; ++kb)
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk) {
             const uint64_t a_hi = desc_sw128(base + kb * TILE_A + kk * 32), a_lo = desc_sw128(base + (2 + kb) * TILE_A + kk * 32);
             const uint64_t b_hi = desc_sw128(base + OFF_B + kb * 32768u + kk * 32), b_lo = desc_sw128(base + OFF_B + 65536u + kb * 32768u + kk * 32);
-            // the cross terms (2^-11 of the main one) have an accumulator of their own: the main accumulator then sees
-            // 8 truncating updates instead of 24 (tensor-core accumulation rounds toward zero)
-            tc_mma_f16(tmem_base + NE, a_lo, b_hi, idesc1, (kb | kk) ? 1u : 0u);
-            tc_mma_f16(tmem_base + NE, a_hi, b_lo, idesc1, 1u);
-            tc_mma_f16(tmem_base, a_hi, b_hi, idesc1, (kb | kk) ? 1u : 0u);
+            tc_mma_f16(tmem_base, a_lo, b_hi, idesc1, (kb | kk) ? 1u : 0u);
+            tc_mma_f16(tmem_base, a_hi, b_lo, idesc1, 1u);
           }
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)
+            tc_mma_f16(tmem_base, desc_sw128(base + kb * TILE_A + kk * 32), desc_sw128(base + OFF_B + kb * 32768u + kk * 32), idesc1, 1u);
         tc_commit(BAR(BAR_P));
         mbar_wait(BAR(BAR_P), ph);                          // pass 1 retired: the table region may be overwritten
         if (!G.want_grad) continue;
@@ -235,10 +240,10 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
         mbar_wait(BAR(BAR_V0), ph);
         tc_fence_after();
         // Both table arrays are contracted with the same operand V (the row's factor f on the D_t part is applied when the
-        // accumulators are read): acc^(s) = sum_e V[e] C^(s)[i][e].  The accumulators reuse the columns of P (dead once V is
-        // being written): s = 0 main / cross terms at columns 0 / NA, s = 1 at 2 NA / 3 NA.
+        // accumulators are read): acc^(s) = sum_e V[e] C^(s)[i][e], cross terms first (see pass 1).  The accumulators reuse the
+        // columns of P (dead once V is being written): s = 0 at columns 0, s = 1 at NA.
 #pragma unroll
-        for (int s = 0; s < 2; ++s)
+        for (int s = 0; s < 2; ++s) {
 #pragma unroll
           for (int kb = 0; kb < 2; ++kb)
 #pragma unroll
@@ -246,10 +251,15 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
               const int eb = 2 * s + kb;
               const uint64_t a_hi = desc_sw128(base + kb * TILE_A + kk * 32), a_lo = desc_sw128(base + (2 + kb) * TILE_A + kk * 32);
               const uint64_t b_hi = desc_sw128(base + OFF_B + eb * 16384u + kk * 32), b_lo = desc_sw128(base + OFF_B + 65536u + eb * 16384u + kk * 32);
-              tc_mma_f16(tmem_base + (2 * s + 1) * NA, a_lo, b_hi, idesc2, (kb | kk) ? 1u : 0u);
-              tc_mma_f16(tmem_base + (2 * s + 1) * NA, a_hi, b_lo, idesc2, 1u);
-              tc_mma_f16(tmem_base + 2 * s * NA, a_hi, b_hi, idesc2, (kb | kk) ? 1u : 0u);
+              tc_mma_f16(tmem_base + s * NA, a_lo, b_hi, idesc2, (kb | kk) ? 1u : 0u);
+              tc_mma_f16(tmem_base + s * NA, a_hi, b_lo, idesc2, 1u);
             }
+#pragma unroll
+          for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)
+              tc_mma_f16(tmem_base + s * NA, desc_sw128(base + kb * TILE_A + kk * 32), desc_sw128(base + OFF_B + (2 * s + kb) * 16384u + kk * 32), idesc2, 1u);
+        }
         tc_commit(BAR(BAR_M1));
         mbar_wait(BAR(BAR_M1), ph);                         // pass 2 retired: both regions are free for the next tile
       }
@@ -375,16 +385,15 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         if ((c & 1) == h && 16 * c < E) {
-          uint32_t v0[16], v1[16], x0[16], x1[16];
+          uint32_t v0[16], v1[16];
           TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
-          TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
           tld_wait();
 #pragma unroll
           for (int k = 0; k < 16; ++k) {
             const int e = 16 * c + k, j = e / NB, b = e % NB;
             if (j < 16) {
-              S0[b] = fmaf(m[j], __uint_as_float(v0[k]) + __uint_as_float(x0[k]), S0[b]);
-              S1[b] = fmaf(m[j], __uint_as_float(v1[k]) + __uint_as_float(x1[k]), S1[b]);
+              S0[b] = fmaf(m[j], __uint_as_float(v0[k]), S0[b]);
+              S1[b] = fmaf(m[j], __uint_as_float(v1[k]), S1[b]);
             }
           }
         }
@@ -448,14 +457,13 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
           if ((c & 1) == h && 16 * c < E) {
-            uint32_t v0[16], v1[16], x0[16], x1[16];
+            uint32_t v0[16], v1[16];
             TLD16(tlane + 16 * c, v0); TLD16(tlane + 128 + 16 * c, v1);
-            TLD16(tlane + NE + 16 * c, x0); TLD16(tlane + NE + 128 + 16 * c, x1);
             tld_wait();
 #pragma unroll
             for (int k = 0; k < 16; ++k) {
               const int e = 16 * c + k, j = e / NB, b = e % NB;
-              if (j < 16) mb[j] = fmaf(sbar[b], fmaf(fu1, __uint_as_float(v1[k]) + __uint_as_float(x1[k]), u0 * (__uint_as_float(v0[k]) + __uint_as_float(x0[k]))), mb[j]);
+              if (j < 16) mb[j] = fmaf(sbar[b], fmaf(fu1, __uint_as_float(v1[k]), u0 * __uint_as_float(v0[k])), mb[j]);
             }
           }
         }
@@ -533,12 +541,11 @@ approx_tc_kernel(TableDev T, ApproxArgs G, RowBuffers B, const __grid_constant__
       float4* stage = reinterpret_cast<float4*>(gbase);                   // [TM][32] float4
 #pragma unroll 1
       for (int c = 4 * h; c < 4 * h + 4; ++c) {
-        uint32_t v[16], x[16], v1[16], x1[16];
-        TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, x); TLD16(tlane + 2 * NA + 16 * c, v1); TLD16(tlane + 3 * NA + 16 * c, x1);
+        uint32_t v[16], v1[16];
+        TLD16(tlane + 16 * c, v); TLD16(tlane + NA + 16 * c, v1);
         tld_wait();
 #pragma unroll
-        for (int k = 0; k < 16; ++k)
-          v[k] = __float_as_uint(fmaf(fa, __uint_as_float(v1[k]) + __uint_as_float(x1[k]), __uint_as_float(v[k]) + __uint_as_float(x[k])));
+        for (int k = 0; k < 16; ++k) v[k] = __float_as_uint(fmaf(fa, __uint_as_float(v1[k]), __uint_as_float(v[k])));
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
           float4 o;
