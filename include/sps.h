@@ -225,6 +225,8 @@ typedef struct {
   int32_t* depth_hist;  /* [11]               NUTS: kept transitions per final tree depth 0..10       */
 } sps_hmc_summary;
 
+/* (sps_hmc_run and sps_leapfrog take their per-run device buffers from a process-wide cache of blocks and hand them back at
+ * the end: no cudaFree per call; sps_destroy_table releases the blocks that are not in use.) */
 /* sps_hmc_run: n_gal galaxies x n_chain chains of (n_warmup + n_sample) transitions.
  * obs_flux_dev/obs_sigma_dev [n_gal,n_band]; path_of_gal_dev [n_gal] int32 or NULL;
  * theta0_unb_dev [n_gal*n_chain,13] or NULL (R17: xi + 0.1 omega N(0,1));

@@ -57,6 +57,11 @@ sps_status sps_require_device();
 Workspace* sps_workspace(const sps_table* t, cudaStream_t s);                 // never null; thread-safe
 sps_status sps_ensure_row_buffers(const sps_table* t, Workspace& ws, int64_t n, cudaStream_t s);
 void sps_free_workspace(Workspace* ws);
+// process-wide cache of device blocks for the samplers' per-run state (sps_api.cu): alloc reuses a free block of a fitting
+// size, free hands the block back (no cudaFree), release_unused frees the idle ones (sps_destroy_table)
+cudaError_t sps_pool_alloc(void** p, size_t bytes);
+void sps_pool_free(void* p);
+void sps_pool_release_unused();
 sps_status sps_prior_to_dev(const sps_table* t, const sps_prior* p, PriorDev& out);
 // SPS_OPT_CHECK_FINITE: device reduction over the given arrays (any may be null); SPS_ENONFINITE if one entry is not finite
 // or a `positive` entry is <= 0.  No-op (SPS_OK) when the option is off.

@@ -12,11 +12,11 @@ __global__ void gal_of_chain_kernel(int* out, int* rng_id, const int* __restrict
 }
 
 static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n_gal, const int32_t* path_of_gal_dev) {
-  sps_status st = sps_check_cuda(cudaMalloc(&Q.gal_of_chain, Q.n * sizeof(int)), "gal_of_chain allocation");
-  if (st == SPS_OK) st = sps_check_cuda(cudaMalloc(&Q.rng_id, Q.n * sizeof(int)), "rng_id allocation");
+  sps_status st = sps_check_cuda(sps_pool_alloc((void**)&Q.gal_of_chain, Q.n * sizeof(int)), "gal_of_chain allocation");
+  if (st == SPS_OK) st = sps_check_cuda(sps_pool_alloc((void**)&Q.rng_id, Q.n * sizeof(int)), "rng_id allocation");
   if (st != SPS_OK) return st;
   gal_of_chain_kernel<<<(unsigned)((Q.n + 255) / 256), 256>>>(Q.gal_of_chain, Q.rng_id, cfg->gal_id_dev, Q.n, cfg->n_chain); sps_count_launch();
-  st = sps_check_cuda(cudaMalloc(&Q.path_of_chain, Q.n), "path_of_chain allocation");
+  st = sps_check_cuda(sps_pool_alloc((void**)&Q.path_of_chain, Q.n), "path_of_chain allocation");
   if (st != SPS_OK) return st;
   if (!path_of_gal_dev) {
     if (cfg->path != SPS_PATH_EXACT && cfg->path != SPS_PATH_APPROX) { sps_set_error("bad path"); return SPS_EINVAL; }
@@ -25,7 +25,7 @@ static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int
     if (Q.n_groups > 1) {                                     // row groups need an explicit (identity) list to offset into
       std::vector<int> ident(Q.n);
       for (int64_t i = 0; i < Q.n; ++i) ident[i] = (int)i;
-      st = sps_check_cuda(cudaMalloc(&Q.rows_path[cfg->path], Q.n * sizeof(int)), "row list allocation");
+      st = sps_check_cuda(sps_pool_alloc((void**)&Q.rows_path[cfg->path], Q.n * sizeof(int)), "row list allocation");
       if (st != SPS_OK) return st;
       cudaMemcpy(Q.rows_path[cfg->path], ident.data(), Q.n * sizeof(int), cudaMemcpyHostToDevice);
     }
@@ -44,7 +44,7 @@ static sps_status hmc_problem_fill(HmcProblem& Q, const sps_hmc_config* cfg, int
   for (int p = 0; p < 2; ++p) {
     Q.n_rows_path[p] = (int64_t)rows[p].size();
     if (rows[p].empty()) continue;
-    st = sps_check_cuda(cudaMalloc(&Q.rows_path[p], rows[p].size() * sizeof(int)), "row list allocation");
+    st = sps_check_cuda(sps_pool_alloc((void**)&Q.rows_path[p], rows[p].size() * sizeof(int)), "row list allocation");
     if (st != SPS_OK) return st;
     cudaMemcpy(Q.rows_path[p], rows[p].data(), rows[p].size() * sizeof(int), cudaMemcpyHostToDevice);
   }
@@ -67,10 +67,10 @@ sps_status hmc_problem_setup(HmcProblem& Q, const sps_hmc_config* cfg, int64_t n
 }
 
 void hmc_problem_free(HmcProblem& Q) {
-  if (Q.gal_of_chain) cudaFree(Q.gal_of_chain);
-  if (Q.rng_id) cudaFree(Q.rng_id);
-  if (Q.path_of_chain) cudaFree(Q.path_of_chain);
-  for (int p = 0; p < 2; ++p) if (Q.rows_path[p]) cudaFree(Q.rows_path[p]);
+  if (Q.gal_of_chain) sps_pool_free(Q.gal_of_chain);
+  if (Q.rng_id) sps_pool_free(Q.rng_id);
+  if (Q.path_of_chain) sps_pool_free(Q.path_of_chain);
+  for (int p = 0; p < 2; ++p) if (Q.rows_path[p]) sps_pool_free(Q.rows_path[p]);
   memset(&Q, 0, sizeof(Q));
 }
 
@@ -119,7 +119,7 @@ extern "C" sps_status sps_leapfrog(const sps_table* t, const sps_prior* prior, i
   if (t->dev.model != SPS_MODEL_GAUSS_TEST) { st = sps_ensure_row_buffers(t, ws, n, s); if (st != SPS_OK) return st; }
   float* w = nullptr;
   const size_t nv = (size_t)n * SPS_NDIM;
-  st = sps_check_cuda(cudaMalloc(&w, (3 * nv + n) * sizeof(float)), "sps_leapfrog scratch"); if (st != SPS_OK) return st;
+  st = sps_check_cuda(sps_pool_alloc((void**)&w, (3 * nv + n) * sizeof(float)), "sps_leapfrog scratch"); if (st != SPS_OK) return st;
   float *theta_w = w, *p_w = w + nv, *grad_w = w + 2 * nv, *logp_w = w + 3 * nv;
   const unsigned eb = (unsigned)((nv + 255) / 256);
   st = sps_eval(t, ws, P, path, theta0, n, true, true, nullptr, gal_of_row, obs_flux, obs_sigma, nullptr, true, logp_w, grad_w, s);
@@ -129,6 +129,6 @@ extern "C" sps_status sps_leapfrog(const sps_table* t, const sps_prior* prior, i
     if (st == SPS_OK) { lf_record_kernel<<<eb, 256, 0, s>>>(n, k, grad_w, logp_w, eps, inv_mass, theta_w, p_w, traj, logp_traj); sps_count_launch(); }
   }
   cudaStreamSynchronize(s);
-  cudaFree(w);
+  sps_pool_free(w);
   return st == SPS_OK ? sps_check_cuda(cudaGetLastError(), "sps_leapfrog") : st;
 }

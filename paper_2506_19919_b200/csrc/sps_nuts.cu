@@ -229,10 +229,10 @@ sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const 
   if (cfg->n_warmup + cfg->n_sample == 0) return SPS_OK;
   NutsScalars S; memset(&S, 0, sizeof(S));
   float* fbase = nullptr; int* ibase = nullptr; int* lists = nullptr;
-  sps_status st = sps_check_cuda(cudaMalloc(&fbase, 5 * n * sizeof(float)), "NUTS state");
-  if (st == SPS_OK) st = sps_check_cuda(cudaMalloc(&ibase, (6 * n + 4 + NUTS_MAX_DEPTH + 1 + 4) * sizeof(int)), "NUTS state");
-  if (st == SPS_OK) st = sps_check_cuda(cudaMalloc(&lists, 3 * n * sizeof(int)), "NUTS live lists");
-  if (st != SPS_OK) { if (fbase) cudaFree(fbase); if (ibase) cudaFree(ibase); if (lists) cudaFree(lists); return st; }
+  sps_status st = sps_check_cuda(sps_pool_alloc((void**)&fbase, 5 * n * sizeof(float)), "NUTS state");
+  if (st == SPS_OK) st = sps_check_cuda(sps_pool_alloc((void**)&ibase, (6 * n + 4 + NUTS_MAX_DEPTH + 1 + 4) * sizeof(int)), "NUTS state");
+  if (st == SPS_OK) st = sps_check_cuda(sps_pool_alloc((void**)&lists, 3 * n * sizeof(int)), "NUTS live lists");
+  if (st != SPS_OK) { if (fbase) sps_pool_free(fbase); if (ibase) sps_pool_free(ibase); if (lists) sps_pool_free(lists); return st; }
   S.logW = fbase; S.logW_sub = fbase + n; S.acc_sum = fbase + 2 * n; S.prop_lp = fbase + 3 * n; S.sub_lp = fbase + 4 * n;
   S.it = ibase; S.depth = ibase + n; S.leaf = ibase + 2 * n; S.n_leaf = ibase + 3 * n; S.flags = ibase + 4 * n; S.done = ibase + 5 * n;
   S.n_done = ibase + 6 * n; S.depth_hist = ibase + 6 * n + 4;
@@ -275,6 +275,6 @@ sps_status nuts_run(const sps_table* t, Workspace& ws, const PriorDev& P, const 
   if (st == SPS_OK && depth_hist_out)                       // kept transitions per final tree depth
     cudaMemcpyAsync(depth_hist_out, S.depth_hist, (NUTS_MAX_DEPTH + 1) * sizeof(int), cudaMemcpyDeviceToDevice, s);
   cudaStreamSynchronize(s);
-  cudaFree(fbase); cudaFree(ibase); cudaFree(lists);
+  sps_pool_free(fbase); sps_pool_free(ibase); sps_pool_free(lists);
   return st;
 }

@@ -152,7 +152,7 @@ sps_status chain_state_alloc(ChainState& C, int64_t n, int ckpt_vectors) {
   const size_t ns = 17;                             // scalars per chain
   const size_t bytes = n * (nv * SPS_NDIM + ns) * sizeof(float);
   float* base = nullptr;
-  sps_status st = sps_check_cuda(cudaMalloc(&base, bytes), "chain state allocation");
+  sps_status st = sps_check_cuda(sps_pool_alloc((void**)&base, bytes), "chain state allocation");
   if (st != SPS_OK) return st;
   cudaMemset(base, 0, bytes);
   C.base = base;
@@ -169,7 +169,7 @@ sps_status chain_state_alloc(ChainState& C, int64_t n, int ckpt_vectors) {
   C.nuts_sc = sca();   // 5 scalars left for NUTS
   return SPS_OK;
 }
-void chain_state_free(ChainState& C) { if (C.base) cudaFree(C.base); C.base = nullptr; }
+void chain_state_free(ChainState& C) { if (C.base) sps_pool_free(C.base); C.base = nullptr; }
 
 // R14 windows (restated): <20 warmup steps: step size only.  >=150: 75 | 25,50,100,... | 50; else 15% | one window | 10%.
 void warmup_schedule(int W, std::vector<int>& ends, int& slow_lo, int& slow_hi) {
@@ -301,7 +301,7 @@ extern "C" sps_status sps_hmc_run(const sps_table* t, const sps_prior* prior, co
     // Plain launches are used when per-kernel profiling is on, with SPS_OPT_NO_GRAPH, or if capture fails.
     const int n_tr = cfg->n_warmup + cfg->n_sample;
     HmcCtl* ctl = nullptr;
-    st = sps_check_cuda(cudaMalloc(&ctl, sizeof(HmcCtl)), "HMC control block");
+    st = sps_check_cuda(sps_pool_alloc((void**)&ctl, sizeof(HmcCtl)), "HMC control block");
     if (st == SPS_OK) cudaMemsetAsync(ctl, 0xff, sizeof(int), s);          // it = -1
     auto enqueue_transition = [&]() -> sps_status {
       hmc_ctl_kernel<<<1, 1, 0, s>>>(ctl, W);
@@ -342,7 +342,7 @@ extern "C" sps_status sps_hmc_run(const sps_table* t, const sps_prior* prior, co
       else st = enqueue_transition();
     }
     if (exec) { cudaStreamSynchronize(s); cudaGraphExecDestroy(exec); }
-    if (ctl) { cudaStreamSynchronize(s); cudaFree(ctl); }
+    if (ctl) { cudaStreamSynchronize(s); sps_pool_free(ctl); }
   } else if (st == SPS_OK) {
     st = nuts_run(t, ws, P, cfg, Q, C, samples, summary ? summary->depth_hist : nullptr, s);
   }

@@ -340,6 +340,7 @@ extern "C" sps_status sps_destroy_table(sps_table* t) {
   sps_approx_tc_teardown(t);
   for (auto& kv : t->ws) sps_free_workspace(kv.second);
   t->ws.clear();
+  sps_pool_release_unused();
   if (t->own_stream) cudaStreamDestroy(t->own_stream);
   for (cudaStream_t a : t->aux_stream) if (a) cudaStreamDestroy(a);
   delete t;
