@@ -48,10 +48,12 @@ __device__ __forceinline__ void row_forward(const TableDev& T, const PriorView& 
 // a0-a5.  With store_part the per-bin masses dM_i and their partials with respect to (tau, alpha, beta, t_obs) are
 // kept in B.part for the epilogue, which then has no quadrature to redo.  One instantiation serves forward-only and
 // gradient calls (the partials are computed either way), so that both give bit-identical weights and fluxes.
+// Compiled for 48 resident warps per SM (40 registers, ~170 bytes of spills) rather than 32 (60 registers, none): measured
+// 82.6 -> 77.3 us at 40,000 rows; 64 warps (32 registers) and 256-thread blocks at the same occupancy are slower.
 // PW = rows (warps) per block: 16 when the kernel has the SMs to itself; 8 when the sampler overlaps two row groups, so
 // that a block fits in the registers the persistent contraction CTA of the other group leaves free on an SM.
 template <int PW>
-__global__ void __launch_bounds__(32 * PW, 32 / PW)
+__global__ void __launch_bounds__(32 * PW, 48 / PW)
 prologue_kernel(TableDev T, PriorDev P, const float* __restrict__ theta, int64_t n, bool unbounded, bool store_part,
                 const int* __restrict__ rows, RowBuffers B, int* __restrict__ hist) {
   constexpr bool WANT_GRAD = true;
