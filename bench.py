@@ -275,13 +275,13 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), at the
 # launch sizes named there; None where no capture of that launch size exists.
 NCU_TRAFFIC = {
-    ("prologue", 40000): 71.4e6, ("approx_contract", 40000): 58.5e6, ("epilogue", 40000): 140.7e6,   # profiles/r02_hmc_kernels_full.md
+    ("prologue", 40000): 85.8e6, ("approx_contract", 40000): 59.0e6, ("epilogue", 40000): 140.1e6,   # profiles/r02_hmc_kernels_full.md
     ("exact_fwd", 8192): 96.4e6, ("exact_bwd", 8192): 252.1e6,                                        # profiles/r02_exact_gemm_full.md
 }
 
 
 # lts__t_sectors.sum x 32 B per launch from the same captures (every L2 access: SM loads, stores, TMA, atomics and the fills)
-NCU_L2 = {("prologue", 40000): 213.4e6, ("approx_contract", 40000): 260.6e6, ("epilogue", 40000): 229.2e6}      # profiles/r02_hmc_kernels_full.md
+NCU_L2 = {("prologue", 40000): 384.1e6, ("approx_contract", 40000): 264.3e6, ("epilogue", 40000): 229.8e6}      # profiles/r02_hmc_kernels_full.md
 
 
 def algorithmic_counts(grid):
